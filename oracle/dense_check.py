@@ -1,0 +1,94 @@
+"""Exact dense 2^N Heisenberg evolution - the yardstick the ORACLE is pinned against.
+
+TEST INFRASTRUCTURE ONLY (see ``oracle/pepo_oracle.py`` header).  Deliberately shares no
+code with ``pepo_oracle.py`` (own Pauli matrices, own lattice enumeration, 2^N x 2^N complex
+matrices instead of Pauli-transfer matrices), so that agreement between the two is a real
+cross-check (SURVEY.md §8(c) pin P1).
+
+Follows PAPER.md eq. (3)-(5) (L52-L80): Z_c(t+dt) = U^dag Z_c(t) U, C(t) = Tr[Z_c(t) Z_c]/2^N
+(eq. (4)), with the Hamiltonian and Trotter splitting BASELINE.json fixes (DESIGN.md
+readings R1, R2):  H = -J sum_<ij> B_i B_j - h sum_i F_i,  U_step = U_field * U_bond with
+U_field = prod_i exp(+i h dt F_i), U_bond = prod_<ij> exp(+i J dt B_i B_j), so that
+U_step^dag O U_step applies the field conjugation first and the bond conjugation second.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+_I2 = np.eye(2, dtype=complex)
+_SIG = {
+    "I": _I2,
+    "X": np.array([[0, 1], [1, 0]], dtype=complex),
+    "Y": np.array([[0, -1j], [1j, 0]], dtype=complex),
+    "Z": np.array([[1, 0], [0, -1]], dtype=complex),
+}
+
+
+def _embed(ops: dict, n: int) -> np.ndarray:
+    """Kronecker product over sites 0..n-1 with ``ops[site]`` where given, identity elsewhere."""
+    out = np.ones((1, 1), dtype=complex)
+    for s in range(n):
+        out = np.kron(out, ops.get(s, _I2))
+    return out
+
+
+def _bonds(Lx: int, Ly: int):
+    b = []
+    for y in range(Ly):
+        for x in range(Lx):
+            if x + 1 < Lx:
+                b.append((y * Lx + x, y * Lx + x + 1))
+            if y + 1 < Ly:
+                b.append((y * Lx + x, (y + 1) * Lx + x))
+    return b
+
+
+def hamiltonian(Lx, Ly, J, h, bond="Z", field="X"):
+    n = Lx * Ly
+    H = np.zeros((2 ** n, 2 ** n), dtype=complex)
+    for (i, j) in _bonds(Lx, Ly):
+        H -= J * _embed({i: _SIG[bond], j: _SIG[bond]}, n)
+    for i in range(n):
+        H -= h * _embed({i: _SIG[field]}, n)
+    return H
+
+
+def _expm_herm(A: np.ndarray, coeff: complex) -> np.ndarray:
+    """exp(coeff * A) for Hermitian A through its eigendecomposition."""
+    w, V = np.linalg.eigh(A)
+    return (V * np.exp(coeff * w)) @ V.conj().T
+
+
+def trotter_unitary(Lx, Ly, J, h, dt, bond="Z", field="X"):
+    n = Lx * Ly
+    Hf = np.zeros((2 ** n, 2 ** n), dtype=complex)
+    for i in range(n):
+        Hf += h * _embed({i: _SIG[field]}, n)
+    Hb = np.zeros((2 ** n, 2 ** n), dtype=complex)
+    for (i, j) in _bonds(Lx, Ly):
+        Hb += J * _embed({i: _SIG[bond], j: _SIG[bond]}, n)
+    return _expm_herm(Hf, 1j * dt) @ _expm_herm(Hb, 1j * dt)
+
+
+def dense_trotter_correlation(Lx, Ly, cx, cy, J, h, dt, n_steps, bond="Z", field="X", obs="Z"):
+    """C after each of ``n_steps`` first-order Trotter steps, by 2^N x 2^N conjugation."""
+    n = Lx * Ly
+    c = cy * Lx + cx
+    Zc = _embed({c: _SIG[obs]}, n)
+    U = trotter_unitary(Lx, Ly, J, h, dt, bond, field)
+    O = Zc.copy()
+    out = []
+    for _ in range(n_steps):
+        O = U.conj().T @ O @ U
+        out.append(float(np.trace(O @ Zc).real) / 2 ** n)
+    return out
+
+
+def dense_exact_correlation(Lx, Ly, cx, cy, J, h, t, bond="Z", field="X", obs="Z"):
+    """Tr[e^{iHt} Z_c e^{-iHt} Z_c]/2^N with the exact propagator (Trotter-error context)."""
+    n = Lx * Ly
+    c = cy * Lx + cx
+    Zc = _embed({c: _SIG[obs]}, n)
+    U = _expm_herm(hamiltonian(Lx, Ly, J, h, bond, field), -1j * t)
+    O = U.conj().T @ Zc @ U
+    return float(np.trace(O @ Zc).real) / 2 ** n

@@ -1,0 +1,287 @@
+"""Pins of the CPU oracle against things other than itself.
+
+All -m "not gpu".  Paper citations are /root/reference/PAPER.md lines.
+"""
+import itertools
+import math
+
+import numpy as np
+import pytest
+
+from oracle import dense_check as dc
+from oracle import pepo_oracle as po
+
+J, H, DT = 1.0, 0.9, 0.05
+
+
+# ---------------------------------------------------------------- gates (R2, R15) ---------
+def test_field_gate_is_yz_rotation():
+    """PTM of exp(+i theta X): I, X fixed; c_Y' = cos2t c_Y - sin2t c_Z, c_Z' = sin2t c_Y + cos2t c_Z."""
+    th = H * DT
+    G = po.ptm_one_site(th, "X")
+    c, s = math.cos(2 * th), math.sin(2 * th)
+    expect = np.array([[1, 0, 0, 0], [0, 1, 0, 0], [0, 0, c, -s], [0, 0, s, c]])
+    assert np.allclose(G, expect, atol=1e-15)
+    assert np.allclose(G @ G.T, np.eye(4), atol=1e-15)      # real orthogonal
+
+
+def test_zz_gate_structure():
+    """R15: closed-form entries of the ZZ PTM, orthogonality, operator-Schmidt rank 4."""
+    th = J * DT
+    G = po.ptm_two_site(th, "Z")
+    c, s = math.cos(2 * th), math.sin(2 * th)
+    assert np.allclose(G @ G.T, np.eye(16), atol=1e-14)
+    idx = lambda a, b: "IXYZ".index(a) * 4 + "IXYZ".index(b)
+    for ab in ["II", "IZ", "ZI", "ZZ", "XX", "XY", "YX", "YY"]:
+        assert abs(G[idx(*ab), idx(*ab)] - 1) < 1e-15
+    for ab in ["IX", "IY", "XI", "YI", "ZX", "ZY", "XZ", "YZ"]:
+        assert abs(G[idx(*ab), idx(*ab)] - c) < 1e-15
+    pairs = [("IX", "ZY", -s), ("ZY", "IX", +s), ("IY", "ZX", +s), ("ZX", "IY", -s),
+             ("XI", "YZ", -s), ("YZ", "XI", +s), ("YI", "XZ", +s), ("XZ", "YI", -s)]
+    off = np.zeros((16, 16))
+    for (r, cc, v) in pairs:
+        assert abs(G[idx(*r), idx(*cc)] - v) < 1e-15
+        off[idx(*r), idx(*cc)] = v
+    assert np.allclose(G - np.diag(np.diag(G)), off, atol=1e-15)       # nothing else off-diagonal
+    # operator-Schmidt rank across site1|site2
+    T = G.reshape(4, 4, 4, 4).transpose(0, 2, 1, 3).reshape(16, 16)
+    sv = np.linalg.svd(T, compute_uv=False)
+    assert np.sum(sv > 1e-12) == 4
+    assert np.allclose(sv[:4], [3.990, 0.1997, 0.1997, 0.00999], atol=2e-3)
+
+
+def test_gate_ptm_matches_dense_conjugation():
+    """One ZZ gate + field gate on 2 sites through the PTM equals 4x4 dense conjugation."""
+    rng = np.random.default_rng(0)
+    coef = rng.standard_normal(16)
+    paulis = [dc._SIG[k] for k in "IXYZ"]
+    O = sum(coef[a * 4 + b] * np.kron(paulis[a], paulis[b]) for a in range(4) for b in range(4))
+    U = dc._expm_herm(np.kron(paulis[3], paulis[3]), 1j * J * DT)
+    O2 = U.conj().T @ O @ U
+    c2 = po.ptm_two_site(J * DT, "Z") @ coef
+    O2p = sum(c2[a * 4 + b] * np.kron(paulis[a], paulis[b]) for a in range(4) for b in range(4))
+    assert np.allclose(O2, O2p, atol=1e-14)
+
+
+# ---------------------------------------------------------------- P1 / P2 / P3 / P4 ---------
+@pytest.mark.parametrize("case", [(2, 2, 0, 0), (3, 3, 1, 1), (1, 4, 0, 1), (2, 3, 0, 1)])
+def test_untruncated_network_equals_dense(case, golden_dense):
+    """P1+P2: exact contraction of the untruncated network = dense Trotter evolution (<=1e-13 for 4 steps, <=1e-10 for 8);
+    P4: BP/Bethe within 1e-10 of dense for <=8 steps on loopy grids."""
+    Lx, Ly, cx, cy = case
+    gold = golden_dense[case]
+    st = po.PEPOState(Lx, Ly, cx, cy, J, H, DT, chi_max=256)
+    for step in range(8):
+        st.trotter_step()
+        # eps_cut=1e-11 pruning itself moves the network by ~1e-11 from step ~5 on (R8 note)
+        assert abs(st.exact_contraction() - gold[step]) < (1e-13 if step < 4 else 1e-10), (case, step)
+        status, sweeps, delta = st.bp_converge(1e-12, 0.0, 200)
+        assert status == 0
+        assert abs(st.correlation() - gold[step]) < 1e-10, (case, step)
+
+
+def test_golden_file_is_what_dense_check_computes(golden_dense):
+    vals = dc.dense_trotter_correlation(2, 2, 0, 0, J, H, DT, 10)
+    assert np.allclose(vals, golden_dense[(2, 2, 0, 0)], atol=1e-14)
+    # step 1 = cos(2 h dt) on every grid: ZZ commutes with Z_c
+    for k, v in golden_dense.items():
+        assert abs(v[0] - math.cos(2 * H * DT)) < 1e-14
+
+
+@pytest.mark.parametrize("case", [(1, 4, 0, 1), (1, 6, 0, 2)])
+def test_bp_exact_on_trees(case, golden_dense):
+    """P3: BP is exact on trees: 1xN chains, untruncated, 10 steps."""
+    Lx, Ly, cx, cy = case
+    st, out = po.run_trajectory(Lx, Ly, cx, cy, J, H, DT, 256, 10, 1e-13)
+    for o, g in zip(out, golden_dense[case]):
+        assert abs(o["C"] - g) < 1e-13
+
+
+def test_chain_orientation_equivalence(golden_dense):
+    """Nx1 equals 1xN (legs L/R instead of U/D exercise the other permutation cases)."""
+    st, out = po.run_trajectory(4, 1, 1, 0, J, H, DT, 256, 10, 1e-13)
+    for o, g in zip(out, golden_dense[(1, 4, 0, 1)]):
+        assert abs(o["C"] - g) < 1e-13
+
+
+# ---------------------------------------------------------------- P5 closed forms -----------
+def test_closed_forms():
+    """J=0: C(n dt) = cos(2 h n dt), all chi stay 1.  h=0: C == 1, all chi stay 1.  C(0)=1 (L350)."""
+    st = po.PEPOState(3, 3, 1, 1, 0.0, H, DT, 8)
+    st.bp_converge(1e-12)
+    assert abs(st.correlation() - 1.0) < 1e-15          # C(0) = 1
+    for n in range(1, 7):
+        st.trotter_step()
+        st.bp_converge(1e-12)
+        assert abs(st.correlation() - math.cos(2 * H * n * DT)) < 1e-14
+        assert set(st.bond_dims()) == {1}
+    st = po.PEPOState(3, 3, 1, 1, J, 0.0, DT, 8)
+    for n in range(1, 5):
+        st.trotter_step()
+        st.bp_converge(1e-12)
+        assert abs(st.correlation() - 1.0) < 1e-14
+        assert set(st.bond_dims()) == {1}
+
+
+# ---------------------------------------------------------------- P6 config 1 ---------------
+def test_config1_close_to_dense(golden_dense):
+    """BASELINE config 1 (3x3, chi_max=8, truncating from step 4) stays within 5e-9 of dense."""
+    st, out = po.run_trajectory(3, 3, 1, 1, J, H, DT, 8, 10, 1e-10, 0.0)
+    gold = golden_dense[(3, 3, 1, 1)]
+    assert max(st.bond_dims()) == 8
+    for o, g in zip(out, gold):
+        assert o["status"] == 0
+        assert abs(o["C"] - g) < 5e-9
+
+
+# ---------------------------------------------------------------- P7 / P8 / P13 -------------
+def test_c4_symmetry_and_lightcone():
+    st = po.PEPOState(5, 5, 2, 2, J, H, DT, 64)
+    lat = st.lat
+    expected = {1: [2, 1, 1, 1], 2: [4, 2, 1, 1], 3: [9, None, 2, 1], 4: [15, None, 5, 2]}
+    for step in range(1, 5):
+        st.trotter_step()
+        dims = st.bond_dims()
+        by_d = {}
+        for e in range(lat.n_bonds):
+            v1, _, v2, _ = lat.bond_sites(e)
+            d = min(abs(x - 2) + abs(y - 2) for (x, y) in (lat.xy(v1), lat.xy(v2)))
+            by_d.setdefault(d, set()).add(dims[e])
+        for d, want in enumerate(expected[step]):
+            if want is not None:
+                assert by_d[d] == {want}, (step, d, by_d)
+    # P7: the four bonds touching the centre have identical Schmidt spectra (C4)
+    c = lat.site(2, 2)
+    spectra = [st.lam[lat.bond_id(c, d)] for d in "UDLR"]
+    for s in spectra[1:]:
+        assert np.allclose(s, spectra[0], atol=1e-12)
+
+
+def test_exact_symmetries_of_C():
+    """P13: C(J,h) = C(-J,h) = C(J,-h); reflection (1,1) == (2,2) on 4x4."""
+    ref = [o["C"] for o in po.run_trajectory(4, 4, 1, 1, J, H, DT, 8, 8, 1e-12)[1]]
+    for (j, h, cx, cy) in [(-J, H, 1, 1), (J, -H, 1, 1), (J, H, 2, 2), (J, H, 2, 1)]:
+        got = [o["C"] for o in po.run_trajectory(4, 4, cx, cy, j, h, DT, 8, 8, 1e-12)[1]]
+        if (cx, cy) == (2, 1):
+            ref2 = [o["C"] for o in po.run_trajectory(4, 4, 1, 2, J, H, DT, 8, 8, 1e-12)[1]]
+            assert np.allclose(got, ref2, atol=1e-12)
+        else:
+            assert np.allclose(got, ref, atol=1e-12)
+
+
+def test_grid_independence_early_times():
+    """P8 / PAPER L364: C identical across grids until the front returns from the boundary."""
+    a = [o["C"] for o in po.run_trajectory(3, 3, 1, 1, J, H, DT, 8, 2, 1e-12)[1]]
+    b = [o["C"] for o in po.run_trajectory(4, 4, 1, 1, J, H, DT, 8, 2, 1e-12)[1]]
+    assert np.allclose(a, b, atol=1e-14)
+
+
+def test_bp_is_read_only():
+    """R16: bp_converge / correlation do not change (psi, lambda)."""
+    s1 = po.PEPOState(3, 3, 1, 1, J, H, DT, 8)
+    s2 = po.PEPOState(3, 3, 1, 1, J, H, DT, 8)
+    for _ in range(5):
+        s1.trotter_step(); s1.bp_converge(1e-10); s1.correlation()
+        s2.trotter_step()
+    for a, b in zip(s1.psi, s2.psi):
+        assert np.array_equal(a, b)
+
+
+# ---------------------------------------------------------------- P9 permutation ------------
+def test_permutation_listing1_vs_loops_and_transpose():
+    rng = np.random.default_rng(3)
+    shape = [3, 2, 4, 2, 4]
+    src = rng.standard_normal(int(np.prod(shape)))
+    arr = src.reshape(shape, order="F")
+    for perm in itertools.permutations(range(5)):
+        got = po.permute_listing1(src, shape, perm)
+        assert np.array_equal(got, np.transpose(arr, perm).flatten(order="F"))
+    for perm in [(0, 1, 2, 3, 4), (1, 2, 3, 0, 4), (4, 3, 2, 1, 0), (2, 0, 4, 1, 3)]:
+        got = po.permute_listing1(src, shape, perm)
+        assert np.array_equal(got, po.permute_nested_loops(src, shape, perm))
+        inv = np.argsort(perm)
+        back = po.permute_listing1(got, [shape[p] for p in perm], list(inv))
+        assert np.array_equal(back, src)                       # perm o perm^-1 = identity
+    # bijection: permuting arange gives a permutation of arange
+    ar = np.arange(src.size, dtype=np.float64)
+    assert np.array_equal(np.sort(po.permute_listing1(ar, shape, (3, 1, 4, 0, 2))), ar)
+    # rank 3 / rank 1 / size-1 dims
+    assert np.array_equal(po.permute_listing1(ar[:6], [2, 3, 1], (1, 2, 0)),
+                          np.transpose(ar[:6].reshape([2, 3, 1], order="F"), (1, 2, 0)).flatten(order="F"))
+
+
+# ---------------------------------------------------------------- P10 QR / SVD --------------
+def test_qr_invariants_and_cholqr_agrees():
+    rng = np.random.default_rng(5)
+    for (m, n) in [(50, 8), (8, 8), (5, 12), (300, 24)]:
+        A = rng.standard_normal((m, n))
+        Q, R = po.householder_qr(A)
+        k = min(m, n)
+        assert Q.shape == (m, k) and R.shape == (k, n)
+        assert np.linalg.norm(A - Q @ R) / np.linalg.norm(A) < 1e-13
+        assert np.linalg.norm(Q.T @ Q - np.eye(k)) < 1e-13
+        assert np.allclose(R, np.triu(R))
+        if m >= n:
+            Qc, Rc = po.cholesky_qr(A)                          # eq. (10)
+            assert np.all(np.diag(Rc) > 0) and np.allclose(Rc, np.triu(Rc))
+            assert np.linalg.norm(A - Qc @ Rc) / np.linalg.norm(A) < 1e-13
+            assert np.linalg.norm(Qc.T @ Qc - np.eye(n)) < 1e-10
+            sgn = np.sign(np.diag(R))
+            assert np.allclose(Rc, sgn[:, None] * R, atol=1e-10)   # QR unique up to row signs of R
+    with pytest.raises(np.linalg.LinAlgError):
+        A = rng.standard_normal((20, 4)); A[:, 3] = 0.0
+        po.cholesky_qr(A)                                       # potrf_info != 0
+
+
+def test_truncation_rule():
+    s = np.array([1.0, 0.5, 1e-3, 2e-11, 1e-11, 0.9e-11, 0.0])
+    assert po.truncation_rank(s, 100, 1e-11) == 5               # eq. (11): s_i >= eps*s_0 inclusive
+    assert po.truncation_rank(s, 3, 1e-11) == 3
+    assert po.truncation_rank(np.zeros(3), 3, 1e-11) == 0
+
+
+def test_gate_update_preserves_two_site_operator():
+    """A single untruncated Alg.1 equals the gate applied to the contracted two-site tensor, and
+    lambda are the singular values of the environment-weighted two-site tensor (Vidal gauge)."""
+    st = po.PEPOState(2, 3, 0, 1, J, H, DT, 256)
+    for _ in range(3):
+        st.trotter_step()
+    st.apply_field_gate()
+    lat = st.lat
+    e = lat.bond_id(lat.site(0, 1), "R")
+    v1, d1, v2, d2 = lat.bond_sites(e)
+    a, b = st.psi[v1].copy(), st.psi[v2].copy()
+    # theta[u1,d1_,p1,u2,d2_,p2] = sum_c a[u,d,c(R),p] b[u,d,c(L),p]; legs of v1: U,D,R ; v2: U,D,L
+    theta = np.einsum("udcp,efcq->udpefq", a, b)
+    G4 = st.G2.reshape(4, 4, 4, 4)
+    want = np.einsum("xypq,udpefq->udxefy", G4, theta)
+    st.apply_bond_gate(e)
+    got = np.einsum("udcp,efcq->udpefq", st.psi[v1], st.psi[v2])
+    # equality holds in the environment-weighted norm the simple update optimises (the 1e-11 pruning of
+    # eq. (11) is amplified by the deabsorb division in the unweighted norm)
+    w = lambda v: (np.sqrt(st.lam[lat.bond_id(v, "U")])[:, None] * np.sqrt(st.lam[lat.bond_id(v, "D")])[None, :])
+    W = w(v1)[:, :, None, None, None, None] * w(v2)[None, None, None, :, :, None]
+    assert np.linalg.norm((got - want) * W) / np.linalg.norm(want * W) < 1e-10
+    assert abs(np.sum(st.lam[e] ** 2) - 1) < 1e-14 and np.all(np.diff(st.lam[e]) <= 0)
+
+
+# ---------------------------------------------------------------- P11 memory model ----------
+def test_paper_memory_model_tables():
+    """eq. (15)-(17) with sizeof(float)=4 reproduce Table 9 (L649-L656) and Table 10 (L660-L670), decimal GB."""
+    gb = lambda k, l, chi: sum(po.paper_memory_model_bytes(k, l, chi)) / 1e9
+    assert abs(gb(4, 4, 50) - 0.82) < 0.005
+    assert abs(gb(4, 4, 80) - 5.31) < 0.005
+    assert abs(gb(4, 4, 100) - 12.94) < 0.005
+    assert abs(gb(10, 10, 100) - 109.3) < 0.05
+    assert abs(gb(8, 8, 90) - 42.3) < 0.05
+    assert abs(gb(5, 5, 70) - 5.1) < 0.05
+    lat = po.Lattice(8, 8)
+    assert lat.n_bonds == 2 * 8 * 7
+    cls = lat.colour_classes()
+    assert sorted(sum(cls, [])) == list(range(lat.n_bonds))
+    for c in cls:                                               # no shared site in a class
+        seen = set()
+        for e in c:
+            v1, _, v2, _ = lat.bond_sites(e)
+            assert v1 not in seen and v2 not in seen
+            seen.update((v1, v2))
