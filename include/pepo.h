@@ -1,0 +1,181 @@
+/*
+ * pepo.h - C ABI of the B200-native Heisenberg-picture PEPO hot path
+ * (arxiv/paper_2606_30985: Trotter bond update + BP sweeps + Bethe evaluation of
+ *  C(t) = Tr[Z_c(t) Z_c]/2^N on the 2D transverse-field Ising model).
+ *
+ * Citations are "PAPER.md:L<line>" (the paper text) and "R<n>" (DESIGN.md readings, which
+ * restate SURVEY.md section 8(c) C1..C18).
+ *
+ * Conventions
+ *   - All tensors are fp64.  A site tensor psi_v has the legs [U,D,L,R] that exist at the
+ *     site (neighbours U=(x,y-1), D=(x,y+1), L=(x-1,y), R=(x+1,y)) followed by the Pauli leg
+ *     P (dim 4: I,X,Y,Z), stored column-major: first leg fastest, P slowest, packed at the
+ *     LIVE bond dimensions (R11, R12).
+ *   - Bond ids: horizontal bonds (x,y)-(x+1,y) first, id = y*(Lx-1)+x; then vertical bonds
+ *     (x,y)-(x,y+1), id = Ly*(Lx-1) + y*Lx + x.  Site id = y*Lx + x.
+ *   - "d_" pointers are DEVICE pointers, "h_" pointers are HOST pointers.  `stream` is a
+ *     cudaStream_t passed as void* (0 = default stream).
+ *   - Return value: 0 = OK, >0 = soft status, <0 = hard error:
+ *       -1 bad argument, -2 arena too small, -3 CUDA error, -4 numerical failure
+ *       (NaN, s0 = 0, Z_e = 0).  pepo_last_error() returns a text for the last error of
+ *     the calling thread.  No exception or abort crosses this boundary.
+ *   - Nothing in this library allocates device memory after pepo_init(): the caller owns one
+ *     arena (e.g. a torch tensor) and the context sub-allocates it ("zero-malloc",
+ *     PAPER.md:L132-L160).  There is no CPU fallback of any step.
+ */
+#ifndef PEPO_H_
+#define PEPO_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pepo_ctx pepo_ctx;
+
+typedef struct pepo_stats {
+  double gate_err;          /* sum over the gates of the last trotter_step of the discarded
+                               weight sum_{i>=chi_new} s_i^2 / sum_i s_i^2 (Table 1) */
+  double min_cut_gap;       /* min over gates of the last step of (s[chi_new-1]-s[chi_new])/s[chi_new-1]
+                               when truncation by chi_max was active (R8); 1.0 if never */
+  long long n_cholesky;     /* site QRs done by the Cholesky path since init */
+  long long n_householder;  /* site QRs done by the Householder path since init (L223-L229) */
+  long long n_chol_failed;  /* Cholesky attempts rejected (pivot <= 0 or diag ratio < tau_c, R9) */
+  long long jacobi_sweeps;  /* Jacobi sweeps summed over the SVDs of the last step */
+  long long kernel_launches;/* kernels launched by this context since init */
+  int last_bp_sweeps;       /* sweeps of the last bp_converge (both phases) */
+  int last_bp_status;       /* 0 converged, 1 budget exhausted */
+  double last_bp_delta;     /* delta of eq. (14) */
+  size_t arena_high_water;  /* bytes of the arena actually handed out */
+  size_t arena_model_bytes; /* closed-form model for the same configuration (eq. (15)-(17) analogue) */
+  int max_inflight_gates;   /* gates of one colour class processed concurrently */
+  int chi_max_live;         /* largest live bond dimension */
+} pepo_stats;
+
+const char* pepo_last_error(void);
+
+/* Analytic memory model (eq. (15)-(17), re-derived for this layout:
+ * DESIGN.md "Memory model").  Bytes of arena pepo_init() needs.  max_inflight <= 0 picks the
+ * default (as many gates of a colour class as fit a 170 GB budget, at most 16). */
+size_t pepo_arena_bytes(int Lx, int Ly, int chi_max);
+size_t pepo_arena_bytes_ex(int Lx, int Ly, int chi_max, int max_inflight);
+
+/* Create a context for the Lx x Ly open-boundary grid, observable Z at site
+ * (cx,cy) (L308), H = -J sum ZZ - h sum X (R1), first-order Trotter step dt (R2), bond cap
+ * chi_max (L68), BP tolerance and damping d (m <- d m_old + (1-d) m_hat, eq. (19), R7).
+ * State is initialised to the product operator: all bonds chi=1, lambda=[1] (L70, L311).
+ * d_arena: device buffer of arena_bytes >= pepo_arena_bytes(...) owned by the caller for the
+ * lifetime of the context.  Errors: -1 (cx,cy outside grid, chi_max<1, dt<=0, Lx/Ly<1),
+ * -2 (arena too small; pepo_last_error() states the bytes needed), -3. */
+int pepo_init(pepo_ctx** out, int Lx, int Ly, int cx, int cy, double J, double h, double dt,
+              int chi_max, double bp_tol, double bp_damping, void* d_arena, size_t arena_bytes,
+              void* stream);
+/* As pepo_init with explicit max_inflight (<=0: default) and the Paulis of the model as
+ * indices 0..3 = I,X,Y,Z (defaults: bond 3, field 1, observable 3; the paper's own eq. (1)
+ * convention is bond 1, field 3). */
+int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, double J, double h, double dt,
+                 int chi_max, double bp_tol, double bp_damping, void* d_arena,
+                 size_t arena_bytes, void* stream, int max_inflight, int bond_pauli,
+                 int field_pauli, int obs_pauli);
+int pepo_destroy(pepo_ctx* ctx);
+
+/* Options (key, value): "eps_cut" (1e-11, eq. (11)), "bp_max_sweeps" (100, L256),
+ * "bp_max_sweeps_damped" (1000, R7), "chol_min_ratio" (Cholesky when m >= ratio*n, 4, R9),
+ * "chol_tau" (diag-ratio rejection threshold 1e-7, R9), "force_householder" (0/1),
+ * "jacobi_tol" (1e-15), "jacobi_max_sweeps" (60).  -1 on unknown key. */
+int pepo_set_option(pepo_ctx* ctx, const char* key, double value);
+
+/* One full first-order Trotter step (Fig. 1; R2, R3): field gate on all
+ * sites (a1), then the four colour classes of ZZ bond gates, each gate = Algorithm 1
+ * (L258-L288): absorb + permute (a2-a4), QR (a5/a6), core + gate (a7/a8), Jacobi SVD +
+ * truncation (a9), bridge + reconstruction (a10), inverse permute + deabsorb + write-back
+ * (a11-a13).  Asynchronous work on the context stream with one host read of the new bond
+ * dimensions per batch of gates. */
+int pepo_trotter_step(pepo_ctx* ctx);
+/* The two halves, for gate-replay tests. */
+int pepo_apply_field(pepo_ctx* ctx);
+int pepo_apply_bond(pepo_ctx* ctx, int bond);
+
+/* BP on the pinned single-layer network (eq. (13),(14),(19) PAPER.md:L243-L256, L444-L449; R6,
+ * R7): Jacobi-schedule sweeps from the deterministic init until delta < tol or the budget
+ * is spent; undamped phase first, damped restart if configured.  Writes the total sweep
+ * count and the last delta.  Returns 0 converged, 1 budget exhausted. */
+int pepo_bp_converge(pepo_ctx* ctx, int* h_sweeps, double* h_delta);
+/* Bethe evaluation (eq. (7)-(9) PAPER.md:L112-L128) from the current messages, log-space with
+ * sign tracking.  -4 if some Z_e is 0 (R14). */
+int pepo_correlation(pepo_ctx* ctx, double* h_C);
+
+int pepo_get_stats(pepo_ctx* ctx, pepo_stats* h_stats);
+int pepo_n_bonds(pepo_ctx* ctx);
+int pepo_get_bond_dims(pepo_ctx* ctx, int* h_chi /* n_bonds */);
+/* Set all live bond dimensions (1..chi_max); site tensors and lambdas become undefined until
+ * set with pepo_set_site / pepo_set_lambda.  For tests and synthetic workloads. */
+int pepo_set_bond_dims(pepo_ctx* ctx, const int* h_chi /* n_bonds */);
+size_t pepo_site_size(pepo_ctx* ctx, int x, int y);              /* elements at live dims */
+int pepo_get_site(pepo_ctx* ctx, int x, int y, double* h_dst, size_t n);
+int pepo_set_site(pepo_ctx* ctx, int x, int y, const double* h_src, size_t n);
+int pepo_get_lambda(pepo_ctx* ctx, int bond, double* h_dst, int n);
+int pepo_set_lambda(pepo_ctx* ctx, int bond, const double* h_src, int n);
+/* Device pointer of a packed site tensor (valid until the next gate touching the site). */
+double* pepo_site_ptr(pepo_ctx* ctx, int x, int y);
+
+/* ------------------------------------------------------------------------------------
+ * Kernel-level entry points (BASELINE config 3 and the parity tests).  Device pointers,
+ * caller's stream, asynchronous unless stated.
+ * ------------------------------------------------------------------------------------ */
+
+/* Tensor permutation, section 4.1 Listing 1 (L183-L208), R10: d_src is a packed
+ * column-major tensor of `rank` <= 8 dims `shape` (first dim fastest); output dim j is input
+ * dim perm[j] (numpy.transpose convention on the column-major shape); d_dst gets the packed
+ * column-major result.  Bit-exact copy.  d_src and d_dst must not overlap. */
+int pepo_permute(const double* d_src, double* d_dst, const int* h_shape, const int* h_perm,
+                 int rank, void* stream);
+/* Same, fused with the diagonal environment absorption / de-absorption of a3 / a12
+ * (PAPER.md:L93, L103, L267, L283, L318, L336): dst = permute(src * prod_d scale_d[i_d]);
+ * h_scale is a HOST array of `rank` DEVICE pointers, entry d pointing to shape[d] multipliers
+ * for input dim d (sqrt(lambda) to absorb, 1/sqrt(lambda) to de-absorb) or NULL. */
+int pepo_permute_scaled(const double* d_src, double* d_dst, const int* h_shape,
+                        const int* h_perm, int rank, const double* const* h_scale,
+                        void* stream);
+
+/* Gram matrix C = A^T A of a column-major m x n matrix (eq. (10)) on the
+ * fp64 tensor cores (DMMA), deterministic split-K.  d_ws: workspace of
+ * pepo_gram_ws_bytes(m,n) bytes.  d_C: n x n column-major, ldc = n, both triangles. */
+size_t pepo_gram_ws_bytes(long long m, int n);
+int pepo_gram(const double* d_A, long long m, int n, long long lda, double* d_C, void* d_ws,
+              size_t ws_bytes, void* stream);
+
+/* Cholesky-QR (eq. (10)): C = A^T A, R = chol(C) upper, Q = A R^{-1} (via the inverted
+ * triangular factor, the paper's Rinv slots L140).  d_Q: m x n (ldq = lda), d_R: n x n
+ * (ldr = n, strictly-lower part zeroed).  d_info (device int): 0 ok, j>0 = pivot j <= 0
+ * (the paper's potrf_info).  Q is left unspecified when info != 0. */
+size_t pepo_cholqr_ws_bytes(long long m, int n);
+int pepo_cholqr(const double* d_A, long long m, int n, long long lda, double* d_Q, double* d_R,
+                int* d_info, void* d_ws, size_t ws_bytes, void* stream);
+
+/* Householder QR (R13), reduced: A (m x n, column-major, lda) = Q R,
+ * k = min(m,n), d_Q m x k (ldq = m), d_R k x n (ldr = k, upper trapezoidal).  A is not
+ * modified.  Works for m < n and rank-deficient A. */
+size_t pepo_householder_ws_bytes(long long m, int n);
+int pepo_householder_qr(const double* d_A, long long m, int n, long long lda, double* d_Q,
+                        double* d_R, void* d_ws, size_t ws_bytes, void* stream);
+
+/* One-sided Jacobi SVD (a9, eq. (11)-(12) PAPER.md:L233-L241): A (m x n column-major, lda)
+ * = U diag(s) V^T with r = min(m,n); d_U m x r (ldu = m), d_s r (descending), d_V n x r
+ * (ldv = n).  d_sweeps (device int, may be NULL) gets the sweep count. */
+size_t pepo_svd_ws_bytes(int m, int n);
+int pepo_svd_jacobi(const double* d_A, int m, int n, int lda, double* d_U, double* d_s,
+                    double* d_V, int* d_sweeps, void* d_ws, size_t ws_bytes, void* stream);
+
+/* C (M x N, ldc) = op(A) op(B) on the fp64 tensor cores; transA/transB = 0 ('N') or 1 ('T'),
+ * column-major operands (a10 reconstruction GEMM). */
+int pepo_dgemm(int transA, int transB, long long M, int N, int K, const double* d_A,
+               long long lda, const double* d_B, long long ldb, double* d_C, long long ldc,
+               void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PEPO_H_ */

@@ -1,0 +1,274 @@
+"""Thin ctypes binding of the C ABI in ``include/pepo.h`` (argument marshalling only: every
+step of the hot path runs in the CUDA kernels of ``libpepo_b200.so``).
+
+PyTorch supplies device memory (the arena, kernel-level tensors) and the stream.  There is no
+CPU fallback: importing this module without the built library raises, and every call raises
+``PepoError`` on a negative return code.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpepo_b200.so")
+
+
+class PepoError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("pepo error %d: %s" % (code, msg))
+        self.code = code
+
+
+class PepoStats(C.Structure):
+    _fields_ = [("gate_err", C.c_double), ("min_cut_gap", C.c_double),
+                ("n_cholesky", C.c_longlong), ("n_householder", C.c_longlong),
+                ("n_chol_failed", C.c_longlong), ("jacobi_sweeps", C.c_longlong),
+                ("kernel_launches", C.c_longlong), ("last_bp_sweeps", C.c_int),
+                ("last_bp_status", C.c_int), ("last_bp_delta", C.c_double),
+                ("arena_high_water", C.c_size_t), ("arena_model_bytes", C.c_size_t),
+                ("max_inflight_gates", C.c_int), ("chi_max_live", C.c_int)]
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            "libpepo_b200.so is not built (run `python -m paper_2606_30985_b200.build`); "
+            "there is no CPU fallback for the hot path")
+    lib = C.CDLL(LIB_PATH)
+    vp, dp, ip, sz, ll, i, d = (C.c_void_p, C.c_void_p, C.POINTER(C.c_int), C.c_size_t,
+                                C.c_longlong, C.c_int, C.c_double)
+    sig = {
+        "pepo_last_error": (C.c_char_p, []),
+        "pepo_arena_bytes": (sz, [i, i, i]),
+        "pepo_arena_bytes_ex": (sz, [i, i, i, i]),
+        "pepo_init": (i, [C.POINTER(vp), i, i, i, i, d, d, d, i, d, d, vp, sz, vp]),
+        "pepo_init_ex": (i, [C.POINTER(vp), i, i, i, i, d, d, d, i, d, d, vp, sz, vp, i, i, i, i]),
+        "pepo_destroy": (i, [vp]),
+        "pepo_set_option": (i, [vp, C.c_char_p, d]),
+        "pepo_trotter_step": (i, [vp]),
+        "pepo_apply_field": (i, [vp]),
+        "pepo_apply_bond": (i, [vp, i]),
+        "pepo_bp_converge": (i, [vp, ip, C.POINTER(d)]),
+        "pepo_correlation": (i, [vp, C.POINTER(d)]),
+        "pepo_get_stats": (i, [vp, C.POINTER(PepoStats)]),
+        "pepo_n_bonds": (i, [vp]),
+        "pepo_get_bond_dims": (i, [vp, ip]),
+        "pepo_set_bond_dims": (i, [vp, ip]),
+        "pepo_site_size": (sz, [vp, i, i]),
+        "pepo_get_site": (i, [vp, i, i, vp, sz]),
+        "pepo_set_site": (i, [vp, i, i, vp, sz]),
+        "pepo_get_lambda": (i, [vp, i, vp, i]),
+        "pepo_set_lambda": (i, [vp, i, vp, i]),
+        "pepo_site_ptr": (vp, [vp, i, i]),
+        "pepo_permute": (i, [dp, dp, ip, ip, i, vp]),
+        "pepo_permute_scaled": (i, [dp, dp, ip, ip, i, C.POINTER(vp), vp]),
+        "pepo_gram_ws_bytes": (sz, [ll, i]),
+        "pepo_gram": (i, [dp, ll, i, ll, dp, vp, sz, vp]),
+        "pepo_cholqr_ws_bytes": (sz, [ll, i]),
+        "pepo_cholqr": (i, [dp, ll, i, ll, dp, dp, vp, vp, sz, vp]),
+        "pepo_householder_ws_bytes": (sz, [ll, i]),
+        "pepo_householder_qr": (i, [dp, ll, i, ll, dp, dp, vp, sz, vp]),
+        "pepo_svd_ws_bytes": (sz, [i, i]),
+        "pepo_svd_jacobi": (i, [dp, i, i, i, dp, dp, dp, vp, vp, sz, vp]),
+        "pepo_dgemm": (i, [i, i, ll, i, i, dp, ll, dp, ll, dp, ll, vp]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    return lib, sorted(sig)
+
+
+_lib, EXPORTED = _load()
+
+
+def last_error() -> str:
+    return _lib.pepo_last_error().decode()
+
+
+def _check(rc):
+    if rc < 0:
+        raise PepoError(rc, last_error())
+    return rc
+
+
+def _stream(stream=None):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def _iarr(v):
+    return (C.c_int * len(v))(*[int(x) for x in v])
+
+
+def _f64(t, name):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError("%s must be a contiguous CUDA float64 tensor" % name)
+    return C.c_void_p(t.data_ptr())
+
+
+def arena_bytes(Lx, Ly, chi_max, max_inflight=0):
+    return int(_lib.pepo_arena_bytes_ex(Lx, Ly, chi_max, max_inflight))
+
+
+class Pepo:
+    """Context of one simulation (see ``include/pepo.h``).  Owns the arena tensor."""
+
+    def __init__(self, Lx, Ly, cx, cy, J, h, dt, chi_max, bp_tol, bp_damping=0.0, device="cuda:0",
+                 max_inflight=0, bond_pauli=3, field_pauli=1, obs_pauli=3, arena=None):
+        self.Lx, self.Ly, self.chi_max = Lx, Ly, chi_max
+        self.device = torch.device(device)
+        need = arena_bytes(Lx, Ly, chi_max, max_inflight)
+        if need == 0:
+            raise PepoError(-1, "bad grid / chi_max")
+        with torch.cuda.device(self.device):
+            self.arena = arena if arena is not None else torch.empty(need, dtype=torch.uint8, device=self.device)
+            self.stream = torch.cuda.current_stream()
+            h_ = C.c_void_p()
+            _check(_lib.pepo_init_ex(C.byref(h_), Lx, Ly, cx, cy, J, h, dt, chi_max, bp_tol, bp_damping,
+                                     C.c_void_p(self.arena.data_ptr()), self.arena.numel(),
+                                     _stream(self.stream), max_inflight, bond_pauli, field_pauli, obs_pauli))
+        self._h = h_
+        self.n_bonds = _lib.pepo_n_bonds(self._h)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.pepo_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_option(self, key, value):
+        _check(_lib.pepo_set_option(self._h, key.encode(), float(value)))
+
+    def trotter_step(self):
+        _check(_lib.pepo_trotter_step(self._h))
+
+    def apply_field(self):
+        _check(_lib.pepo_apply_field(self._h))
+
+    def apply_bond(self, bond):
+        _check(_lib.pepo_apply_bond(self._h, int(bond)))
+
+    def bp_converge(self):
+        sw, de = C.c_int(0), C.c_double(0.0)
+        status = _check(_lib.pepo_bp_converge(self._h, C.byref(sw), C.byref(de)))
+        return status, sw.value, de.value
+
+    def correlation(self):
+        out = C.c_double(0.0)
+        _check(_lib.pepo_correlation(self._h, C.byref(out)))
+        return out.value
+
+    def stats(self):
+        s = PepoStats()
+        _check(_lib.pepo_get_stats(self._h, C.byref(s)))
+        return {k: getattr(s, k) for k, _ in PepoStats._fields_}
+
+    def bond_dims(self):
+        arr = (C.c_int * max(self.n_bonds, 1))()
+        _check(_lib.pepo_get_bond_dims(self._h, arr))
+        return [arr[i] for i in range(self.n_bonds)]
+
+    def set_bond_dims(self, chi):
+        assert len(chi) == self.n_bonds
+        _check(_lib.pepo_set_bond_dims(self._h, _iarr(chi) if chi else (C.c_int * 1)()))
+
+    def site_size(self, x, y):
+        return int(_lib.pepo_site_size(self._h, x, y))
+
+    def get_site(self, x, y):
+        out = np.empty(self.site_size(x, y), dtype=np.float64)
+        _check(_lib.pepo_get_site(self._h, x, y, out.ctypes.data_as(C.c_void_p), out.size))
+        return out
+
+    def set_site(self, x, y, flat):
+        flat = np.ascontiguousarray(flat, dtype=np.float64).ravel()
+        _check(_lib.pepo_set_site(self._h, x, y, flat.ctypes.data_as(C.c_void_p), flat.size))
+
+    def get_lambda(self, bond):
+        n = self.bond_dims()[bond]
+        out = np.empty(n, dtype=np.float64)
+        _check(_lib.pepo_get_lambda(self._h, bond, out.ctypes.data_as(C.c_void_p), n))
+        return out
+
+    def set_lambda(self, bond, lam):
+        lam = np.ascontiguousarray(lam, dtype=np.float64).ravel()
+        _check(_lib.pepo_set_lambda(self._h, bond, lam.ctypes.data_as(C.c_void_p), lam.size))
+
+
+# ---- kernel-level entry points (device tensors in, device tensors out) ------------------------
+def permute(src, shape, perm, dst=None, scale=None):
+    """``src``: flat CUDA f64 tensor holding a packed column-major tensor of dims ``shape``
+    (first fastest).  Returns the packed column-major permuted tensor (flat)."""
+    _f64(src, "src")
+    if dst is None:
+        dst = torch.empty_like(src)
+    if scale is None:
+        _check(_lib.pepo_permute(_f64(src, "src"), _f64(dst, "dst"), _iarr(shape), _iarr(perm), len(shape), _stream()))
+    else:
+        ptrs = (C.c_void_p * len(shape))(*[C.c_void_p(s.data_ptr()) if s is not None else C.c_void_p(0) for s in scale])
+        _check(_lib.pepo_permute_scaled(_f64(src, "src"), _f64(dst, "dst"), _iarr(shape), _iarr(perm), len(shape),
+                                        ptrs, _stream()))
+    return dst
+
+
+def _ws(nbytes, device):
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+
+
+def gram(A_cm, m, n, ws=None):
+    """A_cm: flat column-major m x n.  Returns C (n x n column-major, flat)."""
+    Cm = torch.empty(n * n, dtype=torch.float64, device=A_cm.device)
+    ws = ws if ws is not None else _ws(_lib.pepo_gram_ws_bytes(m, n), A_cm.device)
+    _check(_lib.pepo_gram(_f64(A_cm, "A"), m, n, m, _f64(Cm, "C"), C.c_void_p(ws.data_ptr()), ws.numel(), _stream()))
+    return Cm
+
+
+def cholqr(A_cm, m, n, Q=None, ws=None):
+    Q = Q if Q is not None else torch.empty(m * n, dtype=torch.float64, device=A_cm.device)
+    R = torch.empty(n * n, dtype=torch.float64, device=A_cm.device)
+    info = torch.zeros(1, dtype=torch.int32, device=A_cm.device)
+    ws = ws if ws is not None else _ws(_lib.pepo_cholqr_ws_bytes(m, n), A_cm.device)
+    _check(_lib.pepo_cholqr(_f64(A_cm, "A"), m, n, m, _f64(Q, "Q"), _f64(R, "R"), C.c_void_p(info.data_ptr()),
+                            C.c_void_p(ws.data_ptr()), ws.numel(), _stream()))
+    return Q, R, info
+
+
+def householder_qr(A_cm, m, n):
+    k = min(m, n)
+    Q = torch.empty(m * k, dtype=torch.float64, device=A_cm.device)
+    R = torch.empty(k * n, dtype=torch.float64, device=A_cm.device)
+    ws = _ws(_lib.pepo_householder_ws_bytes(m, n), A_cm.device)
+    _check(_lib.pepo_householder_qr(_f64(A_cm, "A"), m, n, m, _f64(Q, "Q"), _f64(R, "R"),
+                                    C.c_void_p(ws.data_ptr()), ws.numel(), _stream()))
+    return Q, R
+
+
+def svd_jacobi(A_cm, m, n):
+    r = min(m, n)
+    U = torch.empty(m * r, dtype=torch.float64, device=A_cm.device)
+    s = torch.empty(r, dtype=torch.float64, device=A_cm.device)
+    V = torch.empty(n * r, dtype=torch.float64, device=A_cm.device)
+    sweeps = torch.zeros(1, dtype=torch.int32, device=A_cm.device)
+    ws = _ws(_lib.pepo_svd_ws_bytes(m, n), A_cm.device)
+    _check(_lib.pepo_svd_jacobi(_f64(A_cm, "A"), m, n, m, _f64(U, "U"), _f64(s, "s"), _f64(V, "V"),
+                                C.c_void_p(sweeps.data_ptr()), C.c_void_p(ws.data_ptr()), ws.numel(), _stream()))
+    return U, s, V, sweeps
+
+
+def dgemm(transA, transB, M, N, K, A, lda, B, ldb, Cout=None, ldc=None):
+    ldc = ldc or M
+    Cout = Cout if Cout is not None else torch.empty(ldc * N, dtype=torch.float64, device=A.device)
+    _check(_lib.pepo_dgemm(int(transA), int(transB), M, N, K, _f64(A, "A"), lda, _f64(B, "B"), ldb,
+                           _f64(Cout, "C"), ldc, _stream()))
+    return Cout

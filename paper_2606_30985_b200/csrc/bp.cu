@@ -1,0 +1,285 @@
+// bp.cu - belief-propagation message sweep (a14: eq. (13), (14), (19) PAPER.md:L243-L256,
+// L444-L449; readings R6, R7), the single-site field gate (a1, L313, L339) and the log-space,
+// sign-tracked Bethe evaluation (a15: eq. (7)-(9), L112-L128).
+//
+// A sweep reads the pinned slab T_v = psi_v[..., p_v] of every site ONCE and produces all of
+// the site's outgoing messages from that single pass (the paper issues one strided-batched
+// GEMV per message, L247): block (l, r) of site v reduces the dU x dD slice
+//     pU[u] = sum_d T[u,d,l,r] mD[d],  pD[d] = sum_u T[u,d,l,r] mU[u],  s = sum_u mU[u] pU[u]
+// and stores w*pU, w*pD (w = mL[l] mR[r]) and s as partials; `bp_finalize_kernel` sums the
+// partials in a fixed order (deterministic, no floating-point atomics), L2-normalises,
+// sign-aligns, damps and takes delta = max |m_new - m_old| (atomicMax on the bit pattern of a
+// non-negative double is order-independent).
+#include "bp.cuh"
+#include <algorithm>
+
+namespace pepo {
+namespace {
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+constexpr int BP_THREADS = 256;
+constexpr int BP_MAXK = 8;     // dU <= 256
+
+__global__ void __launch_bounds__(BP_THREADS) bp_partial_kernel(BpBatch b) {
+  __shared__ double sU[BP_THREADS / 32][32 * BP_MAXK];
+  const int t = blockIdx.y;
+  const BpSite& S = b.s[t];
+  const int dU = S.d[0], dD = S.d[1], dL = S.d[2], dR = S.d[3];
+  const int lr = blockIdx.x;
+  if (lr >= dL * dR) return;
+  const int l = lr % dL, r = lr / dL;
+  const double* T = S.T + (long long)lr * dU * dD;
+  const double* mU = S.in[0];
+  const double* mD = S.in[1];
+  const double w = S.in[2][l] * S.in[3][r];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = BP_THREADS / 32;
+  double accU[BP_MAXK];
+  double mu[BP_MAXK];
+#pragma unroll
+  for (int k = 0; k < BP_MAXK; k++) {
+    accU[k] = 0.0;
+    int u = lane + 32 * k;
+    mu[k] = (u < dU) ? mU[u] : 0.0;
+  }
+  double* partD = S.partD + (long long)lr * dD;
+  for (int d = warp; d < dD; d += nw) {
+    const double md = mD[d];
+    const double* col = T + (long long)d * dU;
+    double cs = 0.0;
+#pragma unroll
+    for (int k = 0; k < BP_MAXK; k++) {
+      int u = lane + 32 * k;
+      if (u < dU) {
+        double tv = col[u];
+        accU[k] += tv * md;
+        cs += tv * mu[k];
+      }
+    }
+    cs = warp_sum(cs);
+    if (lane == 0) partD[d] = w * cs;
+  }
+#pragma unroll
+  for (int k = 0; k < BP_MAXK; k++) sU[warp][lane + 32 * k] = accU[k];
+  __syncthreads();
+  double sdot = 0.0;
+  for (int u = threadIdx.x; u < dU; u += BP_THREADS) {
+    double p = 0.0;
+#pragma unroll
+    for (int w2 = 0; w2 < nw; w2++) p += sU[w2][u];
+    S.partU[(long long)lr * dU + u] = w * p;
+    sdot += p * mU[u];
+  }
+  // s = sum_u mU[u] pU[u]  (dU <= 256 = one pass of the block)
+  __shared__ double sred[BP_THREADS / 32];
+  sdot = warp_sum(sdot);
+  if (lane == 0) sred[warp] = sdot;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double s = 0.0;
+    for (int w2 = 0; w2 < nw; w2++) s += sred[w2];
+    S.partS[lr] = s;
+  }
+}
+
+// one block per (site, leg slot)
+__global__ void __launch_bounds__(256) bp_finalize_kernel(BpBatch b, double damping, int update,
+                                                          unsigned long long* delta_bits,
+                                                          int* flag) {
+  __shared__ double sred[8];
+  __shared__ double s_bcast[2];
+  const int t = blockIdx.y;
+  const int slot = blockIdx.x;
+  const BpSite& S = b.s[t];
+  if (!S.present[slot]) return;
+  const int dU = S.d[0], dD = S.d[1], dL = S.d[2], dR = S.d[3];
+  const int dl = S.d[slot];
+  const int nlr = dL * dR;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  extern __shared__ double mhat[];      // dl doubles
+  double nrm2 = 0.0, dot_old = 0.0, dot_in = 0.0;
+  const double* old = S.out_old[slot];
+  const double* inc = S.in[slot];
+  for (int i = threadIdx.x; i < dl; i += blockDim.x) {
+    double v = 0.0;
+    if (slot == 0) {
+      for (int k = 0; k < nlr; k++) v += S.partU[(long long)k * dU + i];
+    } else if (slot == 1) {
+      for (int k = 0; k < nlr; k++) v += S.partD[(long long)k * dD + i];
+    } else if (slot == 2) {
+      for (int r = 0; r < dR; r++) v += S.in[3][r] * S.partS[i + dL * r];
+    } else {
+      for (int l = 0; l < dL; l++) v += S.in[2][l] * S.partS[l + dL * i];
+    }
+    mhat[i] = v;
+    nrm2 += v * v;
+    dot_old += v * old[i];
+    dot_in += v * inc[i];
+  }
+  // block reductions (fixed order)
+  double vals[3] = {nrm2, dot_old, dot_in};
+  double red[3];
+  for (int q = 0; q < 3; q++) {
+    double v = warp_sum(vals[q]);
+    __syncthreads();
+    if (lane == 0) sred[warp] = v;
+    __syncthreads();
+    double s = 0.0;
+    for (int w = 0; w < 8; w++) s += sred[w];
+    red[q] = s;
+  }
+  if (threadIdx.x == 0 && slot == S.first_slot) *S.vs = red[2];     // eq. (7): site value
+  if (!update) return;
+  const double nrm = sqrt(red[0]);
+  double* outn = S.out_new[slot];
+  if (!(nrm > 0.0) || !isfinite(nrm)) {
+    for (int i = threadIdx.x; i < dl; i += blockDim.x) outn[i] = old[i];
+    if (threadIdx.x == 0) atomicOr(flag, 1);
+    return;
+  }
+  const double sgn = (red[1] < 0.0) ? -1.0 : 1.0;
+  double dmax = 0.0;
+  for (int i = threadIdx.x; i < dl; i += blockDim.x) {
+    double mh = sgn * (mhat[i] / nrm);
+    double o = old[i];
+    double mn = damping * o + (1.0 - damping) * mh;
+    outn[i] = mn;
+    dmax = fmax(dmax, fabs(mn - o));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) dmax = fmax(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
+  if (lane == 0) atomicMax(delta_bits, (unsigned long long)__double_as_longlong(dmax));
+  (void)s_bcast;
+}
+
+__global__ void bp_init_kernel(double* msgs, const int* chi_of_msg, int n_msgs, int chi_max) {
+  const int mIdx = blockIdx.x;
+  if (mIdx >= n_msgs) return;
+  const int chi = chi_of_msg[mIdx];
+  const double v = 1.0 / sqrt((double)chi);
+  for (int i = threadIdx.x; i < chi_max; i += blockDim.x)
+    msgs[(long long)mIdx * chi_max + i] = (i < chi) ? v : 0.0;
+}
+
+// eq. (8), (9): C = prod vs_v / prod Z_e in log space with sign tracking
+__global__ void __launch_bounds__(256) bethe_kernel(const double* vs, int n_sites,
+                                                    const double* msgs, const int* chi_of_msg,
+                                                    int n_bonds, int chi_max, double* out_C,
+                                                    int* out_status) {
+  extern __shared__ double Ze[];
+  for (int e = threadIdx.x; e < n_bonds; e += blockDim.x) {
+    const double* a = msgs + (long long)(2 * e) * chi_max;
+    const double* c = msgs + (long long)(2 * e + 1) * chi_max;
+    const int chi = chi_of_msg[2 * e];
+    double s = 0.0;
+    for (int i = 0; i < chi; i++) s += a[i] * c[i];
+    Ze[e] = s;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double lognum = 0.0, logden = 0.0, sign = 1.0;
+    int status = 0;
+    bool zero = false;
+    for (int v = 0; v < n_sites; v++) {
+      double x = vs[v];
+      if (!isfinite(x)) status = -4;
+      if (x == 0.0) { zero = true; continue; }
+      lognum += log(fabs(x));
+      if (x < 0.0) sign = -sign;
+    }
+    for (int e = 0; e < n_bonds; e++) {
+      double z = Ze[e];
+      if (z == 0.0 || !isfinite(z)) { status = -4; continue; }
+      logden += log(fabs(z));
+      if (z < 0.0) sign = -sign;
+    }
+    *out_C = zero ? 0.0 : exp(lognum - logden) * sign;
+    *out_status = status;
+  }
+}
+
+// a1: psi[.., p'] = sum_p G1[p', p] psi[.., p] on the four contiguous Pauli slabs; rows of G1
+// equal to the identity row are skipped (X field: only the Y and Z slabs move).
+__global__ void __launch_bounds__(256) field_gate_kernel(FieldBatch b) {
+  const int t = blockIdx.y;
+  double* psi = b.psi[t];
+  const long long slab = b.slab[t];
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < slab;
+       i += (long long)gridDim.x * blockDim.x) {
+    double v[4], o[4];
+#pragma unroll
+    for (int p = 0; p < 4; p++) v[p] = (b.col_mask >> p & 1) ? psi[i + p * slab] : 0.0;
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+      if (b.row_mask >> q & 1) {
+        o[q] = 0.0;
+#pragma unroll
+        for (int p = 0; p < 4; p++) o[q] += b.G[q * 4 + p] * v[p];
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < 4; q++)
+      if (b.row_mask >> q & 1) psi[i + q * slab] = o[q];
+  }
+}
+
+}  // namespace
+
+int launch_bp_partial(cudaStream_t st, const BpBatch& b) {
+  if (b.count == 0) return 0;
+  int maxlr = 1;
+  for (int t = 0; t < b.count; t++) maxlr = std::max(maxlr, b.s[t].d[2] * b.s[t].d[3]);
+  dim3 grid(maxlr, b.count);
+  bp_partial_kernel<<<grid, BP_THREADS, 0, st>>>(b);
+  PEPO_COUNT_LAUNCH();
+  PEPO_CUDA_OK(cudaGetLastError());
+  return 0;
+}
+
+int launch_bp_finalize(cudaStream_t st, const BpBatch& b, double damping, int update,
+                       unsigned long long* delta_bits, int* flag) {
+  if (b.count == 0) return 0;
+  int dmax = 1;
+  for (int t = 0; t < b.count; t++)
+    for (int k = 0; k < 4; k++) dmax = std::max(dmax, b.s[t].d[k]);
+  dim3 grid(4, b.count);
+  bp_finalize_kernel<<<grid, 256, dmax * sizeof(double), st>>>(b, damping, update, delta_bits, flag);
+  PEPO_COUNT_LAUNCH();
+  PEPO_CUDA_OK(cudaGetLastError());
+  return 0;
+}
+
+int launch_bp_init(cudaStream_t st, double* msgs, const int* chi_of_msg, int n_msgs, int chi_max) {
+  if (n_msgs == 0) return 0;
+  bp_init_kernel<<<n_msgs, 128, 0, st>>>(msgs, chi_of_msg, n_msgs, chi_max);
+  PEPO_COUNT_LAUNCH();
+  PEPO_CUDA_OK(cudaGetLastError());
+  return 0;
+}
+
+int launch_bethe(cudaStream_t st, const double* vs, int n_sites, const double* msgs,
+                 const int* chi_of_msg, int n_bonds, int chi_max, double* out_C, int* out_status) {
+  bethe_kernel<<<1, 256, std::max(1, n_bonds) * sizeof(double), st>>>(vs, n_sites, msgs, chi_of_msg,
+                                                                     n_bonds, chi_max, out_C, out_status);
+  PEPO_COUNT_LAUNCH();
+  PEPO_CUDA_OK(cudaGetLastError());
+  return 0;
+}
+
+int launch_field_gate(cudaStream_t st, const FieldBatch& b) {
+  if (b.count == 0) return 0;
+  long long smax = 1;
+  for (int t = 0; t < b.count; t++) smax = std::max(smax, b.slab[t]);
+  long long g = std::min<long long>((smax + 255) / 256, 148 * 8);
+  dim3 grid((unsigned)g, b.count);
+  field_gate_kernel<<<grid, 256, 0, st>>>(b);
+  PEPO_COUNT_LAUNCH();
+  PEPO_CUDA_OK(cudaGetLastError());
+  return 0;
+}
+
+}  // namespace pepo

@@ -1,0 +1,38 @@
+// bp.cuh - BP sweep / Bethe / field-gate launchers (see bp.cu).
+#pragma once
+#include "common.cuh"
+
+namespace pepo {
+
+#define PEPO_BP_MAXS 32
+
+struct BpSite {
+  const double* T;            // pinned slab psi_v[..., p_v], dims d[0..3] = (U,D,L,R), 1 if absent
+  int d[4];
+  int present[4];
+  int first_slot;             // first present leg (site value vs_v is taken there)
+  const double* in[4];        // incoming message per slot (a constant [1.0] if absent)
+  const double* out_old[4];   // current outgoing message per slot
+  double* out_new[4];         // next outgoing message per slot
+  double* partU; double* partD; double* partS;
+  double* vs;                 // site scalar of eq. (7)
+};
+struct BpBatch { int count; BpSite s[PEPO_BP_MAXS]; };
+
+struct FieldBatch {
+  int count;
+  double* psi[PEPO_BP_MAXS];
+  long long slab[PEPO_BP_MAXS];
+  double G[16];
+  int row_mask, col_mask;
+};
+
+int launch_bp_partial(cudaStream_t st, const BpBatch& b);
+int launch_bp_finalize(cudaStream_t st, const BpBatch& b, double damping, int update,
+                       unsigned long long* delta_bits, int* flag);
+int launch_bp_init(cudaStream_t st, double* msgs, const int* chi_of_msg, int n_msgs, int chi_max);
+int launch_bethe(cudaStream_t st, const double* vs, int n_sites, const double* msgs,
+                 const int* chi_of_msg, int n_bonds, int chi_max, double* out_C, int* out_status);
+int launch_field_gate(cudaStream_t st, const FieldBatch& b);
+
+}  // namespace pepo

@@ -1,0 +1,1075 @@
+// ctx.cu - the context behind the C ABI of include/pepo.h: lattice bookkeeping, the single
+// pre-sized device arena ("zero-malloc"), the analytic memory model
+// (eq. (15)-(17) L292-L304 re-derived for this layout), the Trotter step scheduler (Fig. 1
+// L310-L342; colour classes L87) and the BP / Bethe drivers.
+//
+// Schedule of one bond-gate batch (<= max_inflight gates of one colour class, disjoint sites):
+//   A. per site: cv = permute(psi * sqrt(lambda_env))             (a2-a4, fused)
+//   B. tall sites (m >= ratio*n): C = cv^T cv on DMMA, S = dressed Gram, Rx = chol(S)   (a5)
+//      -> host reads the potrf flags of the batch (the paper's potrf_info, L221)
+//   C. rejected / short sites: Householder cv = Q R, X = dress(R), Householder X = Qx Rx (a6)
+//   D. per gate: K = Rx1 (Sigma x I) Rx2^T, Jacobi SVD, truncation, lambda           (a7-a9)
+//      -> host reads chi_new of the batch (the paper's host threshold, L344)
+//   E. per site: Cholesky path  W = dress(Rx^-1 U sqrt(S)), cv_new = cv W (DMMA)
+//                Householder    cv_new = Q [dress(Qx [U sqrt(S); 0]); 0]              (a10)
+//   F. per site: psi = inverse-permute(cv_new) / sqrt(lambda_env)  (a11-a13, fused)
+// The gate is applied in Schmidt-dressed form: G = sum_a sigma_a Ahat_a (x) Bhat_a (operator-
+// Schmidt decomposition of the 16x16 Pauli-transfer matrix, rank 4 for ZZ), so that the core
+// the Jacobi SVD sees is (NA chi) x (NA chi) instead of the literal (16 chi)^2.
+#include "../../include/pepo.h"
+#include "bp.cuh"
+#include "common.cuh"
+#include "dense.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <complex>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+namespace pepo {
+
+long long g_launch_count = 0;
+static thread_local char g_err[512] = "";
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+const char* last_error() { return g_err; }
+
+// ------------------------------------------------------------------------------------------
+// host-side gate tables
+// ------------------------------------------------------------------------------------------
+typedef std::complex<double> cplx;
+static void pauli(int p, cplx m[2][2]) {
+  static const cplx I(0, 1);
+  cplx z(0, 0), o(1, 0);
+  switch (p) {
+    case 0: m[0][0] = o; m[0][1] = z; m[1][0] = z; m[1][1] = o; break;
+    case 1: m[0][0] = z; m[0][1] = o; m[1][0] = o; m[1][1] = z; break;
+    case 2: m[0][0] = z; m[0][1] = -I; m[1][0] = I; m[1][1] = z; break;
+    default: m[0][0] = o; m[0][1] = z; m[1][0] = z; m[1][1] = -o; break;
+  }
+}
+// dense d x d helpers
+static void matmul(const std::vector<cplx>& A, const std::vector<cplx>& B, std::vector<cplx>& C, int d) {
+  C.assign((size_t)d * d, cplx(0, 0));
+  for (int i = 0; i < d; i++)
+    for (int k = 0; k < d; k++)
+      for (int j = 0; j < d; j++) C[i * d + j] += A[i * d + k] * B[k * d + j];
+}
+static std::vector<cplx> dagger(const std::vector<cplx>& A, int d) {
+  std::vector<cplx> R((size_t)d * d);
+  for (int i = 0; i < d; i++)
+    for (int j = 0; j < d; j++) R[i * d + j] = std::conj(A[j * d + i]);
+  return R;
+}
+static std::vector<cplx> kron2(int a, int b) {
+  cplx A[2][2], B[2][2];
+  pauli(a, A); pauli(b, B);
+  std::vector<cplx> R(16);
+  for (int i = 0; i < 2; i++) for (int j = 0; j < 2; j++)
+    for (int k = 0; k < 2; k++) for (int l = 0; l < 2; l++) R[(i * 2 + k) * 4 + (j * 2 + l)] = A[i][j] * B[k][l];
+  return R;
+}
+// PTM of conjugation by U = exp(+i theta P): G[a][b] = Tr[P_a U^dag P_b U]/2  (R2)
+static void ptm_one_site(double theta, int fp, double G[16]) {
+  cplx P[2][2]; pauli(fp, P);
+  std::vector<cplx> U(4), Pa(4), Pb(4), T1, T2, T3;
+  for (int i = 0; i < 2; i++) for (int j = 0; j < 2; j++)
+    U[i * 2 + j] = (i == j ? cplx(std::cos(theta), 0) : cplx(0, 0)) + cplx(0, std::sin(theta)) * P[i][j];
+  std::vector<cplx> Ud = dagger(U, 2);
+  for (int a = 0; a < 4; a++) for (int b = 0; b < 4; b++) {
+    cplx A[2][2], B[2][2]; pauli(a, A); pauli(b, B);
+    for (int i = 0; i < 2; i++) for (int j = 0; j < 2; j++) { Pa[i * 2 + j] = A[i][j]; Pb[i * 2 + j] = B[i][j]; }
+    matmul(Pa, Ud, T1, 2); matmul(T1, Pb, T2, 2); matmul(T2, U, T3, 2);
+    G[a * 4 + b] = (T3[0] + T3[3]).real() / 2.0;
+  }
+}
+// 16x16 PTM of exp(+i theta P (x) P); row p1'*4+p2', column p1*4+p2 (R15)
+static void ptm_two_site(double theta, int bp, double G[256]) {
+  std::vector<cplx> PP = kron2(bp, bp), U(16), T1, T2, T3;
+  for (int i = 0; i < 4; i++) for (int j = 0; j < 4; j++)
+    U[i * 4 + j] = (i == j ? cplx(std::cos(theta), 0) : cplx(0, 0)) + cplx(0, std::sin(theta)) * PP[i * 4 + j];
+  std::vector<cplx> Ud = dagger(U, 4);
+  for (int a1 = 0; a1 < 4; a1++) for (int a2 = 0; a2 < 4; a2++) {
+    std::vector<cplx> Pa = kron2(a1, a2);
+    for (int b1 = 0; b1 < 4; b1++) for (int b2 = 0; b2 < 4; b2++) {
+      std::vector<cplx> Pb = kron2(b1, b2);
+      matmul(Pa, Ud, T1, 4); matmul(T1, Pb, T2, 4); matmul(T2, U, T3, 4);
+      cplx tr(0, 0);
+      for (int i = 0; i < 4; i++) tr += T3[i * 4 + i];
+      G[(a1 * 4 + a2) * 16 + (b1 * 4 + b2)] = tr.real() / 4.0;
+    }
+  }
+}
+// one-sided Jacobi SVD of a 16x16 host matrix (column-major A = U S V^T); returns sorted.
+static void host_svd16(const double* Ain, double* U, double* s, double* V) {
+  const int n = 16;
+  double G[256], W[256];
+  memcpy(G, Ain, sizeof(G));
+  for (int i = 0; i < 256; i++) W[i] = (i % n == i / n) ? 1.0 : 0.0;
+  for (int sweep = 0; sweep < 100; sweep++) {
+    bool rot = false;
+    for (int p = 0; p < n; p++) for (int q = p + 1; q < n; q++) {
+      double al = 0, be = 0, ga = 0;
+      for (int k = 0; k < n; k++) { al += G[p * n + k] * G[p * n + k]; be += G[q * n + k] * G[q * n + k]; ga += G[p * n + k] * G[q * n + k]; }
+      if (al < 1e-300 || be < 1e-300) continue;
+      if (std::fabs(ga) <= 1e-16 * std::sqrt(al * be)) continue;
+      rot = true;
+      double zeta = (be - al) / (2 * ga);
+      double t = (zeta >= 0 ? 1.0 : -1.0) / (std::fabs(zeta) + std::sqrt(1 + zeta * zeta));
+      double c = 1 / std::sqrt(1 + t * t), sn = c * t;
+      for (int k = 0; k < n; k++) {
+        double x = G[p * n + k], y = G[q * n + k];
+        G[p * n + k] = c * x - sn * y; G[q * n + k] = sn * x + c * y;
+        x = W[p * n + k]; y = W[q * n + k];
+        W[p * n + k] = c * x - sn * y; W[q * n + k] = sn * x + c * y;
+      }
+    }
+    if (!rot) break;
+  }
+  double nr[16]; int ord[16];
+  for (int j = 0; j < n; j++) { double a = 0; for (int k = 0; k < n; k++) a += G[j * n + k] * G[j * n + k]; nr[j] = std::sqrt(a); ord[j] = j; }
+  std::stable_sort(ord, ord + n, [&](int a, int b) { return nr[a] > nr[b]; });
+  for (int c = 0; c < n; c++) {
+    int j = ord[c];
+    s[c] = nr[j];
+    for (int k = 0; k < n; k++) { U[c * n + k] = nr[j] > 0 ? G[j * n + k] / nr[j] : 0.0; V[c * n + k] = W[j * n + k]; }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// lattice
+// ------------------------------------------------------------------------------------------
+static const int DXY[4][2] = {{0, -1}, {0, 1}, {-1, 0}, {1, 0}};   // U, D, L, R
+static const int OPP[4] = {1, 0, 3, 2};
+
+struct SiteInfo {
+  int x, y;
+  int nlegs;
+  int leg_dir[4];     // canonical order, present legs only
+  int leg_bond[4];
+  int nbr[4];         // per direction: neighbour site or -1
+  int bond_of_dir[4];
+  double* psi;        // device slot
+  size_t cap;         // doubles
+};
+struct BondInfo { int v1, d1, v2, d2; };
+
+struct SiteWs {       // per lane, per site-slot
+  double *cv, *out, *C, *Rx, *Rxinv, *Rbuf, *X, *T, *W, *Mx, *beta1, *tau1, *beta2, *tau2, *part;
+  int* info;          // device int (in the lane readback block)
+};
+struct LaneWs {
+  SiteWs s[2];
+  double *K, *Ks, *G, *V, *sv, *Us, *Vs;
+  int* order;
+  int* ints;          // [chi_new, sweeps, info0, info1]
+  double* dbls;       // [discarded, gap]
+};
+
+struct Arena {
+  char* base = nullptr; size_t size = 0, top = 0;
+  bool dry = false; size_t model = 0;     // dry run: only account (model = unaligned sum)
+  void* take(size_t bytes) {
+    model += bytes;
+    size_t off = (top + 255) & ~(size_t)255;
+    top = off + bytes;
+    if (dry) return nullptr;
+    return base ? base + off : nullptr;
+  }
+};
+
+}  // namespace pepo
+
+using namespace pepo;
+
+struct pepo_ctx {
+  int Lx, Ly, cx, cy, center;
+  double J, h, dt, bp_tol, bp_damping;
+  int chi_max, B;      // B = max inflight gates
+  int bondP, fieldP, obsP;
+  double eps_cut = 1e-11, chol_ratio = 4.0, chol_tau = 1e-7, jacobi_tol = 1e-15;
+  int bp_max_sweeps = 100, bp_max_sweeps_damped = 1000, jacobi_max_sweeps = 60;
+  int force_hh = 0;
+  cudaStream_t st;
+  int n_sites, n_bonds, n_hb;
+  std::vector<SiteInfo> sites;
+  std::vector<BondInfo> bonds;
+  std::vector<std::vector<int>> classes;
+  std::vector<int> chi;
+  // device
+  Arena arena;
+  double *lambda, *sqrt_l, *isqrt_l;     // n_bonds * chi_max each
+  double *msgs[2];                        // 2*n_bonds*chi_max each
+  int* chi_of_msg;                        // device 2*n_bonds
+  double* ones;                           // [1.0]
+  double* vs;                             // n_sites
+  double* bp_scalars;                     // [C]
+  unsigned long long* delta_bits;
+  int* bp_ints;                           // [flag, status]
+  std::vector<double*> partU, partD, partS;
+  double *dG1, *dGamma[2], *dAhat[2], *dSigma;
+  int NA;
+  double G1[16];
+  int f_row_mask, f_col_mask;
+  std::vector<LaneWs> lanes;
+  int* lane_ints; double* lane_dbls;      // device readback blocks (B*4 ints, B*2 doubles)
+  // pinned host
+  int* h_ints; double* h_dbls; int* h_chi_msg; double* h_scal; unsigned long long* h_delta; int* h_bpints;
+  int cur_msg = 0;
+  bool msgs_valid = false;
+  long long launches0 = 0;
+  pepo_stats stats;
+  size_t model_bytes = 0;
+};
+
+namespace {
+
+size_t ipow(size_t b, int e) { size_t r = 1; while (e-- > 0) r *= b; return r; }
+
+void build_lattice(int Lx, int Ly, std::vector<SiteInfo>& sites, std::vector<BondInfo>& bonds,
+                   std::vector<std::vector<int>>& classes, int& n_hb) {
+  const int ns = Lx * Ly;
+  n_hb = Ly * (Lx - 1);
+  const int nb = n_hb + (Ly - 1) * Lx;
+  sites.assign(ns, SiteInfo());
+  bonds.assign(nb, BondInfo());
+  for (int e = 0; e < nb; e++) {
+    if (e < n_hb) { int y = e / (Lx - 1), x = e % (Lx - 1); bonds[e] = {y * Lx + x, 3, y * Lx + x + 1, 2}; }
+    else { int q = e - n_hb; int y = q / Lx, x = q % Lx; bonds[e] = {y * Lx + x, 1, (y + 1) * Lx + x, 0}; }
+  }
+  for (int v = 0; v < ns; v++) {
+    SiteInfo& s = sites[v];
+    s.x = v % Lx; s.y = v / Lx; s.nlegs = 0;
+    for (int d = 0; d < 4; d++) {
+      int x2 = s.x + DXY[d][0], y2 = s.y + DXY[d][1];
+      s.nbr[d] = -1; s.bond_of_dir[d] = -1;
+      if (x2 < 0 || x2 >= Lx || y2 < 0 || y2 >= Ly) continue;
+      s.nbr[d] = y2 * Lx + x2;
+      int e;
+      if (d == 3) e = s.y * (Lx - 1) + s.x;
+      else if (d == 2) e = s.y * (Lx - 1) + s.x - 1;
+      else if (d == 1) e = n_hb + s.y * Lx + s.x;
+      else e = n_hb + (s.y - 1) * Lx + s.x;
+      s.bond_of_dir[d] = e;
+      s.leg_dir[s.nlegs] = d; s.leg_bond[s.nlegs] = e; s.nlegs++;
+    }
+  }
+  classes.assign(4, std::vector<int>());
+  for (int y = 0; y < Ly; y++) for (int x = 0; x + 1 < Lx; x++) classes[x % 2].push_back(y * (Lx - 1) + x);
+  for (int y = 0; y + 1 < Ly; y++) for (int x = 0; x < Lx; x++) classes[2 + y % 2].push_back(n_hb + y * Lx + x);
+}
+
+size_t gram_part_cap(int chi_max, size_t m_max) {
+  size_t best = 0;
+  for (int c = 1; c <= chi_max; c++) {
+    int ks, kc; int n = 4 * c;
+    gram_plan((long long)m_max, n, &ks, &kc);
+    best = std::max(best, (size_t)ks * n * n);
+  }
+  return best;
+}
+
+// Lays out (or, with arena.dry, only accounts) every device buffer.  The same routine is the
+// memory model: arena.model = plain sum of the buffer sizes.
+int layout(pepo_ctx* c) {
+  Arena& A = c->arena;
+  const size_t chi = c->chi_max;
+  const int NA = c->NA;
+  const size_t nmax = 4 * chi, Nmax = (size_t)NA * chi;
+  int degmax = 0;
+  for (auto& s : c->sites) degmax = std::max(degmax, s.nlegs);
+  for (auto& s : c->sites) {
+    s.cap = 4 * ipow(chi, s.nlegs);
+    s.psi = (double*)A.take(s.cap * 8);
+  }
+  const size_t nb = c->n_bonds;
+  c->lambda = (double*)A.take(nb * chi * 8);
+  c->sqrt_l = (double*)A.take(nb * chi * 8);
+  c->isqrt_l = (double*)A.take(nb * chi * 8);
+  c->msgs[0] = (double*)A.take(2 * nb * chi * 8 + 8);
+  c->msgs[1] = (double*)A.take(2 * nb * chi * 8 + 8);
+  c->chi_of_msg = (int*)A.take(2 * nb * 4 + 4);
+  c->ones = (double*)A.take(8);
+  c->vs = (double*)A.take(c->n_sites * 8);
+  c->bp_scalars = (double*)A.take(16);
+  c->delta_bits = (unsigned long long*)A.take(8);
+  c->bp_ints = (int*)A.take(16);
+  c->partU.assign(c->n_sites, nullptr); c->partD.assign(c->n_sites, nullptr); c->partS.assign(c->n_sites, nullptr);
+  for (int v = 0; v < c->n_sites; v++) {
+    const SiteInfo& s = c->sites[v];
+    int hU = s.nbr[0] >= 0, hD = s.nbr[1] >= 0, hL = s.nbr[2] >= 0, hR = s.nbr[3] >= 0;
+    c->partU[v] = (double*)A.take(ipow(chi, hL + hR + hU) * 8);
+    c->partD[v] = (double*)A.take(ipow(chi, hL + hR + hD) * 8);
+    c->partS[v] = (double*)A.take(ipow(chi, hL + hR) * 8);
+  }
+  c->dG1 = (double*)A.take(16 * 8);
+  for (int i = 0; i < 2; i++) {
+    c->dGamma[i] = (double*)A.take((size_t)NA * NA * 16 * 8);
+    c->dAhat[i] = (double*)A.take((size_t)NA * 16 * 8);
+  }
+  c->dSigma = (double*)A.take(NA * 8);
+  c->lane_ints = (int*)A.take((size_t)c->B * 4 * 4);
+  c->lane_dbls = (double*)A.take((size_t)c->B * 2 * 8);
+  const size_t m_max = ipow(chi, std::max(degmax - 1, 0));
+  const size_t ld_max = (m_max + 1) & ~(size_t)1;
+  const size_t cvcap = ld_max * nmax;
+  const size_t partcap = (degmax >= 1) ? gram_part_cap(c->chi_max, m_max) : 0;
+  c->lanes.assign(c->B, LaneWs());
+  for (int l = 0; l < c->B; l++) {
+    LaneWs& L = c->lanes[l];
+    L.ints = c->lane_ints ? c->lane_ints + 4 * l : nullptr;
+    L.dbls = c->lane_dbls ? c->lane_dbls + 2 * l : nullptr;
+    for (int i = 0; i < 2; i++) {
+      SiteWs& S = L.s[i];
+      S.cv = (double*)A.take(cvcap * 8);
+      S.out = (double*)A.take(cvcap * 8);
+      S.C = (double*)A.take(nmax * nmax * 8);
+      S.Rx = (double*)A.take(Nmax * Nmax * 8);
+      S.Rxinv = (double*)A.take(Nmax * Nmax * 8);
+      S.Rbuf = (double*)A.take(nmax * nmax * 8);
+      S.X = (double*)A.take(4 * nmax * Nmax * 8);
+      S.T = (double*)A.take(Nmax * chi * 8);
+      S.W = (double*)A.take(nmax * 4 * chi * 8);
+      S.Mx = (double*)A.take(4 * nmax * chi * 8);
+      S.beta1 = (double*)A.take(nmax * 8); S.tau1 = (double*)A.take(nmax * 8);
+      S.beta2 = (double*)A.take(Nmax * 8); S.tau2 = (double*)A.take(Nmax * 8);
+      S.part = (double*)A.take(partcap * 8);
+      S.info = L.ints ? L.ints + 2 + i : nullptr;
+    }
+    L.K = (double*)A.take(Nmax * Nmax * 8);
+    L.Ks = (double*)A.take(Nmax * Nmax * 8);
+    L.G = (double*)A.take(Nmax * Nmax * 8);
+    L.V = (double*)A.take(Nmax * Nmax * 8);
+    L.sv = (double*)A.take(Nmax * 8);
+    L.Us = (double*)A.take(Nmax * chi * 8);
+    L.Vs = (double*)A.take(Nmax * chi * 8);
+    L.order = (int*)A.take(Nmax * 4);
+  }
+  return 0;
+}
+
+int max_class_size(int Lx, int Ly) {
+  std::vector<SiteInfo> s; std::vector<BondInfo> b; std::vector<std::vector<int>> cl; int nh;
+  build_lattice(Lx, Ly, s, b, cl, nh);
+  size_t m = 1;
+  for (auto& c : cl) m = std::max(m, c.size());
+  return (int)m;
+}
+
+size_t model_bytes_for(int Lx, int Ly, int chi_max, int B, int NA, size_t* aligned_top) {
+  pepo_ctx tmp;
+  tmp.Lx = Lx; tmp.Ly = Ly; tmp.chi_max = chi_max; tmp.B = B; tmp.NA = NA;
+  build_lattice(Lx, Ly, tmp.sites, tmp.bonds, tmp.classes, tmp.n_hb);
+  tmp.n_sites = Lx * Ly; tmp.n_bonds = (int)tmp.bonds.size();
+  tmp.arena.dry = true;
+  layout(&tmp);
+  if (aligned_top) *aligned_top = tmp.arena.top;
+  return tmp.arena.model;
+}
+
+int default_inflight(int Lx, int Ly, int chi_max, int NA) {
+  int B = std::min(max_class_size(Lx, Ly), 16);
+  const double budget = 170e9;
+  while (B > 1) {
+    size_t top;
+    model_bytes_for(Lx, Ly, chi_max, B, NA, &top);
+    if ((double)top <= budget) break;
+    B--;
+  }
+  return std::max(B, 1);
+}
+
+inline double* bond_vec(double* base, int e, int chi_max) { return base + (size_t)e * chi_max; }
+
+}  // namespace
+
+// ============================================================================================
+// C ABI: lifetime
+// ============================================================================================
+extern "C" const char* pepo_last_error(void) { return pepo::last_error(); }
+
+extern "C" size_t pepo_arena_bytes_ex(int Lx, int Ly, int chi_max, int max_inflight) {
+  if (Lx < 1 || Ly < 1 || chi_max < 1) return 0;
+  int B = max_inflight > 0 ? std::min(max_inflight, PEPO_MAXT / 2) : default_inflight(Lx, Ly, chi_max, 4);
+  size_t top;
+  model_bytes_for(Lx, Ly, chi_max, B, 4, &top);
+  return top + 256;
+}
+extern "C" size_t pepo_arena_bytes(int Lx, int Ly, int chi_max) {
+  return pepo_arena_bytes_ex(Lx, Ly, chi_max, 0);
+}
+
+static int upload(pepo_ctx* c, void* dst, const void* src, size_t bytes) {
+  PEPO_CUDA_OK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, c->st));
+  PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
+  return 0;
+}
+
+static int reset_state(pepo_ctx* c) {
+  // product operator: all bonds chi = 1, lambda = [1]
+  std::fill(c->chi.begin(), c->chi.end(), 1);
+  for (int v = 0; v < c->n_sites; v++) {
+    double t[4] = {0, 0, 0, 0};
+    t[v == c->center ? c->obsP : 0] = 1.0;
+    int rc = upload(c, c->sites[v].psi, t, sizeof(t));
+    if (rc) return rc;
+  }
+  std::vector<double> one((size_t)c->n_bonds * c->chi_max, 0.0);
+  for (int e = 0; e < c->n_bonds; e++) one[(size_t)e * c->chi_max] = 1.0;
+  if (c->n_bonds) {
+    int rc = upload(c, c->lambda, one.data(), one.size() * 8); if (rc) return rc;
+    rc = upload(c, c->sqrt_l, one.data(), one.size() * 8); if (rc) return rc;
+    rc = upload(c, c->isqrt_l, one.data(), one.size() * 8); if (rc) return rc;
+  }
+  c->msgs_valid = false;
+  return 0;
+}
+
+extern "C" int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, double J, double h,
+                            double dt, int chi_max, double bp_tol, double bp_damping,
+                            void* d_arena, size_t arena_bytes, void* stream, int max_inflight,
+                            int bond_pauli, int field_pauli, int obs_pauli) {
+  if (!out) { set_error("init: out is NULL"); return -1; }
+  *out = nullptr;
+  if (Lx < 1 || Ly < 1 || cx < 0 || cx >= Lx || cy < 0 || cy >= Ly || chi_max < 1 || chi_max > 256 ||
+      !(dt > 0.0) || bond_pauli < 1 || bond_pauli > 3 || field_pauli < 1 || field_pauli > 3 ||
+      obs_pauli < 1 || obs_pauli > 3 || bp_damping < 0.0 || bp_damping >= 1.0 || !d_arena) {
+    set_error("init: bad argument (grid %dx%d centre (%d,%d) chi_max %d dt %g)", Lx, Ly, cx, cy, chi_max, dt);
+    return -1;
+  }
+  pepo_ctx* c = new pepo_ctx();
+  c->Lx = Lx; c->Ly = Ly; c->cx = cx; c->cy = cy; c->center = cy * Lx + cx;
+  c->J = J; c->h = h; c->dt = dt; c->bp_tol = bp_tol; c->bp_damping = bp_damping;
+  c->chi_max = chi_max; c->bondP = bond_pauli; c->fieldP = field_pauli; c->obsP = obs_pauli;
+  c->st = (cudaStream_t)stream;
+  build_lattice(Lx, Ly, c->sites, c->bonds, c->classes, c->n_hb);
+  c->n_sites = Lx * Ly; c->n_bonds = (int)c->bonds.size();
+  c->chi.assign(c->n_bonds, 1);
+  // gate tables: field PTM, bond PTM and its operator-Schmidt decomposition
+  ptm_one_site(h * dt, field_pauli, c->G1);
+  c->f_row_mask = 0; c->f_col_mask = 0;
+  for (int q = 0; q < 4; q++) {
+    bool ident = true;
+    for (int p = 0; p < 4; p++) if (std::fabs(c->G1[q * 4 + p] - (p == q ? 1.0 : 0.0)) > 0.0) ident = false;
+    if (!ident) {
+      c->f_row_mask |= 1 << q;
+      for (int p = 0; p < 4; p++) if (c->G1[q * 4 + p] != 0.0) c->f_col_mask |= 1 << p;
+    }
+  }
+  double G2[256];
+  ptm_two_site(J * dt, bond_pauli, G2);
+  // T[(p1',p1),(p2',p2)] = G2[(p1'p2'),(p1p2)], column-major 16x16
+  double Tm[256], U[256], S[16], V[256];
+  for (int a1 = 0; a1 < 4; a1++) for (int a2 = 0; a2 < 4; a2++) for (int b1 = 0; b1 < 4; b1++) for (int b2 = 0; b2 < 4; b2++)
+    Tm[(a1 * 4 + b1) + 16 * (a2 * 4 + b2)] = G2[(a1 * 4 + a2) * 16 + (b1 * 4 + b2)];
+  host_svd16(Tm, U, S, V);
+  int NA = 0;
+  for (int a = 0; a < 16; a++) if (S[a] > 1e-13 * S[0]) NA = a + 1;
+  if (NA > 4) { set_error("init: gate with operator-Schmidt rank %d > 4 unsupported", NA); delete c; return -1; }
+  c->NA = 4;     // fixed layout (N = 4 chi); unused components get sigma = 0
+  std::vector<double> Ahat[2], Gam[2], sig(4, 0.0);
+  for (int i = 0; i < 2; i++) {
+    const double* F = i == 0 ? U : V;
+    Ahat[i].assign(4 * 16, 0.0);
+    for (int a = 0; a < NA; a++)
+      for (int pp = 0; pp < 4; pp++) for (int p = 0; p < 4; p++) Ahat[i][(a * 4 + pp) * 4 + p] = F[a * 16 + (pp * 4 + p)];
+    // unused components: keep an orthonormal completion so that the dressed Gram stays SPD
+    for (int a = NA; a < 4; a++)
+      for (int pp = 0; pp < 4; pp++) for (int p = 0; p < 4; p++) Ahat[i][(a * 4 + pp) * 4 + p] = F[a * 16 + (pp * 4 + p)];
+    Gam[i].assign(4 * 4 * 16, 0.0);
+    for (int a = 0; a < 4; a++) for (int a2 = 0; a2 < 4; a2++) for (int p = 0; p < 4; p++) for (int q = 0; q < 4; q++) {
+      double s = 0;
+      for (int pp = 0; pp < 4; pp++) s += Ahat[i][(a * 4 + pp) * 4 + p] * Ahat[i][(a2 * 4 + pp) * 4 + q];
+      Gam[i][((a * 4 + a2) * 4 + p) * 4 + q] = s;
+    }
+  }
+  for (int a = 0; a < NA; a++) sig[a] = S[a];
+  // workspace sizing
+  c->B = max_inflight > 0 ? std::min(max_inflight, PEPO_MAXT / 2) : default_inflight(Lx, Ly, chi_max, 4);
+  size_t top;
+  c->model_bytes = model_bytes_for(Lx, Ly, chi_max, c->B, 4, &top);
+  size_t need = top + 256;
+  if (arena_bytes < need) {
+    set_error("init: arena too small: %zu bytes given, %zu needed", arena_bytes, need);
+    delete c; return -2;
+  }
+  size_t mis = (size_t)((uintptr_t)d_arena & 255);
+  c->arena.base = (char*)d_arena + (mis ? 256 - mis : 0);
+  c->arena.size = arena_bytes;
+  layout(c);
+  // pinned host buffers
+  if (cudaMallocHost((void**)&c->h_ints, (size_t)c->B * 4 * 4 + 16) != cudaSuccess ||
+      cudaMallocHost((void**)&c->h_dbls, (size_t)c->B * 2 * 8 + 16) != cudaSuccess ||
+      cudaMallocHost((void**)&c->h_chi_msg, (size_t)2 * c->n_bonds * 4 + 16) != cudaSuccess ||
+      cudaMallocHost((void**)&c->h_scal, 64) != cudaSuccess ||
+      cudaMallocHost((void**)&c->h_delta, 16) != cudaSuccess ||
+      cudaMallocHost((void**)&c->h_bpints, 16) != cudaSuccess) {
+    set_error("init: cudaMallocHost failed"); delete c; return -3;
+  }
+  int rc = 0;
+  double one = 1.0;
+  rc |= upload(c, c->ones, &one, 8);
+  rc |= upload(c, c->dG1, c->G1, 128);
+  for (int i = 0; i < 2; i++) {
+    rc |= upload(c, c->dGamma[i], Gam[i].data(), Gam[i].size() * 8);
+    rc |= upload(c, c->dAhat[i], Ahat[i].data(), Ahat[i].size() * 8);
+  }
+  rc |= upload(c, c->dSigma, sig.data(), 32);
+  if (!rc) rc = reset_state(c);
+  if (rc) { delete c; return -3; }
+  memset(&c->stats, 0, sizeof(c->stats));
+  c->stats.min_cut_gap = 1.0;
+  c->launches0 = g_launch_count;
+  *out = c;
+  return 0;
+}
+
+extern "C" int pepo_init(pepo_ctx** out, int Lx, int Ly, int cx, int cy, double J, double h,
+                         double dt, int chi_max, double bp_tol, double bp_damping, void* d_arena,
+                         size_t arena_bytes, void* stream) {
+  return pepo_init_ex(out, Lx, Ly, cx, cy, J, h, dt, chi_max, bp_tol, bp_damping, d_arena,
+                      arena_bytes, stream, 0, 3, 1, 3);
+}
+
+extern "C" int pepo_destroy(pepo_ctx* c) {
+  if (!c) return 0;
+  cudaStreamSynchronize(c->st);
+  cudaFreeHost(c->h_ints); cudaFreeHost(c->h_dbls); cudaFreeHost(c->h_chi_msg);
+  cudaFreeHost(c->h_scal); cudaFreeHost(c->h_delta); cudaFreeHost(c->h_bpints);
+  delete c;
+  return 0;
+}
+
+extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
+  if (!c || !key) { set_error("set_option: NULL"); return -1; }
+  std::string k(key);
+  if (k == "eps_cut") c->eps_cut = v;
+  else if (k == "bp_max_sweeps") c->bp_max_sweeps = (int)v;
+  else if (k == "bp_max_sweeps_damped") c->bp_max_sweeps_damped = (int)v;
+  else if (k == "chol_min_ratio") c->chol_ratio = v;
+  else if (k == "chol_tau") c->chol_tau = v;
+  else if (k == "force_householder") c->force_hh = (int)v;
+  else if (k == "jacobi_tol") c->jacobi_tol = v;
+  else if (k == "jacobi_max_sweeps") c->jacobi_max_sweeps = (int)v;
+  else if (k == "bp_tol") c->bp_tol = v;
+  else if (k == "bp_damping") c->bp_damping = v;
+  else { set_error("set_option: unknown key %s", key); return -1; }
+  return 0;
+}
+
+// ============================================================================================
+// state access
+// ============================================================================================
+static size_t site_live_size(const pepo_ctx* c, int v) {
+  size_t n = 4;
+  const SiteInfo& s = c->sites[v];
+  for (int l = 0; l < s.nlegs; l++) n *= c->chi[s.leg_bond[l]];
+  return n;
+}
+extern "C" int pepo_n_bonds(pepo_ctx* c) { return c ? c->n_bonds : -1; }
+extern "C" int pepo_get_bond_dims(pepo_ctx* c, int* h_chi) {
+  if (!c || !h_chi) { set_error("get_bond_dims: NULL"); return -1; }
+  for (int e = 0; e < c->n_bonds; e++) h_chi[e] = c->chi[e];
+  return 0;
+}
+extern "C" int pepo_set_bond_dims(pepo_ctx* c, const int* h_chi) {
+  if (!c || !h_chi) { set_error("set_bond_dims: NULL"); return -1; }
+  for (int e = 0; e < c->n_bonds; e++)
+    if (h_chi[e] < 1 || h_chi[e] > c->chi_max) { set_error("set_bond_dims: chi[%d]=%d out of range", e, h_chi[e]); return -1; }
+  for (int e = 0; e < c->n_bonds; e++) c->chi[e] = h_chi[e];
+  c->msgs_valid = false;
+  return 0;
+}
+extern "C" size_t pepo_site_size(pepo_ctx* c, int x, int y) {
+  if (!c || x < 0 || x >= c->Lx || y < 0 || y >= c->Ly) return 0;
+  return site_live_size(c, y * c->Lx + x);
+}
+extern "C" double* pepo_site_ptr(pepo_ctx* c, int x, int y) {
+  if (!c || x < 0 || x >= c->Lx || y < 0 || y >= c->Ly) return nullptr;
+  return c->sites[y * c->Lx + x].psi;
+}
+extern "C" int pepo_get_site(pepo_ctx* c, int x, int y, double* h_dst, size_t n) {
+  if (!c || !h_dst || x < 0 || x >= c->Lx || y < 0 || y >= c->Ly) { set_error("get_site: bad argument"); return -1; }
+  int v = y * c->Lx + x;
+  if (n != site_live_size(c, v)) { set_error("get_site: size %zu != live size %zu", n, site_live_size(c, v)); return -1; }
+  PEPO_CUDA_OK(cudaMemcpyAsync(h_dst, c->sites[v].psi, n * 8, cudaMemcpyDeviceToHost, c->st));
+  PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
+  return 0;
+}
+extern "C" int pepo_set_site(pepo_ctx* c, int x, int y, const double* h_src, size_t n) {
+  if (!c || !h_src || x < 0 || x >= c->Lx || y < 0 || y >= c->Ly) { set_error("set_site: bad argument"); return -1; }
+  int v = y * c->Lx + x;
+  if (n != site_live_size(c, v)) { set_error("set_site: size %zu != live size %zu", n, site_live_size(c, v)); return -1; }
+  c->msgs_valid = false;
+  return upload(c, c->sites[v].psi, h_src, n * 8);
+}
+extern "C" int pepo_get_lambda(pepo_ctx* c, int bond, double* h_dst, int n) {
+  if (!c || !h_dst || bond < 0 || bond >= c->n_bonds || n != c->chi[bond]) { set_error("get_lambda: bad argument"); return -1; }
+  PEPO_CUDA_OK(cudaMemcpyAsync(h_dst, bond_vec(c->lambda, bond, c->chi_max), n * 8, cudaMemcpyDeviceToHost, c->st));
+  PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
+  return 0;
+}
+extern "C" int pepo_set_lambda(pepo_ctx* c, int bond, const double* h_src, int n) {
+  if (!c || !h_src || bond < 0 || bond >= c->n_bonds || n != c->chi[bond]) { set_error("set_lambda: bad argument"); return -1; }
+  std::vector<double> sq(n), isq(n);
+  for (int i = 0; i < n; i++) {
+    if (!(h_src[i] > 0.0)) { set_error("set_lambda: non-positive entry"); return -1; }
+    sq[i] = std::sqrt(h_src[i]); isq[i] = 1.0 / sq[i];
+  }
+  int rc = upload(c, bond_vec(c->lambda, bond, c->chi_max), h_src, n * 8);
+  rc |= upload(c, bond_vec(c->sqrt_l, bond, c->chi_max), sq.data(), n * 8);
+  rc |= upload(c, bond_vec(c->isqrt_l, bond, c->chi_max), isq.data(), n * 8);
+  return rc ? -3 : 0;
+}
+
+extern "C" int pepo_get_stats(pepo_ctx* c, pepo_stats* s) {
+  if (!c || !s) { set_error("get_stats: NULL"); return -1; }
+  c->stats.kernel_launches = g_launch_count - c->launches0;
+  c->stats.arena_high_water = c->arena.top;
+  c->stats.arena_model_bytes = c->model_bytes;
+  c->stats.max_inflight_gates = c->B;
+  int m = 1;
+  for (int e = 0; e < c->n_bonds; e++) m = std::max(m, c->chi[e]);
+  c->stats.chi_max_live = m;
+  *s = c->stats;
+  return 0;
+}
+
+// ============================================================================================
+// Trotter step
+// ============================================================================================
+extern "C" int pepo_apply_field(pepo_ctx* c) {
+  if (!c) { set_error("apply_field: NULL"); return -1; }
+  if (c->f_row_mask == 0) return 0;
+  for (int v0 = 0; v0 < c->n_sites; v0 += PEPO_BP_MAXS) {
+    FieldBatch fb;
+    fb.count = std::min(PEPO_BP_MAXS, c->n_sites - v0);
+    for (int i = 0; i < fb.count; i++) {
+      fb.psi[i] = c->sites[v0 + i].psi;
+      fb.slab[i] = (long long)(site_live_size(c, v0 + i) / 4);
+    }
+    memcpy(fb.G, c->G1, sizeof(fb.G));
+    fb.row_mask = c->f_row_mask; fb.col_mask = c->f_col_mask;
+    int rc = launch_field_gate(c->st, fb);
+    if (rc) return rc;
+  }
+  c->msgs_valid = false;
+  return 0;
+}
+
+namespace {
+
+struct TaskGeo {           // one site of one gate
+  int v, lane, slot, site_idx;     // site_idx: 0 = v1 (first Schmidt factor), 1 = v2
+  int nlegs, cut_leg;
+  int dims[5];             // live dims incl. Pauli
+  int env_legs[3], n_env;
+  long long m, ld;
+  int n, chi_c, N, k, r;   // k = min(m,n); r = rows of Rx
+  bool chol;
+  int chi_new;
+};
+
+int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
+  const int ng = (int)gate_bonds.size();
+  if (ng == 0) return 0;
+  cudaStream_t st = c->st;
+  const int NA = c->NA;
+  GateTables gt;
+  gt.Gamma[0] = c->dGamma[0]; gt.Gamma[1] = c->dGamma[1];
+  gt.Ahat[0] = c->dAhat[0]; gt.Ahat[1] = c->dAhat[1];
+  gt.sigma = c->dSigma;
+  std::vector<TaskGeo> T(2 * ng);
+  // ---- A: geometry + absorb/permute ----------------------------------------------------------
+  for (int g = 0; g < ng; g++) {
+    const BondInfo& b = c->bonds[gate_bonds[g]];
+    for (int i = 0; i < 2; i++) {
+      TaskGeo& t = T[2 * g + i];
+      t.v = i == 0 ? b.v1 : b.v2;
+      const int dcut = i == 0 ? b.d1 : b.d2;
+      t.lane = g; t.slot = i; t.site_idx = i;
+      const SiteInfo& s = c->sites[t.v];
+      t.nlegs = s.nlegs; t.n_env = 0; t.m = 1; t.cut_leg = -1;
+      for (int l = 0; l < s.nlegs; l++) {
+        t.dims[l] = c->chi[s.leg_bond[l]];
+        if (s.leg_dir[l] == dcut) t.cut_leg = l;
+        else { t.env_legs[t.n_env++] = l; t.m *= t.dims[l]; }
+      }
+      t.dims[s.nlegs] = 4;
+      t.chi_c = t.dims[t.cut_leg];
+      t.n = 4 * t.chi_c; t.N = NA * t.chi_c;
+      t.ld = (t.m + 1) & ~1ll;
+      t.k = (int)std::min<long long>(t.m, t.n);
+      t.chol = !c->force_hh && (double)t.m >= c->chol_ratio * t.n;
+      t.r = t.chol ? t.N : std::min(4 * t.k, t.N);
+      SiteWs& W = c->lanes[g].s[i];
+      PermuteDesc pd;
+      pd.rank = s.nlegs + 1; pd.power = 1.0;
+      long long sstr = 1;
+      for (int l = 0; l <= s.nlegs; l++) { pd.shape[l] = t.dims[l]; pd.src_stride[l] = sstr; sstr *= t.dims[l]; pd.scale[l] = nullptr; }
+      long long dstr = 1;
+      for (int j = 0; j < t.n_env; j++) {
+        int l = t.env_legs[j];
+        pd.perm[j] = l; pd.dst_stride[j] = dstr; dstr *= t.dims[l];
+        pd.scale[l] = bond_vec(c->sqrt_l, s.leg_bond[l], c->chi_max);
+      }
+      pd.perm[t.n_env] = t.cut_leg; pd.dst_stride[t.n_env] = t.ld;
+      pd.perm[t.n_env + 1] = s.nlegs; pd.dst_stride[t.n_env + 1] = t.ld * t.chi_c;
+      int rc = launch_permute(st, s.psi, W.cv, pd);
+      if (rc) return rc;
+    }
+  }
+  // ---- B: Cholesky path ------------------------------------------------------------------------
+  {
+    MatBatch pb; pb.count = 0;
+    DressBatch db; db.count = 0; db.NA = NA;
+    int* infos[PEPO_MAXT];
+    for (auto& t : T) {
+      if (!t.chol) continue;
+      SiteWs& W = c->lanes[t.lane].s[t.slot];
+      int ks, kc;
+      gram_plan(t.m, t.n, &ks, &kc);
+      GemmProb gp;
+      gp.A = W.cv; gp.B = W.cv; gp.C = W.C; gp.lda = t.ld; gp.ldb = t.ld; gp.ldc = t.n;
+      gp.M = t.n; gp.N = t.n; gp.K = (int)t.m;
+      int rc = launch_dgemm(st, 1, 0, gp, ks, kc, W.part, true);
+      if (rc) return rc;
+      if (ks > 1) rc = launch_gram_reduce(st, W.part, ks, t.n, W.C, t.n);
+      else {
+        // single split wrote the upper tiles straight into C: mirror through the same reducer
+        rc = launch_gram_reduce(st, W.C, 1, t.n, W.C, t.n);
+      }
+      if (rc) return rc;
+      int q = db.count++;
+      db.in[q] = W.C; db.out[q] = W.Rx; db.chi[q] = t.chi_c; db.k[q] = t.n; db.site[q] = t.site_idx;
+      db.ld_in[q] = t.n; db.ld_out[q] = t.N;
+      int p = pb.count++;
+      pb.A[p] = W.Rx; pb.ld[p] = t.N; pb.m[p] = t.N; pb.n[p] = t.N; infos[p] = W.info;
+    }
+    if (db.count) {
+      int rc = launch_dress_gram(st, db, gt); if (rc) return rc;
+      rc = launch_potrf(st, pb, infos, c->chol_tau); if (rc) return rc;
+      PEPO_CUDA_OK(cudaMemcpyAsync(c->h_ints, c->lane_ints, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
+      PEPO_CUDA_OK(cudaStreamSynchronize(st));
+      for (auto& t : T) {
+        if (!t.chol) continue;
+        int info = c->h_ints[4 * t.lane + 2 + t.slot];
+        if (info != 0) {
+          t.chol = false; t.r = std::min(4 * t.k, t.N);
+          c->stats.n_chol_failed++;
+        }
+      }
+    }
+  }
+  // ---- C: Householder path / finish Cholesky path ----------------------------------------------
+  {
+    HHBatch h1; h1.count = 0;
+    HHBatch h2; h2.count = 0;
+    DressBatch dr; dr.count = 0; dr.NA = NA;
+    double* Rout1[PEPO_MAXT]; long long ldr1[PEPO_MAXT];
+    double* Rout2[PEPO_MAXT]; long long ldr2[PEPO_MAXT];
+    MatBatch zl; zl.count = 0;
+    MatBatch ti; ti.count = 0;
+    for (auto& t : T) {
+      SiteWs& W = c->lanes[t.lane].s[t.slot];
+      if (t.chol) {
+        int q = zl.count++;
+        zl.A[q] = W.Rx; zl.ld[q] = t.N; zl.m[q] = t.N; zl.n[q] = t.N;
+        ti.A[q] = W.Rxinv; ti.ld[q] = t.N; ti.m[q] = t.N; ti.n[q] = t.N; ti.count = zl.count;
+        c->stats.n_cholesky++;
+      } else {
+        int q = h1.count++;
+        h1.A[q] = W.cv; h1.lda[q] = t.ld; h1.m[q] = t.m; h1.n[q] = t.n; h1.beta[q] = W.beta1; h1.tau[q] = W.tau1;
+        Rout1[q] = W.Rbuf; ldr1[q] = t.k;
+        dr.in[q] = W.Rbuf; dr.out[q] = W.X; dr.chi[q] = t.chi_c; dr.k[q] = t.k; dr.site[q] = t.site_idx;
+        dr.ld_in[q] = t.k; dr.ld_out[q] = 4ll * t.k; dr.count = h1.count;
+        h2.A[q] = W.X; h2.lda[q] = 4ll * t.k; h2.m[q] = 4ll * t.k; h2.n[q] = t.N; h2.beta[q] = W.beta2; h2.tau[q] = W.tau2;
+        h2.count = h1.count;
+        Rout2[q] = W.Rx; ldr2[q] = t.r;
+        c->stats.n_householder++;
+      }
+    }
+    int rc = 0;
+    if (zl.count) { rc = launch_zero_lower(st, zl); if (rc) return rc; rc = launch_trtri(st, zl, ti); if (rc) return rc; }
+    if (h1.count) {
+      rc = launch_hh_factor(st, h1); if (rc) return rc;
+      rc = launch_hh_extract_r(st, h1, Rout1, ldr1); if (rc) return rc;
+      rc = launch_dress_R(st, dr, gt); if (rc) return rc;
+      rc = launch_hh_factor(st, h2); if (rc) return rc;
+      rc = launch_hh_extract_r(st, h2, Rout2, ldr2); if (rc) return rc;
+    }
+  }
+  // ---- D: core, SVD, truncation ------------------------------------------------------------------
+  {
+    DressBatch sc; sc.count = ng; sc.NA = NA;
+    SvdBatch sb; sb.count = ng;
+    SvdFinishBatch fb; fb.count = ng;
+    for (int g = 0; g < ng; g++) {
+      TaskGeo& t1 = T[2 * g]; TaskGeo& t2 = T[2 * g + 1];
+      LaneWs& L = c->lanes[g];
+      const int e = gate_bonds[g];
+      sc.in[g] = L.s[0].Rx; sc.out[g] = L.Ks; sc.chi[g] = t1.chi_c; sc.k[g] = t1.r; sc.site[g] = 0;
+      sc.ld_in[g] = t1.r; sc.ld_out[g] = t1.r;
+      sb.K[g] = L.K; sb.ldk[g] = t1.r; sb.r1[g] = t1.r; sb.r2[g] = t2.r;
+      sb.G[g] = L.G; sb.V[g] = L.V; sb.sv[g] = L.sv; sb.order[g] = L.order; sb.sweeps[g] = L.ints + 1;
+      fb.r1[g] = t1.r; fb.r2[g] = t2.r; fb.G[g] = L.G; fb.V[g] = L.V; fb.sv[g] = L.sv; fb.order[g] = L.order;
+      fb.Us[g] = L.Us; fb.ldus[g] = t1.r; fb.Vs[g] = L.Vs; fb.ldvs[g] = t2.r;
+      fb.lambda[g] = bond_vec(c->lambda, e, c->chi_max);
+      fb.sqrt_l[g] = bond_vec(c->sqrt_l, e, c->chi_max);
+      fb.isqrt_l[g] = bond_vec(c->isqrt_l, e, c->chi_max);
+      fb.chi_new[g] = L.ints; fb.gate_stats[g] = L.dbls;
+    }
+    int rc = launch_scale_sigma(st, sc, gt); if (rc) return rc;
+    for (int g = 0; g < ng; g++) {
+      TaskGeo& t1 = T[2 * g]; TaskGeo& t2 = T[2 * g + 1];
+      LaneWs& L = c->lanes[g];
+      GemmProb gp;
+      gp.A = L.Ks; gp.lda = t1.r; gp.B = L.s[1].Rx; gp.ldb = t2.r; gp.C = L.K; gp.ldc = t1.r;
+      gp.M = t1.r; gp.N = t2.r; gp.K = t1.N;
+      rc = launch_dgemm(st, 0, 1, gp, 1, 0, nullptr, false); if (rc) return rc;
+    }
+    rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps); if (rc) return rc;
+    rc = launch_svd_truncate(st, fb, c->chi_max, c->eps_cut); if (rc) return rc;
+    PEPO_CUDA_OK(cudaMemcpyAsync(c->h_ints, c->lane_ints, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
+    PEPO_CUDA_OK(cudaMemcpyAsync(c->h_dbls, c->lane_dbls, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
+    PEPO_CUDA_OK(cudaStreamSynchronize(st));
+    int chi_cap = 1;
+    for (int g = 0; g < ng; g++) {
+      int cn = c->h_ints[4 * g];
+      if (cn < 1) { set_error("gate on bond %d: s0 = 0 or NaN in the core SVD", gate_bonds[g]); return -4; }
+      T[2 * g].chi_new = T[2 * g + 1].chi_new = cn;
+      chi_cap = std::max(chi_cap, cn);
+      c->stats.jacobi_sweeps += c->h_ints[4 * g + 1];
+      c->stats.gate_err += c->h_dbls[2 * g];
+      c->stats.min_cut_gap = std::min(c->stats.min_cut_gap, c->h_dbls[2 * g + 1]);
+    }
+    rc = launch_svd_bridge(st, fb, chi_cap); if (rc) return rc;
+  }
+  // ---- E: bridge + reconstruction ------------------------------------------------------------------
+  {
+    DressBatch bw; bw.count = 0; bw.NA = NA;
+    int* cn_w[PEPO_MAXT];
+    HHApplyBatch a2; a2.count = 0;
+    DressBatch rs; rs.count = 0; rs.NA = NA;
+    int* cn_r[PEPO_MAXT]; long long mrows[PEPO_MAXT];
+    HHApplyBatch a1; a1.count = 0;
+    MatBatch padsrc; padsrc.count = 0;
+    int rc = 0;
+    for (auto& t : T) {
+      SiteWs& W = c->lanes[t.lane].s[t.slot];
+      LaneWs& L = c->lanes[t.lane];
+      const double* UV = t.slot == 0 ? L.Us : L.Vs;
+      if (t.chol) {
+        // T = Rx^-1 (U sqrt S)   (N x chi_new)
+        GemmProb gp;
+        gp.A = W.Rxinv; gp.lda = t.N; gp.B = UV; gp.ldb = t.r; gp.C = W.T; gp.ldc = t.N;
+        gp.M = t.N; gp.N = t.chi_new; gp.K = t.N;
+        rc = launch_dgemm(st, 0, 0, gp, 1, 0, nullptr, false); if (rc) return rc;
+        int q = bw.count++;
+        bw.in[q] = W.T; bw.out[q] = W.W; bw.chi[q] = t.chi_c; bw.k[q] = t.chi_new; bw.site[q] = t.site_idx;
+        bw.ld_in[q] = t.N; bw.ld_out[q] = t.n; cn_w[q] = L.ints;
+      } else {
+        int q = a2.count++;
+        // Mx = [U sqrt S ; 0] (4k x chi_new), then Qx applied
+        padsrc.A[q] = const_cast<double*>(UV); padsrc.ld[q] = t.r; padsrc.m[q] = t.r; padsrc.n[q] = t.chi_new;
+        padsrc.count = a2.count;
+        a2.A[q] = W.X; a2.lda[q] = 4ll * t.k; a2.m[q] = 4ll * t.k; a2.k[q] = t.r;
+        a2.beta[q] = W.beta2; a2.tau[q] = W.tau2; a2.Y[q] = W.Mx; a2.ldy[q] = 4ll * t.k; a2.ncols[q] = t.chi_new;
+        rs.in[q] = W.Mx; rs.out[q] = W.out; rs.chi[q] = t.chi_new; rs.k[q] = t.k; rs.site[q] = t.site_idx;
+        rs.ld_in[q] = 4ll * t.k; rs.ld_out[q] = t.ld; rs.count = a2.count;
+        cn_r[q] = L.ints; mrows[q] = t.m;
+        a1.A[q] = W.cv; a1.lda[q] = t.ld; a1.m[q] = t.m; a1.k[q] = t.k; a1.beta[q] = W.beta1; a1.tau[q] = W.tau1;
+        a1.Y[q] = W.out; a1.ldy[q] = t.ld; a1.ncols[q] = 4 * t.chi_new; a1.count = a2.count;
+      }
+    }
+    if (bw.count) {
+      rc = launch_build_W(st, bw, gt, cn_w); if (rc) return rc;
+      for (auto& t : T) {
+        if (!t.chol) continue;
+        SiteWs& W = c->lanes[t.lane].s[t.slot];
+        GemmProb gp;
+        gp.A = W.cv; gp.lda = t.ld; gp.B = W.W; gp.ldb = t.n; gp.C = W.out; gp.ldc = t.ld;
+        gp.M = t.m; gp.N = 4 * t.chi_new; gp.K = t.n;
+        rc = launch_dgemm(st, 0, 0, gp, 1, 0, nullptr, false); if (rc) return rc;
+      }
+    }
+    if (a2.count) {
+      // pad-copy through the reshuffle kernel's sibling: use launch_copy_pad
+      rc = launch_copy_pad(st, padsrc, a2); if (rc) return rc;
+      rc = launch_hh_apply_q(st, a2); if (rc) return rc;
+      rc = launch_reshuffle_M(st, rs, cn_r, mrows); if (rc) return rc;
+      rc = launch_hh_apply_q(st, a1); if (rc) return rc;
+    }
+  }
+  // ---- F: inverse permute + deabsorb + write-back ----------------------------------------------------
+  for (auto& t : T) {
+    const SiteInfo& s = c->sites[t.v];
+    SiteWs& W = c->lanes[t.lane].s[t.slot];
+    PermuteDesc pd;
+    pd.rank = s.nlegs + 1; pd.power = 1.0;
+    // source dims in cv order: env legs, cut (chi_new), P
+    int newdims[5];
+    for (int l = 0; l < s.nlegs; l++) newdims[l] = (l == t.cut_leg) ? t.chi_new : t.dims[l];
+    newdims[s.nlegs] = 4;
+    long long dst_stride_of_leg[5];
+    long long ds = 1;
+    for (int l = 0; l <= s.nlegs; l++) { dst_stride_of_leg[l] = ds; ds *= newdims[l]; }
+    long long sstr = 1;
+    int src_leg[5];
+    for (int j = 0; j < t.n_env; j++) {
+      int l = t.env_legs[j];
+      src_leg[j] = l; pd.shape[j] = t.dims[l]; pd.src_stride[j] = sstr; sstr *= t.dims[l];
+      pd.scale[j] = bond_vec(c->isqrt_l, s.leg_bond[l], c->chi_max);
+    }
+    src_leg[t.n_env] = t.cut_leg; pd.shape[t.n_env] = t.chi_new; pd.src_stride[t.n_env] = t.ld; pd.scale[t.n_env] = nullptr;
+    src_leg[t.n_env + 1] = s.nlegs; pd.shape[t.n_env + 1] = 4; pd.src_stride[t.n_env + 1] = t.ld * t.chi_new; pd.scale[t.n_env + 1] = nullptr;
+    // output dim j (canonical leg j) is source dim whose leg is j
+    for (int j = 0; j <= s.nlegs; j++) {
+      int sd = -1;
+      for (int q = 0; q <= s.nlegs; q++) if (src_leg[q] == j) sd = q;
+      pd.perm[j] = sd; pd.dst_stride[j] = dst_stride_of_leg[j];
+    }
+    int rc = launch_permute(st, W.out, s.psi, pd);
+    if (rc) return rc;
+  }
+  for (int g = 0; g < ng; g++) c->chi[gate_bonds[g]] = T[2 * g].chi_new;
+  c->msgs_valid = false;
+  return 0;
+}
+
+}  // namespace
+
+extern "C" int pepo_apply_bond(pepo_ctx* c, int bond) {
+  if (!c || bond < 0 || bond >= c->n_bonds) { set_error("apply_bond: bad bond"); return -1; }
+  std::vector<int> g(1, bond);
+  return run_batch(c, g);
+}
+
+extern "C" int pepo_trotter_step(pepo_ctx* c) {
+  if (!c) { set_error("trotter_step: NULL"); return -1; }
+  c->stats.gate_err = 0.0; c->stats.min_cut_gap = 1.0; c->stats.jacobi_sweeps = 0;
+  int rc = pepo_apply_field(c);
+  if (rc) return rc;
+  for (auto& cls : c->classes) {
+    for (size_t i0 = 0; i0 < cls.size(); i0 += c->B) {
+      std::vector<int> g(cls.begin() + i0, cls.begin() + std::min(cls.size(), i0 + (size_t)c->B));
+      rc = run_batch(c, g);
+      if (rc) return rc;
+    }
+  }
+  return 0;
+}
+
+// ============================================================================================
+// BP + Bethe
+// ============================================================================================
+namespace {
+
+int msg_index(const pepo_ctx* c, int v, int dir, bool outgoing) {
+  const SiteInfo& s = c->sites[v];
+  int e = s.bond_of_dir[dir];
+  const BondInfo& b = c->bonds[e];
+  bool is_v1 = (b.v1 == v);
+  // message 2e: v1 -> v2 ; 2e+1: v2 -> v1
+  int out = is_v1 ? 2 * e : 2 * e + 1;
+  return outgoing ? out : (out ^ 1);
+}
+
+void fill_bp_site(pepo_ctx* c, int v, int cur, BpSite& S) {
+  const SiteInfo& s = c->sites[v];
+  size_t slab = site_live_size(c, v) / 4;
+  int pv = (v == c->center) ? c->obsP : 0;
+  S.T = s.psi + slab * pv;
+  S.first_slot = -1;
+  for (int d = 0; d < 4; d++) {
+    if (s.nbr[d] >= 0) {
+      int e = s.bond_of_dir[d];
+      S.d[d] = c->chi[e]; S.present[d] = 1;
+      if (S.first_slot < 0) S.first_slot = d;
+      S.in[d] = c->msgs[cur] + (size_t)msg_index(c, v, d, false) * c->chi_max;
+      S.out_old[d] = c->msgs[cur] + (size_t)msg_index(c, v, d, true) * c->chi_max;
+      S.out_new[d] = c->msgs[cur ^ 1] + (size_t)msg_index(c, v, d, true) * c->chi_max;
+    } else {
+      S.d[d] = 1; S.present[d] = 0;
+      S.in[d] = c->ones; S.out_old[d] = c->ones; S.out_new[d] = nullptr;
+    }
+  }
+  S.partU = c->partU[v]; S.partD = c->partD[v]; S.partS = c->partS[v];
+  S.vs = c->vs + v;
+}
+
+int bp_sweep(pepo_ctx* c, double damping, int update) {
+  for (int v0 = 0; v0 < c->n_sites; v0 += PEPO_BP_MAXS) {
+    BpBatch bb;
+    bb.count = std::min(PEPO_BP_MAXS, c->n_sites - v0);
+    for (int i = 0; i < bb.count; i++) fill_bp_site(c, v0 + i, c->cur_msg, bb.s[i]);
+    int rc = launch_bp_partial(c->st, bb); if (rc) return rc;
+    rc = launch_bp_finalize(c->st, bb, damping, update, c->delta_bits, c->bp_ints); if (rc) return rc;
+  }
+  return 0;
+}
+
+int bp_init_messages(pepo_ctx* c) {
+  for (int e = 0; e < c->n_bonds; e++) { c->h_chi_msg[2 * e] = c->chi[e]; c->h_chi_msg[2 * e + 1] = c->chi[e]; }
+  if (c->n_bonds) {
+    PEPO_CUDA_OK(cudaMemcpyAsync(c->chi_of_msg, c->h_chi_msg, (size_t)2 * c->n_bonds * 4, cudaMemcpyHostToDevice, c->st));
+    int rc = launch_bp_init(c->st, c->msgs[c->cur_msg], c->chi_of_msg, 2 * c->n_bonds, c->chi_max);
+    if (rc) return rc;
+  }
+  PEPO_CUDA_OK(cudaMemsetAsync(c->bp_ints, 0, 16, c->st));
+  return 0;
+}
+
+}  // namespace
+
+extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
+  if (!c) { set_error("bp_converge: NULL"); return -1; }
+  int sweeps = 0;
+  double delta = INFINITY;
+  int status = 1;
+  for (int phase = 0; phase < 2 && status; phase++) {
+    const double damping = phase == 0 ? 0.0 : c->bp_damping;
+    const int budget = phase == 0 ? c->bp_max_sweeps : c->bp_max_sweeps_damped;
+    if (phase == 1 && !(c->bp_damping > 0.0)) break;
+    int rc = bp_init_messages(c); if (rc) return rc;
+    for (int it = 0; it < budget; it++) {
+      PEPO_CUDA_OK(cudaMemsetAsync(c->delta_bits, 0, 8, c->st));
+      rc = bp_sweep(c, damping, 1); if (rc) return rc;
+      PEPO_CUDA_OK(cudaMemcpyAsync(c->h_delta, c->delta_bits, 8, cudaMemcpyDeviceToHost, c->st));
+      PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
+      c->cur_msg ^= 1;
+      sweeps++;
+      memcpy(&delta, c->h_delta, 8);
+      if (c->n_bonds == 0) delta = 0.0;
+      if (delta < c->bp_tol) { status = 0; break; }
+    }
+  }
+  c->msgs_valid = true;
+  c->stats.last_bp_sweeps = sweeps; c->stats.last_bp_status = status; c->stats.last_bp_delta = delta;
+  if (h_sweeps) *h_sweeps = sweeps;
+  if (h_delta) *h_delta = delta;
+  return status;
+}
+
+extern "C" int pepo_correlation(pepo_ctx* c, double* h_C) {
+  if (!c || !h_C) { set_error("correlation: NULL"); return -1; }
+  if (!c->msgs_valid) { set_error("correlation: no converged messages (call pepo_bp_converge after the last state change)"); return -1; }
+  int rc = bp_sweep(c, 0.0, 0); if (rc) return rc;
+  rc = launch_bethe(c->st, c->vs, c->n_sites, c->msgs[c->cur_msg], c->chi_of_msg, c->n_bonds, c->chi_max,
+                    c->bp_scalars, c->bp_ints + 1);
+  if (rc) return rc;
+  PEPO_CUDA_OK(cudaMemcpyAsync(c->h_scal, c->bp_scalars, 8, cudaMemcpyDeviceToHost, c->st));
+  PEPO_CUDA_OK(cudaMemcpyAsync(c->h_bpints, c->bp_ints, 8, cudaMemcpyDeviceToHost, c->st));
+  PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
+  *h_C = c->h_scal[0];
+  if (c->h_bpints[1] != 0) { set_error("correlation: zero or non-finite Z_e / vs_v"); return -4; }
+  return 0;
+}

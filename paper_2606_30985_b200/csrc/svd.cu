@@ -1,0 +1,264 @@
+// svd.cu - hand-written one-sided (Hestenes) Jacobi SVD of the small bond core, the
+// truncation rule eq. (11) and the Vidal normalisation eq. (12) (PAPER.md:L233-L241,
+// L277-L279, L329-L330; a9), all on the device (the paper does the threshold on the host,
+// L344).  K (r1 x r2) = U diag(s) V^T.
+//
+// One CTA per problem.  Columns of G (= K or K^T, tall) are orthogonalised pairwise in the
+// round-robin ("circle") order, one warp per pair; V accumulates the rotations.  Columns whose
+// squared norm is below 1e-30 ||K||_F^2 are numerically zero (the rank threshold of eq. (11)
+// is 1e-11 s_0, i.e. 1e-22 in squared norm) and are not rotated, so exactly rank-deficient
+// cores (the norm at early layers) converge.
+#include "dense.cuh"
+#include <algorithm>
+
+namespace pepo {
+namespace {
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+__global__ void __launch_bounds__(1024) jacobi_svd_kernel(SvdBatch b, double tol, int max_sweeps) {
+  extern __shared__ double snorm[];     // Nc doubles
+  __shared__ double s_red[32];
+  __shared__ int s_rot;
+  __shared__ double s_ref;
+  const int t = blockIdx.x;
+  const int r1 = b.r1[t], r2 = b.r2[t];
+  const bool tr = r1 < r2;
+  const int M = tr ? r2 : r1, Nc = tr ? r1 : r2;
+  const double* K = b.K[t];
+  const int ldk = b.ldk[t];
+  double* G = b.G[t];
+  double* V = b.V[t];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = blockDim.x >> 5;
+  // load
+  double fro = 0.0;
+  for (int e = tid; e < M * Nc; e += blockDim.x) {
+    int i = e % M, j = e / M;
+    double v = tr ? K[j + (long long)i * ldk] : K[i + (long long)j * ldk];
+    G[e] = v;
+    fro += v * v;
+  }
+  for (int e = tid; e < Nc * Nc; e += blockDim.x) V[e] = ((e % Nc) == (e / Nc)) ? 1.0 : 0.0;
+  fro = warp_sum(fro);
+  if (lane == 0) s_red[warp] = fro;
+  __syncthreads();
+  if (tid == 0) {
+    double s = 0.0;
+    for (int w = 0; w < nw; w++) s += s_red[w];
+    s_ref = s;
+  }
+  __syncthreads();
+  const double noise2 = 1e-30 * s_ref;
+  const int npos = (Nc & 1) ? Nc + 1 : Nc;
+  int sweeps = 0;
+  if (Nc >= 2 && s_ref > 0.0 && isfinite(s_ref)) {
+    for (int sw = 0; sw < max_sweeps; sw++) {
+      if (tid == 0) s_rot = 0;
+      __syncthreads();
+      for (int r = 0; r < npos - 1; r++) {
+        for (int i = warp; i < npos / 2; i += nw) {
+          int a, c;
+          if (i == 0) { a = npos - 1; c = r; }
+          else { a = (r + i) % (npos - 1); c = (r - i + npos - 1) % (npos - 1); }
+          int p = min(a, c), q = max(a, c);
+          if (q >= Nc) continue;
+          double* gp = G + (long long)p * M;
+          double* gq = G + (long long)q * M;
+          double al = 0.0, be = 0.0, ga = 0.0;
+          for (int k = lane; k < M; k += 32) {
+            double x = gp[k], y = gq[k];
+            al += x * x; be += y * y; ga += x * y;
+          }
+          al = warp_sum(al); be = warp_sum(be); ga = warp_sum(ga);
+          if (al < noise2 || be < noise2 || !(al > 0.0) || !(be > 0.0)) continue;
+          if (fabs(ga) <= tol * sqrt(al) * sqrt(be)) continue;
+          double zeta = (be - al) / (2.0 * ga);
+          double tt = ((zeta >= 0.0) ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+          double cs = 1.0 / sqrt(1.0 + tt * tt), sn = cs * tt;
+          for (int k = lane; k < M; k += 32) {
+            double x = gp[k], y = gq[k];
+            gp[k] = cs * x - sn * y;
+            gq[k] = sn * x + cs * y;
+          }
+          double* vp = V + (long long)p * Nc;
+          double* vq = V + (long long)q * Nc;
+          for (int k = lane; k < Nc; k += 32) {
+            double x = vp[k], y = vq[k];
+            vp[k] = cs * x - sn * y;
+            vq[k] = sn * x + cs * y;
+          }
+          if (lane == 0) s_rot = 1;
+        }
+        __syncthreads();
+      }
+      sweeps = sw + 1;
+      int rot = s_rot;
+      __syncthreads();
+      if (!rot) break;
+    }
+  }
+  // singular values = column norms; sort descending (rank by counting, ties by index)
+  for (int j = warp; j < Nc; j += nw) {
+    double s = 0.0;
+    for (int k = lane; k < M; k += 32) { double x = G[(long long)j * M + k]; s += x * x; }
+    s = warp_sum(s);
+    if (lane == 0) snorm[j] = sqrt(s);
+  }
+  __syncthreads();
+  for (int j = tid; j < Nc; j += blockDim.x) {
+    double sj = snorm[j];
+    int rank = 0;
+    for (int l = 0; l < Nc; l++) {
+      double sl = snorm[l];
+      rank += (sl > sj || (sl == sj && l < j)) ? 1 : 0;
+    }
+    b.order[t][rank] = j;
+    b.sv[t][rank] = sj;
+  }
+  if (tid == 0 && b.sweeps[t]) *b.sweeps[t] = sweeps;
+}
+
+__global__ void svd_truncate_kernel(SvdFinishBatch b, int chi_max, double eps_cut) {
+  const int t = blockIdx.x;
+  if (threadIdx.x != 0) return;
+  const int Nc = min(b.r1[t], b.r2[t]);
+  const double* s = b.sv[t];
+  const double s0 = (Nc > 0) ? s[0] : 0.0;
+  int chin = 0;
+  double tot = 0.0, kept = 0.0, gap = 1.0;
+  if (s0 > 0.0 && isfinite(s0)) {
+    int count = 0;
+    for (int i = 0; i < Nc; i++) {
+      tot += s[i] * s[i];
+      if (s[i] >= eps_cut * s0) count++;
+    }
+    chin = min(count, chi_max);
+    for (int i = 0; i < chin; i++) kept += s[i] * s[i];
+    const double nrm = sqrt(kept);
+    for (int i = 0; i < chin; i++) {
+      double l = s[i] / nrm;
+      b.lambda[t][i] = l;
+      double sq = sqrt(l);
+      b.sqrt_l[t][i] = sq;
+      b.isqrt_l[t][i] = 1.0 / sq;
+    }
+    if (count > chi_max && chin < Nc) gap = (s[chin - 1] - s[chin]) / s[chin - 1];
+    double disc = 0.0;
+    for (int i = chin; i < Nc; i++) disc += s[i] * s[i];
+    b.gate_stats[t][0] = disc / tot;
+    b.gate_stats[t][1] = gap;
+  } else {
+    b.gate_stats[t][0] = 0.0;
+    b.gate_stats[t][1] = 1.0;
+  }
+  *b.chi_new[t] = chin;
+}
+
+// Us = U sqrt(S), Vs = V sqrt(S) restricted to the kept chi_new triplets
+__global__ void svd_bridge_kernel(SvdFinishBatch b) {
+  const int t = blockIdx.y;
+  const int r1 = b.r1[t], r2 = b.r2[t];
+  const bool tr = r1 < r2;
+  const int M = tr ? r2 : r1, Nc = tr ? r1 : r2;
+  const int chin = *b.chi_new[t];
+  const double* G = b.G[t];
+  const double* V = b.V[t];
+  const long long tot = (long long)(r1 + r2) * chin;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < tot;
+       e += (long long)gridDim.x * blockDim.x) {
+    int row = (int)(e % (r1 + r2)), c = (int)(e / (r1 + r2));
+    int j = b.order[t][c];
+    double rs = sqrt(b.sv[t][c]);
+    // G columns are (left vectors of the tall problem) * s ; V columns the right vectors
+    if (row < r1) {
+      double v = tr ? V[row + (long long)j * Nc] * rs : G[row + (long long)j * M] / rs;
+      b.Us[t][row + (long long)c * b.ldus[t]] = v;
+    } else {
+      int rr = row - r1;
+      double v = tr ? G[rr + (long long)j * M] / rs : V[rr + (long long)j * Nc] * rs;
+      b.Vs[t][rr + (long long)c * b.ldvs[t]] = v;
+    }
+  }
+}
+
+__global__ void svd_vectors_kernel(const double* G, const double* V, const double* s,
+                                   const int* order, int m, int n, double* U, double* Vout) {
+  const bool tr = m < n;
+  const int M = tr ? n : m, Nc = tr ? m : n;
+  const long long tot = (long long)(m + n) * Nc;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < tot;
+       e += (long long)gridDim.x * blockDim.x) {
+    int row = (int)(e % (m + n)), c = (int)(e / (m + n));
+    int j = order[c];
+    double sv = s[c];
+    double inv = sv > 0.0 ? 1.0 / sv : 0.0;
+    if (row < m) U[row + (long long)c * m] = tr ? V[row + (long long)j * Nc] : G[row + (long long)j * M] * inv;
+    else { int rr = row - m; Vout[rr + (long long)c * n] = tr ? G[rr + (long long)j * M] * inv : V[rr + (long long)j * Nc]; }
+  }
+}
+
+__global__ void set_identity_kernel(double* Q, long long m, int k) {
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < m * k;
+       e += (long long)gridDim.x * blockDim.x) {
+    long long i = e % m; int j = (int)(e / m);
+    Q[e] = (i == j) ? 1.0 : 0.0;
+  }
+}
+
+}  // namespace
+
+int launch_svd_vectors(cudaStream_t st, const double* G, const double* V, const double* s,
+                       const int* order, int m, int n, double* U, double* Vout) {
+  long long w = (long long)(m + n) * std::min(m, n);
+  long long g = std::min<long long>(std::max<long long>((w + 255) / 256, 1), 148 * 4);
+  svd_vectors_kernel<<<(unsigned)g, 256, 0, st>>>(G, V, s, order, m, n, U, Vout);
+  PEPO_COUNT_LAUNCH();
+  PEPO_CUDA_OK(cudaGetLastError());
+  return 0;
+}
+
+int launch_set_identity(cudaStream_t st, double* Q, long long m, int k) {
+  long long w = m * k;
+  long long g = std::min<long long>(std::max<long long>((w + 255) / 256, 1), 148 * 8);
+  set_identity_kernel<<<(unsigned)g, 256, 0, st>>>(Q, m, k);
+  PEPO_COUNT_LAUNCH();
+  PEPO_CUDA_OK(cudaGetLastError());
+  return 0;
+}
+
+int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps) {
+  if (b.count == 0) return 0;
+  int ncmax = 1;
+  for (int t = 0; t < b.count; t++) ncmax = std::max(ncmax, std::min(b.r1[t], b.r2[t]));
+  size_t smem = (size_t)ncmax * sizeof(double);
+  jacobi_svd_kernel<<<b.count, 1024, smem, st>>>(b, tol, max_sweeps);
+  PEPO_COUNT_LAUNCH();
+  PEPO_CUDA_OK(cudaGetLastError());
+  return 0;
+}
+
+int launch_svd_truncate(cudaStream_t st, const SvdFinishBatch& b, int chi_max, double eps_cut) {
+  if (b.count == 0) return 0;
+  svd_truncate_kernel<<<b.count, 32, 0, st>>>(b, chi_max, eps_cut);
+  PEPO_COUNT_LAUNCH();
+  PEPO_CUDA_OK(cudaGetLastError());
+  return 0;
+}
+
+int launch_svd_bridge(cudaStream_t st, const SvdFinishBatch& b, int chi_cap) {
+  if (b.count == 0) return 0;
+  long long w = 0;
+  for (int t = 0; t < b.count; t++) w = std::max(w, (long long)(b.r1[t] + b.r2[t]) * chi_cap);
+  long long g = std::min<long long>(std::max<long long>((w + 255) / 256, 1), 148 * 4);
+  dim3 grid((unsigned)g, b.count);
+  svd_bridge_kernel<<<grid, 256, 0, st>>>(b);
+  PEPO_COUNT_LAUNCH();
+  PEPO_CUDA_OK(cudaGetLastError());
+  return 0;
+}
+
+}  // namespace pepo

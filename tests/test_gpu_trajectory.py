@@ -1,0 +1,141 @@
+"""GPU-vs-oracle parity of the full hot path through the C ABI (-m gpu): C(t) trajectories,
+bond dimensions, Schmidt spectra, BP sweep counts.  Tolerances from BASELINE.json north_star:
+1e-10 absolute on untruncated configs, 1e-6 absolute on truncated configs."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+J, H, DT = 1.0, 0.9, 0.05
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2606_30985_b200 import binding
+    return torch, binding
+
+
+def _run_gpu(B, Lx, Ly, cx, cy, chi_max, steps, tol, damping=0.0, opts=None, **kw):
+    sim = B.Pepo(Lx, Ly, cx, cy, J, H, DT, chi_max, tol, damping, **kw)
+    for k, v in (opts or {}).items():
+        sim.set_option(k, v)
+    out = []
+    for _ in range(steps):
+        sim.trotter_step()
+        status, sweeps, delta = sim.bp_converge()
+        out.append(dict(C=sim.correlation(), status=status, sweeps=sweeps, delta=delta,
+                        chi=sim.bond_dims(), gate_err=sim.stats()["gate_err"]))
+    return sim, out
+
+
+def _compare(out_g, out_o, tol_c, sweeps_slack=0):
+    for t, (g, o) in enumerate(zip(out_g, out_o)):
+        assert g["chi"] == o["chi"], "bond dims differ at step %d: %s vs %s" % (t + 1, g["chi"], o["chi"])
+        assert abs(g["C"] - o["C"]) <= tol_c, "C differs at step %d: %.15g vs %.15g" % (t + 1, g["C"], o["C"])
+        assert g["status"] == o["status"]
+        assert abs(g["sweeps"] - o["sweeps"]) <= sweeps_slack, (t + 1, g["sweeps"], o["sweeps"])
+        assert abs(g["gate_err"] - o["gate_err"]) <= 1e-9 + 1e-6 * o["gate_err"]
+
+
+def test_config1_3x3_chi8(gpu, golden_dense):
+    """BASELINE configs[0]: 3x3, chi_max 8, 10 steps, centre (1,1), BP tol 1e-10 undamped."""
+    torch, B = gpu
+    from oracle import pepo_oracle as po
+    sim, out_g = _run_gpu(B, 3, 3, 1, 1, 8, 10, 1e-10)
+    st, out_o = po.run_trajectory(3, 3, 1, 1, J, H, DT, 8, 10, 1e-10)
+    _compare(out_g, out_o, 1e-10, sweeps_slack=1)
+    # pin P6: within 2e-9 of the dense Trotterised evolution (tests/golden/dense_trotter.txt)
+    dense = golden_dense[(3, 3, 1, 1)]
+    for t in range(10):
+        assert abs(out_g[t]["C"] - dense[t]) < 5e-9
+    # lambda spectra agree bond by bond
+    for e in range(sim.n_bonds):
+        assert np.allclose(sim.get_lambda(e), st.lam[e], rtol=0, atol=1e-10)
+    s = sim.stats()
+    assert s["arena_high_water"] <= s["arena_model_bytes"] * 1.02 + 65536
+    sim.close()
+
+
+@pytest.mark.parametrize("Lx,Ly,cx,cy", [(2, 2, 0, 0), (1, 4, 0, 1), (2, 3, 0, 1), (1, 6, 0, 2)])
+def test_untruncated_small_grids_vs_dense(gpu, golden_dense, Lx, Ly, cx, cy):
+    """Untruncated (chi_max 64 >= any live chi for 8 steps): GPU == oracle to 1e-10 and, on
+    trees (1xN) or for <= 8 steps, == exact dense evolution (pins P1-P4)."""
+    torch, B = gpu
+    from oracle import pepo_oracle as po
+    sim, out_g = _run_gpu(B, Lx, Ly, cx, cy, 64, 8, 1e-12)
+    st, out_o = po.run_trajectory(Lx, Ly, cx, cy, J, H, DT, 64, 8, 1e-12)
+    _compare(out_g, out_o, 1e-10, sweeps_slack=2)
+    dense = golden_dense[(Lx, Ly, cx, cy)]
+    for t in range(8):
+        assert abs(out_g[t]["C"] - dense[t]) < 2e-10, (t, out_g[t]["C"], dense[t])
+    sim.close()
+
+
+def test_closed_forms(gpu):
+    """P5: J=0 -> C(n dt) = cos(2 h n dt), all chi stay 1; h=0 -> C = 1."""
+    torch, B = gpu
+    sim = B.Pepo(3, 3, 1, 1, 0.0, H, DT, 8, 1e-12)
+    for n in range(1, 6):
+        sim.trotter_step(); sim.bp_converge()
+        assert abs(sim.correlation() - np.cos(2 * H * n * DT)) < 1e-13
+        assert set(sim.bond_dims()) == {1}
+    sim.close()
+    sim = B.Pepo(3, 3, 1, 1, J, 0.0, DT, 8, 1e-12)
+    for n in range(1, 4):
+        sim.trotter_step(); sim.bp_converge()
+        assert abs(sim.correlation() - 1.0) < 1e-13
+        assert set(sim.bond_dims()) == {1}
+    sim.close()
+
+
+@pytest.mark.parametrize("chi_max,steps", [(8, 24), (16, 16)])
+def test_config2_twin_4x4(gpu, chi_max, steps):
+    """Reduced-chi twin of BASELINE configs[1] (4x4, centre (1,1), damping 0.5 on
+    non-convergence): heavily truncated trajectory, tolerance 1e-6."""
+    torch, B = gpu
+    from oracle import pepo_oracle as po
+    sim, out_g = _run_gpu(B, 4, 4, 1, 1, chi_max, steps, 1e-10, 0.5)
+    st, out_o = po.run_trajectory(4, 4, 1, 1, J, H, DT, chi_max, steps, 1e-10, 0.5)
+    _compare(out_g, out_o, 1e-6, sweeps_slack=3)
+    sim.close()
+
+
+def test_householder_only_matches_adaptive(gpu):
+    """Cholesky path and forced Householder path give the same trajectory (R9)."""
+    torch, B = gpu
+    sim1, a = _run_gpu(B, 3, 3, 1, 1, 8, 8, 1e-10)
+    sim2, b = _run_gpu(B, 3, 3, 1, 1, 8, 8, 1e-10, opts={"force_householder": 1})
+    for x, y in zip(a, b):
+        assert x["chi"] == y["chi"] and abs(x["C"] - y["C"]) < 1e-11
+    assert sim2.stats()["n_cholesky"] == 0
+    sim1.close(); sim2.close()
+
+
+def test_bp_is_read_only(gpu):
+    """R16: bp_converge / correlation do not change (psi, lambda); skipping them cannot change
+    later results."""
+    torch, B = gpu
+    sim1, a = _run_gpu(B, 3, 3, 1, 1, 8, 5, 1e-10)
+    sim2 = B.Pepo(3, 3, 1, 1, J, H, DT, 8, 1e-10)
+    for _ in range(5):
+        sim2.trotter_step()
+    sim2.bp_converge()
+    assert sim2.correlation() == a[-1]["C"]
+    sim1.close(); sim2.close()
+
+
+def test_init_errors(gpu):
+    torch, B = gpu
+    with pytest.raises(B.PepoError) as e:
+        B.Pepo(3, 3, 5, 1, J, H, DT, 8, 1e-10)
+    assert e.value.code == -1
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.PepoError) as e:
+        B.Pepo(3, 3, 1, 1, J, H, DT, 8, 1e-10, arena=small)
+    assert e.value.code == -2 and "needed" in str(e.value)
+    sim = B.Pepo(2, 2, 0, 0, J, H, DT, 4, 1e-10)
+    with pytest.raises(B.PepoError):
+        sim.correlation()          # no messages yet
+    sim.close()
