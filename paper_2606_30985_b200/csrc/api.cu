@@ -22,7 +22,7 @@ struct Carver {
 
 static int permute_common(const double* d_src, double* d_dst, const int* shape, const int* perm,
                           int rank, const double* const* scale, void* stream) {
-  if (!d_src || !d_dst || !shape || !perm || rank < 1 || rank > PEPO_MAX_RANK) {
+  if (!shape || !perm || rank < 1 || rank > PEPO_MAX_RANK) {
     set_error("permute: bad argument"); return -1;
   }
   bool seen[PEPO_MAX_RANK] = {false};
@@ -31,6 +31,10 @@ static int permute_common(const double* d_src, double* d_dst, const int* shape, 
     seen[perm[j]] = true;
     if (shape[j] < 0) { set_error("permute: negative extent"); return -1; }
   }
+  long long total = 1;
+  for (int j = 0; j < rank; j++) total *= shape[j];
+  if (total == 0) return 0;                 // empty tensor: nothing to move
+  if (!d_src || !d_dst) { set_error("permute: NULL tensor pointer"); return -1; }
   PermuteDesc pd;
   pd.rank = rank; pd.power = 1.0;
   long long s = 1;
