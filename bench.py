@@ -1,0 +1,444 @@
+#!/usr/bin/env python
+"""bench.py - Trotter steps/s of the B200-native PEPO hot path (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload physical|synthetic] [--grid 4] [--chi 60]
+
+One "step" = one pass of the whole hot path:
+pepo_trotter_step (field gate + 4 colour classes of bond gates) + pepo_bp_converge +
+pepo_correlation.  Workload at N=1: BASELINE configs[1], the 4x4 grid at chi_max = 60 with
+every bond saturated.  `--workload physical` (default) reaches that state by running the real
+dynamics from the product operator (untimed preparation) and then times the next K steps;
+`--workload synthetic` loads the seeded random saturated state of SURVEY.md 8(d)(iii).
+Prints ONE JSON line (contract in the task statement).  N > 1: independent replicas, one per
+GPU, no collective on the data path ("replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+J, H, DT = 1.0, 0.9, 0.05
+FP64_NOMINAL_RATIO = 45.0 / 2250.0     # B200 fp64 tensor / bf16 tensor, blackwell guide table
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="physical", choices=["physical", "synthetic"])
+    ap.add_argument("--grid", type=int, default=4)
+    ap.add_argument("--cx", type=int, default=1)
+    ap.add_argument("--cy", type=int, default=1)
+    ap.add_argument("--chi", type=int, default=60)
+    ap.add_argument("--prep-max", type=int, default=60, help="max untimed preparation steps")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--bp-tol", type=float, default=1e-10)
+    ap.add_argument("--bp-damping", type=float, default=0.5)
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks: sample nvidia-smi DURING the timed region
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for k, nm in enumerate(names):
+                if len(r) > 3 + k and r[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return {"hbm_gbs": p["hbm_gbs"], "bf16_tflops": p["bf16_tflops"],
+                "bf16_tflops_sustained": p.get("bf16_tflops_sustained", p["bf16_tflops"]), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+# ---------------------------------------------------------------------------------------------
+# workload preparation (GPU arm)
+# ---------------------------------------------------------------------------------------------
+def load_synthetic(sim, L, chi):
+    from paper_2606_30985_b200 import inputs
+    chis, psi, lam = inputs.synthetic_state(L, L, chi)
+    sim.set_bond_dims(chis)
+    for e, l in enumerate(lam):
+        sim.set_lambda(e, l)
+    for v, t in psi.items():
+        sim.set_site(v % L, v // L, t)
+    return chis, psi, lam
+
+
+def prepare(sim, args):
+    """Bring the context to the saturated state the metric is quoted on.  Returns a dict that
+    describes what was done (untimed)."""
+    L, chi = args.grid, args.chi
+    if args.workload == "synthetic":
+        load_synthetic(sim, L, chi)
+        return {"prep": "synthetic saturated state (SURVEY 8(d)(iii))"}
+    n = 0
+    while n < args.prep_max and min(sim.bond_dims()) < chi:
+        sim.trotter_step()
+        n += 1
+    if min(sim.bond_dims()) < chi:
+        raise RuntimeError("bonds did not saturate in %d preparation steps: %s" % (n, sim.bond_dims()))
+    return {"prep": "%d physical Trotter steps from the product operator (all bonds = %d)" % (n, chi),
+            "prep_steps": n}
+
+
+def one_step(sim):
+    sim.trotter_step()
+    status, sweeps, delta = sim.bp_converge()
+    c = sim.correlation()
+    return c, status, sweeps
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_30985_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    torch.cuda.set_device(dev)
+    L, chi = args.grid, args.chi
+    sim = B.Pepo(L, L, args.cx, args.cy, J, H, DT, chi, args.bp_tol, args.bp_damping, device=str(dev))
+    info = prepare(sim, args)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing ---------------------------------------------------------------
+    for _ in range(args.warmup):
+        one_step(sim)
+    sim.set_option("profile", 2)
+    launches0 = sim.stats()["kernel_launches"]
+    sampler = ClockSampler(local)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_trot, sweeps_tot, jac = 0.0, 0, 0
+    ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    c_last = None
+    for _ in range(args.steps):
+        ea.record()
+        sim.trotter_step()
+        eb.record()
+        status, sweeps, delta = sim.bp_converge()
+        c_last = sim.correlation()
+        t_trot += ea.elapsed_time(eb)        # bp_converge synchronised the stream
+        sweeps_tot += sweeps
+        jac += sim.stats()["jacobi_sweeps"]
+    e1.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms = e0.elapsed_time(e1)
+    prof = sim.profile()
+    sim.set_option("profile", 0)
+    launches = sim.stats()["kernel_launches"] - launches0
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    stats = sim.stats()
+
+    # ---- end-to-end: host buffers in, host scalar out, copies inside the timed region ----------
+    e2e = None
+    if not args.no_e2e:
+        host = {}
+        for y in range(L):
+            for x in range(L):
+                a = sim.get_site(x, y)
+                p = torch.empty(a.size, dtype=torch.float64).pin_memory()
+                p.numpy()[:] = a
+                host[(x, y)] = p
+        lam = [sim.get_lambda(e) for e in range(sim.n_bonds)]
+        chis = sim.bond_dims()
+        h2d = sum(p.numel() * 8 for p in host.values()) + sum(l.size * 8 for l in lam)
+
+        def e2e_step():
+            sim.set_bond_dims(chis)
+            for e, l in enumerate(lam):
+                sim.set_lambda(e, l)
+            for (x, y), p in host.items():
+                sim.set_site(x, y, p.numpy())
+            return one_step(sim)
+
+        for _ in range(max(1, args.warmup // 2)):
+            e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            e2e_step()
+        barrier()
+        dt_e2e = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt_e2e], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt_e2e = float(t.item())
+        e2e = {"value": world * args.steps / dt_e2e, "unit": "Trotter steps/s",
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": 8 + 8 + 4 * sim.n_bonds,
+               "note": "state uploaded from pinned host memory every step, C(t) read back"}
+
+    peaks = measured_peaks()
+    # dominant kernel class by accumulated device time
+    dom = max(prof, key=lambda k: prof[k]["ms"])
+    fp64_peak = peaks["bf16_tflops_sustained"] * FP64_NOMINAL_RATIO
+    per = {}
+    for k, v in prof.items():
+        if v["count"] == 0:
+            continue
+        per[k] = {"ms_per_step": v["ms"] / args.steps, "share": v["ms"] / max(ms, 1e-9),
+                  "launch_groups_per_step": v["count"] / args.steps}
+        if v["flops"] > 0 and v["ms"] > 0:
+            per[k]["tflops"] = v["flops"] / v["ms"] * 1e-9
+        if v["bytes"] > 0 and v["ms"] > 0:
+            per[k]["gbs"] = v["bytes"] / v["ms"] * 1e-6
+    d = prof[dom]
+    if dom in ("gram", "apply_gemm", "small_gemm"):
+        ach = d["flops"] / d["ms"] * 1e-9
+        roof = {"kernel": dom, "bound": "tensor", "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s",
+                "frac": ach / fp64_peak, "traffic": None,
+                "peak_source": "%s bf16 sustained %.1f TF/s x nominal fp64/bf16 ratio 45/2250 (of %s); DMMA "
+                               "microbenchmark on this pool: 36.9 TF/s" % (peaks["source"], peaks["bf16_tflops_sustained"], peaks["source"])}
+    elif dom in ("permute", "field", "bp"):
+        ach = d["bytes"] / d["ms"] * 1e-6
+        roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": ach / peaks["hbm_gbs"], "traffic": None, "peak_source": "hbm_gbs of " + peaks["source"]}
+    else:
+        # latency-bound small dense kernel (Jacobi SVD / Cholesky): no flop or byte roofline applies;
+        # report against the fp64 ALU peak (148 SMs x 64 FMA/clk x 2 x 1.965 GHz)
+        alu_peak = 148 * 64 * 2 * 1.965e9 * 1e-12
+        roof = {"kernel": dom, "bound": "alu", "achieved": None, "peak": alu_peak, "unit": "TFLOP/s",
+                "frac": None, "traffic": None,
+                "peak_source": "fp64 DFMA peak from unit counts (latency-bound kernel: see profiles/)"}
+    line = {
+        "metric": "Trotter steps/sec (4x4 chi=60 fp64)" if (L, chi) == (4, 60) else "Trotter steps/sec (%dx%d chi=%d fp64)" % (L, L, chi),
+        "value": world * args.steps / (ms * 1e-3), "unit": "Trotter steps/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE configs[1]: %dx%d open grid, TFIM J=1 h=0.9 dt=0.05, Z at (%d,%d), chi_max=%d, "
+                               "all bonds saturated; step = trotter_step + bp_converge(tol %g, damping %g) + correlation"
+                               % (L, L, args.cx, args.cy, chi, args.bp_tol, args.bp_damping),
+                   "state": info["prep"], "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": "working set per step (%.1f GB of site tensors) exceeds the 126 MB L2" % (stats["arena_high_water"] / 1e9)},
+        "trotter_only_steps_per_s": world * args.steps / (t_trot * 1e-3),
+        "trotter_ms_per_step": t_trot / args.steps,
+        "bp_sweeps_per_step": sweeps_tot / args.steps, "jacobi_sweeps_per_step": jac / args.steps,
+        "last_C": c_last, "gate_err_last_step": stats["gate_err"],
+        "qr": {"cholesky": stats["n_cholesky"], "householder": stats["n_householder"], "chol_rejected": stats["n_chol_failed"]},
+        "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "kernels": per,
+        "arena": {"high_water_bytes": stats["arena_high_water"], "model_bytes": stats["arena_model_bytes"],
+                  "inflight_gates": stats["max_inflight_gates"]},
+        "e2e": e2e,
+    }
+    sim.close()
+    return line, rank, world
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle arm (cpu_baseline leg and --impl reference): the oracle as it stands, timed on the
+# host cores on a bounded sample of the same workload
+# ---------------------------------------------------------------------------------------------
+def oracle_state(L, chi, cx, cy):
+    """Oracle PEPOState holding the seeded synthetic saturated state (same generator as the GPU
+    arm's --workload synthetic)."""
+    import numpy as np
+    from oracle import pepo_oracle as po
+    from paper_2606_30985_b200 import inputs
+    st = po.PEPOState(L, L, cx, cy, J, H, DT, chi)
+    chis, psi, lam = inputs.synthetic_state(L, L, chi)
+    for v in range(L * L):
+        x, y = v % L, v // L
+        dims = [chis[inputs.bond_id(L, L, x, y, d)] for d in inputs.site_legs(L, L, x, y)] + [4]
+        st.psi[v] = np.asarray(psi[v]).reshape(dims, order="F").copy()
+    st.lam = [np.asarray(l) for l in lam]
+    return st
+
+
+def bond_classes(L):
+    """Group the bonds of the LxL grid by the degrees of their two sites; returns
+    {(deg1, deg2): [bond ids]} - gates of one class cost the same."""
+    from oracle import pepo_oracle as po
+    lat = po.Lattice(L, L)
+    out = {}
+    for e in range(lat.n_bonds):
+        v1, _, v2, _ = lat.bond_sites(e)
+        key = tuple(sorted((len(lat.legs(v1)), len(lat.legs(v2)))))
+        out.setdefault(key, []).append(e)
+    return out
+
+
+def gate_flops(chi, key):
+    """6 m n^2 per site (Householder QR + explicit Q + Q M), m = chi^(deg-1), n = 4 chi."""
+    return sum(6.0 * chi ** (d - 1) * (4 * chi) ** 2 for d in key)
+
+
+def oracle_sample(st, L, chi, budget_s):
+    """Time one oracle bond gate per bond class, cheapest class first, while the projected
+    total stays within budget_s; classes not timed are extrapolated by the flop model from the
+    most expensive timed class.  Returns (seconds per full Trotter step, description)."""
+    classes = bond_classes(L)
+    order = sorted(classes, key=lambda k: gate_flops(chi, k))
+    timed, spent = {}, 0.0
+    t0 = time.perf_counter()
+    st.apply_field_gate()
+    t_field = time.perf_counter() - t0
+    spent += t_field
+    for key in order:
+        if timed:
+            last = max(timed, key=lambda k: gate_flops(chi, k))
+            projected = timed[last] * gate_flops(chi, key) / gate_flops(chi, last)
+            if spent + projected > budget_s:
+                break
+        e = classes[key][0]
+        t0 = time.perf_counter()
+        st.apply_bond_gate(e)
+        timed[key] = time.perf_counter() - t0
+        spent += timed[key]
+    ref = max(timed, key=lambda k: gate_flops(chi, k))
+    total = t_field
+    for key, bonds in classes.items():
+        t = timed.get(key, timed[ref] * gate_flops(chi, key) / gate_flops(chi, ref))
+        total += t * len(bonds)
+    desc = ("field gate on all sites + one oracle bond gate for each of the bond classes %s of the %dx%d chi=%d "
+            "synthetic saturated state (%.1f s of CPU work); other classes %s extrapolated by 6mn^2; "
+            "BP/Bethe not included" % (sorted(timed), L, L, chi, spent,
+                                       sorted(k for k in classes if k not in timed)))
+    return total, desc, spent
+
+
+def host_threads():
+    try:
+        import threadpoolctl
+        n = max((p.get("num_threads", 1) for p in threadpoolctl.threadpool_info()), default=1)
+        return int(n)
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_cpu_baseline(args, budget_s=25.0):
+    import numpy  # noqa: F401  (loads the BLAS whose threads are counted)
+    st = oracle_state(args.grid, args.chi, args.cx, args.cy)
+    total, desc, spent = oracle_sample(st, args.grid, args.chi, budget_s)
+    return {"value": 1.0 / total, "unit": "Trotter steps/s", "cores": host_threads(), "kind": "oracle",
+            "sample": desc}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, K timed 'steps' after W warm-ups, each
+    step a bounded sample (see oracle_sample) sized so that the run ends within minutes."""
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank != 0:
+        return None, rank, world
+    L, chi = args.grid, args.chi
+    n_runs = max(1, args.steps + args.warmup)
+    budget = max(2.0, 150.0 / n_runs)
+    st = oracle_state(L, chi, args.cx, args.cy)
+    totals, desc = [], ""
+    for i in range(n_runs):
+        total, desc, spent = oracle_sample(st, L, chi, budget)
+        if i >= args.warmup:
+            totals.append(total)
+    mean = sum(totals) / len(totals)
+    val = 1.0 / mean
+    line = {
+        "impl": "reference",
+        "metric": "Trotter steps/sec (4x4 chi=60 fp64)" if (L, chi) == (4, 60) else "Trotter steps/sec (%dx%d chi=%d fp64)" % (L, L, chi),
+        "value": val, "unit": "Trotter steps/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": mean * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": "BASELINE configs[1]: %dx%d open grid, TFIM J=1 h=0.9 dt=0.05, Z at (%d,%d), chi_max=%d, "
+                               "all bonds saturated (seeded synthetic state); Trotter step only" % (L, L, args.cx, args.cy, chi)},
+        "cpu_baseline": {"value": val, "unit": "Trotter steps/s", "cores": host_threads(), "kind": "oracle", "sample": desc},
+        "e2e": {"value": val, "unit": "Trotter steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    return line, rank, world
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        line, rank, world = run_reference(args)
+        if line is not None:
+            print(json.dumps(line), flush=True)
+        return 0
+    line, rank, world = run_ours(args)
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = run_cpu_baseline(args)
+        else:
+            line["cpu_baseline"] = None
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -108,6 +108,14 @@ int pepo_bp_converge(pepo_ctx* ctx, int* h_sweeps, double* h_delta);
 int pepo_correlation(pepo_ctx* ctx, double* h_C);
 
 int pepo_get_stats(pepo_ctx* ctx, pepo_stats* h_stats);
+/* In-situ per-kernel-class timing (option "profile": 1 on, 0 off, 2 on + reset): CUDA-event
+ * pairs on the context stream around each launch group, summed per class.  Classes, in order:
+ * 0 permute(+absorb/deabsorb), 1 Gram, 2 reconstruction GEMM, 3 small core GEMMs, 4 Cholesky +
+ * triangular inverse, 5 Householder, 6 gate dressing, 7 Jacobi SVD + truncation, 8 field gate,
+ * 9 BP sweep.  Fills the first n entries of each non-NULL array with accumulated milliseconds,
+ * algorithmic flops, algorithmic bytes and launch-group counts; returns the class count. */
+int pepo_get_profile(pepo_ctx* ctx, int n, double* h_ms, double* h_flops, double* h_bytes,
+                     long long* h_count);
 int pepo_n_bonds(pepo_ctx* ctx);
 int pepo_get_bond_dims(pepo_ctx* ctx, int* h_chi /* n_bonds */);
 /* Set all live bond dimensions (1..chi_max); site tensors and lambdas become undefined until

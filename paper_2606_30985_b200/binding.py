@@ -55,6 +55,7 @@ def _load():
         "pepo_bp_converge": (i, [vp, ip, C.POINTER(d)]),
         "pepo_correlation": (i, [vp, C.POINTER(d)]),
         "pepo_get_stats": (i, [vp, C.POINTER(PepoStats)]),
+        "pepo_get_profile": (i, [vp, i, C.POINTER(d), C.POINTER(d), C.POINTER(d), C.POINTER(ll)]),
         "pepo_n_bonds": (i, [vp]),
         "pepo_get_bond_dims": (i, [vp, ip]),
         "pepo_set_bond_dims": (i, [vp, ip]),
@@ -173,6 +174,16 @@ class Pepo:
         s = PepoStats()
         _check(_lib.pepo_get_stats(self._h, C.byref(s)))
         return {k: getattr(s, k) for k, _ in PepoStats._fields_}
+
+    PROFILE_CLASSES = ("permute", "gram", "apply_gemm", "small_gemm", "cholesky", "householder",
+                       "dress", "svd", "field", "bp")
+
+    def profile(self):
+        n = len(self.PROFILE_CLASSES)
+        ms, fl, by = (C.c_double * n)(), (C.c_double * n)(), (C.c_double * n)()
+        cnt = (C.c_longlong * n)()
+        _check(_lib.pepo_get_profile(self._h, n, ms, fl, by, cnt))
+        return {k: dict(ms=ms[i], flops=fl[i], bytes=by[i], count=cnt[i]) for i, k in enumerate(self.PROFILE_CLASSES)}
 
     def bond_dims(self):
         arr = (C.c_int * max(self.n_bonds, 1))()

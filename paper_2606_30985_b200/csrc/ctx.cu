@@ -186,6 +186,19 @@ struct Arena {
   }
 };
 
+// ---- optional in-situ profiling: CUDA-event pairs around every launch group, accumulated per
+// category at the existing host sync points (option "profile").  Events are created at init.
+enum ProfCat { PC_PERMUTE = 0, PC_GRAM, PC_APPLY, PC_SMALL_GEMM, PC_CHOL, PC_HOUSEHOLDER, PC_DRESS,
+               PC_SVD, PC_FIELD, PC_BP, PC_COUNT };
+struct Prof {
+  bool on = false;
+  std::vector<cudaEvent_t> ev;
+  std::vector<int> cat;          // category of pair i
+  size_t used = 0;               // pairs in flight
+  double ms[PC_COUNT] = {0}, flops[PC_COUNT] = {0}, bytes[PC_COUNT] = {0};
+  long long cnt[PC_COUNT] = {0};
+};
+
 }  // namespace pepo
 
 using namespace pepo;
@@ -228,7 +241,36 @@ struct pepo_ctx {
   long long launches0 = 0;
   pepo_stats stats;
   size_t model_bytes = 0;
+  Prof prof;
 };
+
+namespace {
+void prof_flush(pepo_ctx* c) {        // call only after a stream synchronize
+  Prof& P = c->prof;
+  for (size_t i = 0; i < P.used; i++) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, P.ev[2 * i], P.ev[2 * i + 1]) == cudaSuccess) P.ms[P.cat[i]] += ms;
+  }
+  P.used = 0;
+}
+struct ProfScope {
+  pepo_ctx* c; bool active;
+  ProfScope(pepo_ctx* c_, int cat, double flops, double bytes) : c(c_), active(false) {
+    Prof& P = c->prof;
+    if (!P.on) return;
+    if (2 * (P.used + 1) > P.ev.size()) { cudaStreamSynchronize(c->st); prof_flush(c); }
+    P.cat[P.used] = cat; P.cnt[cat]++; P.flops[cat] += flops; P.bytes[cat] += bytes;
+    cudaEventRecord(P.ev[2 * P.used], c->st);
+    active = true;
+  }
+  ~ProfScope() {
+    if (!active) return;
+    Prof& P = c->prof;
+    cudaEventRecord(P.ev[2 * P.used + 1], c->st);
+    P.used++;
+  }
+};
+}  // namespace
 
 namespace {
 
@@ -559,6 +601,16 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "force_householder") c->force_hh = (int)v;
   else if (k == "jacobi_tol") c->jacobi_tol = v;
   else if (k == "jacobi_max_sweeps") c->jacobi_max_sweeps = (int)v;
+  else if (k == "profile") {
+    Prof& P = c->prof;
+    if (v != 0.0 && P.ev.empty()) {
+      P.ev.resize(2 * 4096); P.cat.assign(4096, 0);
+      for (auto& e : P.ev) if (cudaEventCreate(&e) != cudaSuccess) { set_error("profile: cudaEventCreate failed"); return -3; }
+    }
+    cudaStreamSynchronize(c->st); prof_flush(c);
+    P.on = (v != 0.0);
+    if (v == 2.0) for (int i = 0; i < PC_COUNT; i++) { P.ms[i] = P.flops[i] = P.bytes[i] = 0; P.cnt[i] = 0; }
+  }
   else if (k == "bp_tol") c->bp_tol = v;
   else if (k == "bp_damping") c->bp_damping = v;
   else { set_error("set_option: unknown key %s", key); return -1; }
@@ -658,6 +710,8 @@ extern "C" int pepo_apply_field(pepo_ctx* c) {
     }
     memcpy(fb.G, c->G1, sizeof(fb.G));
     fb.row_mask = c->f_row_mask; fb.col_mask = c->f_col_mask;
+    double fbytes = 0; for (int i = 0; i < fb.count; i++) fbytes += 8.0 * fb.slab[i] * 2 * __builtin_popcount(fb.row_mask);
+    ProfScope ps(c, PC_FIELD, 0, fbytes);
     int rc = launch_field_gate(c->st, fb);
     if (rc) return rc;
   }
@@ -723,6 +777,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       }
       pd.perm[t.n_env] = t.cut_leg; pd.dst_stride[t.n_env] = t.ld;
       pd.perm[t.n_env + 1] = s.nlegs; pd.dst_stride[t.n_env + 1] = t.ld * t.chi_c;
+      ProfScope ps(c, PC_PERMUTE, 0, 16.0 * t.m * t.n);
       int rc = launch_permute(st, s.psi, W.cv, pd);
       if (rc) return rc;
     }
@@ -740,6 +795,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       GemmProb gp;
       gp.A = W.cv; gp.B = W.cv; gp.C = W.C; gp.lda = t.ld; gp.ldb = t.ld; gp.ldc = t.n;
       gp.M = t.n; gp.N = t.n; gp.K = (int)t.m;
+      ProfScope ps(c, PC_GRAM, (double)t.m * t.n * (t.n + 1), 8.0 * t.m * t.n);
       int rc = launch_dgemm(st, 1, 0, gp, ks, kc, W.part, true);
       if (rc) return rc;
       if (ks > 1) rc = launch_gram_reduce(st, W.part, ks, t.n, W.C, t.n);
@@ -755,10 +811,12 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       pb.A[p] = W.Rx; pb.ld[p] = t.N; pb.m[p] = t.N; pb.n[p] = t.N; infos[p] = W.info;
     }
     if (db.count) {
-      int rc = launch_dress_gram(st, db, gt); if (rc) return rc;
-      rc = launch_potrf(st, pb, infos, c->chol_tau); if (rc) return rc;
+      int rc;
+      { ProfScope ps(c, PC_DRESS, 0, 0); rc = launch_dress_gram(st, db, gt); if (rc) return rc; }
+      { ProfScope ps(c, PC_CHOL, 0, 0); rc = launch_potrf(st, pb, infos, c->chol_tau); if (rc) return rc; }
       PEPO_CUDA_OK(cudaMemcpyAsync(c->h_ints, c->lane_ints, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
       PEPO_CUDA_OK(cudaStreamSynchronize(st));
+      prof_flush(c);
       for (auto& t : T) {
         if (!t.chol) continue;
         int info = c->h_ints[4 * t.lane + 2 + t.slot];
@@ -798,8 +856,9 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       }
     }
     int rc = 0;
-    if (zl.count) { rc = launch_zero_lower(st, zl); if (rc) return rc; rc = launch_trtri(st, zl, ti); if (rc) return rc; }
+    if (zl.count) { ProfScope ps(c, PC_CHOL, 0, 0); rc = launch_zero_lower(st, zl); if (rc) return rc; rc = launch_trtri(st, zl, ti); if (rc) return rc; }
     if (h1.count) {
+      ProfScope ps(c, PC_HOUSEHOLDER, 0, 0);
       rc = launch_hh_factor(st, h1); if (rc) return rc;
       rc = launch_hh_extract_r(st, h1, Rout1, ldr1); if (rc) return rc;
       rc = launch_dress_R(st, dr, gt); if (rc) return rc;
@@ -834,13 +893,18 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       GemmProb gp;
       gp.A = L.Ks; gp.lda = t1.r; gp.B = L.s[1].Rx; gp.ldb = t2.r; gp.C = L.K; gp.ldc = t1.r;
       gp.M = t1.r; gp.N = t2.r; gp.K = t1.N;
+      ProfScope ps(c, PC_SMALL_GEMM, 2.0 * t1.r * t2.r * t1.N, 0);
       rc = launch_dgemm(st, 0, 1, gp, 1, 0, nullptr, false); if (rc) return rc;
     }
-    rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps); if (rc) return rc;
-    rc = launch_svd_truncate(st, fb, c->chi_max, c->eps_cut); if (rc) return rc;
+    {
+      ProfScope ps(c, PC_SVD, 0, 0);
+      rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps); if (rc) return rc;
+      rc = launch_svd_truncate(st, fb, c->chi_max, c->eps_cut); if (rc) return rc;
+    }
     PEPO_CUDA_OK(cudaMemcpyAsync(c->h_ints, c->lane_ints, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
     PEPO_CUDA_OK(cudaMemcpyAsync(c->h_dbls, c->lane_dbls, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
     PEPO_CUDA_OK(cudaStreamSynchronize(st));
+    prof_flush(c);
     int chi_cap = 1;
     for (int g = 0; g < ng; g++) {
       int cn = c->h_ints[4 * g];
@@ -872,7 +936,8 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
         GemmProb gp;
         gp.A = W.Rxinv; gp.lda = t.N; gp.B = UV; gp.ldb = t.r; gp.C = W.T; gp.ldc = t.N;
         gp.M = t.N; gp.N = t.chi_new; gp.K = t.N;
-        rc = launch_dgemm(st, 0, 0, gp, 1, 0, nullptr, false); if (rc) return rc;
+        { ProfScope ps(c, PC_SMALL_GEMM, 2.0 * t.N * t.N * t.chi_new, 0);
+          rc = launch_dgemm(st, 0, 0, gp, 1, 0, nullptr, false); if (rc) return rc; }
         int q = bw.count++;
         bw.in[q] = W.T; bw.out[q] = W.W; bw.chi[q] = t.chi_c; bw.k[q] = t.chi_new; bw.site[q] = t.site_idx;
         bw.ld_in[q] = t.N; bw.ld_out[q] = t.n; cn_w[q] = L.ints;
@@ -891,18 +956,20 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       }
     }
     if (bw.count) {
-      rc = launch_build_W(st, bw, gt, cn_w); if (rc) return rc;
+      { ProfScope ps(c, PC_DRESS, 0, 0); rc = launch_build_W(st, bw, gt, cn_w); if (rc) return rc; }
       for (auto& t : T) {
         if (!t.chol) continue;
         SiteWs& W = c->lanes[t.lane].s[t.slot];
         GemmProb gp;
         gp.A = W.cv; gp.lda = t.ld; gp.B = W.W; gp.ldb = t.n; gp.C = W.out; gp.ldc = t.ld;
         gp.M = t.m; gp.N = 4 * t.chi_new; gp.K = t.n;
+        ProfScope ps(c, PC_APPLY, 2.0 * t.m * t.n * 4 * t.chi_new, 8.0 * t.m * (t.n + 4 * t.chi_new));
         rc = launch_dgemm(st, 0, 0, gp, 1, 0, nullptr, false); if (rc) return rc;
       }
     }
     if (a2.count) {
       // pad-copy through the reshuffle kernel's sibling: use launch_copy_pad
+      ProfScope ps(c, PC_HOUSEHOLDER, 0, 0);
       rc = launch_copy_pad(st, padsrc, a2); if (rc) return rc;
       rc = launch_hh_apply_q(st, a2); if (rc) return rc;
       rc = launch_reshuffle_M(st, rs, cn_r, mrows); if (rc) return rc;
@@ -937,6 +1004,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       for (int q = 0; q <= s.nlegs; q++) if (src_leg[q] == j) sd = q;
       pd.perm[j] = sd; pd.dst_stride[j] = dst_stride_of_leg[j];
     }
+    ProfScope ps(c, PC_PERMUTE, 0, 16.0 * t.m * 4 * t.chi_new);
     int rc = launch_permute(st, W.out, s.psi, pd);
     if (rc) return rc;
   }
@@ -1011,6 +1079,8 @@ int bp_sweep(pepo_ctx* c, double damping, int update) {
     BpBatch bb;
     bb.count = std::min(PEPO_BP_MAXS, c->n_sites - v0);
     for (int i = 0; i < bb.count; i++) fill_bp_site(c, v0 + i, c->cur_msg, bb.s[i]);
+    double bbytes = 0; for (int i = 0; i < bb.count; i++) bbytes += 8.0 * bb.s[i].d[0] * bb.s[i].d[1] * bb.s[i].d[2] * bb.s[i].d[3];
+    ProfScope ps(c, PC_BP, 0, bbytes);
     int rc = launch_bp_partial(c->st, bb); if (rc) return rc;
     rc = launch_bp_finalize(c->st, bb, damping, update, c->delta_bits, c->bp_ints); if (rc) return rc;
   }
@@ -1045,6 +1115,7 @@ extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
       rc = bp_sweep(c, damping, 1); if (rc) return rc;
       PEPO_CUDA_OK(cudaMemcpyAsync(c->h_delta, c->delta_bits, 8, cudaMemcpyDeviceToHost, c->st));
       PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
+      prof_flush(c);
       c->cur_msg ^= 1;
       sweeps++;
       memcpy(&delta, c->h_delta, 8);
@@ -1072,4 +1143,18 @@ extern "C" int pepo_correlation(pepo_ctx* c, double* h_C) {
   *h_C = c->h_scal[0];
   if (c->h_bpints[1] != 0) { set_error("correlation: zero or non-finite Z_e / vs_v"); return -4; }
   return 0;
+}
+
+extern "C" int pepo_get_profile(pepo_ctx* c, int n, double* h_ms, double* h_flops, double* h_bytes,
+                                long long* h_count) {
+  if (!c || n < 0) { set_error("get_profile: bad argument"); return -1; }
+  cudaStreamSynchronize(c->st);
+  prof_flush(c);
+  for (int i = 0; i < n && i < PC_COUNT; i++) {
+    if (h_ms) h_ms[i] = c->prof.ms[i];
+    if (h_flops) h_flops[i] = c->prof.flops[i];
+    if (h_bytes) h_bytes[i] = c->prof.bytes[i];
+    if (h_count) h_count[i] = c->prof.cnt[i];
+  }
+  return PC_COUNT;
 }
