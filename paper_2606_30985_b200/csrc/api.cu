@@ -132,7 +132,7 @@ extern "C" int pepo_householder_qr(const double* d_A, long long m, int n, long l
 extern "C" size_t pepo_svd_ws_bytes(int m, int n) {
   if (m < 1 || n < 1) return 0;
   size_t M = std::max(m, n), Nc = std::min(m, n);
-  return al(M * Nc * 8) + al(Nc * Nc * 8) + al(Nc * 8) + al(Nc * 4) + 4 * 256 + al(16) + al(3 * Nc * 8) + al(16);
+  return al(M * Nc * 8) + al((Nc * Nc + Nc) * 8) + al(Nc * 8) + al(Nc * 4) + 4 * 256 + al(16) + al(3 * Nc * 8) + al(16);
 }
 extern "C" int pepo_svd_jacobi(const double* d_A, int m, int n, int lda, double* d_U, double* d_s,
                                double* d_V, int* d_sweeps, void* d_ws, size_t ws_bytes,
@@ -143,7 +143,7 @@ extern "C" int pepo_svd_jacobi(const double* d_A, int m, int n, int lda, double*
   const int Nc = std::min(m, n), M = std::max(m, n);
   Carver cv{(char*)d_ws, ws_bytes};
   double* G = (double*)cv.take((size_t)M * Nc * 8);
-  double* V = (double*)cv.take((size_t)Nc * Nc * 8);
+  double* V = (double*)cv.take(((size_t)Nc * Nc + Nc) * 8);
   int* order = (int*)cv.take((size_t)Nc * 4);
   int* ints = (int*)cv.take(16);
   double* lam3 = (double*)cv.take((size_t)3 * Nc * 8);

@@ -389,7 +389,7 @@ int layout(pepo_ctx* c) {
     L.K = (double*)A.take(Nmax * Nmax * 8);
     L.Ks = (double*)A.take(Nmax * Nmax * 8);
     L.G = (double*)A.take(Nmax * Nmax * 8);
-    L.V = (double*)A.take(Nmax * Nmax * 8);
+    L.V = (double*)A.take((Nmax * Nmax + Nmax) * 8);     // + Nmax: unsorted norms scratch
     L.sv = (double*)A.take(Nmax * 8);
     L.Us = (double*)A.take(Nmax * chi * 8);
     L.Vs = (double*)A.take(Nmax * chi * 8);

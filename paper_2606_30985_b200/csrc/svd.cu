@@ -10,6 +10,8 @@
 // cores (the norm at early layers) converge.
 #include "dense.cuh"
 #include <algorithm>
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
 
 namespace pepo {
 namespace {
@@ -122,6 +124,190 @@ __global__ void __launch_bounds__(1024) jacobi_svd_kernel(SvdBatch b, double tol
   if (tid == 0 && b.sweeps[t]) *b.sweeps[t] = sweeps;
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Cluster version: the columns of [G; V] (length LEN = M + Nc) live in the shared memory of a
+// thread-block cluster of CS CTAs, two blocks of `bs` columns per CTA (2 CS blocks in all).
+// One sweep = all pairs inside every block, then 2 CS - 1 super-rounds in which every CTA
+// orthogonalises its two resident blocks against each other (bs local rounds of bs disjoint
+// pairs, one warp per pair, __syncthreads only) and the blocks then move one position along
+// the round-robin circle through distributed shared memory (staged in registers between two
+// cluster barriers).  No global-memory traffic inside the iteration.
+// ---------------------------------------------------------------------------------------------
+constexpr int JC_THREADS = 1024;
+constexpr int JC_STAGE = 26;            // doubles staged per thread during a block exchange
+constexpr size_t JC_SMEM_CAP = 200 * 1024;
+
+__device__ __forceinline__ bool rotate_pair(double* cp, double* cq, int M, int LEN, double tol,
+                                            double noise2, int lane) {
+  double al = 0.0, be = 0.0, ga = 0.0;
+  for (int k = lane; k < M; k += 32) {
+    double x = cp[k], y = cq[k];
+    al += x * x; be += y * y; ga += x * y;
+  }
+  al = warp_sum(al); be = warp_sum(be); ga = warp_sum(ga);
+  if (al < noise2 || be < noise2 || !(al > 0.0) || !(be > 0.0)) return false;
+  if (fabs(ga) <= tol * sqrt(al) * sqrt(be)) return false;
+  double zeta = (be - al) / (2.0 * ga);
+  double tt = ((zeta >= 0.0) ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+  double cs = 1.0 / sqrt(1.0 + tt * tt), sn = cs * tt;
+  for (int k = lane; k < LEN; k += 32) {
+    double x = cp[k], y = cq[k];
+    cp[k] = cs * x - sn * y;
+    cq[k] = sn * x + cs * y;
+  }
+  return true;
+}
+
+__global__ void __launch_bounds__(JC_THREADS, 1)
+jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS) {
+  extern __shared__ double jsm[];
+  cg::cluster_group cluster = cg::this_cluster();
+  const int crank = (int)cluster.block_rank();
+  const int t = blockIdx.x / CS;
+  const int r1 = b.r1[t], r2 = b.r2[t];
+  const bool tr = r1 < r2;
+  const int M = tr ? r2 : r1, Nc = tr ? r1 : r2;
+  const int LEN = M + Nc;
+  const double* K = b.K[t];
+  const int ldk = b.ldk[t];
+  // shared layout: cols[2][bs][LEN], ids[2][bs] (as double-aligned ints), scal[4]
+  double* cols = jsm;
+  int* ids = (int*)(cols + (size_t)2 * bs * LEN);
+  double* scal = (double*)(ids + 2 * bs + (2 * bs & 1));     // [0] partial fro, [1] rotated flag
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = JC_THREADS / 32;
+  const int blk_of_slot[2] = {crank, 2 * CS - 1 - crank};
+  // ---- load ---------------------------------------------------------------------------------
+  double fro = 0.0;
+  for (int e = tid; e < 2 * bs * LEN; e += JC_THREADS) {
+    int k = e % LEN, ci = e / LEN;               // ci = slot*bs + i
+    int j = blk_of_slot[ci / bs] * bs + (ci % bs);
+    double v = 0.0;
+    if (j < Nc) {
+      if (k < M) { v = tr ? K[j + (long long)k * ldk] : K[k + (long long)j * ldk]; fro += v * v; }
+      else v = (k - M == j) ? 1.0 : 0.0;
+    }
+    cols[e] = v;
+  }
+  for (int e = tid; e < 2 * bs; e += JC_THREADS) ids[e] = blk_of_slot[e / bs] * bs + (e % bs);
+  __shared__ double s_red[32];
+  fro = warp_sum(fro);
+  if (lane == 0) s_red[warp] = fro;
+  __syncthreads();
+  if (tid == 0) {
+    double s = 0.0;
+    for (int w = 0; w < nw; w++) s += s_red[w];
+    scal[0] = s; scal[1] = 0.0;
+  }
+  cluster.sync();
+  double ref = 0.0;
+  for (int c = 0; c < CS; c++) ref += cluster.map_shared_rank(scal, c)[0];
+  const double noise2 = 1e-30 * ref;
+  int sweeps = 0;
+  const bool active = (Nc >= 2) && (ref > 0.0) && isfinite(ref);
+  double* top = cols;
+  double* bot = cols + (size_t)bs * LEN;
+  const int nb2 = (bs & 1) ? bs + 1 : bs;        // circle size for the intra-block pairs
+  for (int sw = 0; active && sw < max_sweeps; sw++) {
+    bool rot = false;
+    // intra-block pairs (both blocks at once)
+    for (int r = 0; r < nb2 - 1; r++) {
+      for (int w = warp; w < nb2; w += nw) {
+        int slot = w / (nb2 / 2), i = w % (nb2 / 2);
+        int a, c;
+        if (i == 0) { a = nb2 - 1; c = r; }
+        else { a = (r + i) % (nb2 - 1); c = (r - i + nb2 - 1) % (nb2 - 1); }
+        if (a >= bs || c >= bs) continue;
+        double* base = slot ? bot : top;
+        rot |= rotate_pair(base + (size_t)min(a, c) * LEN, base + (size_t)max(a, c) * LEN, M, LEN, tol, noise2, lane);
+      }
+      __syncthreads();
+    }
+    // super-rounds
+    for (int sr = 0; sr < 2 * CS - 1; sr++) {
+      for (int r = 0; r < bs; r++) {
+        for (int i = warp; i < bs; i += nw) {
+          int j = i + r; if (j >= bs) j -= bs;
+          rot |= rotate_pair(top + (size_t)i * LEN, bot + (size_t)j * LEN, M, LEN, tol, noise2, lane);
+        }
+        __syncthreads();
+      }
+      if (CS > 1) {
+        cluster.sync();                           // A: every CTA finished computing
+        const int per = bs * LEN;                 // doubles per block
+        // sources of the new top / bottom blocks
+        const double* src_top; const int* src_top_id;
+        if (crank == 0) { src_top = nullptr; src_top_id = nullptr; }
+        else if (crank == 1) { src_top = cluster.map_shared_rank(bot, 0); src_top_id = cluster.map_shared_rank(ids + bs, 0); }
+        else { src_top = cluster.map_shared_rank(top, crank - 1); src_top_id = cluster.map_shared_rank(ids, crank - 1); }
+        const double* src_bot; const int* src_bot_id;
+        if (crank == CS - 1) { src_bot = top; src_bot_id = ids; }
+        else { src_bot = cluster.map_shared_rank(bot, crank + 1); src_bot_id = cluster.map_shared_rank(ids + bs, crank + 1); }
+        double stage[JC_STAGE];
+        int id_stage = -1;
+#pragma unroll
+        for (int q = 0; q < JC_STAGE; q++) {
+          int e = tid + q * JC_THREADS;
+          double v = 0.0;
+          if (e < per) { if (src_top) v = src_top[e]; }
+          else if (e < 2 * per) v = src_bot[e - per];
+          stage[q] = v;
+        }
+        if (tid < bs) { if (src_top_id) id_stage = src_top_id[tid]; }
+        else if (tid < 2 * bs) id_stage = src_bot_id[tid - bs];
+        cluster.sync();                           // B: every CTA finished reading
+#pragma unroll
+        for (int q = 0; q < JC_STAGE; q++) {
+          int e = tid + q * JC_THREADS;
+          if (e < per) { if (src_top) top[e] = stage[q]; }
+          else if (e < 2 * per) bot[e - per] = stage[q];
+        }
+        if (tid < bs) { if (src_top_id) ids[tid] = id_stage; }
+        else if (tid < 2 * bs) ids[tid] = id_stage;
+        __syncthreads();
+      }
+    }
+    sweeps = sw + 1;
+    // cluster-wide "any rotation" (uniform decision)
+    int anyrot = __syncthreads_or(rot ? 1 : 0);
+    if (tid == 0) scal[1] = anyrot ? 1.0 : 0.0;
+    cluster.sync();
+    double tot = 0.0;
+    for (int c = 0; c < CS; c++) tot += cluster.map_shared_rank(scal, c)[1];
+    cluster.sync();                               // flags read before anyone overwrites them
+    if (tot == 0.0) break;
+  }
+  // ---- write back: column id -> global column id of G / V, norm -> sv scratch (unsorted) -------
+  double* G = b.G[t];
+  double* V = b.V[t];
+  double* svu = b.V[t] + (size_t)Nc * Nc;         // unsorted norms: Nc doubles after V (caller sizes V as Nc*(Nc+1))
+  for (int ci = warp; ci < 2 * bs; ci += nw) {
+    int id = ids[ci];
+    if (id >= Nc) continue;
+    const double* col = cols + (size_t)ci * LEN;
+    double s = 0.0;
+    for (int k = lane; k < M; k += 32) { double x = col[k]; s += x * x; G[(size_t)id * M + k] = x; }
+    for (int k = lane; k < Nc; k += 32) V[(size_t)id * Nc + k] = col[M + k];
+    s = warp_sum(s);
+    if (lane == 0) svu[id] = sqrt(s);
+  }
+  __threadfence();
+  cluster.sync();
+  if (crank == 0) {
+    for (int j = tid; j < Nc; j += JC_THREADS) {
+      double sj = svu[j];
+      int rank = 0;
+      for (int l = 0; l < Nc; l++) {
+        double sl = svu[l];
+        rank += (sl > sj || (sl == sj && l < j)) ? 1 : 0;
+      }
+      b.order[t][rank] = j;
+      b.sv[t][rank] = sj;
+    }
+    if (tid == 0 && b.sweeps[t]) *b.sweeps[t] = sweeps;
+  }
+}
+
 __global__ void svd_truncate_kernel(SvdFinishBatch b, int chi_max, double eps_cut) {
   const int t = blockIdx.x;
   if (threadIdx.x != 0) return;
@@ -232,8 +418,37 @@ int launch_set_identity(cudaStream_t st, double* Q, long long m, int k) {
 
 int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps) {
   if (b.count == 0) return 0;
-  int ncmax = 1;
-  for (int t = 0; t < b.count; t++) ncmax = std::max(ncmax, std::min(b.r1[t], b.r2[t]));
+  int ncmax = 1, lenmax = 2;
+  for (int t = 0; t < b.count; t++) {
+    int nc = std::min(b.r1[t], b.r2[t]), mm = std::max(b.r1[t], b.r2[t]);
+    ncmax = std::max(ncmax, nc); lenmax = std::max(lenmax, mm + nc);
+  }
+  // smallest cluster whose per-CTA share of the columns fits shared memory and the staging regs
+  for (int CS = 1; CS <= 16; CS *= 2) {
+    int bs = (ncmax + 2 * CS - 1) / (2 * CS);
+    size_t smem = ((size_t)2 * bs * lenmax) * 8 + (size_t)(2 * bs + 2) * 4 + 64;
+    bool fits = smem <= JC_SMEM_CAP && (CS == 1 || (size_t)2 * bs * lenmax <= (size_t)JC_STAGE * JC_THREADS);
+    if (!fits) continue;
+    static bool attr_done = false;
+    if (!attr_done) {
+      PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
+      PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+      attr_done = true;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(b.count * CS));
+    cfg.blockDim = dim3(JC_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel, b, tol, max_sweeps, bs, CS);
+    if (e == cudaSuccess) { PEPO_COUNT_LAUNCH(); return 0; }
+    (void)cudaGetLastError();                      // e.g. cluster of 16 not schedulable: try the fallback
+    break;
+  }
   size_t smem = (size_t)ncmax * sizeof(double);
   jacobi_svd_kernel<<<b.count, 1024, smem, st>>>(b, tol, max_sweeps);
   PEPO_COUNT_LAUNCH();
