@@ -27,10 +27,12 @@ __global__ void __launch_bounds__(512) potrf_upper_kernel(MatBatch b, InfoPtrs i
   const int n = b.n[t];
   double* D = sm;                 // PB x (PB+1)
   double* Ps = sm + PB * (PB + 1);  // PB x pitch (pitch = n rounded)
+  double* dg = Ps + (size_t)PB * max(n, 1);   // original diagonal G_jj = ||column j||^2
   __shared__ int s_fail;
-  __shared__ double s_dmin, s_dmax;
+  __shared__ double s_rmin;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (tid == 0) { s_fail = 0; s_dmin = 1e300; s_dmax = 0.0; }
+  if (tid == 0) { s_fail = 0; s_rmin = 1e300; }
+  for (int j = tid; j < n; j += blockDim.x) dg[j] = A[j + (long long)j * ld];
   __syncthreads();
   for (int jb = 0; jb < n; jb += PB) {
     const int nb = min(PB, n - jb);
@@ -49,9 +51,9 @@ __global__ void __launch_bounds__(512) potrf_upper_kernel(MatBatch b, InfoPtrs i
           break;
         }
         double rkk = sqrt(piv);
-        if (lane == 0) {
-          s_dmin = fmin(s_dmin, rkk); s_dmax = fmax(s_dmax, rkk);
-        }
+        // scale-invariant conditioning measure (R9): R_kk / ||column k|| = sine of the angle between
+        // column k and the span of the previous columns
+        if (lane == 0) s_rmin = fmin(s_rmin, rkk / sqrt(dg[jb + k]));
         __syncwarp();
         double rkj = 0.0;
         if (lane < nb && lane >= k) {
@@ -113,7 +115,7 @@ __global__ void __launch_bounds__(512) potrf_upper_kernel(MatBatch b, InfoPtrs i
   }
   if (tid == 0) {
     int inf = s_fail;
-    if (inf == 0 && n > 0 && s_dmin < tau * s_dmax) inf = -1;
+    if (inf == 0 && n > 0 && s_rmin < tau) inf = -1;
     *info.p[t] = inf;
   }
 }
@@ -491,7 +493,7 @@ int launch_potrf(cudaStream_t st, const MatBatch& b, int* const* info, double ta
   InfoPtrs ip;
   int nmax = 0;
   for (int t = 0; t < b.count; t++) { ip.p[t] = info[t]; nmax = std::max(nmax, b.n[t]); }
-  size_t smem = (size_t)(PB * (PB + 1) + PB * std::max(nmax, 1)) * sizeof(double);
+  size_t smem = (size_t)(PB * (PB + 1) + (PB + 1) * std::max(nmax, 1)) * sizeof(double);
   static size_t attr = 0;
   if (smem > attr) {
     PEPO_CUDA_OK(cudaFuncSetAttribute(potrf_upper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(smem, (size_t)48 * 1024)));
