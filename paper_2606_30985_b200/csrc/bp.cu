@@ -26,18 +26,19 @@ constexpr int BP_THREADS = 256;
 constexpr int BP_MAXK = 8;     // dU <= 256
 
 __global__ void __launch_bounds__(BP_THREADS) bp_partial_kernel(BpBatch b) {
-  __shared__ double sU[BP_THREADS / 32][32 * BP_MAXK];
+  constexpr int nw = BP_THREADS / 32;
+  __shared__ double sU[nw][32 * BP_MAXK];
+  __shared__ double sS[PEPO_BP_MAXCHUNK][nw];
   const int t = blockIdx.y;
   const BpSite& S = b.s[t];
+  const int blk = blockIdx.x;
+  if (blk >= S.nchunks) return;
   const int dU = S.d[0], dD = S.d[1], dL = S.d[2], dR = S.d[3];
-  const int lr = blockIdx.x;
-  if (lr >= dL * dR) return;
-  const int l = lr % dL, r = lr / dL;
-  const double* T = S.T + (long long)lr * dU * dD;
+  const int nlr = dL * dR;
+  const int lr0 = blk * S.chunk, lr1 = min(nlr, lr0 + S.chunk);
   const double* mU = S.in[0];
   const double* mD = S.in[1];
-  const double w = S.in[2][l] * S.in[3][r];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = BP_THREADS / 32;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   double accU[BP_MAXK];
   double mu[BP_MAXK];
 #pragma unroll
@@ -46,43 +47,65 @@ __global__ void __launch_bounds__(BP_THREADS) bp_partial_kernel(BpBatch b) {
     int u = lane + 32 * k;
     mu[k] = (u < dU) ? mU[u] : 0.0;
   }
-  double* partD = S.partD + (long long)lr * dD;
-  for (int d = warp; d < dD; d += nw) {
-    const double md = mD[d];
-    const double* col = T + (long long)d * dU;
-    double cs = 0.0;
+  // lane j of warp wp owns pD[d] for d = wp + nw*j (dD <= 256)
+  double accD = 0.0;
+  const double myD = (warp + nw * lane < dD) ? mD[warp + nw * lane] : 0.0;
+  for (int lr = lr0; lr < lr1; lr++) {
+    const int l = lr % dL, r = lr / dL;
+    const double w = S.in[2][l] * S.in[3][r];
+    const double* T = S.T + (long long)lr * dU * dD;
+    double ssum = 0.0;
+    int j = 0;
+    for (int d = warp; d < dD; d += 2 * nw, j += 2) {
+      const int d2 = d + nw;
+      const bool has2 = d2 < dD;
+      const double md = __shfl_sync(0xffffffffu, myD, j);
+      const double md2 = __shfl_sync(0xffffffffu, myD, (j + 1) & 31);
+      const double* col = T + (long long)d * dU;
+      const double* col2 = T + (long long)(has2 ? d2 : d) * dU;
+      const double mdw = md * w, mdw2 = has2 ? md2 * w : 0.0;
+      double cs = 0.0, cs2 = 0.0;
 #pragma unroll
-    for (int k = 0; k < BP_MAXK; k++) {
-      int u = lane + 32 * k;
-      if (u < dU) {
-        double tv = col[u];
-        accU[k] += tv * md;
-        cs += tv * mu[k];
+      for (int k = 0; k < BP_MAXK; k++) {
+        int u = lane + 32 * k;
+        if (u < dU) {
+          double tv = col[u], tv2 = col2[u];
+          accU[k] += tv * mdw;
+          cs += tv * mu[k];
+          accU[k] += tv2 * mdw2;
+          cs2 += tv2 * mu[k];
+        }
+      }
+      cs = warp_sum(cs);
+      cs2 = warp_sum(cs2);
+      if (lane == j) accD += w * cs;
+      ssum += md * cs;
+      if (has2) {
+        if (lane == j + 1) accD += w * cs2;
+        ssum += md2 * cs2;
       }
     }
-    cs = warp_sum(cs);
-    if (lane == 0) partD[d] = w * cs;
+    if (lane == 0) sS[lr - lr0][warp] = ssum;
   }
 #pragma unroll
   for (int k = 0; k < BP_MAXK; k++) sU[warp][lane + 32 * k] = accU[k];
   __syncthreads();
-  double sdot = 0.0;
   for (int u = threadIdx.x; u < dU; u += BP_THREADS) {
     double p = 0.0;
 #pragma unroll
     for (int w2 = 0; w2 < nw; w2++) p += sU[w2][u];
-    S.partU[(long long)lr * dU + u] = w * p;
-    sdot += p * mU[u];
+    S.partU[(long long)blk * dU + u] = p;
   }
-  // s = sum_u mU[u] pU[u]  (dU <= 256 = one pass of the block)
-  __shared__ double sred[BP_THREADS / 32];
-  sdot = warp_sum(sdot);
-  if (lane == 0) sred[warp] = sdot;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    double s = 0.0;
-    for (int w2 = 0; w2 < nw; w2++) s += sred[w2];
-    S.partS[lr] = s;
+  {
+    const int d = warp + nw * lane;
+    if (d < dD) S.partD[(long long)blk * dD + d] = accD;
+  }
+  // s(l,r) = sum_d mD[d] (sum_u T[u,d,l,r] mU[u])
+  for (int i = threadIdx.x; i < lr1 - lr0; i += BP_THREADS) {
+    double sv = 0.0;
+#pragma unroll
+    for (int w2 = 0; w2 < nw; w2++) sv += sS[i][w2];
+    S.partS[lr0 + i] = sv;
   }
 }
 
@@ -107,9 +130,9 @@ __global__ void __launch_bounds__(256) bp_finalize_kernel(BpBatch b, double damp
   for (int i = threadIdx.x; i < dl; i += blockDim.x) {
     double v = 0.0;
     if (slot == 0) {
-      for (int k = 0; k < nlr; k++) v += S.partU[(long long)k * dU + i];
+      for (int k = 0; k < S.nchunks; k++) v += S.partU[(long long)k * dU + i];
     } else if (slot == 1) {
-      for (int k = 0; k < nlr; k++) v += S.partD[(long long)k * dD + i];
+      for (int k = 0; k < S.nchunks; k++) v += S.partD[(long long)k * dD + i];
     } else if (slot == 2) {
       for (int r = 0; r < dR; r++) v += S.in[3][r] * S.partS[i + dL * r];
     } else {
@@ -232,7 +255,7 @@ __global__ void __launch_bounds__(256) field_gate_kernel(FieldBatch b) {
 int launch_bp_partial(cudaStream_t st, const BpBatch& b) {
   if (b.count == 0) return 0;
   int maxlr = 1;
-  for (int t = 0; t < b.count; t++) maxlr = std::max(maxlr, b.s[t].d[2] * b.s[t].d[3]);
+  for (int t = 0; t < b.count; t++) maxlr = std::max(maxlr, b.s[t].nchunks);
   dim3 grid(maxlr, b.count);
   bp_partial_kernel<<<grid, BP_THREADS, 0, st>>>(b);
   PEPO_COUNT_LAUNCH();

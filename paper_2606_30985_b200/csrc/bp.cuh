@@ -5,6 +5,7 @@
 namespace pepo {
 
 #define PEPO_BP_MAXS 32
+#define PEPO_BP_MAXCHUNK 32
 
 struct BpSite {
   const double* T;            // pinned slab psi_v[..., p_v], dims d[0..3] = (U,D,L,R), 1 if absent
@@ -14,7 +15,8 @@ struct BpSite {
   const double* in[4];        // incoming message per slot (a constant [1.0] if absent)
   const double* out_old[4];   // current outgoing message per slot
   double* out_new[4];         // next outgoing message per slot
-  double* partU; double* partD; double* partS;
+  double* partU; double* partD; double* partS;   // partU/partD: one row per chunk of (l,r) slices
+  int chunk, nchunks;         // (l,r) slices per CTA of bp_partial_kernel, CTAs for this site
   double* vs;                 // site scalar of eq. (7)
 };
 struct BpBatch { int count; BpSite s[PEPO_BP_MAXS]; };

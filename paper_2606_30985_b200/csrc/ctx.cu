@@ -729,6 +729,7 @@ struct TaskGeo {           // one site of one gate
   long long m, ld;
   int n, chi_c, N, k, r;   // k = min(m,n); r = rows of Rx
   bool chol;
+  bool skip1, skip2;       // Householder path: Q = I when m <= n (R = cv); Qx = I when 4k <= N (Rx = X)
   int chi_new;
 };
 
@@ -764,6 +765,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       t.k = (int)std::min<long long>(t.m, t.n);
       t.chol = !c->force_hh && (double)t.m >= c->chol_ratio * t.n;
       t.r = t.chol ? t.N : std::min(4 * t.k, t.N);
+      t.skip1 = t.m <= t.n; t.skip2 = 4 * t.k <= t.N;
       SiteWs& W = c->lanes[g].s[i];
       PermuteDesc pd;
       pd.rank = s.nlegs + 1; pd.power = 1.0;
@@ -844,26 +846,40 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
         ti.A[q] = W.Rxinv; ti.ld[q] = t.N; ti.m[q] = t.N; ti.n[q] = t.N; ti.count = zl.count;
         c->stats.n_cholesky++;
       } else {
-        int q = h1.count++;
-        h1.A[q] = W.cv; h1.lda[q] = t.ld; h1.m[q] = t.m; h1.n[q] = t.n; h1.beta[q] = W.beta1; h1.tau[q] = W.tau1;
-        Rout1[q] = W.Rbuf; ldr1[q] = t.k;
-        dr.in[q] = W.Rbuf; dr.out[q] = W.X; dr.chi[q] = t.chi_c; dr.k[q] = t.k; dr.site[q] = t.site_idx;
-        dr.ld_in[q] = t.k; dr.ld_out[q] = 4ll * t.k; dr.count = h1.count;
-        h2.A[q] = W.X; h2.lda[q] = 4ll * t.k; h2.m[q] = 4ll * t.k; h2.n[q] = t.N; h2.beta[q] = W.beta2; h2.tau[q] = W.tau2;
-        h2.count = h1.count;
-        Rout2[q] = W.Rx; ldr2[q] = t.r;
+        // first factor: cv = Q R (k x n); for m <= n take Q = I, R = cv (any factor with orthonormal Q serves)
+        const double* Rsrc = W.Rbuf; long long ldR = t.k;
+        if (t.skip1) { Rsrc = W.cv; ldR = t.ld; }
+        else {
+          int q = h1.count++;
+          h1.A[q] = W.cv; h1.lda[q] = t.ld; h1.m[q] = t.m; h1.n[q] = t.n; h1.beta[q] = W.beta1; h1.tau[q] = W.tau1;
+          Rout1[q] = W.Rbuf; ldr1[q] = t.k;
+        }
+        // X = dress(R) (4k x N); when 4k <= N it is already the small factor Rx (Qx = I)
+        int q = dr.count++;
+        dr.in[q] = Rsrc; dr.chi[q] = t.chi_c; dr.k[q] = t.k; dr.site[q] = t.site_idx; dr.ld_in[q] = ldR;
+        if (t.skip2) { dr.out[q] = W.Rx; dr.ld_out[q] = t.r; }
+        else {
+          dr.out[q] = W.X; dr.ld_out[q] = 4ll * t.k;
+          int q2 = h2.count++;
+          h2.A[q2] = W.X; h2.lda[q2] = 4ll * t.k; h2.m[q2] = 4ll * t.k; h2.n[q2] = t.N; h2.beta[q2] = W.beta2; h2.tau[q2] = W.tau2;
+          Rout2[q2] = W.Rx; ldr2[q2] = t.r;
+        }
         c->stats.n_householder++;
       }
     }
     int rc = 0;
     if (zl.count) { ProfScope ps(c, PC_CHOL, 0, 0); rc = launch_zero_lower(st, zl); if (rc) return rc; rc = launch_trtri(st, zl, ti); if (rc) return rc; }
-    if (h1.count) {
+    if (dr.count) {
       ProfScope ps(c, PC_HOUSEHOLDER, 0, 0);
-      rc = launch_hh_factor(st, h1); if (rc) return rc;
-      rc = launch_hh_extract_r(st, h1, Rout1, ldr1); if (rc) return rc;
+      if (h1.count) {
+        rc = launch_hh_factor(st, h1); if (rc) return rc;
+        rc = launch_hh_extract_r(st, h1, Rout1, ldr1); if (rc) return rc;
+      }
       rc = launch_dress_R(st, dr, gt); if (rc) return rc;
-      rc = launch_hh_factor(st, h2); if (rc) return rc;
-      rc = launch_hh_extract_r(st, h2, Rout2, ldr2); if (rc) return rc;
+      if (h2.count) {
+        rc = launch_hh_factor(st, h2); if (rc) return rc;
+        rc = launch_hh_extract_r(st, h2, Rout2, ldr2); if (rc) return rc;
+      }
     }
   }
   // ---- D: core, SVD, truncation ------------------------------------------------------------------
@@ -925,6 +941,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
     DressBatch rs; rs.count = 0; rs.NA = NA;
     int* cn_r[PEPO_MAXT]; long long mrows[PEPO_MAXT];
     HHApplyBatch a1; a1.count = 0;
+    HHApplyBatch pad; pad.count = 0;
     MatBatch padsrc; padsrc.count = 0;
     int rc = 0;
     for (auto& t : T) {
@@ -942,17 +959,24 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
         bw.in[q] = W.T; bw.out[q] = W.W; bw.chi[q] = t.chi_c; bw.k[q] = t.chi_new; bw.site[q] = t.site_idx;
         bw.ld_in[q] = t.N; bw.ld_out[q] = t.n; cn_w[q] = L.ints;
       } else {
-        int q = a2.count++;
-        // Mx = [U sqrt S ; 0] (4k x chi_new), then Qx applied
-        padsrc.A[q] = const_cast<double*>(UV); padsrc.ld[q] = t.r; padsrc.m[q] = t.r; padsrc.n[q] = t.chi_new;
-        padsrc.count = a2.count;
-        a2.A[q] = W.X; a2.lda[q] = 4ll * t.k; a2.m[q] = 4ll * t.k; a2.k[q] = t.r;
-        a2.beta[q] = W.beta2; a2.tau[q] = W.tau2; a2.Y[q] = W.Mx; a2.ldy[q] = 4ll * t.k; a2.ncols[q] = t.chi_new;
-        rs.in[q] = W.Mx; rs.out[q] = W.out; rs.chi[q] = t.chi_new; rs.k[q] = t.k; rs.site[q] = t.site_idx;
-        rs.ld_in[q] = 4ll * t.k; rs.ld_out[q] = t.ld; rs.count = a2.count;
-        cn_r[q] = L.ints; mrows[q] = t.m;
-        a1.A[q] = W.cv; a1.lda[q] = t.ld; a1.m[q] = t.m; a1.k[q] = t.k; a1.beta[q] = W.beta1; a1.tau[q] = W.tau1;
-        a1.Y[q] = W.out; a1.ldy[q] = t.ld; a1.ncols[q] = 4 * t.chi_new; a1.count = a2.count;
+        // Mx = Qx [U sqrt S ; 0] (4k x chi_new); Qx = I when 4k <= N (then r = 4k: plain copy)
+        int qp = padsrc.count++;
+        padsrc.A[qp] = const_cast<double*>(UV); padsrc.ld[qp] = t.r; padsrc.m[qp] = t.r; padsrc.n[qp] = t.chi_new;
+        pad.Y[qp] = W.Mx; pad.ldy[qp] = 4ll * t.k; pad.m[qp] = 4ll * t.k; pad.ncols[qp] = t.chi_new; pad.count = padsrc.count;
+        if (!t.skip2) {
+          int q = a2.count++;
+          a2.A[q] = W.X; a2.lda[q] = 4ll * t.k; a2.m[q] = 4ll * t.k; a2.k[q] = t.r;
+          a2.beta[q] = W.beta2; a2.tau[q] = W.tau2; a2.Y[q] = W.Mx; a2.ldy[q] = 4ll * t.k; a2.ncols[q] = t.chi_new;
+        }
+        int qr = rs.count++;
+        rs.in[qr] = W.Mx; rs.out[qr] = W.out; rs.chi[qr] = t.chi_new; rs.k[qr] = t.k; rs.site[qr] = t.site_idx;
+        rs.ld_in[qr] = 4ll * t.k; rs.ld_out[qr] = t.ld;
+        cn_r[qr] = L.ints; mrows[qr] = t.m;
+        if (!t.skip1) {
+          int q = a1.count++;
+          a1.A[q] = W.cv; a1.lda[q] = t.ld; a1.m[q] = t.m; a1.k[q] = t.k; a1.beta[q] = W.beta1; a1.tau[q] = W.tau1;
+          a1.Y[q] = W.out; a1.ldy[q] = t.ld; a1.ncols[q] = 4 * t.chi_new;
+        }
       }
     }
     if (bw.count) {
@@ -967,13 +991,12 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
         rc = launch_dgemm(st, 0, 0, gp, 1, 0, nullptr, false); if (rc) return rc;
       }
     }
-    if (a2.count) {
-      // pad-copy through the reshuffle kernel's sibling: use launch_copy_pad
+    if (rs.count) {
       ProfScope ps(c, PC_HOUSEHOLDER, 0, 0);
-      rc = launch_copy_pad(st, padsrc, a2); if (rc) return rc;
-      rc = launch_hh_apply_q(st, a2); if (rc) return rc;
+      rc = launch_copy_pad(st, padsrc, pad); if (rc) return rc;
+      if (a2.count) { rc = launch_hh_apply_q(st, a2); if (rc) return rc; }
       rc = launch_reshuffle_M(st, rs, cn_r, mrows); if (rc) return rc;
-      rc = launch_hh_apply_q(st, a1); if (rc) return rc;
+      if (a1.count) { rc = launch_hh_apply_q(st, a1); if (rc) return rc; }
     }
   }
   // ---- F: inverse permute + deabsorb + write-back ----------------------------------------------------
@@ -1080,6 +1103,16 @@ int bp_sweep(pepo_ctx* c, double damping, int update) {
     bb.count = std::min(PEPO_BP_MAXS, c->n_sites - v0);
     for (int i = 0; i < bb.count; i++) fill_bp_site(c, v0 + i, c->cur_msg, bb.s[i]);
     double bbytes = 0; for (int i = 0; i < bb.count; i++) bbytes += 8.0 * bb.s[i].d[0] * bb.s[i].d[1] * bb.s[i].d[2] * bb.s[i].d[3];
+    // chunking: ~8 CTAs per SM over the batch, each CTA a contiguous run of (l,r) slices
+    const double per_cta = std::max(bbytes / (148.0 * 8.0), 32768.0);
+    for (int i = 0; i < bb.count; i++) {
+      BpSite& S = bb.s[i];
+      const double slice = 8.0 * S.d[0] * S.d[1];
+      const int nlr = S.d[2] * S.d[3];
+      int ch = (int)std::min<double>(std::max(per_cta / slice, 1.0), (double)PEPO_BP_MAXCHUNK);
+      S.chunk = std::min(ch, nlr);
+      S.nchunks = (nlr + S.chunk - 1) / S.chunk;
+    }
     ProfScope ps(c, PC_BP, 0, bbytes);
     int rc = launch_bp_partial(c->st, bb); if (rc) return rc;
     rc = launch_bp_finalize(c->st, bb, damping, update, c->delta_bits, c->bp_ints); if (rc) return rc;
