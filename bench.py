@@ -47,6 +47,8 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--bp-tol", type=float, default=1e-10)
     ap.add_argument("--bp-damping", type=float, default=0.5)
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="pepo_set_option tunable (repeatable), e.g. svd_min_cluster=8")
     return ap.parse_args()
 
 
@@ -161,6 +163,9 @@ def run_ours(args):
     torch.cuda.set_device(dev)
     L, chi = args.grid, args.chi
     sim = B.Pepo(L, L, args.cx, args.cy, J, H, DT, chi, args.bp_tol, args.bp_damping, device=str(dev))
+    for kv in args.opt:
+        k, v = kv.split("=")
+        sim.set_option(k, float(v))
     info = prepare(sim, args)
 
     def barrier():

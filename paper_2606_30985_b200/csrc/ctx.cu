@@ -601,6 +601,7 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "force_householder") c->force_hh = (int)v;
   else if (k == "jacobi_tol") c->jacobi_tol = v;
   else if (k == "jacobi_max_sweeps") c->jacobi_max_sweeps = (int)v;
+  else if (k == "svd_min_cluster") set_svd_min_cluster((int)v);
   else if (k == "profile") {
     Prof& P = c->prof;
     if (v != 0.0 && P.ev.empty()) {
@@ -886,7 +887,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
   {
     DressBatch sc; sc.count = ng; sc.NA = NA;
     SvdBatch sb; sb.count = ng;
-    SvdFinishBatch fb; fb.count = ng;
+    SvdFinishBatch fb; fb.count = ng; fb.with_v = 0;
     for (int g = 0; g < ng; g++) {
       TaskGeo& t1 = T[2 * g]; TaskGeo& t2 = T[2 * g + 1];
       LaneWs& L = c->lanes[g];
@@ -895,6 +896,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       sc.ld_in[g] = t1.r; sc.ld_out[g] = t1.r;
       sb.K[g] = L.K; sb.ldk[g] = t1.r; sb.r1[g] = t1.r; sb.r2[g] = t2.r;
       sb.G[g] = L.G; sb.V[g] = L.V; sb.sv[g] = L.sv; sb.order[g] = L.order; sb.sweeps[g] = L.ints + 1;
+      fb.K[g] = L.K; fb.ldk[g] = t1.r;
       fb.r1[g] = t1.r; fb.r2[g] = t2.r; fb.G[g] = L.G; fb.V[g] = L.V; fb.sv[g] = L.sv; fb.order[g] = L.order;
       fb.Us[g] = L.Us; fb.ldus[g] = t1.r; fb.Vs[g] = L.Vs; fb.ldvs[g] = t2.r;
       fb.lambda[g] = bond_vec(c->lambda, e, c->chi_max);
@@ -914,7 +916,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
     }
     {
       ProfScope ps(c, PC_SVD, 0, 0);
-      rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps); if (rc) return rc;
+      rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps, false); if (rc) return rc;
       rc = launch_svd_truncate(st, fb, c->chi_max, c->eps_cut); if (rc) return rc;
     }
     PEPO_CUDA_OK(cudaMemcpyAsync(c->h_ints, c->lane_ints, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));

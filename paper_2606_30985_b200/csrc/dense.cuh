@@ -56,13 +56,17 @@ struct SvdBatch {
   int* order[PEPO_MAXT];                            // Nc ints scratch
   int* sweeps[PEPO_MAXT];                           // device int
 };
-int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps);
+// with_v = false: V is not accumulated (launch_svd_bridge then derives it from K, SvdFinishBatch::K)
+int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v);
+void set_svd_min_cluster(int cs);
 
 struct SvdFinishBatch {
   int count;
   int r1[PEPO_MAXT]; int r2[PEPO_MAXT];
   const double* G[PEPO_MAXT]; const double* V[PEPO_MAXT]; const double* sv[PEPO_MAXT];
   const int* order[PEPO_MAXT];
+  int with_v;                                       // 1: V accumulated by the Jacobi kernel; 0: derive from K
+  const double* K[PEPO_MAXT]; int ldk[PEPO_MAXT];   // the core (needed when with_v = 0)
   double* Us[PEPO_MAXT]; int ldus[PEPO_MAXT];       // r1 x chi_new
   double* Vs[PEPO_MAXT]; int ldvs[PEPO_MAXT];       // r2 x chi_new
   double* lambda[PEPO_MAXT]; double* sqrt_l[PEPO_MAXT]; double* isqrt_l[PEPO_MAXT];

@@ -134,41 +134,55 @@ __global__ void __launch_bounds__(1024) jacobi_svd_kernel(SvdBatch b, double tol
 // the round-robin circle through distributed shared memory (staged in registers between two
 // cluster barriers).  No global-memory traffic inside the iteration.
 // ---------------------------------------------------------------------------------------------
+int g_svd_min_cluster = 1;              // tunable (option "svd_min_cluster"): smallest cluster size tried
 constexpr int JC_THREADS = 1024;
 constexpr int JC_STAGE = 26;            // doubles staged per thread during a block exchange
 constexpr size_t JC_SMEM_CAP = 200 * 1024;
 
-__device__ __forceinline__ bool rotate_pair(double* cp, double* cq, int M, int LEN, double tol,
+// cp, cq: 16-byte aligned columns; MP2 = (padded) number of double2 of the G part that enter the
+// inner products, LEN2 = double2 per column (G part + optional V part); pad entries are zero.
+__device__ __forceinline__ bool rotate_pair(double* cp, double* cq, int MP2, int LEN2, double tol2,
                                             double noise2, int lane) {
+  double2* p2 = reinterpret_cast<double2*>(cp);
+  double2* q2 = reinterpret_cast<double2*>(cq);
   double al = 0.0, be = 0.0, ga = 0.0;
-  for (int k = lane; k < M; k += 32) {
-    double x = cp[k], y = cq[k];
-    al += x * x; be += y * y; ga += x * y;
+  for (int k = lane; k < MP2; k += 32) {
+    double2 x = p2[k], y = q2[k];
+    al += x.x * x.x; be += y.x * y.x; ga += x.x * y.x;
+    al += x.y * x.y; be += y.y * y.y; ga += x.y * y.y;
   }
   al = warp_sum(al); be = warp_sum(be); ga = warp_sum(ga);
   if (al < noise2 || be < noise2 || !(al > 0.0) || !(be > 0.0)) return false;
-  if (fabs(ga) <= tol * sqrt(al) * sqrt(be)) return false;
-  double zeta = (be - al) / (2.0 * ga);
-  double tt = ((zeta >= 0.0) ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-  double cs = 1.0 / sqrt(1.0 + tt * tt), sn = cs * tt;
-  for (int k = lane; k < LEN; k += 32) {
-    double x = cp[k], y = cq[k];
-    cp[k] = cs * x - sn * y;
-    cq[k] = sn * x + cs * y;
+  if (ga * ga <= tol2 * al * be) return false;          // |ga| <= tol ||p|| ||q||
+  // tan of the rotation angle, smaller root: t = sgn(zeta)/(|zeta| + sqrt(1 + zeta^2)), zeta =
+  // (be - al)/(2 ga), written with one sqrt and one division
+  const double d = be - al, g2 = 2.0 * ga;
+  const double tt = g2 / (d + copysign(sqrt(d * d + g2 * g2), d));
+  const double cs = rsqrt(1.0 + tt * tt), sn = cs * tt;
+  for (int k = lane; k < LEN2; k += 32) {
+    double2 x = p2[k], y = q2[k];
+    double2 xn, yn;
+    xn.x = cs * x.x - sn * y.x; yn.x = sn * x.x + cs * y.x;
+    xn.y = cs * x.y - sn * y.y; yn.y = sn * x.y + cs * y.y;
+    p2[k] = xn; q2[k] = yn;
   }
   return true;
 }
 
 __global__ void __launch_bounds__(JC_THREADS, 1)
-jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS) {
-  extern __shared__ double jsm[];
+jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int with_v, int LEN) {
+  extern __shared__ __align__(16) double jsm[];
   cg::cluster_group cluster = cg::this_cluster();
   const int crank = (int)cluster.block_rank();
   const int t = blockIdx.x / CS;
   const int r1 = b.r1[t], r2 = b.r2[t];
   const bool tr = r1 < r2;
   const int M = tr ? r2 : r1, Nc = tr ? r1 : r2;
-  const int LEN = M + Nc;
+  // column layout: [G part: M, zero-padded to MP (even)] [V part: Nc, zero-padded, only with_v];
+  // LEN (even, same for the whole launch) >= MP + (with_v ? Nc : 0)
+  const int MP = (M + 1) & ~1;
+  const int MP2 = MP >> 1, LEN2 = LEN >> 1;
+  const double tol2 = tol * tol;
   const double* K = b.K[t];
   const int ldk = b.ldk[t];
   // shared layout: cols[2][bs][LEN], ids[2][bs] (as double-aligned ints), scal[4]
@@ -185,7 +199,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS) {
     double v = 0.0;
     if (j < Nc) {
       if (k < M) { v = tr ? K[j + (long long)k * ldk] : K[k + (long long)j * ldk]; fro += v * v; }
-      else v = (k - M == j) ? 1.0 : 0.0;
+      else if (with_v && k >= MP) v = (k - MP == j) ? 1.0 : 0.0;
     }
     cols[e] = v;
   }
@@ -219,7 +233,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS) {
         else { a = (r + i) % (nb2 - 1); c = (r - i + nb2 - 1) % (nb2 - 1); }
         if (a >= bs || c >= bs) continue;
         double* base = slot ? bot : top;
-        rot |= rotate_pair(base + (size_t)min(a, c) * LEN, base + (size_t)max(a, c) * LEN, M, LEN, tol, noise2, lane);
+        rot |= rotate_pair(base + (size_t)min(a, c) * LEN, base + (size_t)max(a, c) * LEN, MP2, LEN2, tol2, noise2, lane);
       }
       __syncthreads();
     }
@@ -228,7 +242,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS) {
       for (int r = 0; r < bs; r++) {
         for (int i = warp; i < bs; i += nw) {
           int j = i + r; if (j >= bs) j -= bs;
-          rot |= rotate_pair(top + (size_t)i * LEN, bot + (size_t)j * LEN, M, LEN, tol, noise2, lane);
+          rot |= rotate_pair(top + (size_t)i * LEN, bot + (size_t)j * LEN, MP2, LEN2, tol2, noise2, lane);
         }
         __syncthreads();
       }
@@ -287,7 +301,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS) {
     const double* col = cols + (size_t)ci * LEN;
     double s = 0.0;
     for (int k = lane; k < M; k += 32) { double x = col[k]; s += x * x; G[(size_t)id * M + k] = x; }
-    for (int k = lane; k < Nc; k += 32) V[(size_t)id * Nc + k] = col[M + k];
+    if (with_v) for (int k = lane; k < Nc; k += 32) V[(size_t)id * Nc + k] = col[MP + k];
     s = warp_sum(s);
     if (lane == 0) svu[id] = sqrt(s);
   }
@@ -371,6 +385,58 @@ __global__ void svd_bridge_kernel(SvdFinishBatch b) {
   }
 }
 
+// Bridges without an accumulated V (hot path): the Jacobi kernel leaves G = A V = (left vectors
+// of A) * s for the tall problem A (= K, or K^T when r1 < r2).  The other side follows from
+// b_j = A^T a_j / s_j, i.e. Z = A^T G[:, kept] computed here from the untouched core K.
+//   !tr: Us = G/sqrt(s),   Vs = (K^T G)/s^1.5        tr: Vs = G/sqrt(s),   Us = (K G)/s^1.5
+// Error of b_j is u ||K|| / s_j, so s_j b_j (what enters the tensors) is accurate to u ||K||.
+__global__ void __launch_bounds__(256) svd_bridge_nov_kernel(SvdFinishBatch b) {
+  const int t = blockIdx.y;
+  const int r1 = b.r1[t], r2 = b.r2[t];
+  const bool tr = r1 < r2;
+  const int M = tr ? r2 : r1, Nc = tr ? r1 : r2;
+  const int chin = *b.chi_new[t];
+  const double* G = b.G[t];
+  const double* K = b.K[t];
+  const int ldk = b.ldk[t];
+  const int* order = b.order[t];
+  const double* sv = b.sv[t];
+  double* Gside = tr ? b.Vs[t] : b.Us[t];
+  const int ldg = tr ? b.ldvs[t] : b.ldus[t];
+  double* Zside = tr ? b.Us[t] : b.Vs[t];
+  const int ldz = tr ? b.ldus[t] : b.ldvs[t];
+  const long long gtid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  const long long gthreads = (long long)gridDim.x * blockDim.x;
+  for (long long e = gtid; e < (long long)M * chin; e += gthreads) {
+    int row = (int)(e % M), c = (int)(e / M);
+    Gside[row + (long long)c * ldg] = G[row + (long long)order[c] * M] / sqrt(sv[c]);
+  }
+  if (!tr) {
+    // Z[i,c] = sum_k K[k + i ldk] G[k + j M]: one warp per output, lanes along k
+    const int lane = threadIdx.x & 31;
+    const long long gw = gtid >> 5, nwarps = gthreads >> 5;
+    for (long long e = gw; e < (long long)Nc * chin; e += nwarps) {
+      int i = (int)(e % Nc), c = (int)(e / Nc);
+      const double* kc = K + (long long)i * ldk;
+      const double* gc = G + (long long)order[c] * M;
+      double z = 0.0;
+      for (int k = lane; k < M; k += 32) z += kc[k] * gc[k];
+      z = warp_sum(z);
+      if (lane == 0) { double sc = sv[c]; Zside[i + (long long)c * ldz] = z / (sc * sqrt(sc)); }
+    }
+  } else {
+    // Z[i,c] = sum_k K[i + k ldk] G[k + j M]: one thread per output, coalesced along i
+    for (long long e = gtid; e < (long long)Nc * chin; e += gthreads) {
+      int i = (int)(e % Nc), c = (int)(e / Nc);
+      const double* gc = G + (long long)order[c] * M;
+      double z = 0.0;
+      for (int k = 0; k < M; k++) z += K[i + (long long)k * ldk] * gc[k];
+      double sc = sv[c];
+      Zside[i + (long long)c * ldz] = z / (sc * sqrt(sc));
+    }
+  }
+}
+
 __global__ void svd_vectors_kernel(const double* G, const double* V, const double* s,
                                    const int* order, int m, int n, double* U, double* Vout) {
   const bool tr = m < n;
@@ -397,6 +463,8 @@ __global__ void set_identity_kernel(double* Q, long long m, int k) {
 
 }  // namespace
 
+void set_svd_min_cluster(int cs) { g_svd_min_cluster = cs < 1 ? 1 : (cs > 16 ? 16 : cs); }
+
 int launch_svd_vectors(cudaStream_t st, const double* G, const double* V, const double* s,
                        const int* order, int m, int n, double* U, double* Vout) {
   long long w = (long long)(m + n) * std::min(m, n);
@@ -416,15 +484,19 @@ int launch_set_identity(cudaStream_t st, double* Q, long long m, int k) {
   return 0;
 }
 
-int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps) {
+int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v) {
   if (b.count == 0) return 0;
   int ncmax = 1, lenmax = 2;
   for (int t = 0; t < b.count; t++) {
     int nc = std::min(b.r1[t], b.r2[t]), mm = std::max(b.r1[t], b.r2[t]);
-    ncmax = std::max(ncmax, nc); lenmax = std::max(lenmax, mm + nc);
+    ncmax = std::max(ncmax, nc); lenmax = std::max(lenmax, ((mm + 1) & ~1) + (with_v ? ((nc + 1) & ~1) : 0));
   }
   // smallest cluster whose per-CTA share of the columns fits shared memory and the staging regs
-  for (int CS = 1; CS <= 16; CS *= 2) {
+  // a CTA keeps at most ~16 column pairs busy per round (the pair rotations are LSU / issue bound
+  // beyond that, measured), so prefer the cluster size with bs <= 16, up to the portable 8
+  int cs0 = 1;
+  while (cs0 < 8 && (ncmax + 2 * cs0 - 1) / (2 * cs0) > 16) cs0 *= 2;
+  for (int CS = std::max(cs0, g_svd_min_cluster); CS <= 16; CS *= 2) {
     int bs = (ncmax + 2 * CS - 1) / (2 * CS);
     size_t smem = ((size_t)2 * bs * lenmax) * 8 + (size_t)(2 * bs + 2) * 4 + 64;
     bool fits = smem <= JC_SMEM_CAP && (CS == 1 || (size_t)2 * bs * lenmax <= (size_t)JC_STAGE * JC_THREADS);
@@ -444,7 +516,7 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel, b, tol, max_sweeps, bs, CS);
+    cudaError_t e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel, b, tol, max_sweeps, bs, CS, with_v ? 1 : 0, lenmax);
     if (e == cudaSuccess) { PEPO_COUNT_LAUNCH(); return 0; }
     (void)cudaGetLastError();                      // e.g. cluster of 16 not schedulable: try the fallback
     break;
@@ -470,7 +542,8 @@ int launch_svd_bridge(cudaStream_t st, const SvdFinishBatch& b, int chi_cap) {
   for (int t = 0; t < b.count; t++) w = std::max(w, (long long)(b.r1[t] + b.r2[t]) * chi_cap);
   long long g = std::min<long long>(std::max<long long>((w + 255) / 256, 1), 148 * 4);
   dim3 grid((unsigned)g, b.count);
-  svd_bridge_kernel<<<grid, 256, 0, st>>>(b);
+  if (b.with_v) svd_bridge_kernel<<<grid, 256, 0, st>>>(b);
+  else svd_bridge_nov_kernel<<<dim3(148 * 4, b.count), 256, 0, st>>>(b);
   PEPO_COUNT_LAUNCH();
   PEPO_CUDA_OK(cudaGetLastError());
   return 0;
