@@ -38,18 +38,27 @@ def hbm_peak():
     return 6650.0, "fallback"
 
 
-def time_ms(fn, reps, warm=3):
-    for _ in range(warm):
-        fn(0)
+def time_ms(fn, reps, warm=3, inner=6):
+    """Median / min milliseconds of one fn(i) call.  `inner` calls are captured into a CUDA graph
+    and replayed, so the CPU-side launch cost of the ctypes binding (tens of microseconds, more
+    than some of these kernels take) stays out of the measurement."""
+    for i in range(warm):
+        fn(i)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        for i in range(inner):
+            fn(i)
+    g.replay()
     torch.cuda.synchronize()
     ts = []
-    for i in range(reps):
+    for _ in range(reps):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        fn(i)
+        g.replay()
         e1.record()
         e1.synchronize()
-        ts.append(e0.elapsed_time(e1))
+        ts.append(e0.elapsed_time(e1) / inner)
     return statistics.median(ts), min(ts)
 
 
