@@ -74,6 +74,7 @@ struct TiledParams {
   int n[3];                          // full sizes of the three tile dims
   FastDiv tiles[3];                  // number of tiles along each tile dim
   FastDiv fdT[3], fdR[3];            // division by the full tile extent / by the remainder extent
+  FastDiv fdHT[3], fdHR[3];          // ... by half of them (128-bit variant)
   int rem[3];                        // extent of the last (ragged) tile, = T if it divides
   long long ss[3], ds[3];
   const double* scale[3];
@@ -158,6 +159,167 @@ __global__ void __launch_bounds__(256) permute_tiled_kernel(const double* __rest
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// 128-bit variants (the fast path): every global access is a 16-byte vector of two doubles.
+// Preconditions (checked by launch_permute): 16-byte aligned base pointers; the input-fastest
+// and the output-fastest (merged) dims have even extents; every other stride is even.
+// ---------------------------------------------------------------------------------------------
+struct RowsV2Params {
+  int rank;                          // dims incl. dim 0 (counted in double2 units)
+  uint32_t total2;                   // number of double2
+  FastDiv fd[MAXD];                  // fd[0] divides by n0/2
+  long long ss[MAXD], ds[MAXD];      // strides in doubles (ss[0] = ds[0] = 1 -> 2 per vector)
+  const double* scale[MAXD];
+};
+
+template <bool SCALED>
+__global__ void __launch_bounds__(256) permute_rows_v2_kernel(const double* __restrict__ src,
+                                                              double* __restrict__ dst,
+                                                              RowsV2Params P) {
+  constexpr int UNROLL = 4;
+  const uint32_t base = (blockIdx.x * (uint32_t)blockDim.x * UNROLL) + threadIdx.x;
+  double2 v[UNROLL];
+  long long doff[UNROLL];
+#pragma unroll
+  for (int u = 0; u < UNROLL; u++) {
+    const uint32_t idx = base + u * blockDim.x;
+    doff[u] = -1;
+    if (idx < P.total2) {
+      uint32_t rem = fd_div(idx, P.fd[0]);
+      const uint32_t j0 = idx - rem * P.fd[0].d;
+      long long so = 2ll * j0, dof = 2ll * j0;
+      double f = 1.0;
+#pragma unroll
+      for (int d = 1; d < MAXD; d++) {
+        if (d < P.rank) {
+          uint32_t q = fd_div(rem, P.fd[d]);
+          uint32_t c = rem - q * P.fd[d].d;
+          rem = q;
+          so += (long long)c * P.ss[d];
+          dof += (long long)c * P.ds[d];
+          if (SCALED && P.scale[d]) f *= __ldg(P.scale[d] + c);
+        }
+      }
+      double2 x = *reinterpret_cast<const double2*>(src + so);
+      if (SCALED) {
+        double f0 = f, f1 = f;
+        if (P.scale[0]) { f0 *= __ldg(P.scale[0] + 2 * j0); f1 *= __ldg(P.scale[0] + 2 * j0 + 1); }
+        x.x *= f0; x.y *= f1;
+      }
+      v[u] = x;
+      doff[u] = dof;
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < UNROLL; u++)
+    if (doff[u] >= 0) *reinterpret_cast<double2*>(dst + doff[u]) = v[u];
+}
+
+// Tiled transpose, same tile geometry as permute_tiled_kernel (TiledParams); T[0], T[1] and the
+// ragged remainders are even.  Phase 1 reads double2 along the input-fastest dim and stores the
+// two halves as 64-bit shared stores (odd pitch: conflict-free); phase 2 gathers two 64-bit
+// values one pitch apart and writes a double2 along the output-fastest dim.
+template <bool SCALED>
+__global__ void __launch_bounds__(256) permute_tiled_v2_kernel(const double* __restrict__ src,
+                                                               double* __restrict__ dst,
+                                                               TiledParams P) {
+  extern __shared__ double tile[];
+  uint32_t b = blockIdx.x;
+  int tc[3], ext[3];
+  bool ragged[3];
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    uint32_t q = fd_div(b, P.tiles[d]);
+    tc[d] = b - q * P.tiles[d].d;
+    b = q;
+    bool last = (tc[d] == (int)P.tiles[d].d - 1);
+    ext[d] = last ? P.rem[d] : P.T[d];
+    ragged[d] = last && P.rem[d] != P.T[d];
+  }
+  const FastDiv fh0 = ragged[0] ? P.fdHR[0] : P.fdHT[0];   // divide by ext[0]/2
+  const FastDiv fh1 = ragged[1] ? P.fdHR[1] : P.fdHT[1];   // divide by ext[1]/2
+  const FastDiv fe0 = ragged[0] ? P.fdR[0] : P.fdT[0];
+  const FastDiv fe1 = ragged[1] ? P.fdR[1] : P.fdT[1];
+  const FastDiv fe2 = ragged[2] ? P.fdR[2] : P.fdT[2];
+  long long sbase = 0, dbase = 0;
+  double fo = 1.0;
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    sbase += (long long)tc[d] * P.T[d] * P.ss[d];
+    dbase += (long long)tc[d] * P.T[d] * P.ds[d];
+  }
+  for (int d = 0; d < P.n_other; d++) {
+    uint32_t q = fd_div(b, P.ofd[d]);
+    uint32_t c = b - q * P.ofd[d].d;
+    b = q;
+    sbase += (long long)c * P.oss[d];
+    dbase += (long long)c * P.ods[d];
+    if (SCALED && P.oscale[d]) fo *= __ldg(P.oscale[d] + c);
+  }
+  const int pitch0 = P.pitch0, T1 = P.T[1];
+  constexpr int UN = 4;
+  // ---- phase 1 -------------------------------------------------------------------------------
+  {
+    const int E2 = (ext[0] >> 1) * ext[1] * ext[2];
+    for (int e0 = threadIdx.x; e0 < E2; e0 += 256 * UN) {
+      double2 x[UN];
+      int so[UN];
+#pragma unroll
+      for (int u = 0; u < UN; u++) {
+        const int e = e0 + u * 256;
+        so[u] = -1;
+        if (e < E2) {
+          uint32_t q = fd_div(e, fh0);
+          const int j0 = e - q * fh0.d;
+          int i1, i2;
+          if (P.in_b_before_a) { uint32_t q2 = fd_div(q, fe2); i2 = q - q2 * fe2.d; i1 = q2; }
+          else { uint32_t q2 = fd_div(q, fe1); i1 = q - q2 * fe1.d; i2 = q2; }
+          double2 v = *reinterpret_cast<const double2*>(src + sbase + 2 * j0 + i1 * P.ss[1] + i2 * P.ss[2]);
+          if (SCALED) {
+            double f = fo;
+            if (P.scale[1]) f *= __ldg(P.scale[1] + tc[1] * P.T[1] + i1);
+            if (P.scale[2]) f *= __ldg(P.scale[2] + tc[2] * P.T[2] + i2);
+            double f0 = f, f1 = f;
+            if (P.scale[0]) {
+              f0 *= __ldg(P.scale[0] + tc[0] * P.T[0] + 2 * j0);
+              f1 *= __ldg(P.scale[0] + tc[0] * P.T[0] + 2 * j0 + 1);
+            }
+            v.x *= f0; v.y *= f1;
+          }
+          x[u] = v;
+          so[u] = 2 * j0 + pitch0 * (i1 + T1 * i2);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < UN; u++)
+        if (so[u] >= 0) { tile[so[u]] = x[u].x; tile[so[u] + 1] = x[u].y; }
+    }
+  }
+  __syncthreads();
+  // ---- phase 2 -------------------------------------------------------------------------------
+  {
+    const int E2 = ext[0] * (ext[1] >> 1) * ext[2];
+    for (int e = threadIdx.x; e < E2; e += 256) {
+      uint32_t q = fd_div(e, fh1);
+      const int j1 = e - q * fh1.d;
+      int i0, i2;
+      if (P.out_b_before_0) { uint32_t q2 = fd_div(q, fe2); i2 = q - q2 * fe2.d; i0 = q2; }
+      else { uint32_t q2 = fd_div(q, fe0); i0 = q - q2 * fe0.d; i2 = q2; }
+      const int so = i0 + pitch0 * (2 * j1 + T1 * i2);
+      double2 v;
+      v.x = tile[so];
+      v.y = tile[so + pitch0];
+      *reinterpret_cast<double2*>(dst + dbase + i0 * P.ds[0] + 2 * j1 + i2 * P.ds[2]) = v;
+    }
+  }
+}
+
+inline int even_tile(int n, int cap) {      // n even: balanced even tile extent <= ~cap
+  int parts = (n + cap - 1) / cap;
+  int t = (n + parts - 1) / parts;
+  return (t + 1) & ~1;
+}
+
 inline int balanced_tile(int n, int cap) {
   int parts = (n + cap - 1) / cap;
   return (n + parts - 1) / parts;
@@ -203,6 +365,88 @@ int launch_permute(cudaStream_t st, const double* src, double* dst, const Permut
   int a = 0;
   for (int d = 1; d < r; d++) if (ds[d] < ds[a]) a = d;
 
+  // ---- 128-bit fast paths ---------------------------------------------------------------------
+  bool vec = (((uintptr_t)src | (uintptr_t)dst) & 15) == 0 && ss[0] == 1 && ds[a] == 1 &&
+             (n[0] % 2 == 0) && (n[a] % 2 == 0);
+  for (int d = 0; d < r && vec; d++) {
+    if (d != 0 && (ss[d] & 1)) vec = false;
+    if (d != a && (ds[d] & 1)) vec = false;
+  }
+  if (vec && a == 0) {
+    RowsV2Params P;
+    P.rank = r; P.total2 = (uint32_t)(total / 2);
+    for (int d = 0; d < MAXD; d++) {
+      if (d < r) { P.fd[d] = make_fastdiv(d == 0 ? n[0] / 2 : n[d]); P.ss[d] = ss[d]; P.ds[d] = ds[d]; P.scale[d] = sc[d]; }
+      else { P.fd[d] = make_fastdiv(1); P.ss[d] = 0; P.ds[d] = 0; P.scale[d] = nullptr; }
+    }
+    unsigned blocks = (unsigned)((total / 2 + 1023) / 1024);
+    if (scaled) permute_rows_v2_kernel<true><<<blocks, 256, 0, st>>>(src, dst, P);
+    else permute_rows_v2_kernel<false><<<blocks, 256, 0, st>>>(src, dst, P);
+    PEPO_COUNT_LAUNCH();
+    PEPO_CUDA_OK(cudaGetLastError());
+    return 0;
+  }
+  if (vec && total >= 4096) {
+    // tile = (dim 0) x (dim a) [x third dim when the tile would be small]: ~2048-4096 elements
+    const int T0 = even_tile(n[0], 64), Ta = even_tile(n[a], 64);
+    int bdim = -1, Tb = 1;
+    if (T0 * Ta < 2048 && r > 2) {
+      int ob = -1, ib = -1;              // next dim in output order after a / in input order after 0
+      for (int d = 0; d < r; d++) {
+        if (d == a || d == 0) continue;
+        if (ob < 0 || ds[d] < ds[ob]) ob = d;
+        if (ib < 0 || ss[d] < ss[ib]) ib = d;
+      }
+      // a short output run is lengthened by the next output dim unless that is dim 0 itself
+      // (then the run is already n[a]*n[0] long); otherwise lengthen the input side
+      bool out_next_is_0 = true;
+      for (int d = 1; d < r; d++) if (d != a && ds[d] < ds[0]) out_next_is_0 = false;
+      if (Ta < 32 && !out_next_is_0) bdim = ob; else bdim = ib;
+      if (bdim >= 0) {
+        int want = (2048 + T0 * Ta - 1) / (T0 * Ta);
+        Tb = balanced_tile(n[bdim], std::min(n[bdim], want));
+      }
+    }
+    TiledParams P;
+    const int td[3] = {0, a, bdim};
+    const int Tt[3] = {T0, Ta, Tb};
+    long long nblocks = 1;
+    for (int k = 0; k < 3; k++) {
+      int d = td[k];
+      int nn = (d >= 0) ? n[d] : 1;
+      P.T[k] = Tt[k]; P.n[k] = nn;
+      int nt = (nn + Tt[k] - 1) / Tt[k];
+      P.tiles[k] = make_fastdiv(nt);
+      P.rem[k] = nn - (nt - 1) * Tt[k];
+      P.fdT[k] = make_fastdiv(Tt[k]);
+      P.fdR[k] = make_fastdiv(P.rem[k]);
+      P.fdHT[k] = make_fastdiv(std::max(Tt[k] / 2, 1));
+      P.fdHR[k] = make_fastdiv(std::max(P.rem[k] / 2, 1));
+      P.ss[k] = (d >= 0) ? ss[d] : 0;
+      P.ds[k] = (d >= 0) ? ds[d] : 0;
+      P.scale[k] = (d >= 0) ? sc[d] : nullptr;
+      nblocks *= nt;
+    }
+    P.n_other = 0;
+    for (int d = 0; d < MAXD; d++) { P.ofd[d] = make_fastdiv(1); P.oss[d] = 0; P.ods[d] = 0; P.oscale[d] = nullptr; }
+    for (int d = 1; d < r; d++) {
+      if (d == a || d == bdim) continue;
+      int k = P.n_other++;
+      P.ofd[k] = make_fastdiv(n[d]); P.oss[k] = ss[d]; P.ods[k] = ds[d]; P.oscale[k] = sc[d];
+      nblocks *= n[d];
+    }
+    if (nblocks >= (1ll << 31)) { set_error("permute: grid too large"); return -1; }
+    P.pitch0 = T0 | 1;
+    P.in_b_before_a = (bdim >= 0 && ss[bdim] < ss[a]) ? 1 : 0;
+    P.out_b_before_0 = (bdim >= 0 && ds[bdim] < ds[0]) ? 1 : 0;
+    size_t smem = (size_t)P.pitch0 * Ta * Tb * sizeof(double);
+    if (scaled) permute_tiled_v2_kernel<true><<<(unsigned)nblocks, 256, smem, st>>>(src, dst, P);
+    else permute_tiled_v2_kernel<false><<<(unsigned)nblocks, 256, smem, st>>>(src, dst, P);
+    PEPO_COUNT_LAUNCH();
+    PEPO_CUDA_OK(cudaGetLastError());
+    return 0;
+  }
+  // ---- generic 64-bit paths (odd extents / misaligned) ---------------------------------------
   const bool tiled = (a != 0) && ss[0] == 1 && ds[a] == 1 && total >= 4096;
   if (!tiled) {
     RowsParams P;
