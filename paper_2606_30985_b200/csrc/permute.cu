@@ -388,7 +388,10 @@ int launch_permute(cudaStream_t st, const double* src, double* dst, const Permut
   }
   if (vec && total >= 4096) {
     // tile = (dim 0) x (dim a) [x third dim when the tile would be small]: ~2048-4096 elements
-    const int T0 = even_tile(n[0], 64), Ta = even_tile(n[a], 64);
+    // a short side (e.g. the Pauli dim, extent 4) is compensated by a longer other side
+    const int cap0 = (n[a] < 32) ? std::min(1024, 2048 / n[a]) : 64;
+    const int capa = (n[0] < 32) ? std::min(1024, 2048 / n[0]) : 64;
+    const int T0 = even_tile(n[0], cap0), Ta = even_tile(n[a], capa);
     int bdim = -1, Tb = 1;
     if (T0 * Ta < 2048 && r > 2) {
       int ob = -1, ib = -1;              // next dim in output order after a / in input order after 0
