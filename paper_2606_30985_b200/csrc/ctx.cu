@@ -211,6 +211,7 @@ struct pepo_ctx {
   double eps_cut = 1e-11, chol_ratio = 4.0, chol_tau = 1e-7, jacobi_tol = 1e-15;
   int bp_max_sweeps = 100, bp_max_sweeps_damped = 1000, jacobi_max_sweeps = 60;
   int force_hh = 0;
+  int svd_precond_min = 32;            // QR-precondition core SVDs with min(r1,r2) >= this (0: off)
   cudaStream_t st;
   int n_sites, n_bonds, n_hb;
   std::vector<SiteInfo> sites;
@@ -602,6 +603,7 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "jacobi_tol") c->jacobi_tol = v;
   else if (k == "jacobi_max_sweeps") c->jacobi_max_sweeps = (int)v;
   else if (k == "svd_min_cluster") set_svd_min_cluster((int)v);
+  else if (k == "svd_precond_min") c->svd_precond_min = (int)v;
   else if (k == "profile") {
     Prof& P = c->prof;
     if (v != 0.0 && P.ev.empty()) {
@@ -887,7 +889,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
   {
     DressBatch sc; sc.count = ng; sc.NA = NA;
     SvdBatch sb; sb.count = ng;
-    SvdFinishBatch fb; fb.count = ng; fb.with_v = 0;
+    SvdFinishBatch fb; fb.count = ng; fb.with_v = 0; fb.precond_min = c->svd_precond_min;
     for (int g = 0; g < ng; g++) {
       TaskGeo& t1 = T[2 * g]; TaskGeo& t2 = T[2 * g + 1];
       LaneWs& L = c->lanes[g];
@@ -916,7 +918,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
     }
     {
       ProfScope ps(c, PC_SVD, 0, 0);
-      rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps, false); if (rc) return rc;
+      rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps, false, c->svd_precond_min); if (rc) return rc;
       rc = launch_svd_truncate(st, fb, c->chi_max, c->eps_cut); if (rc) return rc;
     }
     PEPO_CUDA_OK(cudaMemcpyAsync(c->h_ints, c->lane_ints, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));

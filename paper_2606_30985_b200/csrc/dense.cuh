@@ -57,7 +57,10 @@ struct SvdBatch {
   int* sweeps[PEPO_MAXT];                           // device int
 };
 // with_v = false: V is not accumulated (launch_svd_bridge then derives it from K, SvdFinishBatch::K)
-int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v);
+// precond_min > 0 (only with_v = false): problems with min(r1,r2) >= precond_min are QR-preconditioned
+// (the Jacobi iteration runs on R^T); launch_svd_bridge must get the same value.
+int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
+                      int precond_min);
 void set_svd_min_cluster(int cs);
 
 struct SvdFinishBatch {
@@ -66,6 +69,7 @@ struct SvdFinishBatch {
   const double* G[PEPO_MAXT]; const double* V[PEPO_MAXT]; const double* sv[PEPO_MAXT];
   const int* order[PEPO_MAXT];
   int with_v;                                       // 1: V accumulated by the Jacobi kernel; 0: derive from K
+  int precond_min;                                  // as passed to launch_svd_jacobi (with_v = 0)
   const double* K[PEPO_MAXT]; int ldk[PEPO_MAXT];   // the core (needed when with_v = 0)
   double* Us[PEPO_MAXT]; int ldus[PEPO_MAXT];       // r1 x chi_new
   double* Vs[PEPO_MAXT]; int ldvs[PEPO_MAXT];       // r2 x chi_new

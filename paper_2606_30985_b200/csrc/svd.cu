@@ -170,7 +170,8 @@ __device__ __forceinline__ bool rotate_pair(double* cp, double* cq, int MP2, int
 }
 
 __global__ void __launch_bounds__(JC_THREADS, 1)
-jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int with_v, int LEN) {
+jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int with_v, int LEN,
+                      int precond_min, int pw) {
   extern __shared__ __align__(16) double jsm[];
   cg::cluster_group cluster = cg::this_cluster();
   const int crank = (int)cluster.block_rank();
@@ -181,7 +182,9 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
   // column layout: [G part: M, zero-padded to MP (even)] [V part: Nc, zero-padded, only with_v];
   // LEN (even, same for the whole launch) >= MP + (with_v ? Nc : 0)
   const int MP = (M + 1) & ~1;
-  const int MP2 = MP >> 1, LEN2 = LEN >> 1;
+  int Mj = M;                             // rows of the matrix the Jacobi iteration works on
+  int MP2 = MP >> 1;
+  const int LEN2 = LEN >> 1;
   const double tol2 = tol * tol;
   const double* K = b.K[t];
   const int ldk = b.ldk[t];
@@ -189,6 +192,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
   double* cols = jsm;
   int* ids = (int*)(cols + (size_t)2 * bs * LEN);
   double* scal = (double*)(ids + 2 * bs + (2 * bs & 1));     // [0] partial fro, [1] rotated flag
+  double* vbuf = scal + 4;                                    // pw x (MP + 2): Householder panel
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = JC_THREADS / 32;
   const int blk_of_slot[2] = {crank, 2 * CS - 1 - crank};
   // ---- load ---------------------------------------------------------------------------------
@@ -217,6 +221,102 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
   double ref = 0.0;
   for (int c = 0; c < CS; c++) ref += cluster.map_shared_rank(scal, c)[0];
   const double noise2 = 1e-30 * ref;
+  // ---- QR preconditioning (Drmac-Veselic): A = Q R by Householder reflections on the columns
+  // resident in the cluster, then iterate on L = R^T (Nc x Nc).  R R^T is one LR step closer to
+  // diagonal than R^T R, which roughly halves the number of sweeps; Q is never needed because
+  // the bridges are rebuilt from the untouched core K (svd_bridge_nov_kernel).
+  const bool precond = !with_v && precond_min > 0 && Nc >= precond_min && ref > 0.0 && isfinite(ref);
+  if (precond) {
+    // panels of <= pw consecutive columns (inside one block, i.e. inside one CTA): the owner
+    // factors the panel locally, broadcasts its reflectors once, every CTA applies them to its
+    // later columns: two cluster barriers per panel instead of per column.
+    const int VS = MP + 2;                               // stride of one reflector in vbuf
+    const int nblk = (Nc + bs - 1) / bs;
+    for (int blk = 0; blk < nblk; blk++) {
+      const int owner = blk < CS ? blk : 2 * CS - 1 - blk;
+      for (int p0 = 0; p0 < bs; p0 += pw) {
+        const int j0 = blk * bs + p0;
+        if (j0 >= Nc) break;
+        const int j1 = min(min(j0 + pw, (blk + 1) * bs), Nc);
+        if (crank == owner) {
+          double* pcols = cols + ((size_t)(blk < CS ? 0 : 1) * bs + p0) * LEN;   // panel columns
+          for (int j = j0; j < j1; j++) {
+            double* col = pcols + (size_t)(j - j0) * LEN;
+            double* vl = vbuf + (size_t)(j - j0) * VS;
+            if (warp == 0) {
+              double ss = 0.0;
+              for (int k = j + lane; k < M; k += 32) { double x = col[k]; ss += x * x; }
+              ss = warp_sum(ss);
+              const double ajj = col[j];
+              const double nrm = sqrt(ss);
+              const double alpha = (ajj > 0.0) ? -nrm : nrm;
+              const double vj = ajj - alpha;
+              const double vtv = ss - ajj * ajj + vj * vj;
+              for (int k = j + lane; k < M; k += 32) {
+                vl[k] = (k == j) ? vj : col[k];
+                col[k] = (k == j) ? alpha : 0.0;               // column j of R
+              }
+              if (lane == 0) vl[MP] = (vtv > 0.0) ? 2.0 / vtv : 0.0;
+            }
+            __syncthreads();
+            const double tau = vl[MP];
+            if (tau != 0.0) {
+              for (int jj = j + 1 + warp; jj < j1; jj += nw) {
+                double* c2 = pcols + (size_t)(jj - j0) * LEN;
+                double w = 0.0;
+                for (int k = j + lane; k < M; k += 32) w += vl[k] * c2[k];
+                w = warp_sum(w) * tau;
+                for (int k = j + lane; k < M; k += 32) c2[k] -= w * vl[k];
+              }
+            }
+            __syncthreads();
+          }
+          const int tot = (j1 - j0) * VS;
+          for (int c = 0; c < CS; c++) {
+            if (c == crank) continue;
+            double* rv = cluster.map_shared_rank(vbuf, c);
+            for (int e = tid; e < tot; e += JC_THREADS) rv[e] = vbuf[e];
+          }
+        }
+        cluster.sync();
+        for (int ci = warp; ci < 2 * bs; ci += nw) {
+          const int id = ids[ci];
+          if (id < j1 || id >= Nc) continue;
+          double* col = cols + (size_t)ci * LEN;
+          for (int j = j0; j < j1; j++) {
+            const double* vl = vbuf + (size_t)(j - j0) * VS;
+            const double tau = vl[MP];
+            if (tau == 0.0) continue;
+            double w = 0.0;
+            for (int k = j + lane; k < M; k += 32) w += vl[k] * col[k];
+            w = warp_sum(w) * tau;
+            for (int k = j + lane; k < M; k += 32) col[k] -= w * vl[k];
+          }
+        }
+        cluster.sync();
+      }
+    }
+    // transpose R through the global scratch G (ld M): new column i = row i of R
+    double* Gs = b.G[t];
+    for (int ci = warp; ci < 2 * bs; ci += nw) {
+      const int id = ids[ci];
+      if (id >= Nc) continue;
+      const double* col = cols + (size_t)ci * LEN;
+      for (int k = lane; k < Nc; k += 32) Gs[k + (size_t)id * M] = (k <= id) ? col[k] : 0.0;
+    }
+    __threadfence();
+    cluster.sync();
+    for (int ci = warp; ci < 2 * bs; ci += nw) {
+      const int id = ids[ci];
+      double* col = cols + (size_t)ci * LEN;
+      for (int k = lane; k < LEN; k += 32)
+        col[k] = (id < Nc && k < Nc && k >= id) ? Gs[id + (size_t)k * M] : 0.0;
+    }
+    __syncthreads();
+    cluster.sync();
+    Mj = Nc;
+    MP2 = ((Nc + 1) & ~1) >> 1;
+  }
   int sweeps = 0;
   const bool active = (Nc >= 2) && (ref > 0.0) && isfinite(ref);
   double* top = cols;
@@ -300,7 +400,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
     if (id >= Nc) continue;
     const double* col = cols + (size_t)ci * LEN;
     double s = 0.0;
-    for (int k = lane; k < M; k += 32) { double x = col[k]; s += x * x; G[(size_t)id * M + k] = x; }
+    for (int k = lane; k < Mj; k += 32) { double x = col[k]; s += x * x; G[(size_t)id * M + k] = x; }
     if (with_v) for (int k = lane; k < Nc; k += 32) V[(size_t)id * Nc + k] = col[MP + k];
     s = warp_sum(s);
     if (lane == 0) svu[id] = sqrt(s);
@@ -395,42 +495,48 @@ __global__ void __launch_bounds__(256) svd_bridge_nov_kernel(SvdFinishBatch b) {
   const int r1 = b.r1[t], r2 = b.r2[t];
   const bool tr = r1 < r2;
   const int M = tr ? r2 : r1, Nc = tr ? r1 : r2;
+  const bool precond = b.precond_min > 0 && Nc >= b.precond_min;
+  // columns of G (ld M): left vectors of the tall problem A (= K, or K^T if tr) times s; with the
+  // QR preconditioner instead its right vectors times s (length Nc).  Either way they are
+  // singular vectors of K on one side, and the other side is op(K) G / s.
+  const bool g_is_v = (tr != precond);                 // G holds right vectors of K
+  const int gr = g_is_v ? r2 : r1, zr = g_is_v ? r1 : r2;
   const int chin = *b.chi_new[t];
   const double* G = b.G[t];
   const double* K = b.K[t];
   const int ldk = b.ldk[t];
   const int* order = b.order[t];
   const double* sv = b.sv[t];
-  double* Gside = tr ? b.Vs[t] : b.Us[t];
-  const int ldg = tr ? b.ldvs[t] : b.ldus[t];
-  double* Zside = tr ? b.Us[t] : b.Vs[t];
-  const int ldz = tr ? b.ldus[t] : b.ldvs[t];
+  double* Gside = g_is_v ? b.Vs[t] : b.Us[t];
+  const int ldg = g_is_v ? b.ldvs[t] : b.ldus[t];
+  double* Zside = g_is_v ? b.Us[t] : b.Vs[t];
+  const int ldz = g_is_v ? b.ldus[t] : b.ldvs[t];
   const long long gtid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   const long long gthreads = (long long)gridDim.x * blockDim.x;
-  for (long long e = gtid; e < (long long)M * chin; e += gthreads) {
-    int row = (int)(e % M), c = (int)(e / M);
+  for (long long e = gtid; e < (long long)gr * chin; e += gthreads) {
+    int row = (int)(e % gr), c = (int)(e / gr);
     Gside[row + (long long)c * ldg] = G[row + (long long)order[c] * M] / sqrt(sv[c]);
   }
-  if (!tr) {
-    // Z[i,c] = sum_k K[k + i ldk] G[k + j M]: one warp per output, lanes along k
+  if (!g_is_v) {
+    // Z = K^T G: Z[i,c] = sum_{k<r1} K[k + i ldk] G[k + j M]: one warp per output, lanes along k
     const int lane = threadIdx.x & 31;
     const long long gw = gtid >> 5, nwarps = gthreads >> 5;
-    for (long long e = gw; e < (long long)Nc * chin; e += nwarps) {
-      int i = (int)(e % Nc), c = (int)(e / Nc);
+    for (long long e = gw; e < (long long)zr * chin; e += nwarps) {
+      int i = (int)(e % zr), c = (int)(e / zr);
       const double* kc = K + (long long)i * ldk;
       const double* gc = G + (long long)order[c] * M;
       double z = 0.0;
-      for (int k = lane; k < M; k += 32) z += kc[k] * gc[k];
+      for (int k = lane; k < gr; k += 32) z += kc[k] * gc[k];
       z = warp_sum(z);
       if (lane == 0) { double sc = sv[c]; Zside[i + (long long)c * ldz] = z / (sc * sqrt(sc)); }
     }
   } else {
-    // Z[i,c] = sum_k K[i + k ldk] G[k + j M]: one thread per output, coalesced along i
-    for (long long e = gtid; e < (long long)Nc * chin; e += gthreads) {
-      int i = (int)(e % Nc), c = (int)(e / Nc);
+    // Z = K G: Z[i,c] = sum_{k<r2} K[i + k ldk] G[k + j M]: one thread per output, coalesced along i
+    for (long long e = gtid; e < (long long)zr * chin; e += gthreads) {
+      int i = (int)(e % zr), c = (int)(e / zr);
       const double* gc = G + (long long)order[c] * M;
       double z = 0.0;
-      for (int k = 0; k < M; k++) z += K[i + (long long)k * ldk] * gc[k];
+      for (int k = 0; k < gr; k++) z += K[i + (long long)k * ldk] * gc[k];
       double sc = sv[c];
       Zside[i + (long long)c * ldz] = z / (sc * sqrt(sc));
     }
@@ -484,7 +590,8 @@ int launch_set_identity(cudaStream_t st, double* Q, long long m, int k) {
   return 0;
 }
 
-int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v) {
+int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
+                      int precond_min) {
   if (b.count == 0) return 0;
   int ncmax = 1, lenmax = 2;
   for (int t = 0; t < b.count; t++) {
@@ -498,7 +605,11 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
   while (cs0 < 8 && (ncmax + 2 * cs0 - 1) / (2 * cs0) > 16) cs0 *= 2;
   for (int CS = std::max(cs0, g_svd_min_cluster); CS <= 16; CS *= 2) {
     int bs = (ncmax + 2 * CS - 1) / (2 * CS);
-    size_t smem = ((size_t)2 * bs * lenmax) * 8 + (size_t)(2 * bs + 2) * 4 + 64;
+    size_t smem0 = ((size_t)2 * bs * lenmax) * 8 + (size_t)(2 * bs + 2) * 4 + 64;
+    int pw = 0;                                        // Householder panel width (preconditioner)
+    if (!with_v && precond_min > 0 && smem0 < JC_SMEM_CAP)
+      pw = (int)std::min<size_t>((size_t)bs, (JC_SMEM_CAP - smem0) / ((size_t)(lenmax + 2) * 8));
+    size_t smem = smem0 + (size_t)std::max(pw, 1) * (lenmax + 2) * 8;
     bool fits = smem <= JC_SMEM_CAP && (CS == 1 || (size_t)2 * bs * lenmax <= (size_t)JC_STAGE * JC_THREADS);
     if (!fits) continue;
     static bool attr_done = false;
@@ -516,11 +627,13 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel, b, tol, max_sweeps, bs, CS, with_v ? 1 : 0, lenmax);
+    cudaError_t e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel, b, tol, max_sweeps, bs, CS, with_v ? 1 : 0, lenmax,
+                                       (with_v || pw < 1) ? 0 : precond_min, std::max(pw, 1));
     if (e == cudaSuccess) { PEPO_COUNT_LAUNCH(); return 0; }
     (void)cudaGetLastError();                      // e.g. cluster of 16 not schedulable: try the fallback
     break;
   }
+  if (!with_v && precond_min > 0) { set_error("svd: cluster launch failed"); return -3; }
   size_t smem = (size_t)ncmax * sizeof(double);
   jacobi_svd_kernel<<<b.count, 1024, smem, st>>>(b, tol, max_sweeps);
   PEPO_COUNT_LAUNCH();
