@@ -9,6 +9,7 @@
 // zero-filled outside the matrix) through a STAGES-deep ring; shared tiles are XOR-swizzled
 // so that the 64-bit fragment loads of a half-warp hit 16 distinct bank pairs.
 #include "common.cuh"
+#include <cstdlib>
 
 namespace pepo {
 
@@ -221,15 +222,39 @@ int launch_trans(cudaStream_t st, int ta, int tb, const GemmProb& p, const GemmP
 
 }  // namespace
 
+// Tile shapes (measured on B200, 216000 x 240 x 240 and 256000 x 160 x 160): two or three
+// resident CTAs per SM matter more than a large tile, because the k loop of these products is
+// short (K = n = 4 chi for the reconstruction GEMM) and one CTA's epilogue must overlap another's
+// main loop; tiles that divide n exactly (80 | 4 chi for chi = 20, 40, 60, 100) waste no DMMA.
+enum TileCfg { T_64x64, T_128x128, T_128x64, T_64x80, T_80x80 };
+
+static TileCfg pick_tile(long long M, int N, int ksplit, bool upper_only) {
+  const long long tiles128 = ((M + 127) / 128) * ((N + 127) / 128) * ksplit;
+  if (upper_only) {
+    if (M == N && N % 80 == 0) return T_80x80;
+    return (tiles128 >= 120 && N > 64) ? T_128x128 : T_64x64;
+  }
+  if (tiles128 < 120 || N <= 64) return T_64x64;
+  if (N % 80 == 0) return T_64x80;
+  return T_128x64;
+}
+
 int launch_dgemm(cudaStream_t st, int transA, int transB, const GemmProb& p, int ksplit,
                  int kchunk, double* part, bool upper_only) {
   if (p.M <= 0 || p.N <= 0) return 0;
   if (ksplit < 1) ksplit = 1;
-  // big tile when the problem fills the machine with it, small tile otherwise
-  long long tiles128 = ((p.M + 127) / 128) * ((p.N + 127) / 128) * ksplit;
-  if (tiles128 >= 120 && p.N > 64)
-    return launch_trans<128, 128, 64, 32, 4>(st, transA, transB, p, nullptr, ksplit, p.M, p.N, ksplit, kchunk, part, upper_only);
-  return launch_trans<64, 64, 32, 32, 4>(st, transA, transB, p, nullptr, ksplit, p.M, p.N, ksplit, kchunk, part, upper_only);
+  switch (pick_tile(p.M, p.N, ksplit, upper_only)) {
+    case T_80x80:
+      return launch_trans<80, 80, 40, 40, 4>(st, transA, transB, p, nullptr, ksplit, p.M, p.N, ksplit, kchunk, part, upper_only);
+    case T_64x80:
+      return launch_trans<64, 80, 32, 40, 4>(st, transA, transB, p, nullptr, ksplit, p.M, p.N, ksplit, kchunk, part, upper_only);
+    case T_128x64:
+      return launch_trans<128, 64, 32, 32, 4>(st, transA, transB, p, nullptr, ksplit, p.M, p.N, ksplit, kchunk, part, upper_only);
+    case T_128x128:
+      return launch_trans<128, 128, 64, 32, 4>(st, transA, transB, p, nullptr, ksplit, p.M, p.N, ksplit, kchunk, part, upper_only);
+    default:
+      return launch_trans<64, 64, 32, 32, 4>(st, transA, transB, p, nullptr, ksplit, p.M, p.N, ksplit, kchunk, part, upper_only);
+  }
 }
 
 int launch_dgemm_batched(cudaStream_t st, int transA, int transB, const GemmProb* probs_dev,
@@ -239,17 +264,17 @@ int launch_dgemm_batched(cudaStream_t st, int transA, int transB, const GemmProb
 }
 
 void gram_plan(long long m, int n, int* ksplit, int* kchunk) {
-  // tiles of the upper triangle at the tile size launch_dgemm will pick
-  int tn128 = (n + 127) / 128;
-  int upper128 = tn128 * (tn128 + 1) / 2;
-  int tn64 = (n + 63) / 64;
-  int upper64 = tn64 * (tn64 + 1) / 2;
-  int target = 148 * 2;
-  int ks = (int)((target + upper128 - 1) / upper128);
-  if (n <= 64) ks = (target + upper64 - 1) / upper64;
+  // upper-triangle tiles at the tile size launch_dgemm will pick (the choice between the 128 and
+  // 64 tiles depends on ksplit itself: plan with the 128 tile first, as before)
+  int bt = 128, target = 148 * 2, cap = 128;
+  if (n % 80 == 0) { bt = 80; target = 148 * 4; cap = 100; }     // 128-thread CTAs, 4 resident per SM
+  else if (n <= 64) bt = 64;
+  const int tn = (n + bt - 1) / bt;
+  const int upper = tn * (tn + 1) / 2;
+  int ks = (target + upper - 1) / upper;
   long long maxsplit = (m + 255) / 256;             // at least 256 rows per split
   if (ks > maxsplit) ks = (int)maxsplit;
-  if (ks > 128) ks = 128;
+  if (ks > cap) ks = cap;
   if (ks < 1) ks = 1;
   long long kc = (m + ks - 1) / ks;
   kc = (kc + 15) / 16 * 16;
