@@ -62,6 +62,7 @@ struct SvdBatch {
 int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
                       int precond_min);
 void set_svd_min_cluster(int cs);
+void set_svd_block(int on);
 
 struct SvdFinishBatch {
   int count;

@@ -22,6 +22,43 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
+// Short-latency fp64 reciprocal square root / reciprocal for the rotation parameters: hardware
+// approximation (MUFU.RSQ64H / RCP64H, ~2^-22) + two Newton steps (-> a few ulp).  The library
+// sqrt()/division are long dependent instruction sequences with special-case branches and sit on
+// the critical path of every pair rotation.  Arguments here are positive, finite and normal
+// (guarded by the noise test); a rotation stays orthogonal to rounding for any c, s = c t.
+__device__ __forceinline__ double fast_rsqrt(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double hx = 0.5 * x;
+#pragma unroll
+  for (int it = 0; it < 2; it++) {
+    const double e = fma(-hx * y, y, 0.5);
+    y = fma(y, e, y);
+  }
+  return y;
+}
+__device__ __forceinline__ double fast_rcp(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+#pragma unroll
+  for (int it = 0; it < 2; it++) {
+    const double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+  }
+  return y;
+}
+// (c, s) of the Jacobi rotation that orthogonalises two columns with squared norms al, be and
+// inner product ga: t = sgn(zeta)/(|zeta| + sqrt(1 + zeta^2)), zeta = (be - al)/(2 ga).
+__device__ __forceinline__ void jacobi_cs(double al, double be, double ga, double& cs, double& sn) {
+  const double d = be - al, g2 = 2.0 * ga;
+  const double h = fma(d, d, g2 * g2);
+  const double r = h * fast_rsqrt(h);                      // sqrt(d^2 + g2^2) > 0
+  const double tt = g2 * fast_rcp(d + copysign(r, d));
+  cs = fast_rsqrt(fma(tt, tt, 1.0));
+  sn = cs * tt;
+}
+
 __global__ void __launch_bounds__(1024) jacobi_svd_kernel(SvdBatch b, double tol, int max_sweeps) {
   extern __shared__ double snorm[];     // Nc doubles
   __shared__ double s_red[32];
@@ -134,6 +171,7 @@ __global__ void __launch_bounds__(1024) jacobi_svd_kernel(SvdBatch b, double tol
 // the round-robin circle through distributed shared memory (staged in registers between two
 // cluster barriers).  No global-memory traffic inside the iteration.
 // ---------------------------------------------------------------------------------------------
+int g_svd_block = 0;                    // tunable (option "svd_block"): block form of the super-rounds
 int g_svd_min_cluster = 1;              // tunable (option "svd_min_cluster"): smallest cluster size tried
 constexpr int JC_THREADS = 1024;
 constexpr int JC_STAGE = 26;            // doubles staged per thread during a block exchange
@@ -156,9 +194,8 @@ __device__ __forceinline__ bool rotate_pair(double* cp, double* cq, int MP2, int
   if (ga * ga <= tol2 * al * be) return false;          // |ga| <= tol ||p|| ||q||
   // tan of the rotation angle, smaller root: t = sgn(zeta)/(|zeta| + sqrt(1 + zeta^2)), zeta =
   // (be - al)/(2 ga), written with one sqrt and one division
-  const double d = be - al, g2 = 2.0 * ga;
-  const double tt = g2 / (d + copysign(sqrt(d * d + g2 * g2), d));
-  const double cs = rsqrt(1.0 + tt * tt), sn = cs * tt;
+  double cs, sn;
+  jacobi_cs(al, be, ga, cs, sn);
   for (int k = lane; k < LEN2; k += 32) {
     double2 x = p2[k], y = q2[k];
     double2 xn, yn;
@@ -169,9 +206,141 @@ __device__ __forceinline__ bool rotate_pair(double* cp, double* cq, int MP2, int
   return true;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Block form of one super-round (top block x bottom block, bs rounds of bs disjoint pairs).
+// The pair rotations of a round need only the Gram matrix of the 2 bs resident columns, so:
+//   A. W = X^T X from the columns (fresh inner products, once per super-round);
+//   B. the bs rounds run on W alone (two-sided update of a 2bs x 2bs matrix) and accumulate the
+//      rotations into J (orthogonal by construction: a product of plane rotations);
+//   C. X <- X J, one pass over the columns (ALU-bound, 2 LEN (2bs)^2 flop).
+// Same pairs, same order, same angle formula as the column-wise rounds; the latency-bound part
+// (reductions + the scalar rotation arithmetic of every pair) now touches 2bs-vectors instead of
+// LEN-vectors.  The "any rotation" flag is taken from the fresh W (step A), i.e. from inner
+// products of the actual columns, as in the column-wise form.
+// Shared: Wm, Jm: n2 x PW (PW even >= n2), rc/rs: bs doubles each.  LEN/2 odd: conflict-free.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void rot_params(double al, double be, double ga, double tol2, double noise2,
+                                           double& cs, double& sn) {
+  cs = 1.0; sn = 0.0;
+  if (al < noise2 || be < noise2 || !(al > 0.0) || !(be > 0.0)) return;
+  if (ga * ga <= tol2 * al * be) return;
+  jacobi_cs(al, be, ga, cs, sn);
+}
+
+__device__ bool block_superround(double* top, int bs, int LEN, int MP2, double tol2, double noise2,
+                                 double* Wm, double* Jm, double* rc, double* rs, int PW) {
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int n2 = 2 * bs, LEN2 = LEN >> 1;
+  const double2* X2 = reinterpret_cast<const double2*>(top);      // column c at X2 + c*LEN2
+  // ---- A: Gram (upper triangle, two threads per entry) ---------------------------------------
+  const int npair = n2 * (n2 + 1) / 2;
+  bool rot = false;
+  for (int e0 = 0; e0 < npair; e0 += JC_THREADS / 2) {
+    const int e = e0 + (tid >> 1);
+    double v = 0.0;
+    int i = 0, j = 0;
+    if (e < npair) {
+      // e -> (i <= j): row-major enumeration of the upper triangle
+      int rem = e;
+      i = 0;
+      int rowlen = n2;
+      while (rem >= rowlen) { rem -= rowlen; rowlen--; i++; }
+      j = i + rem;
+      const double2* xi = X2 + (size_t)i * LEN2;
+      const double2* xj = X2 + (size_t)j * LEN2;
+      for (int k = (tid & 1); k < MP2; k += 2) {
+        const double2 a = xi[k], b = xj[k];
+        v += a.x * b.x;
+        v += a.y * b.y;
+      }
+    }
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    if (e < npair && (tid & 1) == 0) { Wm[i * PW + j] = v; Wm[j * PW + i] = v; }
+  }
+  for (int e = tid; e < n2 * PW; e += JC_THREADS) Jm[e] = ((e / PW) == (e % PW)) ? 1.0 : 0.0;
+  __syncthreads();
+  // ---- B: bs rounds on W, rotations accumulated in J -----------------------------------------
+  for (int r = 0; r < bs; r++) {
+    if (tid < bs) {
+      const int pp = tid;
+      int q = tid + r; if (q >= bs) q -= bs;
+      q += bs;
+      double cs, sn;
+      rot_params(Wm[pp * PW + pp], Wm[q * PW + q], Wm[pp * PW + q], tol2, noise2, cs, sn);
+      rc[tid] = cs; rs[tid] = sn;
+      rot |= (sn != 0.0);
+    }
+    __syncthreads();
+    // column phase: W[:,p], W[:,q] and J[:,p], J[:,q]
+    {
+      const int half = JC_THREADS / 2;
+      double* Mx = (tid < half) ? Wm : Jm;
+      for (int e = (tid < half ? tid : tid - half); e < n2 * bs; e += half) {
+        const int t = e % bs, i = e / bs;
+        int q = t + r; if (q >= bs) q -= bs;
+        q += bs;
+        const double cs = rc[t], sn = rs[t];
+        if (sn != 0.0) {
+          const double x = Mx[i * PW + t], y = Mx[i * PW + q];
+          Mx[i * PW + t] = cs * x - sn * y;
+          Mx[i * PW + q] = sn * x + cs * y;
+        }
+      }
+    }
+    __syncthreads();
+    // row phase: W[p,:], W[q,:]
+    for (int e = tid; e < n2 * bs; e += JC_THREADS) {
+      const int j = e % n2, t = e / n2;
+      int q = t + r; if (q >= bs) q -= bs;
+      q += bs;
+      const double cs = rc[t], sn = rs[t];
+      if (sn != 0.0) {
+        const double x = Wm[t * PW + j], y = Wm[q * PW + j];
+        Wm[t * PW + j] = cs * x - sn * y;
+        Wm[q * PW + j] = sn * x + cs * y;
+      }
+    }
+    __syncthreads();
+  }
+  // ---- C: X <- X J (rows independent: in place after a barrier per pass) ----------------------
+  {
+    double2* Xw = reinterpret_cast<double2*>(top);
+    const int ng = (n2 + 3) / 4;                       // groups of 4 output columns
+    const int rpp = JC_THREADS / ng;                   // row pairs per pass (all groups of a row in one pass)
+    for (int k0 = 0; k0 < LEN2; k0 += rpp) {
+      const int k2 = k0 + tid % rpp, jg = tid / rpp;
+      const bool act = (jg < ng) && (k2 < LEN2);
+      const int j0 = jg * 4;
+      double2 acc0 = make_double2(0.0, 0.0), acc1 = acc0, acc2 = acc0, acc3 = acc0;
+      if (act) {
+        for (int i = 0; i < n2; i++) {
+          const double2 x = Xw[(size_t)i * LEN2 + k2];
+          const double2 ja = *reinterpret_cast<const double2*>(Jm + i * PW + j0);
+          const double2 jb = *reinterpret_cast<const double2*>(Jm + i * PW + j0 + 2);
+          acc0.x += x.x * ja.x; acc0.y += x.y * ja.x;
+          acc1.x += x.x * ja.y; acc1.y += x.y * ja.y;
+          acc2.x += x.x * jb.x; acc2.y += x.y * jb.x;
+          acc3.x += x.x * jb.y; acc3.y += x.y * jb.y;
+        }
+      }
+      __syncthreads();
+      if (act) {
+        Xw[(size_t)j0 * LEN2 + k2] = acc0;
+        if (j0 + 1 < n2) Xw[(size_t)(j0 + 1) * LEN2 + k2] = acc1;
+        if (j0 + 2 < n2) Xw[(size_t)(j0 + 2) * LEN2 + k2] = acc2;
+        if (j0 + 3 < n2) Xw[(size_t)(j0 + 3) * LEN2 + k2] = acc3;
+      }
+      __syncthreads();
+    }
+  }
+  (void)lane;
+  return rot;
+}
+
+template <int STAGE, int NREG>
 __global__ void __launch_bounds__(JC_THREADS, 1)
 jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int with_v, int LEN,
-                      int precond_min, int pw) {
+                      int precond_min, int pw, int use_block) {
   extern __shared__ __align__(16) double jsm[];
   cg::cluster_group cluster = cg::this_cluster();
   const int crank = (int)cluster.block_rank();
@@ -191,8 +360,13 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
   // shared layout: cols[2][bs][LEN], ids[2][bs] (as double-aligned ints), scal[4]
   double* cols = jsm;
   int* ids = (int*)(cols + (size_t)2 * bs * LEN);
-  double* scal = (double*)(ids + 2 * bs + (2 * bs & 1));     // [0] partial fro, [1] rotated flag
+  double* scal = (double*)(ids + ((2 * bs + 3) & ~3));        // [0] partial fro, [1] rotated flag
   double* vbuf = scal + 4;                                    // pw x (MP + 2): Householder panel
+  const int PW = (2 * bs + 3) & ~3;                           // pitch of the small matrices W, J
+  double* Wm = vbuf + (size_t)pw * (MP + 2);                  // block form: Gram of the resident columns
+  double* Jm = Wm + (size_t)2 * bs * PW;                      //             accumulated rotations
+  double* rc = Jm + (size_t)2 * bs * PW;
+  double* rs = rc + bs;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = JC_THREADS / 32;
   const int blk_of_slot[2] = {crank, 2 * CS - 1 - crank};
   // ---- load ---------------------------------------------------------------------------------
@@ -339,12 +513,69 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
     }
     // super-rounds
     for (int sr = 0; sr < 2 * CS - 1; sr++) {
-      for (int r = 0; r < bs; r++) {
-        for (int i = warp; i < bs; i += nw) {
-          int j = i + r; if (j >= bs) j -= bs;
-          rot |= rotate_pair(top + (size_t)i * LEN, bot + (size_t)j * LEN, MP2, LEN2, tol2, noise2, lane);
+      if (use_block) {
+        rot |= block_superround(top, bs, LEN, MP2, tol2, noise2, Wm, Jm, rc, rs, PW);
+      } else if (NREG > 0) {
+        // The pair rotations are shared-memory-bandwidth bound (each touches two LEN-vectors three
+        // times).  Warp i keeps top column i in registers for the bs rounds of the super-round, so
+        // only the bottom column of each pair moves through shared memory.
+        double2 tp[NREG > 0 ? NREG : 1];
+        const bool own = warp < bs;
+        double2* tcol = reinterpret_cast<double2*>(top + (size_t)(own ? warp : 0) * LEN);
+        if (own) {
+#pragma unroll
+          for (int q = 0; q < NREG; q++) {
+            const int k = lane + 32 * q;
+            tp[q] = (k < LEN2) ? tcol[k] : make_double2(0.0, 0.0);
+          }
+        }
+        for (int r = 0; r < bs; r++) {
+          if (own) {
+            int j = warp + r; if (j >= bs) j -= bs;
+            double2* cq = reinterpret_cast<double2*>(bot + (size_t)j * LEN);
+            double2 y[NREG > 0 ? NREG : 1];
+            double al = 0.0, be = 0.0, ga = 0.0;
+#pragma unroll
+            for (int q = 0; q < NREG; q++) {
+              const int k = lane + 32 * q;
+              y[q] = (k < LEN2) ? cq[k] : make_double2(0.0, 0.0);
+              if (k < MP2) {
+                al += tp[q].x * tp[q].x; be += y[q].x * y[q].x; ga += tp[q].x * y[q].x;
+                al += tp[q].y * tp[q].y; be += y[q].y * y[q].y; ga += tp[q].y * y[q].y;
+              }
+            }
+            al = warp_sum(al); be = warp_sum(be); ga = warp_sum(ga);
+            if (!(al < noise2 || be < noise2 || !(al > 0.0) || !(be > 0.0)) && !(ga * ga <= tol2 * al * be)) {
+              double cs, sn;
+              jacobi_cs(al, be, ga, cs, sn);
+#pragma unroll
+              for (int q = 0; q < NREG; q++) {
+                const int k = lane + 32 * q;
+                const double2 x = tp[q];
+                tp[q].x = cs * x.x - sn * y[q].x; tp[q].y = cs * x.y - sn * y[q].y;
+                if (k < LEN2) cq[k] = make_double2(sn * x.x + cs * y[q].x, sn * x.y + cs * y[q].y);
+              }
+              rot = true;
+            }
+          }
+          __syncthreads();
+        }
+        if (own) {
+#pragma unroll
+          for (int q = 0; q < NREG; q++) {
+            const int k = lane + 32 * q;
+            if (k < LEN2) tcol[k] = tp[q];
+          }
         }
         __syncthreads();
+      } else {
+        for (int r = 0; r < bs; r++) {
+          for (int i = warp; i < bs; i += nw) {
+            int j = i + r; if (j >= bs) j -= bs;
+            rot |= rotate_pair(top + (size_t)i * LEN, bot + (size_t)j * LEN, MP2, LEN2, tol2, noise2, lane);
+          }
+          __syncthreads();
+        }
       }
       if (CS > 1) {
         cluster.sync();                           // A: every CTA finished computing
@@ -357,10 +588,10 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
         const double* src_bot; const int* src_bot_id;
         if (crank == CS - 1) { src_bot = top; src_bot_id = ids; }
         else { src_bot = cluster.map_shared_rank(bot, crank + 1); src_bot_id = cluster.map_shared_rank(ids + bs, crank + 1); }
-        double stage[JC_STAGE];
+        double stage[STAGE];
         int id_stage = -1;
 #pragma unroll
-        for (int q = 0; q < JC_STAGE; q++) {
+        for (int q = 0; q < STAGE; q++) {
           int e = tid + q * JC_THREADS;
           double v = 0.0;
           if (e < per) { if (src_top) v = src_top[e]; }
@@ -371,7 +602,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
         else if (tid < 2 * bs) id_stage = src_bot_id[tid - bs];
         cluster.sync();                           // B: every CTA finished reading
 #pragma unroll
-        for (int q = 0; q < JC_STAGE; q++) {
+        for (int q = 0; q < STAGE; q++) {
           int e = tid + q * JC_THREADS;
           if (e < per) { if (src_top) top[e] = stage[q]; }
           else if (e < 2 * per) bot[e - per] = stage[q];
@@ -569,6 +800,7 @@ __global__ void set_identity_kernel(double* Q, long long m, int k) {
 
 }  // namespace
 
+void set_svd_block(int on) { g_svd_block = on ? 1 : 0; }
 void set_svd_min_cluster(int cs) { g_svd_min_cluster = cs < 1 ? 1 : (cs > 16 ? 16 : cs); }
 
 int launch_svd_vectors(cudaStream_t st, const double* G, const double* V, const double* s,
@@ -599,25 +831,22 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
     ncmax = std::max(ncmax, nc); lenmax = std::max(lenmax, ((mm + 1) & ~1) + (with_v ? ((nc + 1) & ~1) : 0));
   }
   // smallest cluster whose per-CTA share of the columns fits shared memory and the staging regs
+  if (((lenmax >> 1) & 1) == 0) lenmax += 2;          // LEN/2 odd: columns start in distinct 16-byte bank groups
   // a CTA keeps at most ~16 column pairs busy per round (the pair rotations are LSU / issue bound
   // beyond that, measured), so prefer the cluster size with bs <= 16, up to the portable 8
   int cs0 = 1;
   while (cs0 < 8 && (ncmax + 2 * cs0 - 1) / (2 * cs0) > 16) cs0 *= 2;
   for (int CS = std::max(cs0, g_svd_min_cluster); CS <= 16; CS *= 2) {
     int bs = (ncmax + 2 * CS - 1) / (2 * CS);
-    size_t smem0 = ((size_t)2 * bs * lenmax) * 8 + (size_t)(2 * bs + 2) * 4 + 64;
+    const int PW = (2 * bs + 3) & ~3;
+    size_t smem0 = ((size_t)2 * bs * lenmax) * 8 + (size_t)(2 * bs + 4) * 4 + 64 +
+                   ((size_t)4 * bs * PW + 2 * bs) * 8;
     int pw = 0;                                        // Householder panel width (preconditioner)
     if (!with_v && precond_min > 0 && smem0 < JC_SMEM_CAP)
       pw = (int)std::min<size_t>((size_t)bs, (JC_SMEM_CAP - smem0) / ((size_t)(lenmax + 2) * 8));
     size_t smem = smem0 + (size_t)std::max(pw, 1) * (lenmax + 2) * 8;
     bool fits = smem <= JC_SMEM_CAP && (CS == 1 || (size_t)2 * bs * lenmax <= (size_t)JC_STAGE * JC_THREADS);
     if (!fits) continue;
-    static bool attr_done = false;
-    if (!attr_done) {
-      PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
-      PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-      attr_done = true;
-    }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(b.count * CS));
     cfg.blockDim = dim3(JC_THREADS);
@@ -627,8 +856,44 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel, b, tol, max_sweeps, bs, CS, with_v ? 1 : 0, lenmax,
-                                       (with_v || pw < 1) ? 0 : precond_min, std::max(pw, 1));
+    // registers staged per thread during a block exchange: smallest instantiation that holds a CTA's columns
+    const size_t need = (CS == 1) ? 0 : ((size_t)2 * bs * lenmax + JC_THREADS - 1) / JC_THREADS;
+    const int pmin = (with_v || pw < 1) ? 0 : precond_min;
+    const int pwk = std::max(pw, 1), wv = with_v ? 1 : 0;
+    cudaError_t e;
+    if (need <= 8 && lenmax / 2 <= 128 && bs <= JC_THREADS / 32) {
+      static bool done84 = false;
+      if (!done84) {
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<8, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<8, 4>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        done84 = true;
+      }
+      e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel<8, 4>, b, tol, max_sweeps, bs, CS, wv, lenmax, pmin, pwk, g_svd_block);
+    } else if (need <= 8) {
+      static bool done8 = false;
+      if (!done8) {
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<8, 0>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        done8 = true;
+      }
+      e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel<8, 0>, b, tol, max_sweeps, bs, CS, wv, lenmax, pmin, pwk, g_svd_block);
+    } else if (need <= 16) {
+      static bool done16 = false;
+      if (!done16) {
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<16, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<16, 0>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        done16 = true;
+      }
+      e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel<16, 0>, b, tol, max_sweeps, bs, CS, wv, lenmax, pmin, pwk, g_svd_block);
+    } else {
+      static bool done26 = false;
+      if (!done26) {
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<JC_STAGE, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<JC_STAGE, 0>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        done26 = true;
+      }
+      e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel<JC_STAGE, 0>, b, tol, max_sweeps, bs, CS, wv, lenmax, pmin, pwk, g_svd_block);
+    }
     if (e == cudaSuccess) { PEPO_COUNT_LAUNCH(); return 0; }
     (void)cudaGetLastError();                      // e.g. cluster of 16 not schedulable: try the fallback
     break;
