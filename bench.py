@@ -151,16 +151,13 @@ def one_step(sim):
 
 def run_ours(args):
     import torch
-    import torch.distributed as dist
     from paper_2606_30985_b200 import binding as B
+    from paper_2606_30985_b200 import replicas as R
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    world, rank, local = R.world()
     dev = torch.device("cuda", local)
     torch.cuda.set_device(dev)
+    R.init("nccl", dev)
     L, chi = args.grid, args.chi
     sim = B.Pepo(L, L, args.cx, args.cy, J, H, DT, chi, args.bp_tol, args.bp_damping, device=str(dev))
     for kv in args.opt:
@@ -169,9 +166,7 @@ def run_ours(args):
     info = prepare(sim, args)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        R.barrier(dev)
 
     # ---- device-resident timing ---------------------------------------------------------------
     for _ in range(args.warmup):
@@ -203,10 +198,7 @@ def run_ours(args):
     prof = sim.profile()
     sim.set_option("profile", 0)
     launches = sim.stats()["kernel_launches"] - launches0
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = R.max_over_ranks(ms, dev)
     stats = sim.stats()
 
     # ---- end-to-end: host buffers in, host scalar out, copies inside the timed region ----------
@@ -239,10 +231,7 @@ def run_ours(args):
             e2e_step()
         barrier()
         dt_e2e = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt_e2e], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt_e2e = float(t.item())
+        dt_e2e = R.max_over_ranks(dt_e2e, dev)
         e2e = {"value": world * args.steps / dt_e2e, "unit": "Trotter steps/s",
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": 8 + 8 + 4 * sim.n_bonds,
                "note": "state uploaded from pinned host memory every step, C(t) read back"}
@@ -439,9 +428,8 @@ def main():
         else:
             line["cpu_baseline"] = None
         print(json.dumps(line), flush=True)
-    if world > 1:
-        import torch.distributed as dist
-        dist.destroy_process_group()
+    from paper_2606_30985_b200 import replicas as R
+    R.finish()
     return 0
 
 
