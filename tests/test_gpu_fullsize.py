@@ -1,0 +1,177 @@
+"""GPU parity at BASELINE.json's full sizes (-m gpu), in the launch configuration bench.py times:
+
+* config 3: all 120 permutations of the (4,40,40,40,40) tensor bit-exact; Cholesky-QR of the
+  256000 x 40 / 256000 x 160 matrices against the oracle's Householder QR;
+* config 2 sizes: gate replay on the seeded synthetic saturated 4x4 chi = 60 state - the oracle's
+  single Algorithm-1 gate on the same inputs, compared through gauge-invariant quantities
+  (lambda, chi_new, sampled entries of the two-site tensor; reading R17);
+* config 2 physics: the first steps of the real 4x4 chi_max = 60 run against the oracle
+  trajectory (bonds still small, so the oracle finishes in seconds) and, on the saturated state
+  bench.py times, properties that hold at any size (normalised lambda, descending spectrum,
+  read-only BP, |C| <= 1).
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+J, H, DT = 1.0, 0.9, 0.05
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2606_30985_b200 import binding
+    return torch, binding
+
+
+def test_config3_all_120_permutations_bit_exact(gpu):
+    torch, B = gpu
+    from paper_2606_30985_b200 import inputs
+    chi = 40
+    shape = [chi, chi, chi, chi, 4]                       # column-major dims of C-order (4,chi,chi,chi,chi)
+    src = inputs.normal_tensor(shape, seed=1)
+    d_src = torch.from_numpy(src).cuda()
+    d_dst = torch.empty_like(d_src)
+    # oracle on the full tensor: the definition itself (R10 = numpy.transpose on the column-major
+    # shape; oracle.permute_listing1 is pinned to it on small tensors in tests/test_oracle_pins.py)
+    t = src.reshape(shape, order="F")
+    for perm in itertools.permutations(range(5)):
+        want = np.transpose(t, perm).flatten(order="F")
+        got = B.permute(d_src, shape, perm, dst=d_dst).cpu().numpy()
+        assert np.array_equal(got.view(np.int64), want.view(np.int64)), perm
+
+
+@pytest.mark.parametrize("m,n", [(256000, 40), (256000, 160)])
+def test_config3_cholqr_vs_oracle(gpu, m, n):
+    torch, B = gpu
+    from oracle import pepo_oracle as po
+    from paper_2606_30985_b200 import inputs
+    A = inputs.normal_tensor((m, n), seed=1).reshape((m, n), order="F")
+    d_A = torch.from_numpy(np.asfortranarray(A).flatten(order="F")).cuda()
+    Q, R, info = B.cholqr(d_A, m, n)
+    assert int(info.item()) == 0
+    Qh = Q.cpu().numpy().reshape((m, n), order="F")
+    Rh = R.cpu().numpy().reshape((n, n), order="F")
+    assert np.allclose(np.tril(Rh, -1), 0.0)
+    fro = np.linalg.norm(A)
+    assert np.linalg.norm(Qh @ Rh - A) / fro <= 1e-12
+    assert np.linalg.norm(Qh.T @ Qh - np.eye(n)) <= 1e-11
+    # against the oracle's Householder factor, rows sign-normalised (unique for full column rank)
+    _, Ro = po.householder_qr(A)
+    sg = np.sign(np.diag(Rh)) * np.sign(np.diag(Ro))
+    assert np.linalg.norm(Rh - sg[:, None] * Ro) / np.linalg.norm(Ro) <= 1e-11
+
+
+def _load_synthetic(sim, L, chi):
+    from paper_2606_30985_b200 import inputs
+    chis, psi, lam = inputs.synthetic_state(L, L, chi)
+    sim.set_bond_dims(chis)
+    for e, l in enumerate(lam):
+        sim.set_lambda(e, l)
+    for v, t in psi.items():
+        sim.set_site(v % L, v // L, t)
+    return chis, psi, lam
+
+
+def _oracle_state(L, chi):
+    from oracle import pepo_oracle as po
+    from paper_2606_30985_b200 import inputs
+    st = po.PEPOState(L, L, 1, 1, J, H, DT, chi)
+    chis, psi, lam = inputs.synthetic_state(L, L, chi)
+    for v in range(L * L):
+        x, y = v % L, v // L
+        dims = [chis[inputs.bond_id(L, L, x, y, d)] for d in inputs.site_legs(L, L, x, y)] + [4]
+        st.psi[v] = np.asarray(psi[v]).reshape(dims, order="F").copy()
+    st.lam = [np.asarray(l) for l in lam]
+    return st
+
+
+def _two_site_samples(t1, ax1, t2, ax2, idx1, idx2):
+    """Theta[i1, i2] = sum_c t1[i1 with cut=c] t2[i2 with cut=c] on sampled multi-indices."""
+    a = np.moveaxis(t1, ax1, -1)
+    b = np.moveaxis(t2, ax2, -1)
+    return np.einsum("sc,sc->s", a[tuple(idx1.T)], b[tuple(idx2.T)])
+
+
+@pytest.mark.parametrize("which", ["corner-edge", "edge-interior", "interior-interior"])
+def test_gate_replay_4x4_chi60(gpu, which):
+    """One Algorithm-1 gate at full size (chi = 60, m up to 216000) on the same seeded inputs."""
+    torch, B = gpu
+    from paper_2606_30985_b200 import inputs
+    L, chi = 4, 60
+    bond = {"corner-edge": inputs.bond_id(L, L, 0, 0, "R"),
+            "edge-interior": inputs.bond_id(L, L, 0, 1, "R"),
+            "interior-interior": inputs.bond_id(L, L, 1, 1, "R")}[which]
+    sim = B.Pepo(L, L, 1, 1, J, H, DT, chi, 1e-10, 0.5)
+    _load_synthetic(sim, L, chi)
+    st = _oracle_state(L, chi)
+    sim.apply_bond(bond)
+    st.apply_bond_gate(bond)
+    assert sim.bond_dims()[bond] == st.lam[bond].size == chi
+    lam_g = sim.get_lambda(bond)
+    assert np.allclose(lam_g, st.lam[bond], rtol=1e-9, atol=1e-13)
+    v1, d1, v2, d2 = st.lat.bond_sites(bond)
+    legs1, legs2 = st.lat.legs(v1), st.lat.legs(v2)
+    g1 = sim.get_site(v1 % L, v1 // L).reshape(st.psi[v1].shape, order="F")
+    g2 = sim.get_site(v2 % L, v2 // L).reshape(st.psi[v2].shape, order="F")
+    ax1, ax2 = legs1.index(d1), legs2.index(d2)
+    rng = np.random.default_rng(7)
+    ns = 4000
+    sh1 = [s for a, s in enumerate(g1.shape) if a != ax1]
+    sh2 = [s for a, s in enumerate(g2.shape) if a != ax2]
+    idx1 = np.stack([rng.integers(0, s, ns) for s in sh1], axis=1)
+    idx2 = np.stack([rng.integers(0, s, ns) for s in sh2], axis=1)
+    th_g = _two_site_samples(g1, ax1, g2, ax2, idx1, idx2)
+    th_o = _two_site_samples(st.psi[v1], ax1, st.psi[v2], ax2, idx1, idx2)
+    scale = np.linalg.norm(th_o) / np.sqrt(ns)
+    assert np.max(np.abs(th_g - th_o)) <= 1e-9 * scale, np.max(np.abs(th_g - th_o)) / scale
+    sim.close()
+
+
+def test_config2_first_steps_vs_oracle(gpu):
+    """BASELINE configs[1] from the product operator: 8 steps (bonds up to ~41) against the oracle."""
+    torch, B = gpu
+    from oracle import pepo_oracle as po
+    steps = 8
+    sim = B.Pepo(4, 4, 1, 1, J, H, DT, 60, 1e-10, 0.5)
+    st = po.PEPOState(4, 4, 1, 1, J, H, DT, 60)
+    for t in range(steps):
+        sim.trotter_step()
+        st.trotter_step()
+        assert sim.bond_dims() == st.bond_dims(), (t + 1, sim.bond_dims(), st.bond_dims())
+        sg, swg, _ = sim.bp_converge()
+        so, swo, _ = st.bp_converge(1e-10, 0.5)
+        assert sg == so and abs(swg - swo) <= 1
+        assert abs(sim.correlation() - st.correlation()) <= 1e-10
+    sim.close()
+
+
+def test_config2_saturated_properties(gpu):
+    """On the state bench.py times (every bond = 60 after the physical preparation) no oracle run
+    is affordable: check what holds at any size."""
+    torch, B = gpu
+    sim = B.Pepo(4, 4, 1, 1, J, H, DT, 60, 1e-10, 0.5)
+    n = 0
+    while min(sim.bond_dims()) < 60 and n < 40:
+        sim.trotter_step()
+        n += 1
+    assert min(sim.bond_dims()) == 60
+    sim.trotter_step()
+    for e in range(sim.n_bonds):
+        lam = sim.get_lambda(e)
+        assert abs(np.linalg.norm(lam) - 1.0) < 1e-12
+        assert np.all(np.diff(lam) <= 0) and lam[-1] > 0
+    before = [sim.get_site(x, y).copy() for y in range(4) for x in range(4)]
+    status, sweeps, delta = sim.bp_converge()
+    c = sim.correlation()
+    after = [sim.get_site(x, y) for y in range(4) for x in range(4)]
+    assert all(np.array_equal(a, b) for a, b in zip(before, after))          # R16: BP is read-only
+    assert status in (0, 1) and abs(c) <= 1.0 + 1e-9
+    s = sim.stats()
+    assert 0.0 <= s["gate_err"] < 1e-3
+    assert s["arena_high_water"] <= s["arena_model_bytes"] * 1.02 + 65536
+    sim.close()
