@@ -23,11 +23,13 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 constexpr int BP_THREADS = 256;
-constexpr int BP_MAXK = 8;     // dU <= 256
+constexpr int BP_MAXK = 8;     // dU <= 256 (kernel instantiated for 32*KU >= dU, KU in {2,4,8}: fewer
+                               // registers -> more resident CTAs -> more bytes in flight)
 
+template <int KU>
 __global__ void __launch_bounds__(BP_THREADS) bp_partial_kernel(BpBatch b) {
   constexpr int nw = BP_THREADS / 32;
-  __shared__ double sU[nw][32 * BP_MAXK];
+  __shared__ double sU[nw][32 * KU];
   __shared__ double sS[PEPO_BP_MAXCHUNK][nw];
   const int t = blockIdx.y;
   const BpSite& S = b.s[t];
@@ -39,10 +41,10 @@ __global__ void __launch_bounds__(BP_THREADS) bp_partial_kernel(BpBatch b) {
   const double* mU = S.in[0];
   const double* mD = S.in[1];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  double accU[BP_MAXK];
-  double mu[BP_MAXK];
+  double accU[KU];
+  double mu[KU];
 #pragma unroll
-  for (int k = 0; k < BP_MAXK; k++) {
+  for (int k = 0; k < KU; k++) {
     accU[k] = 0.0;
     int u = lane + 32 * k;
     mu[k] = (u < dU) ? mU[u] : 0.0;
@@ -66,7 +68,7 @@ __global__ void __launch_bounds__(BP_THREADS) bp_partial_kernel(BpBatch b) {
       const double mdw = md * w, mdw2 = has2 ? md2 * w : 0.0;
       double cs = 0.0, cs2 = 0.0;
 #pragma unroll
-      for (int k = 0; k < BP_MAXK; k++) {
+      for (int k = 0; k < KU; k++) {
         int u = lane + 32 * k;
         if (u < dU) {
           double tv = col[u], tv2 = col2[u];
@@ -88,7 +90,7 @@ __global__ void __launch_bounds__(BP_THREADS) bp_partial_kernel(BpBatch b) {
     if (lane == 0) sS[lr - lr0][warp] = ssum;
   }
 #pragma unroll
-  for (int k = 0; k < BP_MAXK; k++) sU[warp][lane + 32 * k] = accU[k];
+  for (int k = 0; k < KU; k++) sU[warp][lane + 32 * k] = accU[k];
   __syncthreads();
   for (int u = threadIdx.x; u < dU; u += BP_THREADS) {
     double p = 0.0;
@@ -127,9 +129,22 @@ __global__ void __launch_bounds__(256) bp_finalize_kernel(BpBatch b, double damp
   double nrm2 = 0.0, dot_old = 0.0, dot_in = 0.0;
   const double* old = S.out_old[slot];
   const double* inc = S.in[slot];
+  // slots 0/1: sum of the per-chunk partial vectors, 4 thread groups per entry, fixed order
+  __shared__ double sgrp[4][64];
+  const bool split = (slot < 2) && dl <= 64;
+  if (split) {
+    const int i = threadIdx.x & 63, gq = threadIdx.x >> 6;
+    const double* part = slot == 0 ? S.partU : S.partD;
+    double v = 0.0;
+    if (i < dl) for (int k = gq; k < S.nchunks; k += 4) v += part[(long long)k * dl + i];
+    sgrp[gq][i] = v;
+    __syncthreads();
+  }
   for (int i = threadIdx.x; i < dl; i += blockDim.x) {
     double v = 0.0;
-    if (slot == 0) {
+    if (split) {
+      v = (sgrp[0][i] + sgrp[1][i]) + (sgrp[2][i] + sgrp[3][i]);
+    } else if (slot == 0) {
       for (int k = 0; k < S.nchunks; k++) v += S.partU[(long long)k * dU + i];
     } else if (slot == 1) {
       for (int k = 0; k < S.nchunks; k++) v += S.partD[(long long)k * dD + i];
@@ -257,7 +272,11 @@ int launch_bp_partial(cudaStream_t st, const BpBatch& b) {
   int maxlr = 1;
   for (int t = 0; t < b.count; t++) maxlr = std::max(maxlr, b.s[t].nchunks);
   dim3 grid(maxlr, b.count);
-  bp_partial_kernel<<<grid, BP_THREADS, 0, st>>>(b);
+  int dumax = 1;
+  for (int t = 0; t < b.count; t++) dumax = std::max(dumax, b.s[t].d[0]);
+  if (dumax <= 64) bp_partial_kernel<2><<<grid, BP_THREADS, 0, st>>>(b);
+  else if (dumax <= 128) bp_partial_kernel<4><<<grid, BP_THREADS, 0, st>>>(b);
+  else bp_partial_kernel<8><<<grid, BP_THREADS, 0, st>>>(b);
   PEPO_COUNT_LAUNCH();
   PEPO_CUDA_OK(cudaGetLastError());
   return 0;

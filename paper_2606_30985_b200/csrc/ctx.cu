@@ -933,6 +933,13 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       T[2 * g].chi_new = T[2 * g + 1].chi_new = cn;
       chi_cap = std::max(chi_cap, cn);
       c->stats.jacobi_sweeps += c->h_ints[4 * g + 1];
+      if (c->prof.on) {
+        // algorithmic flops of the one-sided Jacobi iteration: per sweep Nc(Nc-1)/2 pairs, each
+        // 3 inner products (6 L flop) + one plane rotation of two L-vectors (6 L flop)
+        const double Nc = std::min(T[2 * g].r, T[2 * g + 1].r), Mx = std::max(T[2 * g].r, T[2 * g + 1].r);
+        const double Lc = (c->svd_precond_min > 0 && Nc >= c->svd_precond_min) ? Nc : Mx;
+        c->prof.flops[PC_SVD] += c->h_ints[4 * g + 1] * 0.5 * Nc * (Nc - 1) * 12.0 * Lc;
+      }
       c->stats.gate_err += c->h_dbls[2 * g];
       c->stats.min_cut_gap = std::min(c->stats.min_cut_gap, c->h_dbls[2 * g + 1]);
     }
