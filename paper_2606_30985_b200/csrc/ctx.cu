@@ -929,7 +929,16 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
     int chi_cap = 1;
     for (int g = 0; g < ng; g++) {
       int cn = c->h_ints[4 * g];
-      if (cn < 1) { set_error("gate on bond %d: s0 = 0 or NaN in the core SVD", gate_bonds[g]); return -4; }
+      if (cn < 1) {
+        // diagnostics: leading entries of the core and of the computed spectrum
+        double hk[4] = {0, 0, 0, 0}, hs[2] = {0, 0};
+        const int r1 = T[2 * g].r, r2 = T[2 * g + 1].r;
+        cudaMemcpy(hk, c->lanes[g].K, sizeof(double) * std::min(4, r1 * r2), cudaMemcpyDeviceToHost);
+        cudaMemcpy(hs, c->lanes[g].sv, sizeof(double) * std::min(2, std::min(r1, r2)), cudaMemcpyDeviceToHost);
+        set_error("gate on bond %d: s0 = 0 or NaN in the core SVD (core %d x %d, K[0..3] = %g %g %g %g, s[0..1] = %g %g, "
+                  "sweeps %d)", gate_bonds[g], r1, r2, hk[0], hk[1], hk[2], hk[3], hs[0], hs[1], c->h_ints[4 * g + 1]);
+        return -4;
+      }
       T[2 * g].chi_new = T[2 * g + 1].chi_new = cn;
       chi_cap = std::max(chi_cap, cn);
       c->stats.jacobi_sweeps += c->h_ints[4 * g + 1];

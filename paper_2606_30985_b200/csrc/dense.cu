@@ -241,7 +241,11 @@ __device__ void hh_reflect(const double* __restrict__ x, double* __restrict__ y,
   const double nrm = sqrt(sxx);
   double beta = (x0 >= 0.0) ? -nrm : nrm;
   double tau = 0.0;
-  if (nrm > 0.0) tau = 1.0 / (nrm * (nrm + fabs(x0)));
+  // tau = 2 / v^T v overflows for ||x|| < ~1e-154 (underflow-level columns occur at the light-cone
+  // front, where entries are products of rounding noise): such a column is numerically zero, its
+  // reflector is the identity and R_jj = x_0
+  if (sxx > 1e-290) tau = 1.0 / (nrm * (nrm + fabs(x0)));
+  else beta = x0;
   if (beta_out && gtid == 0) { *beta_out = beta; *tau_out = tau; }
   if (!y || tau == 0.0) return;
   const double y0 = y[0];

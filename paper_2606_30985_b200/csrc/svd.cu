@@ -430,7 +430,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
                 vl[k] = (k == j) ? vj : col[k];
                 col[k] = (k == j) ? alpha : 0.0;               // column j of R
               }
-              if (lane == 0) vl[MP] = (vtv > 0.0) ? 2.0 / vtv : 0.0;
+              if (lane == 0) vl[MP] = (vtv > 1e-290) ? 2.0 / vtv : 0.0;     // identity for underflow-level columns
             }
             __syncthreads();
             const double tau = vl[MP];

@@ -1,0 +1,106 @@
+"""Run one of the BASELINE.json configurations end to end through the C ABI and print C(t):
+
+    python -m paper_2606_30985_b200.run --config 2 [--steps N] [--chi CHI] [--json out.json]
+
+configs (BASELINE.json "configs", 1-based; config 3 is the kernel microbenchmark, see
+``python -m paper_2606_30985_b200.microbench``):
+  1: 3x3, centre (1,1), chi_max 8, 10 steps, BP tol 1e-10, no damping
+  2: 4x4, centre (1,1), chi_max 60, 60 steps, BP tol 1e-10, damping 0.5
+  4: 8x8, centre (3,3), chi_max 60, 40 steps, BP tol 1e-9, damping 0.5
+  5: 10x10, centre (4,4), chi_max = largest value whose memory model fits the free HBM
+     (<= 100), 30 steps, BP tol 1e-8, damping 0.5
+TFIM J = 1, h = 0.9, dt = 0.05, first-order Trotter (readings R1, R2).  Every step:
+trotter_step, bp_converge, correlation; wall-clock per phase is measured with CUDA events.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import time
+
+import torch
+
+from . import binding as B
+
+CONFIGS = {
+    1: dict(L=3, c=(1, 1), chi=8, steps=10, tol=1e-10, damping=0.0),
+    2: dict(L=4, c=(1, 1), chi=60, steps=60, tol=1e-10, damping=0.5),
+    4: dict(L=8, c=(3, 3), chi=60, steps=40, tol=1e-9, damping=0.5),
+    5: dict(L=10, c=(4, 4), chi=100, steps=30, tol=1e-8, damping=0.5),
+}
+
+
+def fit_chi(L, chi_cap, free_bytes, inflight=0):
+    """Largest chi_max <= chi_cap whose arena (analytic memory model) fits free_bytes."""
+    for chi in range(chi_cap, 0, -1):
+        need = B.arena_bytes(L, L, chi, inflight)
+        if 0 < need <= free_bytes:
+            return chi, need
+    raise RuntimeError("no chi_max fits %d bytes" % free_bytes)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", type=int, default=1, choices=sorted(CONFIGS))
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--chi", type=int, default=None)
+    ap.add_argument("--inflight", type=int, default=0)
+    ap.add_argument("--json", default=None)
+    args = ap.parse_args()
+    cfg = dict(CONFIGS[args.config])
+    if args.steps is not None:
+        cfg["steps"] = args.steps
+    if args.chi is not None:
+        cfg["chi"] = args.chi
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    L = cfg["L"]
+    free, total = torch.cuda.mem_get_info(dev)
+    inflight = args.inflight
+    if args.config == 5 and inflight == 0:
+        inflight = 2
+    chi, need = fit_chi(L, cfg["chi"], int(free * 0.985), inflight)
+    if chi != cfg["chi"]:
+        print("# chi_max %d does not fit %.1f GB free HBM; memory model picks chi_max = %d (%.1f GB)"
+              % (cfg["chi"], free / 1e9, chi, need / 1e9), flush=True)
+    sim = B.Pepo(L, L, cfg["c"][0], cfg["c"][1], 1.0, 0.9, 0.05, chi, cfg["tol"], cfg["damping"], device=str(dev),
+                 max_inflight=inflight)
+    rows = []
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    t_start = time.perf_counter()
+    for step in range(1, cfg["steps"] + 1):
+        ev[0].record()
+        sim.trotter_step()
+        ev[1].record()
+        status, sweeps, delta = sim.bp_converge()
+        c = sim.correlation()
+        ev[2].record()
+        ev[2].synchronize()
+        st = sim.stats()
+        dims = sim.bond_dims()
+        row = dict(step=step, C=c, trotter_ms=ev[0].elapsed_time(ev[1]), bp_ms=ev[1].elapsed_time(ev[2]),
+                   bp_status=status, bp_sweeps=sweeps, bp_delta=delta, chi_min=min(dims), chi_max=max(dims),
+                   gate_err=st["gate_err"], jacobi_sweeps=st["jacobi_sweeps"], n_cholesky=st["n_cholesky"],
+                   n_householder=st["n_householder"], n_chol_failed=st["n_chol_failed"])
+        rows.append(row)
+        print("step %3d  C = % .12f  trotter %9.2f ms  bp %8.2f ms (%4d sweeps, status %d)  chi [%d, %d]  gate_err %.2e"
+              % (step, c, row["trotter_ms"], row["bp_ms"], sweeps, status, row["chi_min"], row["chi_max"], st["gate_err"]),
+              flush=True)
+    wall = time.perf_counter() - t_start
+    st = sim.stats()
+    sat = [r for r in rows if r["chi_min"] == chi]
+    summary = dict(config=args.config, L=L, chi_max=chi, steps=cfg["steps"], wall_s=wall,
+                   trotter_s=sum(r["trotter_ms"] for r in rows) * 1e-3, bp_s=sum(r["bp_ms"] for r in rows) * 1e-3,
+                   steps_per_s_whole_run=cfg["steps"] / (sum(r["trotter_ms"] for r in rows) * 1e-3),
+                   steps_per_s_saturated=(len(sat) / (sum(r["trotter_ms"] for r in sat) * 1e-3)) if sat else None,
+                   arena_bytes=st["arena_high_water"], arena_model_bytes=st["arena_model_bytes"],
+                   inflight_gates=st["max_inflight_gates"], kernel_launches=st["kernel_launches"])
+    print("# " + json.dumps(summary), flush=True)
+    if args.json:
+        with open(args.json, "w") as f:
+            json.dump(dict(summary=summary, rows=rows), f)
+    sim.close()
+
+
+if __name__ == "__main__":
+    main()
