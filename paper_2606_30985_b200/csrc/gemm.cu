@@ -116,6 +116,9 @@ dgemm_dmma_kernel(GemmProb p0, const GemmProb* __restrict__ probs, int ksplit, i
   const bool alignedA = (((uintptr_t)p.A & 15) == 0) && ((p.lda & 1) == 0) && ((kbeg & 1) == 0);
   const bool alignedB = (((uintptr_t)p.B & 15) == 0) && ((p.ldb & 1) == 0) && ((kbeg & 1) == 0);
 
+  // Gram (upper_only) diagonal tiles: a warp tile strictly below the diagonal is never read by the
+  // reducer, so its warp only helps with the loads (frees its DMMA issue slots for co-resident CTAs)
+  const bool skip_warp = upper_only && tn == tm && BM == BN && (wm0 >= wn0 + WN);
   double acc[MI][NI][2];
 #pragma unroll
   for (int i = 0; i < MI; i++)
@@ -141,6 +144,7 @@ dgemm_dmma_kernel(GemmProb p0, const GemmProb* __restrict__ probs, int ksplit, i
     issue(it + STAGES - 1);
     const double* a_s = sA + (it % STAGES) * BM * BK;
     const double* b_s = sB + (it % STAGES) * BN * BK;
+    if (skip_warp) continue;
 #pragma unroll
     for (int kk = 0; kk < BK; kk += 4) {
       double af[MI], bf[NI];
@@ -164,6 +168,7 @@ dgemm_dmma_kernel(GemmProb p0, const GemmProb* __restrict__ probs, int ksplit, i
   }
   cp_async_wait<0>();
 
+  if (skip_warp) return;
   double* Cb = p.C;
   long long ldc = p.ldc;
   if (ksplit > 1) { Cb = part + (long long)split * M * N; ldc = M; }
