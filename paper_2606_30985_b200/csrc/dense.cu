@@ -101,14 +101,34 @@ __global__ void __launch_bounds__(512) potrf_upper_kernel(MatBatch b, InfoPtrs i
       }
       __syncthreads();
       // trailing update of the upper triangle
-      const long long tot = (long long)rest * rest;
-      for (long long e = tid; e < tot; e += blockDim.x) {
-        int i = (int)(e % rest), j = (int)(e / rest);
-        if (i <= j) {
-          double s = 0.0;
-          for (int l = 0; l < nb; l++) s += Ps[l * rest + i] * Ps[l * rest + j];
-          A[(c0 + i) + (long long)(c0 + j) * ld] -= s;
+      // four independent elements per thread and pass: the global (L2) round trips of the
+      // read-modify-write overlap instead of serialising (this loop was latency-bound)
+      const int tot = rest * rest;
+      for (int e0 = tid; e0 < tot; e0 += 4 * blockDim.x) {
+        double av[4], sv[4];
+        double* ap[4];
+#pragma unroll
+        for (int u = 0; u < 4; u++) {
+          const int e = e0 + u * blockDim.x;
+          ap[u] = nullptr;
+          if (e < tot) {
+            const int i = e % rest, j = e / rest;
+            if (i <= j) { ap[u] = A + (c0 + i) + (long long)(c0 + j) * ld; av[u] = *ap[u]; }
+          }
         }
+#pragma unroll
+        for (int u = 0; u < 4; u++) {
+          const int e = e0 + u * blockDim.x;
+          sv[u] = 0.0;
+          if (ap[u]) {
+            const int i = e % rest, j = e / rest;
+            double s = 0.0;
+            for (int l = 0; l < nb; l++) s += Ps[l * rest + i] * Ps[l * rest + j];
+            sv[u] = s;
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; u++) if (ap[u]) *ap[u] = av[u] - sv[u];
       }
     }
     __syncthreads();
