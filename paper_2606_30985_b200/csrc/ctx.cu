@@ -605,6 +605,7 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "svd_min_cluster") set_svd_min_cluster((int)v);
   else if (k == "svd_precond_min") c->svd_precond_min = (int)v;
   else if (k == "svd_block") set_svd_block((int)v);
+  else if (k == "svd_c16") set_svd_c16((int)v);
   else if (k == "profile") {
     Prof& P = c->prof;
     if (v != 0.0 && P.ev.empty()) {

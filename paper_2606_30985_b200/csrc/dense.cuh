@@ -63,6 +63,7 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
                       int precond_min);
 void set_svd_min_cluster(int cs);
 void set_svd_block(int on);
+void set_svd_c16(int on);
 
 struct SvdFinishBatch {
   int count;

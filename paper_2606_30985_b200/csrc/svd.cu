@@ -22,6 +22,28 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
+// 64-bit butterfly exchange through the two 32-bit halves (keeps the compiler from swapping the
+// halves around a register-pair shuffle) and the reductions built on it.  warp_sum3 interleaves
+// three independent reductions so their shuffle latencies overlap.
+__device__ __forceinline__ double shfl_xor_f64(double v, int o) {
+  int lo = __double2loint(v), hi = __double2hiint(v);
+  lo = __shfl_xor_sync(0xffffffffu, lo, o);
+  hi = __shfl_xor_sync(0xffffffffu, hi, o);
+  return __hiloint2double(hi, lo);
+}
+__device__ __forceinline__ double warp_sum1(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += shfl_xor_f64(v, o);
+  return v;
+}
+__device__ __forceinline__ void warp_sum3(double& a, double& b, double& c) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const double a2 = shfl_xor_f64(a, o), b2 = shfl_xor_f64(b, o), c2 = shfl_xor_f64(c, o);
+    a += a2; b += b2; c += c2;
+  }
+}
+
 // Short-latency fp64 reciprocal square root / reciprocal for the rotation parameters: hardware
 // approximation (MUFU.RSQ64H / RCP64H, ~2^-22) + two Newton steps (-> a few ulp).  The library
 // sqrt()/division are long dependent instruction sequences with special-case branches and sit on
@@ -50,13 +72,17 @@ __device__ __forceinline__ double fast_rcp(double x) {
 }
 // (c, s) of the Jacobi rotation that orthogonalises two columns with squared norms al, be and
 // inner product ga: t = sgn(zeta)/(|zeta| + sqrt(1 + zeta^2)), zeta = (be - al)/(2 ga).
-__device__ __forceinline__ void jacobi_cs(double al, double be, double ga, double& cs, double& sn) {
+__device__ __forceinline__ void jacobi_cst(double al, double be, double ga, double& cs, double& sn, double& tt) {
   const double d = be - al, g2 = 2.0 * ga;
   const double h = fma(d, d, g2 * g2);
   const double r = h * fast_rsqrt(h);                      // sqrt(d^2 + g2^2) > 0
-  const double tt = g2 * fast_rcp(d + copysign(r, d));
+  tt = g2 * fast_rcp(d + copysign(r, d));
   cs = fast_rsqrt(fma(tt, tt, 1.0));
   sn = cs * tt;
+}
+__device__ __forceinline__ void jacobi_cs(double al, double be, double ga, double& cs, double& sn) {
+  double tt;
+  jacobi_cst(al, be, ga, cs, sn, tt);
 }
 
 __global__ void __launch_bounds__(1024) jacobi_svd_kernel(SvdBatch b, double tol, int max_sweeps) {
@@ -172,6 +198,7 @@ __global__ void __launch_bounds__(1024) jacobi_svd_kernel(SvdBatch b, double tol
 // cluster barriers).  No global-memory traffic inside the iteration.
 // ---------------------------------------------------------------------------------------------
 int g_svd_block = 0;                    // tunable (option "svd_block"): block form of the super-rounds
+int g_svd_c16 = 1;                      // tunable (option "svd_c16"): 16-lane hot-path kernel
 int g_svd_min_cluster = 1;              // tunable (option "svd_min_cluster"): smallest cluster size tried
 constexpr int JC_THREADS = 1024;
 constexpr int JC_STAGE = 26;            // doubles staged per thread during a block exchange
@@ -189,7 +216,7 @@ __device__ __forceinline__ bool rotate_pair(double* cp, double* cq, int MP2, int
     al += x.x * x.x; be += y.x * y.x; ga += x.x * y.x;
     al += x.y * x.y; be += y.y * y.y; ga += x.y * y.y;
   }
-  al = warp_sum(al); be = warp_sum(be); ga = warp_sum(ga);
+  warp_sum3(al, be, ga);
   if (al < noise2 || be < noise2 || !(al > 0.0) || !(be > 0.0)) return false;
   if (ga * ga <= tol2 * al * be) return false;          // |ga| <= tol ||p|| ||q||
   // tan of the rotation angle, smaller root: t = sgn(zeta)/(|zeta| + sqrt(1 + zeta^2)), zeta =
@@ -367,6 +394,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
   double* Jm = Wm + (size_t)2 * bs * PW;                      //             accumulated rotations
   double* rc = Jm + (size_t)2 * bs * PW;
   double* rs = rc + bs;
+  double* nrm = rs + bs;                                      // squared norms of the resident columns [2 bs]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = JC_THREADS / 32;
   const int blk_of_slot[2] = {crank, 2 * CS - 1 - crank};
   // ---- load ---------------------------------------------------------------------------------
@@ -511,50 +539,80 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
       }
       __syncthreads();
     }
+    // squared norms of the resident columns, fresh once per sweep (carried through the super-rounds)
+    for (int ci = warp; ci < 2 * bs; ci += nw) {
+      const double2* c2 = reinterpret_cast<const double2*>(cols + (size_t)ci * LEN);
+      double a0 = 0.0;
+      for (int k = lane; k < MP2; k += 32) { const double2 x = c2[k]; a0 = fma(x.x, x.x, a0); a0 = fma(x.y, x.y, a0); }
+      a0 = warp_sum1(a0);
+      if (lane == 0) nrm[ci] = a0;
+    }
+    __syncthreads();
     // super-rounds
     for (int sr = 0; sr < 2 * CS - 1; sr++) {
       if (use_block) {
         rot |= block_superround(top, bs, LEN, MP2, tol2, noise2, Wm, Jm, rc, rs, PW);
       } else if (NREG > 0) {
-        // The pair rotations are shared-memory-bandwidth bound (each touches two LEN-vectors three
-        // times).  Warp i keeps top column i in registers for the bs rounds of the super-round, so
-        // only the bottom column of each pair moves through shared memory.
+        // The pair rotations are shared-memory-bandwidth and latency bound.  Warp i keeps top column
+        // i in registers for the bs rounds of the super-round, so only the bottom column of each pair
+        // moves through shared memory; the squared norms of the columns are carried along (al in a
+        // register, the bottom norms in nrm[]) and updated by ||p'||^2 = al - t ga, ||q'||^2 = be +
+        // t ga, so that a rotation costs ONE warp reduction (the inner product) instead of three.
+        // The carried norms are refreshed from the columns once per sweep (above) and whenever an
+        // update cancels more than two digits.
         double2 tp[NREG > 0 ? NREG : 1];
         const bool own = warp < bs;
         double2* tcol = reinterpret_cast<double2*>(top + (size_t)(own ? warp : 0) * LEN);
+        double al = 0.0;
         if (own) {
 #pragma unroll
           for (int q = 0; q < NREG; q++) {
             const int k = lane + 32 * q;
             tp[q] = (k < LEN2) ? tcol[k] : make_double2(0.0, 0.0);
           }
+          al = nrm[warp];
         }
         for (int r = 0; r < bs; r++) {
           if (own) {
             int j = warp + r; if (j >= bs) j -= bs;
             double2* cq = reinterpret_cast<double2*>(bot + (size_t)j * LEN);
             double2 y[NREG > 0 ? NREG : 1];
-            double al = 0.0, be = 0.0, ga = 0.0;
+            double ga0 = 0.0, ga1 = 0.0;
 #pragma unroll
             for (int q = 0; q < NREG; q++) {
               const int k = lane + 32 * q;
               y[q] = (k < LEN2) ? cq[k] : make_double2(0.0, 0.0);
-              if (k < MP2) {
-                al += tp[q].x * tp[q].x; be += y[q].x * y[q].x; ga += tp[q].x * y[q].x;
-                al += tp[q].y * tp[q].y; be += y[q].y * y[q].y; ga += tp[q].y * y[q].y;
-              }
+              if (k < MP2) { ga0 = fma(tp[q].x, y[q].x, ga0); ga1 = fma(tp[q].y, y[q].y, ga1); }
             }
-            al = warp_sum(al); be = warp_sum(be); ga = warp_sum(ga);
-            if (!(al < noise2 || be < noise2 || !(al > 0.0) || !(be > 0.0)) && !(ga * ga <= tol2 * al * be)) {
-              double cs, sn;
-              jacobi_cs(al, be, ga, cs, sn);
+            const double be = nrm[bs + j];
+            const double ga = warp_sum1(ga0 + ga1);
+            if (al >= noise2 && be >= noise2 && ga * ga > tol2 * al * be) {
+              double cs, sn, tt;
+              jacobi_cst(al, be, ga, cs, sn, tt);
 #pragma unroll
               for (int q = 0; q < NREG; q++) {
                 const int k = lane + 32 * q;
                 const double2 x = tp[q];
                 tp[q].x = cs * x.x - sn * y[q].x; tp[q].y = cs * x.y - sn * y[q].y;
-                if (k < LEN2) cq[k] = make_double2(sn * x.x + cs * y[q].x, sn * x.y + cs * y[q].y);
+                y[q].x = sn * x.x + cs * y[q].x; y[q].y = sn * x.y + cs * y[q].y;
+                if (k < LEN2) cq[k] = y[q];
               }
+              const double tg = tt * ga;
+              double aln = al - tg, ben = be + tg;
+              if (aln < 0.01 * al || ben < 0.01 * be) {         // heavy cancellation (rare): fresh norms
+                double a0 = 0.0, b0 = 0.0, z0 = 0.0;
+#pragma unroll
+                for (int q = 0; q < NREG; q++) {
+                  if (lane + 32 * q < MP2) {
+                    a0 = fma(tp[q].x, tp[q].x, a0); a0 = fma(tp[q].y, tp[q].y, a0);
+                    b0 = fma(y[q].x, y[q].x, b0); b0 = fma(y[q].y, y[q].y, b0);
+                  }
+                }
+                warp_sum3(a0, b0, z0);
+                aln = a0; ben = b0;
+              }
+              al = aln;
+              if (lane == 0) nrm[bs + j] = ben;
               rot = true;
             }
           }
@@ -566,6 +624,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
             const int k = lane + 32 * q;
             if (k < LEN2) tcol[k] = tp[q];
           }
+          if (lane == 0) nrm[warp] = al;
         }
         __syncthreads();
       } else {
@@ -590,6 +649,9 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
         else { src_bot = cluster.map_shared_rank(bot, crank + 1); src_bot_id = cluster.map_shared_rank(ids + bs, crank + 1); }
         double stage[STAGE];
         int id_stage = -1;
+        double nrm_stage = 0.0;
+        const double* src_top_nrm = src_top ? (const double*)cluster.map_shared_rank(nrm, crank == 1 ? 0 : crank - 1) + (crank == 1 ? bs : 0) : nullptr;
+        const double* src_bot_nrm = (crank == CS - 1) ? nrm : (const double*)cluster.map_shared_rank(nrm, crank + 1) + bs;
 #pragma unroll
         for (int q = 0; q < STAGE; q++) {
           int e = tid + q * JC_THREADS;
@@ -598,8 +660,8 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
           else if (e < 2 * per) v = src_bot[e - per];
           stage[q] = v;
         }
-        if (tid < bs) { if (src_top_id) id_stage = src_top_id[tid]; }
-        else if (tid < 2 * bs) id_stage = src_bot_id[tid - bs];
+        if (tid < bs) { if (src_top_id) { id_stage = src_top_id[tid]; nrm_stage = src_top_nrm[tid]; } }
+        else if (tid < 2 * bs) { id_stage = src_bot_id[tid - bs]; nrm_stage = src_bot_nrm[tid - bs]; }
         cluster.sync();                           // B: every CTA finished reading
 #pragma unroll
         for (int q = 0; q < STAGE; q++) {
@@ -607,8 +669,8 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
           if (e < per) { if (src_top) top[e] = stage[q]; }
           else if (e < 2 * per) bot[e - per] = stage[q];
         }
-        if (tid < bs) { if (src_top_id) ids[tid] = id_stage; }
-        else if (tid < 2 * bs) ids[tid] = id_stage;
+        if (tid < bs) { if (src_top_id) { ids[tid] = id_stage; nrm[tid] = nrm_stage; } }
+        else if (tid < 2 * bs) { ids[tid] = id_stage; nrm[tid] = nrm_stage; }
         __syncthreads();
       }
     }
@@ -644,6 +706,369 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
       int rank = 0;
       for (int l = 0; l < Nc; l++) {
         double sl = svu[l];
+        rank += (sl > sj || (sl == sj && l < j)) ? 1 : 0;
+      }
+      b.order[t][rank] = j;
+      b.sv[t][rank] = sj;
+    }
+    if (tid == 0 && b.sweeps[t]) *b.sweeps[t] = sweeps;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Hot-path cluster kernel (no V, 2 <= CS, LEN = 32 NREG doubles per column, bs <= 16).
+// Differences from jacobi_cluster_kernel, each measured on the 4x4 chi = 60 cores (N = 240):
+//  * 16 lanes per column pair, two pairs per warp: the scalar part of a rotation (reduction,
+//    convergence test, rotation parameters) is issued once for two pairs, and 8 warps instead of
+//    15 compete for the issue slots and the fp64 pipe of the SM;
+//  * carried squared norms (||p'||^2 = al - t ga, ||q'||^2 = be + t ga, refreshed from the columns
+//    once per sweep and after heavy cancellation): one reduction per rotation instead of three;
+//  * ping-pong column buffers: in the last round of a super-round the rotated columns are stored
+//    straight into the neighbour's spare buffer through DSMEM (the top column from registers), so
+//    the block exchange costs ONE cluster barrier and no extra pass over the columns;
+//  * the cluster-wide "any rotation" flag rides on the last barrier of the sweep.
+// ---------------------------------------------------------------------------------------------
+constexpr int J16_THREADS = 512;
+
+__device__ __forceinline__ double half_sum1(double v) {
+#pragma unroll
+  for (int o = 8; o > 0; o >>= 1) v += shfl_xor_f64(v, o);
+  return v;
+}
+__device__ __forceinline__ void half_sum3(double& a, double& b, double& c) {
+#pragma unroll
+  for (int o = 8; o > 0; o >>= 1) {
+    const double a2 = shfl_xor_f64(a, o), b2 = shfl_xor_f64(b, o), c2 = shfl_xor_f64(c, o);
+    a += a2; b += b2; c += c2;
+  }
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+template <int NREG>
+__global__ void __launch_bounds__(J16_THREADS, 1)
+jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int precond_min, int pw) {
+  constexpr int LEN = 32 * NREG, LEN2 = 16 * NREG;
+  extern __shared__ __align__(16) double jsm[];
+  cg::cluster_group cluster = cg::this_cluster();
+  const int crank = (int)cluster.block_rank();
+  const int t = blockIdx.x / CS;
+  const int r1 = b.r1[t], r2 = b.r2[t];
+  const bool tr = r1 < r2;
+  const int M = tr ? r2 : r1, Nc = tr ? r1 : r2;
+  const int MP = (M + 1) & ~1;
+  int Mj = M;
+  const double tol2 = tol * tol;
+  const double* K = b.K[t];
+  const int ldk = b.ldk[t];
+  // shared layout: colbuf[2][2 bs][LEN], nrmbuf[2][2 bs], idbuf[2][2 bs], flags[16], scal[4], vbuf
+  const int per = 2 * bs * LEN;
+  double* colbuf = jsm;
+  double* nrmbuf = colbuf + (size_t)2 * per;
+  int* idbuf = (int*)(nrmbuf + 4 * bs);
+  double* flags = (double*)(idbuf + ((4 * bs + 3) & ~3));
+  double* scal = flags + 16;
+  double* vbuf = scal + 4;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = J16_THREADS / 32;
+  const int blk_of_slot[2] = {crank, 2 * CS - 1 - crank};
+  int cur = 0;
+  double* cols = colbuf;
+  int* ids = idbuf;
+  // ---- load ---------------------------------------------------------------------------------
+  double fro = 0.0;
+  for (int e = tid; e < per; e += J16_THREADS) {
+    const int k = e % LEN, ci = e / LEN;
+    const int j = blk_of_slot[ci / bs] * bs + (ci % bs);
+    double v = 0.0;
+    if (j < Nc && k < M) { v = tr ? K[j + (long long)k * ldk] : K[k + (long long)j * ldk]; fro += v * v; }
+    cols[e] = v;
+  }
+  for (int e = tid; e < 2 * bs; e += J16_THREADS) ids[e] = blk_of_slot[e / bs] * bs + (e % bs);
+  __shared__ double s_red[32];
+  __shared__ int s_flag;
+  fro = warp_sum1(fro);
+  if (lane == 0) s_red[warp] = fro;
+  __syncthreads();
+  if (tid == 0) {
+    double s = 0.0;
+    for (int w = 0; w < nw; w++) s += s_red[w];
+    scal[0] = s;
+    s_flag = 0;
+  }
+  cluster.sync();
+  double ref = 0.0;
+  for (int c = 0; c < CS; c++) ref += cluster.map_shared_rank(scal, c)[0];
+  const double noise2 = 1e-30 * ref;
+  // ---- QR preconditioning (as in jacobi_cluster_kernel): iterate on L = R^T ------------------
+  const bool precond = precond_min > 0 && Nc >= precond_min && ref > 0.0 && isfinite(ref);
+  if (precond) {
+    const int VS = MP + 2;
+    const int nblk = (Nc + bs - 1) / bs;
+    for (int blk = 0; blk < nblk; blk++) {
+      const int owner = blk < CS ? blk : 2 * CS - 1 - blk;
+      for (int p0 = 0; p0 < bs; p0 += pw) {
+        const int j0 = blk * bs + p0;
+        if (j0 >= Nc) break;
+        const int j1 = min(min(j0 + pw, (blk + 1) * bs), Nc);
+        if (crank == owner) {
+          double* pcols = cols + ((size_t)(blk < CS ? 0 : 1) * bs + p0) * LEN;
+          for (int j = j0; j < j1; j++) {
+            double* col = pcols + (size_t)(j - j0) * LEN;
+            double* vl = vbuf + (size_t)(j - j0) * VS;
+            if (warp == 0) {
+              double ss = 0.0;
+              for (int k = j + lane; k < M; k += 32) { double x = col[k]; ss += x * x; }
+              ss = warp_sum1(ss);
+              const double ajj = col[j];
+              const double nrm = sqrt(ss);
+              const double alpha = (ajj > 0.0) ? -nrm : nrm;
+              const double vj = ajj - alpha;
+              const double vtv = ss - ajj * ajj + vj * vj;
+              for (int k = j + lane; k < M; k += 32) {
+                vl[k] = (k == j) ? vj : col[k];
+                col[k] = (k == j) ? alpha : 0.0;
+              }
+              if (lane == 0) vl[MP] = (vtv > 1e-290) ? 2.0 / vtv : 0.0;
+            }
+            __syncthreads();
+            const double tau = vl[MP];
+            if (tau != 0.0) {
+              for (int jj = j + 1 + warp; jj < j1; jj += nw) {
+                double* c2 = pcols + (size_t)(jj - j0) * LEN;
+                double w = 0.0;
+                for (int k = j + lane; k < M; k += 32) w += vl[k] * c2[k];
+                w = warp_sum1(w) * tau;
+                for (int k = j + lane; k < M; k += 32) c2[k] -= w * vl[k];
+              }
+            }
+            __syncthreads();
+          }
+          const int tot = (j1 - j0) * VS;
+          for (int c = 0; c < CS; c++) {
+            if (c == crank) continue;
+            double* rv = cluster.map_shared_rank(vbuf, c);
+            for (int e = tid; e < tot; e += J16_THREADS) rv[e] = vbuf[e];
+          }
+        }
+        cluster.sync();
+        for (int ci = warp; ci < 2 * bs; ci += nw) {
+          const int id = ids[ci];
+          if (id < j1 || id >= Nc) continue;
+          double* col = cols + (size_t)ci * LEN;
+          for (int j = j0; j < j1; j++) {
+            const double* vl = vbuf + (size_t)(j - j0) * VS;
+            const double tau = vl[MP];
+            if (tau == 0.0) continue;
+            double w = 0.0;
+            for (int k = j + lane; k < M; k += 32) w += vl[k] * col[k];
+            w = warp_sum1(w) * tau;
+            for (int k = j + lane; k < M; k += 32) col[k] -= w * vl[k];
+          }
+        }
+        cluster.sync();
+      }
+    }
+    double* Gs = b.G[t];
+    for (int ci = warp; ci < 2 * bs; ci += nw) {
+      const int id = ids[ci];
+      if (id >= Nc) continue;
+      const double* col = cols + (size_t)ci * LEN;
+      for (int k = lane; k < Nc; k += 32) Gs[k + (size_t)id * M] = (k <= id) ? col[k] : 0.0;
+    }
+    __threadfence();
+    cluster.sync();
+    for (int ci = warp; ci < 2 * bs; ci += nw) {
+      const int id = ids[ci];
+      double* col = cols + (size_t)ci * LEN;
+      for (int k = lane; k < LEN; k += 32)
+        col[k] = (id < Nc && k < Nc && k >= id) ? Gs[id + (size_t)k * M] : 0.0;
+    }
+    __syncthreads();
+    cluster.sync();
+    Mj = Nc;
+  }
+  // ---- iteration ------------------------------------------------------------------------------
+  int sweeps = 0;
+  const bool active = (Nc >= 2) && (ref > 0.0) && isfinite(ref);
+  const int nb2 = (bs & 1) ? bs + 1 : bs;
+  const int half = lane >> 4, l16 = lane & 15;
+  const int hw = 2 * warp + half;                        // half-warp index
+  const int nrw = (bs + 1) / 2;                          // warps that rotate pairs in the super-rounds
+  // destinations of the block exchange (see header): my top block and my bottom block
+  const int top_dst_rank = (crank == 0 || crank == CS - 1) ? crank : crank + 1;
+  const int top_dst_slot = (crank == CS - 1) ? 1 : 0;
+  const int bot_dst_rank = (crank == 0) ? 1 : crank - 1;
+  const int bot_dst_slot = (crank == 0) ? 0 : 1;
+  double* const rcol_top = cluster.map_shared_rank(colbuf, top_dst_rank);
+  double* const rcol_bot = cluster.map_shared_rank(colbuf, bot_dst_rank);
+  double* const rnrm_top = cluster.map_shared_rank(nrmbuf, top_dst_rank);
+  double* const rnrm_bot = cluster.map_shared_rank(nrmbuf, bot_dst_rank);
+  int* const rid_top = cluster.map_shared_rank(idbuf, top_dst_rank);
+  int* const rid_bot = cluster.map_shared_rank(idbuf, bot_dst_rank);
+  for (int sw = 0; active && sw < max_sweeps; sw++) {
+    double* nrm = nrmbuf + cur * 2 * bs;
+    // intra-block pairs of both resident blocks: nb2 half-warps per round
+    for (int r = 0; r < nb2 - 1; r++) {
+      if (hw < nb2) {
+        const int slot = hw / (nb2 / 2), i = hw % (nb2 / 2);
+        int a, c;
+        if (i == 0) { a = nb2 - 1; c = r; }
+        else { a = (r + i) % (nb2 - 1); c = (r - i + nb2 - 1) % (nb2 - 1); }
+        const bool valid = (a < bs && c < bs);
+        const int p = valid ? min(a, c) : 0, q = valid ? max(a, c) : 0;
+        double2* p2 = reinterpret_cast<double2*>(cols + ((size_t)slot * bs + p) * LEN);
+        double2* q2 = reinterpret_cast<double2*>(cols + ((size_t)slot * bs + q) * LEN);
+        double2 x[NREG], y[NREG];
+        double al = 0.0, be = 0.0, ga = 0.0;
+#pragma unroll
+        for (int u = 0; u < NREG; u++) {
+          x[u] = p2[l16 + 16 * u]; y[u] = q2[l16 + 16 * u];
+          al = fma(x[u].x, x[u].x, al); be = fma(y[u].x, y[u].x, be); ga = fma(x[u].x, y[u].x, ga);
+          al = fma(x[u].y, x[u].y, al); be = fma(y[u].y, y[u].y, be); ga = fma(x[u].y, y[u].y, ga);
+        }
+        half_sum3(al, be, ga);
+        const bool dorot = valid && al >= noise2 && be >= noise2 && ga * ga > tol2 * al * be;
+        if (dorot) {
+          double cs, sn;
+          jacobi_cs(al, be, ga, cs, sn);
+#pragma unroll
+          for (int u = 0; u < NREG; u++) {
+            double2 xn, yn;
+            xn.x = cs * x[u].x - sn * y[u].x; yn.x = sn * x[u].x + cs * y[u].x;
+            xn.y = cs * x[u].y - sn * y[u].y; yn.y = sn * x[u].y + cs * y[u].y;
+            p2[l16 + 16 * u] = xn; q2[l16 + 16 * u] = yn;
+          }
+          s_flag = 1;
+        }
+      }
+      __syncthreads();
+    }
+    // squared norms of the resident columns, fresh once per sweep
+    if (hw < 2 * bs) {
+      const double2* c2 = reinterpret_cast<const double2*>(cols + (size_t)hw * LEN);
+      double a0 = 0.0, a1 = 0.0;
+#pragma unroll
+      for (int u = 0; u < NREG; u++) { const double2 x = c2[l16 + 16 * u]; a0 = fma(x.x, x.x, a0); a1 = fma(x.y, x.y, a1); }
+      a0 = half_sum1(a0 + a1);
+      if (l16 == 0) nrm[hw] = a0;
+    }
+    __syncthreads();
+    // super-rounds
+    for (int sr = 0; sr < 2 * CS - 1; sr++) {
+      const int nxt = cur ^ 1;
+      if (warp < nrw) {
+        const bool own = hw < bs;
+        const int pi = own ? hw : 0;
+        double* top = cols;
+        double* bot = cols + (size_t)bs * LEN;
+        double* nrmc = nrmbuf + cur * 2 * bs;
+        double2 tp[NREG];
+        const double2* tcol = reinterpret_cast<const double2*>(top + (size_t)pi * LEN);
+#pragma unroll
+        for (int u = 0; u < NREG; u++) tp[u] = tcol[l16 + 16 * u];
+        double al = nrmc[pi];
+        for (int r = 0; r < bs; r++) {
+          int j = pi + r; if (j >= bs) j -= bs;
+          double2* cq = reinterpret_cast<double2*>(bot + (size_t)j * LEN);
+          double2 y[NREG];
+          double ga0 = 0.0, ga1 = 0.0;
+#pragma unroll
+          for (int u = 0; u < NREG; u++) {
+            y[u] = cq[l16 + 16 * u];
+            ga0 = fma(tp[u].x, y[u].x, ga0); ga1 = fma(tp[u].y, y[u].y, ga1);
+          }
+          double be = nrmc[bs + j];
+          const double ga = half_sum1(ga0 + ga1);
+          const bool dorot = own && al >= noise2 && be >= noise2 && ga * ga > tol2 * al * be;
+          const bool last = (r == bs - 1);
+          if (__any_sync(0xffffffffu, dorot)) {
+            double cs = 1.0, sn = 0.0, tt = 0.0;
+            jacobi_cst(dorot ? al : 1.0, dorot ? be : 2.0, dorot ? ga : 0.5, cs, sn, tt);
+            if (!dorot) { cs = 1.0; sn = 0.0; tt = 0.0; }
+#pragma unroll
+            for (int u = 0; u < NREG; u++) {
+              const double2 x = tp[u];
+              tp[u].x = cs * x.x - sn * y[u].x; tp[u].y = cs * x.y - sn * y[u].y;
+              y[u].x = sn * x.x + cs * y[u].x; y[u].y = sn * x.y + cs * y[u].y;
+            }
+            const double tg = tt * ga;
+            double aln = al - tg, ben = be + tg;
+            const bool bad = dorot && (aln < 0.01 * al || ben < 0.01 * be);
+            if (__any_sync(0xffffffffu, bad)) {               // heavy cancellation (rare): fresh norms
+              double a0 = 0.0, b0 = 0.0, z0 = 0.0;
+#pragma unroll
+              for (int u = 0; u < NREG; u++) {
+                a0 = fma(tp[u].x, tp[u].x, a0); a0 = fma(tp[u].y, tp[u].y, a0);
+                b0 = fma(y[u].x, y[u].x, b0); b0 = fma(y[u].y, y[u].y, b0);
+              }
+              half_sum3(a0, b0, z0);
+              if (bad) { aln = a0; ben = b0; }
+            }
+            if (dorot) {
+              al = aln; be = ben;
+              s_flag = 1;
+              if (!last) {
+#pragma unroll
+                for (int u = 0; u < NREG; u++) cq[l16 + 16 * u] = y[u];
+                if (l16 == 0) nrmc[bs + j] = ben;
+              }
+            }
+          }
+          if (last && own) {
+            // exchange fused into the last round: bottom column j and top column pi go to the spare
+            // buffers of their next owners
+            double2* dq = reinterpret_cast<double2*>(rcol_bot + (size_t)nxt * per + ((size_t)bot_dst_slot * bs + j) * LEN);
+            double2* dp = reinterpret_cast<double2*>(rcol_top + (size_t)nxt * per + ((size_t)top_dst_slot * bs + pi) * LEN);
+#pragma unroll
+            for (int u = 0; u < NREG; u++) { dq[l16 + 16 * u] = y[u]; dp[l16 + 16 * u] = tp[u]; }
+            if (l16 == 0) {
+              rnrm_bot[nxt * 2 * bs + bot_dst_slot * bs + j] = be;
+              rnrm_top[nxt * 2 * bs + top_dst_slot * bs + pi] = al;
+              rid_bot[nxt * 2 * bs + bot_dst_slot * bs + j] = ids[bs + j];
+              rid_top[nxt * 2 * bs + top_dst_slot * bs + pi] = ids[pi];
+            }
+          }
+          if (!last) named_bar_sync(1, nrw * 32);
+        }
+      }
+      if (sr == 2 * CS - 2) {
+        // last barrier of the sweep carries the "any rotation" flags
+        __syncthreads();
+        if (tid < CS) cluster.map_shared_rank(flags, tid)[crank] = s_flag ? 1.0 : 0.0;
+      }
+      cluster.sync();
+      cur = nxt;
+      cols = colbuf + (size_t)cur * per;
+      ids = idbuf + cur * 2 * bs;
+    }
+    sweeps = sw + 1;
+    double tot = 0.0;
+    for (int c = 0; c < CS; c++) tot += flags[c];
+    if (tid == 0) s_flag = 0;                         // every thread passed the flag push (cluster barrier)
+    __syncthreads();
+    if (tot == 0.0) break;
+  }
+  // ---- write back ------------------------------------------------------------------------------
+  double* G = b.G[t];
+  double* svu = b.V[t] + (size_t)Nc * Nc;
+  for (int ci = warp; ci < 2 * bs; ci += nw) {
+    const int id = ids[ci];
+    if (id >= Nc) continue;
+    const double* col = cols + (size_t)ci * LEN;
+    double s = 0.0;
+    for (int k = lane; k < Mj; k += 32) { double x = col[k]; s += x * x; G[(size_t)id * M + k] = x; }
+    s = warp_sum1(s);
+    if (lane == 0) svu[id] = sqrt(s);
+  }
+  __threadfence();
+  cluster.sync();
+  if (crank == 0) {
+    for (int j = tid; j < Nc; j += J16_THREADS) {
+      const double sj = svu[j];
+      int rank = 0;
+      for (int l = 0; l < Nc; l++) {
+        const double sl = svu[l];
         rank += (sl > sj || (sl == sj && l < j)) ? 1 : 0;
       }
       b.order[t][rank] = j;
@@ -801,6 +1226,7 @@ __global__ void set_identity_kernel(double* Q, long long m, int k) {
 }  // namespace
 
 void set_svd_block(int on) { g_svd_block = on ? 1 : 0; }
+void set_svd_c16(int on) { g_svd_c16 = on ? 1 : 0; }
 void set_svd_min_cluster(int cs) { g_svd_min_cluster = cs < 1 ? 1 : (cs > 16 ? 16 : cs); }
 
 int launch_svd_vectors(cudaStream_t st, const double* G, const double* V, const double* s,
@@ -836,11 +1262,52 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
   // beyond that, measured), so prefer the cluster size with bs <= 16, up to the portable 8
   int cs0 = 1;
   while (cs0 < 8 && (ncmax + 2 * cs0 - 1) / (2 * cs0) > 16) cs0 *= 2;
+  // hot path: 16-lane kernel (no V, cluster >= 2, columns of <= 256 doubles, <= 16 pairs per CTA)
+  if (!with_v && g_svd_c16) {
+    const int CS = std::max(std::max(cs0, g_svd_min_cluster), 2);
+    const int bs = (ncmax + 2 * CS - 1) / (2 * CS);
+    int mmax = 2;
+    for (int t = 0; t < b.count; t++) mmax = std::max(mmax, std::max(b.r1[t], b.r2[t]));
+    const int nreg = (mmax + 31) / 32 <= 2 ? 2 : (mmax + 31) / 32 <= 4 ? 4 : (mmax + 31) / 32 <= 6 ? 6 : 8;
+    if (CS <= 8 && bs <= 16 && mmax <= 256) {
+      const int LENc = 32 * nreg;
+      const size_t base = ((size_t)4 * bs * LENc + 4 * bs) * 8 + (size_t)((4 * bs + 3) & ~3) * 4 + (16 + 4) * 8;
+      const size_t vs8 = (size_t)(((mmax + 1) & ~1) + 2) * 8;
+      int pw = 1;
+      if (precond_min > 0) pw = (int)std::max<size_t>(1, std::min<size_t>((size_t)bs, (JC_SMEM_CAP - base) / vs8));
+      const size_t smem = base + (size_t)pw * vs8;
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)(b.count * CS));
+      cfg.blockDim = dim3(J16_THREADS);
+      cfg.dynamicSmemBytes = smem;
+      cfg.stream = st;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      static bool attr_done = false;
+      if (!attr_done) {
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
+        attr_done = true;
+      }
+      cudaError_t e;
+      if (nreg == 2) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<2>, b, tol, max_sweeps, bs, CS, precond_min, pw);
+      else if (nreg == 4) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<4>, b, tol, max_sweeps, bs, CS, precond_min, pw);
+      else if (nreg == 6) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<6>, b, tol, max_sweeps, bs, CS, precond_min, pw);
+      else e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<8>, b, tol, max_sweeps, bs, CS, precond_min, pw);
+      if (e != cudaSuccess) { set_error("svd: cluster launch failed: %s", cudaGetErrorString(e)); return -3; }
+      PEPO_COUNT_LAUNCH();
+      return 0;
+    }
+  }
   for (int CS = std::max(cs0, g_svd_min_cluster); CS <= 16; CS *= 2) {
     int bs = (ncmax + 2 * CS - 1) / (2 * CS);
     const int PW = (2 * bs + 3) & ~3;
     size_t smem0 = ((size_t)2 * bs * lenmax) * 8 + (size_t)(2 * bs + 4) * 4 + 64 +
-                   ((size_t)4 * bs * PW + 2 * bs) * 8;
+                   ((size_t)4 * bs * PW + 4 * bs) * 8;
     int pw = 0;                                        // Householder panel width (preconditioner)
     if (!with_v && precond_min > 0 && smem0 < JC_SMEM_CAP)
       pw = (int)std::min<size_t>((size_t)bs, (JC_SMEM_CAP - smem0) / ((size_t)(lenmax + 2) * 8));
