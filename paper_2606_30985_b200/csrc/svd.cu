@@ -771,7 +771,6 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
   double* scal = flags + 16;
   double* vbuf = scal + 4;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = J16_THREADS / 32;
-  const int blk_of_slot[2] = {crank, 2 * CS - 1 - crank};
   int cur = 0;
   double* cols = colbuf;
   int* ids = idbuf;
@@ -779,12 +778,12 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
   double fro = 0.0;
   for (int e = tid; e < per; e += J16_THREADS) {
     const int k = e % LEN, ci = e / LEN;
-    const int j = blk_of_slot[ci / bs] * bs + (ci % bs);
+    const int j = ((ci / bs) ? 2 * CS - 1 - crank : crank) * bs + (ci % bs);
     double v = 0.0;
     if (j < Nc && k < M) { v = tr ? K[j + (long long)k * ldk] : K[k + (long long)j * ldk]; fro += v * v; }
     cols[e] = v;
   }
-  for (int e = tid; e < 2 * bs; e += J16_THREADS) ids[e] = blk_of_slot[e / bs] * bs + (e % bs);
+  for (int e = tid; e < 2 * bs; e += J16_THREADS) ids[e] = ((e / bs) ? 2 * CS - 1 - crank : crank) * bs + (e % bs);
   __shared__ double s_red[32];
   __shared__ int s_flag;
   fro = warp_sum1(fro);
@@ -900,12 +899,7 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
   const int top_dst_slot = (crank == CS - 1) ? 1 : 0;
   const int bot_dst_rank = (crank == 0) ? 1 : crank - 1;
   const int bot_dst_slot = (crank == 0) ? 0 : 1;
-  double* const rcol_top = cluster.map_shared_rank(colbuf, top_dst_rank);
-  double* const rcol_bot = cluster.map_shared_rank(colbuf, bot_dst_rank);
-  double* const rnrm_top = cluster.map_shared_rank(nrmbuf, top_dst_rank);
-  double* const rnrm_bot = cluster.map_shared_rank(nrmbuf, bot_dst_rank);
-  int* const rid_top = cluster.map_shared_rank(idbuf, top_dst_rank);
-  int* const rid_bot = cluster.map_shared_rank(idbuf, bot_dst_rank);
+  const int nrt = nrw * 32;
   for (int sw = 0; active && sw < max_sweeps; sw++) {
     double* nrm = nrmbuf + cur * 2 * bs;
     // intra-block pairs of both resident blocks: nb2 half-warps per round
@@ -983,14 +977,15 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
           const bool dorot = own && al >= noise2 && be >= noise2 && ga * ga > tol2 * al * be;
           const bool last = (r == bs - 1);
           if (__any_sync(0xffffffffu, dorot)) {
-            double cs = 1.0, sn = 0.0, tt = 0.0;
+            double cs, sn, tt;
             jacobi_cst(dorot ? al : 1.0, dorot ? be : 2.0, dorot ? ga : 0.5, cs, sn, tt);
-            if (!dorot) { cs = 1.0; sn = 0.0; tt = 0.0; }
+            double ics = fma(tt, tt, 1.0) * cs;                // 1 / cs
+            if (!dorot) { cs = 1.0; sn = 0.0; tt = 0.0; ics = 1.0; }
+            // in place, no temporaries: p' = cs p - sn q, then q' = sn p + cs q = t p' + q / cs
 #pragma unroll
             for (int u = 0; u < NREG; u++) {
-              const double2 x = tp[u];
-              tp[u].x = cs * x.x - sn * y[u].x; tp[u].y = cs * x.y - sn * y[u].y;
-              y[u].x = sn * x.x + cs * y[u].x; y[u].y = sn * x.y + cs * y[u].y;
+              tp[u].x = fma(cs, tp[u].x, -(sn * y[u].x)); tp[u].y = fma(cs, tp[u].y, -(sn * y[u].y));
+              y[u].x = fma(tt, tp[u].x, y[u].x * ics); y[u].y = fma(tt, tp[u].y, y[u].y * ics);
             }
             const double tg = tt * ga;
             double aln = al - tg, ben = be + tg;
@@ -1018,18 +1013,24 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
           if (last && own) {
             // exchange fused into the last round: bottom column j and top column pi go to the spare
             // buffers of their next owners
+            double* const rcol_top = cluster.map_shared_rank(colbuf, top_dst_rank);
+            double* const rcol_bot = cluster.map_shared_rank(colbuf, bot_dst_rank);
             double2* dq = reinterpret_cast<double2*>(rcol_bot + (size_t)nxt * per + ((size_t)bot_dst_slot * bs + j) * LEN);
             double2* dp = reinterpret_cast<double2*>(rcol_top + (size_t)nxt * per + ((size_t)top_dst_slot * bs + pi) * LEN);
 #pragma unroll
             for (int u = 0; u < NREG; u++) { dq[l16 + 16 * u] = y[u]; dp[l16 + 16 * u] = tp[u]; }
             if (l16 == 0) {
+              double* const rnrm_top = cluster.map_shared_rank(nrmbuf, top_dst_rank);
+              double* const rnrm_bot = cluster.map_shared_rank(nrmbuf, bot_dst_rank);
+              int* const rid_top = cluster.map_shared_rank(idbuf, top_dst_rank);
+              int* const rid_bot = cluster.map_shared_rank(idbuf, bot_dst_rank);
               rnrm_bot[nxt * 2 * bs + bot_dst_slot * bs + j] = be;
               rnrm_top[nxt * 2 * bs + top_dst_slot * bs + pi] = al;
               rid_bot[nxt * 2 * bs + bot_dst_slot * bs + j] = ids[bs + j];
               rid_top[nxt * 2 * bs + top_dst_slot * bs + pi] = ids[pi];
             }
           }
-          if (!last) named_bar_sync(1, nrw * 32);
+          if (!last) named_bar_sync(1, nrt);
         }
       }
       if (sr == 2 * CS - 2) {
