@@ -213,6 +213,12 @@ struct pepo_ctx {
   int force_hh = 0;
   int svd_precond_min = 32;            // QR-precondition core SVDs with min(r1,r2) >= this (0: off)
   cudaStream_t st;
+  cudaStream_t cur_st = nullptr;       // stream the profiling events of the current launches go to
+  // pipelined schedule of a colour class (option "pipeline"): second half-batch on st2, the Jacobi
+  // kernels of the two half-batches on the high-priority streams hp[0], hp[1]
+  int pipeline = 1;
+  cudaStream_t st2 = nullptr, hp[2] = {nullptr, nullptr};
+  cudaEvent_t pev[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   int n_sites, n_bonds, n_hb;
   std::vector<SiteInfo> sites;
   std::vector<BondInfo> bonds;
@@ -255,19 +261,24 @@ void prof_flush(pepo_ctx* c) {        // call only after a stream synchronize
   P.used = 0;
 }
 struct ProfScope {
-  pepo_ctx* c; bool active;
+  pepo_ctx* c; bool active; cudaStream_t st = nullptr;
   ProfScope(pepo_ctx* c_, int cat, double flops, double bytes) : c(c_), active(false) {
     Prof& P = c->prof;
     if (!P.on) return;
-    if (2 * (P.used + 1) > P.ev.size()) { cudaStreamSynchronize(c->st); prof_flush(c); }
+    if (2 * (P.used + 1) > P.ev.size()) {
+      cudaStreamSynchronize(c->st);
+      if (c->st2) { cudaStreamSynchronize(c->st2); cudaStreamSynchronize(c->hp[0]); cudaStreamSynchronize(c->hp[1]); }
+      prof_flush(c);
+    }
     P.cat[P.used] = cat; P.cnt[cat]++; P.flops[cat] += flops; P.bytes[cat] += bytes;
-    cudaEventRecord(P.ev[2 * P.used], c->st);
+    st = c->cur_st ? c->cur_st : c->st;
+    cudaEventRecord(P.ev[2 * P.used], st);
     active = true;
   }
   ~ProfScope() {
     if (!active) return;
     Prof& P = c->prof;
-    cudaEventRecord(P.ev[2 * P.used + 1], c->st);
+    cudaEventRecord(P.ev[2 * P.used + 1], st);
     P.used++;
   }
 };
@@ -557,6 +568,15 @@ extern "C" int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, doub
       cudaMallocHost((void**)&c->h_bpints, 16) != cudaSuccess) {
     set_error("init: cudaMallocHost failed"); delete c; return -3;
   }
+  {
+    int lo = 0, hi = 0;
+    cudaDeviceGetStreamPriorityRange(&lo, &hi);          // hi = numerically smallest = highest priority
+    bool ok = cudaStreamCreateWithPriority(&c->st2, cudaStreamNonBlocking, lo) == cudaSuccess;
+    for (int i = 0; i < 2 && ok; i++) ok = cudaStreamCreateWithPriority(&c->hp[i], cudaStreamNonBlocking, hi) == cudaSuccess;
+    for (int i = 0; i < 8 && ok; i++) ok = cudaEventCreateWithFlags(&c->pev[i], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) { set_error("init: stream / event creation failed"); delete c; return -3; }
+  }
+  c->cur_st = c->st;
   int rc = 0;
   double one = 1.0;
   rc |= upload(c, c->ones, &one, 8);
@@ -585,6 +605,9 @@ extern "C" int pepo_init(pepo_ctx** out, int Lx, int Ly, int cx, int cy, double 
 extern "C" int pepo_destroy(pepo_ctx* c) {
   if (!c) return 0;
   cudaStreamSynchronize(c->st);
+  if (c->st2) { cudaStreamSynchronize(c->st2); cudaStreamDestroy(c->st2); }
+  for (int i = 0; i < 2; i++) if (c->hp[i]) { cudaStreamSynchronize(c->hp[i]); cudaStreamDestroy(c->hp[i]); }
+  for (int i = 0; i < 8; i++) if (c->pev[i]) cudaEventDestroy(c->pev[i]);
   cudaFreeHost(c->h_ints); cudaFreeHost(c->h_dbls); cudaFreeHost(c->h_chi_msg);
   cudaFreeHost(c->h_scal); cudaFreeHost(c->h_delta); cudaFreeHost(c->h_bpints);
   delete c;
@@ -606,6 +629,7 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "svd_precond_min") c->svd_precond_min = (int)v;
   else if (k == "svd_block") set_svd_block((int)v);
   else if (k == "svd_c16") set_svd_c16((int)v);
+  else if (k == "pipeline") c->pipeline = (int)v;
   else if (k == "profile") {
     Prof& P = c->prof;
     if (v != 0.0 && P.ev.empty()) {
@@ -738,16 +762,32 @@ struct TaskGeo {           // one site of one gate
   int chi_new;
 };
 
-int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
-  const int ng = (int)gate_bonds.size();
-  if (ng == 0) return 0;
-  cudaStream_t st = c->st;
+struct BatchState {        // one batch of gates moving through the three phases of Algorithm 1
+  std::vector<int> gate_bonds;
+  std::vector<TaskGeo> T;
+  int ng = 0, lane0 = 0;           // lanes [lane0, lane0 + ng) of the workspace
+  cudaStream_t st = nullptr;       // stream of this batch
+  cudaStream_t hp = nullptr;       // high-priority stream for the Jacobi kernel (nullptr: st)
+  cudaEvent_t ev[2] = {nullptr, nullptr};
+  bool piped = false;              // another batch is in flight: keep the profiling events until the class ends
+  bool have_chol = false;
+  SvdFinishBatch fb;
+};
+
+// phase 1: absorb + permute, Gram, dressing, Cholesky (enqueue only; ends with the flag read-back)
+int batch_p1(pepo_ctx* c, BatchState& S) {
+  const int ng = S.ng;
+  cudaStream_t st = S.st;
+  std::vector<TaskGeo>& T = S.T;
+  const std::vector<int>& gate_bonds = S.gate_bonds;
   const int NA = c->NA;
   GateTables gt;
   gt.Gamma[0] = c->dGamma[0]; gt.Gamma[1] = c->dGamma[1];
   gt.Ahat[0] = c->dAhat[0]; gt.Ahat[1] = c->dAhat[1];
   gt.sigma = c->dSigma;
-  std::vector<TaskGeo> T(2 * ng);
+  c->cur_st = st;
+  (void)gate_bonds; (void)gt; (void)NA;
+  T.assign(2 * ng, TaskGeo());
   // ---- A: geometry + absorb/permute ----------------------------------------------------------
   for (int g = 0; g < ng; g++) {
     const BondInfo& b = c->bonds[gate_bonds[g]];
@@ -755,7 +795,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       TaskGeo& t = T[2 * g + i];
       t.v = i == 0 ? b.v1 : b.v2;
       const int dcut = i == 0 ? b.d1 : b.d2;
-      t.lane = g; t.slot = i; t.site_idx = i;
+      t.lane = S.lane0 + g; t.slot = i; t.site_idx = i;
       const SiteInfo& s = c->sites[t.v];
       t.nlegs = s.nlegs; t.n_env = 0; t.m = 1; t.cut_leg = -1;
       for (int l = 0; l < s.nlegs; l++) {
@@ -771,7 +811,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       t.chol = !c->force_hh && (double)t.m >= c->chol_ratio * t.n;
       t.r = t.chol ? t.N : std::min(4 * t.k, t.N);
       t.skip1 = t.m <= t.n; t.skip2 = 4 * t.k <= t.N;
-      SiteWs& W = c->lanes[g].s[i];
+      SiteWs& W = c->lanes[S.lane0 + g].s[i];
       PermuteDesc pd;
       pd.rank = s.nlegs + 1; pd.power = 1.0;
       long long sstr = 1;
@@ -821,16 +861,35 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       int rc;
       { ProfScope ps(c, PC_DRESS, 0, 0); rc = launch_dress_gram(st, db, gt); if (rc) return rc; }
       { ProfScope ps(c, PC_CHOL, 0, 0); rc = launch_potrf(st, pb, infos, c->chol_tau); if (rc) return rc; }
-      PEPO_CUDA_OK(cudaMemcpyAsync(c->h_ints, c->lane_ints, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
-      PEPO_CUDA_OK(cudaStreamSynchronize(st));
-      prof_flush(c);
-      for (auto& t : T) {
-        if (!t.chol) continue;
-        int info = c->h_ints[4 * t.lane + 2 + t.slot];
-        if (info != 0) {
-          t.chol = false; t.r = std::min(4 * t.k, t.N);
-          c->stats.n_chol_failed++;
-        }
+      PEPO_CUDA_OK(cudaMemcpyAsync(c->h_ints + 4 * S.lane0, c->lane_ints + 4 * S.lane0, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
+      S.have_chol = true;
+    }
+  }
+  return 0;
+}
+
+// phase 2: Cholesky flags (host), Householder fallback, core, SVD, truncation (ends with the chi_new read-back)
+int batch_p2(pepo_ctx* c, BatchState& S) {
+  const int ng = S.ng;
+  cudaStream_t st = S.st;
+  std::vector<TaskGeo>& T = S.T;
+  const std::vector<int>& gate_bonds = S.gate_bonds;
+  const int NA = c->NA;
+  GateTables gt;
+  gt.Gamma[0] = c->dGamma[0]; gt.Gamma[1] = c->dGamma[1];
+  gt.Ahat[0] = c->dAhat[0]; gt.Ahat[1] = c->dAhat[1];
+  gt.sigma = c->dSigma;
+  c->cur_st = st;
+  (void)gate_bonds; (void)gt; (void)NA;
+  if (S.have_chol) {
+    PEPO_CUDA_OK(cudaStreamSynchronize(st));
+    if (!S.piped) prof_flush(c);
+    for (auto& t : T) {
+      if (!t.chol) continue;
+      int info = c->h_ints[4 * t.lane + 2 + t.slot];
+      if (info != 0) {
+        t.chol = false; t.r = std::min(4 * t.k, t.N);
+        c->stats.n_chol_failed++;
       }
     }
   }
@@ -891,10 +950,10 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
   {
     DressBatch sc; sc.count = ng; sc.NA = NA;
     SvdBatch sb; sb.count = ng;
-    SvdFinishBatch fb; fb.count = ng; fb.with_v = 0; fb.precond_min = c->svd_precond_min;
+    SvdFinishBatch& fb = S.fb; fb.count = ng; fb.with_v = 0; fb.precond_min = c->svd_precond_min;
     for (int g = 0; g < ng; g++) {
       TaskGeo& t1 = T[2 * g]; TaskGeo& t2 = T[2 * g + 1];
-      LaneWs& L = c->lanes[g];
+      LaneWs& L = c->lanes[S.lane0 + g];
       const int e = gate_bonds[g];
       sc.in[g] = L.s[0].Rx; sc.out[g] = L.Ks; sc.chi[g] = t1.chi_c; sc.k[g] = t1.r; sc.site[g] = 0;
       sc.ld_in[g] = t1.r; sc.ld_out[g] = t1.r;
@@ -911,7 +970,7 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
     int rc = launch_scale_sigma(st, sc, gt); if (rc) return rc;
     for (int g = 0; g < ng; g++) {
       TaskGeo& t1 = T[2 * g]; TaskGeo& t2 = T[2 * g + 1];
-      LaneWs& L = c->lanes[g];
+      LaneWs& L = c->lanes[S.lane0 + g];
       GemmProb gp;
       gp.A = L.Ks; gp.lda = t1.r; gp.B = L.s[1].Rx; gp.ldb = t2.r; gp.C = L.K; gp.ldc = t1.r;
       gp.M = t1.r; gp.N = t2.r; gp.K = t1.N;
@@ -919,39 +978,76 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
       rc = launch_dgemm(st, 0, 1, gp, 1, 0, nullptr, false); if (rc) return rc;
     }
     {
+      // the Jacobi kernel needs whole SMs (a cluster per core): on the pipelined schedule it goes to
+      // a high-priority stream so that it is placed ahead of the other half-batch's GEMM CTAs
+      cudaStream_t ss = st;
+      if (S.hp) {
+        PEPO_CUDA_OK(cudaEventRecord(S.ev[0], st));
+        PEPO_CUDA_OK(cudaStreamWaitEvent(S.hp, S.ev[0], 0));
+        ss = S.hp;
+      }
+      c->cur_st = ss;
+      {
+        ProfScope ps(c, PC_SVD, 0, 0);
+        rc = launch_svd_jacobi(ss, sb, c->jacobi_tol, c->jacobi_max_sweeps, false, c->svd_precond_min); if (rc) return rc;
+      }
+      c->cur_st = st;
+      if (S.hp) {
+        PEPO_CUDA_OK(cudaEventRecord(S.ev[1], S.hp));
+        PEPO_CUDA_OK(cudaStreamWaitEvent(st, S.ev[1], 0));
+      }
       ProfScope ps(c, PC_SVD, 0, 0);
-      rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps, false, c->svd_precond_min); if (rc) return rc;
       rc = launch_svd_truncate(st, fb, c->chi_max, c->eps_cut); if (rc) return rc;
     }
-    PEPO_CUDA_OK(cudaMemcpyAsync(c->h_ints, c->lane_ints, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
-    PEPO_CUDA_OK(cudaMemcpyAsync(c->h_dbls, c->lane_dbls, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
+    PEPO_CUDA_OK(cudaMemcpyAsync(c->h_ints + 4 * S.lane0, c->lane_ints + 4 * S.lane0, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
+    PEPO_CUDA_OK(cudaMemcpyAsync(c->h_dbls + 2 * S.lane0, c->lane_dbls + 2 * S.lane0, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
+  }
+  return 0;
+}
+
+// phase 3: chi_new (host), bridges, reconstruction, inverse permute + de-absorb + write-back
+int batch_p3(pepo_ctx* c, BatchState& S) {
+  const int ng = S.ng;
+  cudaStream_t st = S.st;
+  std::vector<TaskGeo>& T = S.T;
+  const std::vector<int>& gate_bonds = S.gate_bonds;
+  const int NA = c->NA;
+  GateTables gt;
+  gt.Gamma[0] = c->dGamma[0]; gt.Gamma[1] = c->dGamma[1];
+  gt.Ahat[0] = c->dAhat[0]; gt.Ahat[1] = c->dAhat[1];
+  gt.sigma = c->dSigma;
+  c->cur_st = st;
+  (void)gate_bonds; (void)gt; (void)NA;
+  {
+    SvdFinishBatch& fb = S.fb;
+    int rc = 0;
     PEPO_CUDA_OK(cudaStreamSynchronize(st));
-    prof_flush(c);
+    if (!S.piped) prof_flush(c);
     int chi_cap = 1;
     for (int g = 0; g < ng; g++) {
-      int cn = c->h_ints[4 * g];
+      int cn = c->h_ints[4 * (S.lane0 + g)];
       if (cn < 1) {
         // diagnostics: leading entries of the core and of the computed spectrum
         double hk[4] = {0, 0, 0, 0}, hs[2] = {0, 0};
         const int r1 = T[2 * g].r, r2 = T[2 * g + 1].r;
-        cudaMemcpy(hk, c->lanes[g].K, sizeof(double) * std::min(4, r1 * r2), cudaMemcpyDeviceToHost);
-        cudaMemcpy(hs, c->lanes[g].sv, sizeof(double) * std::min(2, std::min(r1, r2)), cudaMemcpyDeviceToHost);
+        cudaMemcpy(hk, c->lanes[S.lane0 + g].K, sizeof(double) * std::min(4, r1 * r2), cudaMemcpyDeviceToHost);
+        cudaMemcpy(hs, c->lanes[S.lane0 + g].sv, sizeof(double) * std::min(2, std::min(r1, r2)), cudaMemcpyDeviceToHost);
         set_error("gate on bond %d: s0 = 0 or NaN in the core SVD (core %d x %d, K[0..3] = %g %g %g %g, s[0..1] = %g %g, "
-                  "sweeps %d)", gate_bonds[g], r1, r2, hk[0], hk[1], hk[2], hk[3], hs[0], hs[1], c->h_ints[4 * g + 1]);
+                  "sweeps %d)", gate_bonds[g], r1, r2, hk[0], hk[1], hk[2], hk[3], hs[0], hs[1], c->h_ints[4 * (S.lane0 + g) + 1]);
         return -4;
       }
       T[2 * g].chi_new = T[2 * g + 1].chi_new = cn;
       chi_cap = std::max(chi_cap, cn);
-      c->stats.jacobi_sweeps += c->h_ints[4 * g + 1];
+      c->stats.jacobi_sweeps += c->h_ints[4 * (S.lane0 + g) + 1];
       if (c->prof.on) {
         // algorithmic flops of the one-sided Jacobi iteration: per sweep Nc(Nc-1)/2 pairs, each
         // 3 inner products (6 L flop) + one plane rotation of two L-vectors (6 L flop)
         const double Nc = std::min(T[2 * g].r, T[2 * g + 1].r), Mx = std::max(T[2 * g].r, T[2 * g + 1].r);
         const double Lc = (c->svd_precond_min > 0 && Nc >= c->svd_precond_min) ? Nc : Mx;
-        c->prof.flops[PC_SVD] += c->h_ints[4 * g + 1] * 0.5 * Nc * (Nc - 1) * 12.0 * Lc;
+        c->prof.flops[PC_SVD] += c->h_ints[4 * (S.lane0 + g) + 1] * 0.5 * Nc * (Nc - 1) * 12.0 * Lc;
       }
-      c->stats.gate_err += c->h_dbls[2 * g];
-      c->stats.min_cut_gap = std::min(c->stats.min_cut_gap, c->h_dbls[2 * g + 1]);
+      c->stats.gate_err += c->h_dbls[2 * (S.lane0 + g)];
+      c->stats.min_cut_gap = std::min(c->stats.min_cut_gap, c->h_dbls[2 * (S.lane0 + g) + 1]);
     }
     rc = launch_svd_bridge(st, fb, chi_cap); if (rc) return rc;
   }
@@ -1058,6 +1154,52 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
   return 0;
 }
 
+int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
+  if (gate_bonds.empty()) return 0;
+  BatchState S;
+  S.gate_bonds = gate_bonds; S.ng = (int)gate_bonds.size(); S.lane0 = 0; S.st = c->st;
+  int rc = batch_p1(c, S);
+  if (!rc) rc = batch_p2(c, S);
+  if (!rc) rc = batch_p3(c, S);
+  return rc;
+}
+
+// Two half-batches of one colour class, skewed by one phase on two streams: the Jacobi SVD of a
+// half-batch is latency-bound on a few SMs (one cluster per core), so the other half-batch's Gram /
+// reconstruction GEMMs and permutations run beside it.  The gates of a class touch disjoint sites
+// and bonds, so the half-batches are independent; results are identical to the serial schedule.
+// Host order: p1(X) | p2(X) (SVD_X goes out first, onto free SMs) | p1(Y) | p2(Y) | p3(X) | p3(Y).
+int run_batch_piped(pepo_ctx* c, const std::vector<int>& gate_bonds) {
+  const int ng = (int)gate_bonds.size();
+  const int nx = (ng + 1) / 2;
+  BatchState X, Y;
+  X.gate_bonds.assign(gate_bonds.begin(), gate_bonds.begin() + nx);
+  Y.gate_bonds.assign(gate_bonds.begin() + nx, gate_bonds.end());
+  X.ng = nx; Y.ng = ng - nx; X.lane0 = 0; Y.lane0 = nx;
+  X.st = c->st; Y.st = c->st2; X.hp = c->hp[0]; Y.hp = c->hp[1];
+  X.ev[0] = c->pev[0]; X.ev[1] = c->pev[1]; Y.ev[0] = c->pev[2]; Y.ev[1] = c->pev[3];
+  X.piped = Y.piped = true;
+  // st2 starts after everything already queued on the caller's stream
+  PEPO_CUDA_OK(cudaEventRecord(c->pev[4], c->st));
+  PEPO_CUDA_OK(cudaStreamWaitEvent(c->st2, c->pev[4], 0));
+  int rc = batch_p1(c, X);
+  if (!rc) rc = batch_p2(c, X);
+  if (!rc) rc = batch_p1(c, Y);
+  if (!rc) rc = batch_p2(c, Y);
+  if (!rc) rc = batch_p3(c, X);
+  if (!rc) rc = batch_p3(c, Y);
+  // join: the caller's stream continues after st2
+  cudaEventRecord(c->pev[5], c->st2);
+  cudaStreamWaitEvent(c->st, c->pev[5], 0);
+  c->cur_st = c->st;
+  if (rc) { cudaStreamSynchronize(c->st2); cudaStreamSynchronize(c->hp[0]); cudaStreamSynchronize(c->hp[1]); return rc; }
+  if (c->prof.on) {
+    cudaStreamSynchronize(c->st); cudaStreamSynchronize(c->st2);
+    prof_flush(c);
+  }
+  return 0;
+}
+
 }  // namespace
 
 extern "C" int pepo_apply_bond(pepo_ctx* c, int bond) {
@@ -1074,7 +1216,8 @@ extern "C" int pepo_trotter_step(pepo_ctx* c) {
   for (auto& cls : c->classes) {
     for (size_t i0 = 0; i0 < cls.size(); i0 += c->B) {
       std::vector<int> g(cls.begin() + i0, cls.begin() + std::min(cls.size(), i0 + (size_t)c->B));
-      rc = run_batch(c, g);
+      if (c->pipeline && g.size() >= 2) rc = run_batch_piped(c, g);
+      else rc = run_batch(c, g);
       if (rc) return rc;
     }
   }

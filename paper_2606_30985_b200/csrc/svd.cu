@@ -1249,8 +1249,36 @@ int launch_set_identity(cudaStream_t st, double* Q, long long m, int k) {
   return 0;
 }
 
+static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
+                            int precond_min);
+
+// The launch configuration (cluster size, columns per CTA, register tile) fixes the order of the
+// pair rotations, i.e. the rounding of the result.  It is therefore chosen per problem SIZE, never
+// from the composition of the batch: problems of equal (min, max) dimension share a launch, and a
+// gate gives bit-identical results whichever other gates run beside it (serial or pipelined class).
 int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
                       int precond_min) {
+  if (b.count == 0) return 0;
+  bool done[PEPO_MAXT] = {false};
+  for (int t0 = 0; t0 < b.count; t0++) {
+    if (done[t0]) continue;
+    const int nc0 = std::min(b.r1[t0], b.r2[t0]), mm0 = std::max(b.r1[t0], b.r2[t0]);
+    SvdBatch g; g.count = 0;
+    for (int t = t0; t < b.count; t++) {
+      if (done[t] || std::min(b.r1[t], b.r2[t]) != nc0 || std::max(b.r1[t], b.r2[t]) != mm0) continue;
+      const int q = g.count++;
+      g.K[q] = b.K[t]; g.ldk[q] = b.ldk[t]; g.r1[q] = b.r1[t]; g.r2[q] = b.r2[t];
+      g.G[q] = b.G[t]; g.V[q] = b.V[t]; g.sv[q] = b.sv[t]; g.order[q] = b.order[t]; g.sweeps[q] = b.sweeps[t];
+      done[t] = true;
+    }
+    int rc = launch_svd_group(st, g, tol, max_sweeps, with_v, precond_min);
+    if (rc) return rc;
+  }
+  return 0;
+}
+
+static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
+                            int precond_min) {
   if (b.count == 0) return 0;
   int ncmax = 1, lenmax = 2;
   for (int t = 0; t < b.count; t++) {
@@ -1270,7 +1298,7 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
     int mmax = 2;
     for (int t = 0; t < b.count; t++) mmax = std::max(mmax, std::max(b.r1[t], b.r2[t]));
     const int nreg = (mmax + 31) / 32 <= 2 ? 2 : (mmax + 31) / 32 <= 4 ? 4 : (mmax + 31) / 32 <= 6 ? 6 : 8;
-    if (CS <= 8 && bs <= 16 && mmax <= 256) {
+    if (CS <= 16 && bs <= 16 && mmax <= 256) {
       const int LENc = 32 * nreg;
       const size_t base = ((size_t)4 * bs * LENc + 4 * bs) * 8 + (size_t)((4 * bs + 3) & ~3) * 4 + (16 + 4) * 8;
       const size_t vs8 = (size_t)(((mmax + 1) & ~1) + 2) * 8;
@@ -1292,6 +1320,10 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<2>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<4>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<6>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<8>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         attr_done = true;
       }
       cudaError_t e;
