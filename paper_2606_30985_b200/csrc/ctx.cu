@@ -29,6 +29,7 @@
 #include <cstring>
 #include <string>
 #include <vector>
+#include <thread>
 
 namespace pepo {
 
@@ -194,6 +195,8 @@ struct Prof {
   bool on = false;
   std::vector<cudaEvent_t> ev;
   std::vector<int> cat;          // category of pair i
+  std::vector<int> strm;         // stream id of pair i (trace)
+  int trace = 0;                 // option "trace": print (category, stream, start, end) of every pair at the flush
   size_t used = 0;               // pairs in flight
   double ms[PC_COUNT] = {0}, flops[PC_COUNT] = {0}, bytes[PC_COUNT] = {0};
   long long cnt[PC_COUNT] = {0};
@@ -214,11 +217,14 @@ struct pepo_ctx {
   int svd_precond_min = 32;            // QR-precondition core SVDs with min(r1,r2) >= this (0: off)
   cudaStream_t st;
   cudaStream_t cur_st = nullptr;       // stream the profiling events of the current launches go to
-  // pipelined schedule of a colour class (option "pipeline"): second half-batch on st2, the Jacobi
-  // kernels of the two half-batches on the high-priority streams hp[0], hp[1]
-  int pipeline = 1;
-  cudaStream_t st2 = nullptr, hp[2] = {nullptr, nullptr};
-  cudaEvent_t pev[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  // pipelined schedule of a Trotter step (option "pipeline" = number of piece streams, 0/1 = serial):
+  // pieces of the colour classes on the streams ps[], their Jacobi kernels on the high-priority
+  // streams hp[]; pev: per stream [svd fork, svd join, read-back], then [fork, join per stream]
+  int pipeline = 4;
+  static constexpr int NSMAX = 4;
+  cudaStream_t ps[NSMAX] = {nullptr, nullptr, nullptr, nullptr}, hp[NSMAX] = {nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t pev[4 * NSMAX + 1] = {nullptr};
+  std::vector<cudaEvent_t> done_ev;    // completion events of the pieces of a pipelined step
   int n_sites, n_bonds, n_hb;
   std::vector<SiteInfo> sites;
   std::vector<BondInfo> bonds;
@@ -257,6 +263,12 @@ void prof_flush(pepo_ctx* c) {        // call only after a stream synchronize
   for (size_t i = 0; i < P.used; i++) {
     float ms = 0.f;
     if (cudaEventElapsedTime(&ms, P.ev[2 * i], P.ev[2 * i + 1]) == cudaSuccess) P.ms[P.cat[i]] += ms;
+    if (P.trace) {
+      float t0 = 0.f, t1 = 0.f;
+      cudaEventElapsedTime(&t0, P.ev[0], P.ev[2 * i]);
+      cudaEventElapsedTime(&t1, P.ev[0], P.ev[2 * i + 1]);
+      fprintf(stderr, "TRACE %d %d %.3f %.3f\n", P.cat[i], P.strm[i], t0, t1);
+    }
   }
   P.used = 0;
 }
@@ -267,11 +279,13 @@ struct ProfScope {
     if (!P.on) return;
     if (2 * (P.used + 1) > P.ev.size()) {
       cudaStreamSynchronize(c->st);
-      if (c->st2) { cudaStreamSynchronize(c->st2); cudaStreamSynchronize(c->hp[0]); cudaStreamSynchronize(c->hp[1]); }
+      for (int i = 0; i < pepo_ctx::NSMAX; i++) if (c->ps[i]) { cudaStreamSynchronize(c->ps[i]); cudaStreamSynchronize(c->hp[i]); }
       prof_flush(c);
     }
     P.cat[P.used] = cat; P.cnt[cat]++; P.flops[cat] += flops; P.bytes[cat] += bytes;
     st = c->cur_st ? c->cur_st : c->st;
+    P.strm[P.used] = 0;
+    for (int i = 0; i < pepo_ctx::NSMAX; i++) { if (st == c->ps[i]) P.strm[P.used] = i; if (st == c->hp[i]) P.strm[P.used] = pepo_ctx::NSMAX + i; }
     cudaEventRecord(P.ev[2 * P.used], st);
     active = true;
   }
@@ -571,9 +585,16 @@ extern "C" int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, doub
   {
     int lo = 0, hi = 0;
     cudaDeviceGetStreamPriorityRange(&lo, &hi);          // hi = numerically smallest = highest priority
-    bool ok = cudaStreamCreateWithPriority(&c->st2, cudaStreamNonBlocking, lo) == cudaSuccess;
-    for (int i = 0; i < 2 && ok; i++) ok = cudaStreamCreateWithPriority(&c->hp[i], cudaStreamNonBlocking, hi) == cudaSuccess;
-    for (int i = 0; i < 8 && ok; i++) ok = cudaEventCreateWithFlags(&c->pev[i], cudaEventDisableTiming) == cudaSuccess;
+    // priorities: Jacobi kernels highest (they need whole SMs as soon as some are free), then the
+    // first piece stream, then the second: when both piece streams hold GEMM work the first one is
+    // served first, which re-creates the half-period skew between them after every join
+    bool ok = true;
+    for (int i = 0; i < pepo_ctx::NSMAX && ok; i++) {
+      const int pr = std::min(lo, hi + 1 + i);           // descending priority, all below the Jacobi streams
+      ok = cudaStreamCreateWithPriority(&c->ps[i], cudaStreamNonBlocking, pr) == cudaSuccess &&
+           cudaStreamCreateWithPriority(&c->hp[i], cudaStreamNonBlocking, hi) == cudaSuccess;
+    }
+    for (int i = 0; i < 4 * pepo_ctx::NSMAX + 1 && ok; i++) ok = cudaEventCreateWithFlags(&c->pev[i], cudaEventDisableTiming) == cudaSuccess;
     if (!ok) { set_error("init: stream / event creation failed"); delete c; return -3; }
   }
   c->cur_st = c->st;
@@ -605,9 +626,12 @@ extern "C" int pepo_init(pepo_ctx** out, int Lx, int Ly, int cx, int cy, double 
 extern "C" int pepo_destroy(pepo_ctx* c) {
   if (!c) return 0;
   cudaStreamSynchronize(c->st);
-  if (c->st2) { cudaStreamSynchronize(c->st2); cudaStreamDestroy(c->st2); }
-  for (int i = 0; i < 2; i++) if (c->hp[i]) { cudaStreamSynchronize(c->hp[i]); cudaStreamDestroy(c->hp[i]); }
-  for (int i = 0; i < 8; i++) if (c->pev[i]) cudaEventDestroy(c->pev[i]);
+  for (int i = 0; i < pepo_ctx::NSMAX; i++) {
+    if (c->ps[i]) { cudaStreamSynchronize(c->ps[i]); cudaStreamDestroy(c->ps[i]); }
+    if (c->hp[i]) { cudaStreamSynchronize(c->hp[i]); cudaStreamDestroy(c->hp[i]); }
+  }
+  for (int i = 0; i < 4 * pepo_ctx::NSMAX + 1; i++) if (c->pev[i]) cudaEventDestroy(c->pev[i]);
+  for (auto e : c->done_ev) cudaEventDestroy(e);
   cudaFreeHost(c->h_ints); cudaFreeHost(c->h_dbls); cudaFreeHost(c->h_chi_msg);
   cudaFreeHost(c->h_scal); cudaFreeHost(c->h_delta); cudaFreeHost(c->h_bpints);
   delete c;
@@ -630,10 +654,11 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "svd_block") set_svd_block((int)v);
   else if (k == "svd_c16") set_svd_c16((int)v);
   else if (k == "pipeline") c->pipeline = (int)v;
+  else if (k == "trace") c->prof.trace = (int)v;
   else if (k == "profile") {
     Prof& P = c->prof;
     if (v != 0.0 && P.ev.empty()) {
-      P.ev.resize(2 * 4096); P.cat.assign(4096, 0);
+      P.ev.resize(2 * 4096); P.cat.assign(4096, 0); P.strm.assign(4096, 0);
       for (auto& e : P.ev) if (cudaEventCreate(&e) != cudaSuccess) { set_error("profile: cudaEventCreate failed"); return -3; }
     }
     cudaStreamSynchronize(c->st); prof_flush(c);
@@ -1164,40 +1189,121 @@ int run_batch(pepo_ctx* c, const std::vector<int>& gate_bonds) {
   return rc;
 }
 
-// Two half-batches of one colour class, skewed by one phase on two streams: the Jacobi SVD of a
-// half-batch is latency-bound on a few SMs (one cluster per core), so the other half-batch's Gram /
-// reconstruction GEMMs and permutations run beside it.  The gates of a class touch disjoint sites
-// and bonds, so the half-batches are independent; results are identical to the serial schedule.
-// Host order: p1(X) | p2(X) (SVD_X goes out first, onto free SMs) | p1(Y) | p2(Y) | p3(X) | p3(Y).
-int run_batch_piped(pepo_ctx* c, const std::vector<int>& gate_bonds) {
-  const int ng = (int)gate_bonds.size();
-  const int nx = (ng + 1) / 2;
-  BatchState X, Y;
-  X.gate_bonds.assign(gate_bonds.begin(), gate_bonds.begin() + nx);
-  Y.gate_bonds.assign(gate_bonds.begin() + nx, gate_bonds.end());
-  X.ng = nx; Y.ng = ng - nx; X.lane0 = 0; Y.lane0 = nx;
-  X.st = c->st; Y.st = c->st2; X.hp = c->hp[0]; Y.hp = c->hp[1];
-  X.ev[0] = c->pev[0]; X.ev[1] = c->pev[1]; Y.ev[0] = c->pev[2]; Y.ev[1] = c->pev[3];
-  X.piped = Y.piped = true;
-  // st2 starts after everything already queued on the caller's stream
-  PEPO_CUDA_OK(cudaEventRecord(c->pev[4], c->st));
-  PEPO_CUDA_OK(cudaStreamWaitEvent(c->st2, c->pev[4], 0));
-  int rc = batch_p1(c, X);
-  if (!rc) rc = batch_p2(c, X);
-  if (!rc) rc = batch_p1(c, Y);
-  if (!rc) rc = batch_p2(c, Y);
-  if (!rc) rc = batch_p3(c, X);
-  if (!rc) rc = batch_p3(c, Y);
-  // join: the caller's stream continues after st2
-  cudaEventRecord(c->pev[5], c->st2);
-  cudaStreamWaitEvent(c->st, c->pev[5], 0);
-  c->cur_st = c->st;
-  if (rc) { cudaStreamSynchronize(c->st2); cudaStreamSynchronize(c->hp[0]); cudaStreamSynchronize(c->hp[1]); return rc; }
-  if (c->prof.on) {
-    cudaStreamSynchronize(c->st); cudaStreamSynchronize(c->st2);
-    prof_flush(c);
+// ---------------------------------------------------------------------------------------------
+// Pipelined Trotter step (option "pipeline", default on).  The Jacobi SVD of a batch is latency-
+// bound on a few SMs (one cluster per core), so each colour class is cut into pieces that run on
+// two streams, skewed against each other: while one piece sits in its SVD the other runs its Gram /
+// reconstruction GEMMs and permutations.  A piece depends only on the earlier pieces that touch one
+// of its sites (same stream: stream order; other stream: an event), so on the square lattice the
+// lower and the upper half of the grid advance through three of the four colour classes without
+// waiting for each other.  The host drives the two streams by polling the read-back events of the
+// phases (Cholesky flags, chi_new).  Gate results do not depend on the schedule: no kernel takes
+// its configuration from the batch composition (tested bit-identical to the serial schedule).
+// ---------------------------------------------------------------------------------------------
+struct Piece {
+  BatchState S;
+  int stream = 0, phase = 0;
+  std::vector<int> sites;
+};
+
+int run_step_piped(pepo_ctx* c) {
+  const int NS = std::min(std::min(c->pipeline, pepo_ctx::NSMAX), c->B);
+  const int hb = c->B / NS;                      // lanes per stream
+  std::vector<Piece> P;
+  for (auto& cls : c->classes) {
+    const int n = (int)cls.size();
+    if (n == 0) continue;
+    int np = (n + hb - 1) / hb;
+    np = ((np + NS - 1) / NS) * NS;              // a multiple of the stream count: stream q % NS keeps its part of the grid
+    np = std::min(np, n);
+    for (int q = 0; q < np; q++) {
+      const int a = (int)((long long)n * q / np), b = (int)((long long)n * (q + 1) / np);
+      if (b <= a) continue;
+      Piece pc;
+      pc.stream = q % NS;
+      pc.S.gate_bonds.assign(cls.begin() + a, cls.begin() + b);
+      pc.S.ng = b - a;
+      for (int e : pc.S.gate_bonds) { pc.sites.push_back(c->bonds[e].v1); pc.sites.push_back(c->bonds[e].v2); }
+      P.push_back(std::move(pc));
+    }
   }
-  return 0;
+  const int np = (int)P.size();
+  while ((int)c->done_ev.size() < np) {
+    cudaEvent_t e;
+    PEPO_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    c->done_ev.push_back(e);
+  }
+  std::vector<int> queue[pepo_ctx::NSMAX];
+  for (int i = 0; i < np; i++) {
+    Piece& pc = P[i];
+    const int s = pc.stream;
+    queue[s].push_back(i);
+    pc.S.lane0 = s * hb;
+    pc.S.st = c->ps[s];
+    pc.S.hp = c->hp[s];
+    pc.S.ev[0] = c->pev[3 * s]; pc.S.ev[1] = c->pev[3 * s + 1];
+    pc.S.piped = true;
+  }
+  // the piece streams start after everything already queued on the caller's stream (the field gate)
+  cudaEvent_t fork = c->pev[3 * pepo_ctx::NSMAX];
+  PEPO_CUDA_OK(cudaEventRecord(fork, c->st));
+  for (int s = 0; s < NS; s++) PEPO_CUDA_OK(cudaStreamWaitEvent(c->ps[s], fork, 0));
+  std::vector<char> mark(c->n_sites, 0);
+  size_t pos[pepo_ctx::NSMAX] = {0, 0, 0, 0};
+  int rc = 0, left = np;
+  while (!rc && left > 0) {
+    bool progressed = false;
+    for (int s = 0; s < NS && !rc; s++) {
+      if (pos[s] >= queue[s].size()) continue;
+      const int i = queue[s][pos[s]];
+      Piece& u = P[i];
+      cudaEvent_t rb = c->pev[3 * s + 2];
+      if (u.phase == 0) {
+        // earlier pieces on the other streams that touch one of my sites
+        for (int v : u.sites) mark[v] = 1;
+        bool ready = true;
+        std::vector<int> deps;
+        for (int d = 0; d < i; d++) {
+          if (P[d].stream == s) continue;
+          bool hit = false;
+          for (int v : P[d].sites) hit |= (mark[v] != 0);
+          if (!hit) continue;
+          if (P[d].phase < 3) { ready = false; break; }
+          deps.push_back(d);
+        }
+        for (int v : u.sites) mark[v] = 0;
+        if (!ready) continue;
+        for (int d : deps) PEPO_CUDA_OK(cudaStreamWaitEvent(u.S.st, c->done_ev[d], 0));
+        rc = batch_p1(c, u.S);
+        if (!rc) { PEPO_CUDA_OK(cudaEventRecord(rb, u.S.st)); }
+        u.phase = 1; progressed = true;
+      } else if (cudaEventQuery(rb) == cudaSuccess) {
+        if (u.phase == 1) {
+          rc = batch_p2(c, u.S);
+          if (!rc) { PEPO_CUDA_OK(cudaEventRecord(rb, u.S.st)); }
+          u.phase = 2;
+        } else {
+          rc = batch_p3(c, u.S);
+          if (!rc) { PEPO_CUDA_OK(cudaEventRecord(c->done_ev[i], u.S.st)); }
+          u.phase = 3; pos[s]++; left--;
+        }
+        progressed = true;
+      }
+    }
+    if (!progressed) std::this_thread::yield();
+  }
+  // join: the caller's stream continues after all piece streams
+  for (int s = 0; s < NS; s++) {
+    cudaEventRecord(c->pev[3 * pepo_ctx::NSMAX + 1 + s], c->ps[s]);
+    cudaStreamWaitEvent(c->st, c->pev[3 * pepo_ctx::NSMAX + 1 + s], 0);
+  }
+  c->cur_st = c->st;
+  if (rc || c->prof.on) {
+    cudaStreamSynchronize(c->st);
+    for (int s = 0; s < NS; s++) { cudaStreamSynchronize(c->ps[s]); cudaStreamSynchronize(c->hp[s]); }
+    if (c->prof.on) prof_flush(c);
+  }
+  return rc;
 }
 
 }  // namespace
@@ -1213,11 +1319,11 @@ extern "C" int pepo_trotter_step(pepo_ctx* c) {
   c->stats.gate_err = 0.0; c->stats.min_cut_gap = 1.0; c->stats.jacobi_sweeps = 0;
   int rc = pepo_apply_field(c);
   if (rc) return rc;
+  if (c->pipeline >= 2 && c->B >= 2) return run_step_piped(c);
   for (auto& cls : c->classes) {
     for (size_t i0 = 0; i0 < cls.size(); i0 += c->B) {
       std::vector<int> g(cls.begin() + i0, cls.begin() + std::min(cls.size(), i0 + (size_t)c->B));
-      if (c->pipeline && g.size() >= 2) rc = run_batch_piped(c, g);
-      else rc = run_batch(c, g);
+      rc = run_batch(c, g);
       if (rc) return rc;
     }
   }
