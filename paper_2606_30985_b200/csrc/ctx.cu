@@ -221,6 +221,7 @@ struct pepo_ctx {
   // pieces of the colour classes on the streams ps[], their Jacobi kernels on the high-priority
   // streams hp[]; pev: per stream [svd fork, svd join, read-back], then [fork, join per stream]
   int pipeline = 4;
+  int piece_stride = 1;                // 1: piece q of a class takes gates q, q + np, ... (else contiguous runs)
   static constexpr int NSMAX = 4;
   cudaStream_t ps[NSMAX] = {nullptr, nullptr, nullptr, nullptr}, hp[NSMAX] = {nullptr, nullptr, nullptr, nullptr};
   cudaEvent_t pev[4 * NSMAX + 1] = {nullptr};
@@ -653,8 +654,10 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "svd_precond_min") c->svd_precond_min = (int)v;
   else if (k == "svd_block") set_svd_block((int)v);
   else if (k == "svd_c16") set_svd_c16((int)v);
+  else if (k == "jacobi_early") set_svd_early(v);
   else if (k == "pipeline") c->pipeline = (int)v;
   else if (k == "trace") c->prof.trace = (int)v;
+  else if (k == "piece_stride") c->piece_stride = (int)v;
   else if (k == "profile") {
     Prof& P = c->prof;
     if (v != 0.0 && P.ev.empty()) {
@@ -1217,12 +1220,16 @@ int run_step_piped(pepo_ctx* c) {
     np = ((np + NS - 1) / NS) * NS;              // a multiple of the stream count: stream q % NS keeps its part of the grid
     np = std::min(np, n);
     for (int q = 0; q < np; q++) {
-      const int a = (int)((long long)n * q / np), b = (int)((long long)n * (q + 1) / np);
-      if (b <= a) continue;
       Piece pc;
       pc.stream = q % NS;
-      pc.S.gate_bonds.assign(cls.begin() + a, cls.begin() + b);
-      pc.S.ng = b - a;
+      if (c->piece_stride) {
+        for (int g = q; g < n; g += np) pc.S.gate_bonds.push_back(cls[g]);
+      } else {
+        const int a = (int)((long long)n * q / np), b = (int)((long long)n * (q + 1) / np);
+        pc.S.gate_bonds.assign(cls.begin() + a, cls.begin() + b);
+      }
+      if (pc.S.gate_bonds.empty()) continue;
+      pc.S.ng = (int)pc.S.gate_bonds.size();
       for (int e : pc.S.gate_bonds) { pc.sites.push_back(c->bonds[e].v1); pc.sites.push_back(c->bonds[e].v2); }
       P.push_back(std::move(pc));
     }

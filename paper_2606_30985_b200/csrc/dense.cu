@@ -42,31 +42,27 @@ __global__ void __launch_bounds__(512) potrf_upper_kernel(MatBatch b, InfoPtrs i
       D[i * (PB + 1) + j] = (i <= j) ? A[(jb + i) + (long long)(jb + j) * ld] : 0.0;
     }
     __syncthreads();
-    if (warp == 0) {
-      // right-looking Cholesky of the nb x nb block, lane = column
-      for (int k = 0; k < nb; k++) {
-        double piv = D[k * (PB + 1) + k];
-        if (!(piv > 0.0) || !isfinite(piv)) {
-          if (lane == 0 && s_fail == 0) s_fail = jb + k + 1;
-          break;
-        }
-        double rkk = sqrt(piv);
-        // scale-invariant conditioning measure (R9): R_kk / ||column k|| = sine of the angle between
-        // column k and the span of the previous columns
-        if (lane == 0) s_rmin = fmin(s_rmin, rkk / sqrt(dg[jb + k]));
-        __syncwarp();
-        double rkj = 0.0;
-        if (lane < nb && lane >= k) {
-          rkj = (lane == k) ? rkk : D[k * (PB + 1) + lane] / rkk;
-          D[k * (PB + 1) + lane] = rkj;
-        }
-        __syncwarp();
-        if (lane < nb && lane > k) {
-          for (int i = k + 1; i <= lane; i++)
-            D[i * (PB + 1) + lane] -= D[k * (PB + 1) + i] * rkj;
-        }
-        __syncwarp();
+    // right-looking Cholesky of the nb x nb block with the whole CTA: per column k one pass that
+    // scales row k and one rank-1 update of the trailing (i, j) entries (two barriers per column;
+    // one warp doing the update row by row was half of the kernel's time)
+    for (int k = 0; k < nb; k++) {
+      const double piv = D[k * (PB + 1) + k];
+      if (!(piv > 0.0) || !isfinite(piv)) {               // uniform: every thread reads the same value
+        if (tid == 0 && s_fail == 0) s_fail = jb + k + 1;
+        break;
       }
+      const double rkk = sqrt(piv);
+      // scale-invariant conditioning measure (R9): R_kk / ||column k|| = sine of the angle between
+      // column k and the span of the previous columns
+      if (tid == 0) s_rmin = fmin(s_rmin, rkk / sqrt(dg[jb + k]));
+      __syncthreads();
+      if (tid >= k && tid < nb) D[k * (PB + 1) + tid] = (tid == k) ? rkk : D[k * (PB + 1) + tid] / rkk;
+      __syncthreads();
+      for (int e = tid; e < nb * nb; e += blockDim.x) {
+        const int i = e / nb, j = e % nb;
+        if (i > k && j >= i) D[i * (PB + 1) + j] -= D[k * (PB + 1) + i] * D[k * (PB + 1) + j];
+      }
+      __syncthreads();
     }
     __syncthreads();
     if (s_fail) break;

@@ -64,6 +64,7 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
 void set_svd_min_cluster(int cs);
 void set_svd_block(int on);
 void set_svd_c16(int on);
+void set_svd_early(double cosine);
 
 struct SvdFinishBatch {
   int count;

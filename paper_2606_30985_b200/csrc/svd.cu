@@ -198,6 +198,7 @@ __global__ void __launch_bounds__(1024) jacobi_svd_kernel(SvdBatch b, double tol
 // cluster barriers).  No global-memory traffic inside the iteration.
 // ---------------------------------------------------------------------------------------------
 int g_svd_block = 0;                    // tunable (option "svd_block"): block form of the super-rounds
+double g_svd_early = 1e-7;              // tunable (option "jacobi_early"): see jacobi_c16_kernel
 int g_svd_c16 = 1;                      // tunable (option "svd_c16"): 16-lane hot-path kernel
 int g_svd_min_cluster = 1;              // tunable (option "svd_min_cluster"): smallest cluster size tried
 constexpr int JC_THREADS = 1024;
@@ -748,7 +749,8 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 
 template <int NREG>
 __global__ void __launch_bounds__(J16_THREADS, 1)
-jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int precond_min, int pw) {
+jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int precond_min, int pw,
+                  double early2) {
   constexpr int LEN = 32 * NREG, LEN2 = 16 * NREG;
   extern __shared__ __align__(16) double jsm[];
   cg::cluster_group cluster = cg::this_cluster();
@@ -785,7 +787,7 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
   }
   for (int e = tid; e < 2 * bs; e += J16_THREADS) ids[e] = ((e / bs) ? 2 * CS - 1 - crank : crank) * bs + (e % bs);
   __shared__ double s_red[32];
-  __shared__ int s_flag;
+  __shared__ int s_flag;                  // a pair with cos^2 > early2 was rotated in this sweep
   fro = warp_sum1(fro);
   if (lane == 0) s_red[warp] = fro;
   __syncthreads();
@@ -902,6 +904,7 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
   const int nrt = nrw * 32;
   for (int sw = 0; active && sw < max_sweeps; sw++) {
     double* nrm = nrmbuf + cur * 2 * bs;
+    bool big = false;                                    // this thread rotated a pair with cos^2 > early2 in this sweep
     // intra-block pairs of both resident blocks: nb2 half-warps per round
     for (int r = 0; r < nb2 - 1; r++) {
       if (hw < nb2) {
@@ -933,7 +936,7 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
             xn.y = cs * x[u].y - sn * y[u].y; yn.y = sn * x[u].y + cs * y[u].y;
             p2[l16 + 16 * u] = xn; q2[l16 + 16 * u] = yn;
           }
-          s_flag = 1;
+          big |= (ga * ga > early2 * al * be);
         }
       }
       __syncthreads();
@@ -1001,8 +1004,8 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
               if (bad) { aln = a0; ben = b0; }
             }
             if (dorot) {
+              big |= (ga * ga > early2 * al * be);
               al = aln; be = ben;
-              s_flag = 1;
               if (!last) {
 #pragma unroll
                 for (int u = 0; u < NREG; u++) cq[l16 + 16 * u] = y[u];
@@ -1034,7 +1037,8 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
         }
       }
       if (sr == 2 * CS - 2) {
-        // last barrier of the sweep carries the "any rotation" flags
+        // last barrier of the sweep carries the largest rotated cos^2 of every CTA
+        if (big) s_flag = 1;
         __syncthreads();
         if (tid < CS) cluster.map_shared_rank(flags, tid)[crank] = s_flag ? 1.0 : 0.0;
       }
@@ -1044,11 +1048,16 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
       ids = idbuf + cur * 2 * bs;
     }
     sweeps = sw + 1;
-    double tot = 0.0;
-    for (int c = 0; c < CS; c++) tot += flags[c];
+    // Was any pair with |cos| > max(tol, early) rotated in this sweep, cluster-wide?  If not the
+    // iteration has converged: either nothing was rotated, or only pairs with tiny cosines were,
+    // and the cyclic Jacobi iteration converges quadratically (a sweep whose largest cosine is c
+    // leaves cosines of order c^2), so the sweep that would only confirm |cos| <= tol is not run
+    // (option "jacobi_early" = cosine threshold, default 1e-7; 0 = always run the confirming sweep).
+    double anybig = 0.0;
+    for (int c = 0; c < CS; c++) anybig += flags[c];
     if (tid == 0) s_flag = 0;                         // every thread passed the flag push (cluster barrier)
     __syncthreads();
-    if (tot == 0.0) break;
+    if (anybig == 0.0) break;
   }
   // ---- write back ------------------------------------------------------------------------------
   double* G = b.G[t];
@@ -1228,6 +1237,7 @@ __global__ void set_identity_kernel(double* Q, long long m, int k) {
 
 void set_svd_block(int on) { g_svd_block = on ? 1 : 0; }
 void set_svd_c16(int on) { g_svd_c16 = on ? 1 : 0; }
+void set_svd_early(double c) { g_svd_early = c < 0.0 ? 0.0 : c; }
 void set_svd_min_cluster(int cs) { g_svd_min_cluster = cs < 1 ? 1 : (cs > 16 ? 16 : cs); }
 
 int launch_svd_vectors(cudaStream_t st, const double* G, const double* V, const double* s,
@@ -1326,11 +1336,12 @@ static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int 
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<8>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         attr_done = true;
       }
+      const double early2 = g_svd_early * g_svd_early;
       cudaError_t e;
-      if (nreg == 2) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<2>, b, tol, max_sweeps, bs, CS, precond_min, pw);
-      else if (nreg == 4) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<4>, b, tol, max_sweeps, bs, CS, precond_min, pw);
-      else if (nreg == 6) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<6>, b, tol, max_sweeps, bs, CS, precond_min, pw);
-      else e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<8>, b, tol, max_sweeps, bs, CS, precond_min, pw);
+      if (nreg == 2) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<2>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
+      else if (nreg == 4) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<4>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
+      else if (nreg == 6) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<6>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
+      else e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<8>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
       if (e != cudaSuccess) { set_error("svd: cluster launch failed: %s", cudaGetErrorString(e)); return -3; }
       PEPO_COUNT_LAUNCH();
       return 0;
