@@ -23,6 +23,7 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 constexpr int BP_THREADS = 256;
+int g_bp_form = 2;             // tunable (option "bp_form"): 1 = per-column reductions, 2 = per-chunk reductions
 constexpr int BP_MAXK = 8;     // dU <= 256 (kernel instantiated for 32*KU >= dU, KU in {2,4,8}: fewer
                                // registers -> more resident CTAs -> more bytes in flight)
 
@@ -103,6 +104,103 @@ __global__ void __launch_bounds__(BP_THREADS) bp_partial_kernel(BpBatch b) {
     if (d < dD) S.partD[(long long)blk * dD + d] = accD;
   }
   // s(l,r) = sum_d mD[d] (sum_u T[u,d,l,r] mU[u])
+  for (int i = threadIdx.x; i < lr1 - lr0; i += BP_THREADS) {
+    double sv = 0.0;
+#pragma unroll
+    for (int w2 = 0; w2 < nw; w2++) sv += sS[i][w2];
+    S.partS[lr0 + i] = sv;
+  }
+}
+
+// Second form of the partial sweep (the one launched): the reduction over u that pD[d] needs is
+// NOT taken per column.  Warp w owns the columns d = w + nw j (j < KD) of every slice of its
+// chunk; each lane accumulates its own share of pD[d] in a register across all slices of the
+// chunk (weight w_lr folded in), and the KD warp reductions happen once per chunk.  Per slice only
+// s(l,r) needs one warp reduction.  Per column that leaves two loads and four FMAs per lane and no
+// shuffle (the first form spent ~30 of its ~45 instructions per column pair on reductions and was
+// issue-bound at 0.35 of the HBM rate); the KD columns of a slice are KU*KD independent loads in
+// flight per lane.  Sums are in a fixed order: deterministic.
+template <int KU, int KD>
+__global__ void __launch_bounds__(BP_THREADS) bp_partial2_kernel(BpBatch b) {
+  constexpr int nw = BP_THREADS / 32;
+  __shared__ double sU[nw][32 * KU];
+  __shared__ double sS[PEPO_BP_MAXCHUNK][nw];
+  const int t = blockIdx.y;
+  const BpSite& S = b.s[t];
+  const int blk = blockIdx.x;
+  if (blk >= S.nchunks) return;
+  const int dU = S.d[0], dD = S.d[1], dL = S.d[2], dR = S.d[3];
+  const int nlr = dL * dR;
+  const int lr0 = blk * S.chunk, lr1 = min(nlr, lr0 + S.chunk);
+  const double* mU = S.in[0];
+  const double* mD = S.in[1];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  double accU[KU], mu[KU], accD[KD], md[KD];
+#pragma unroll
+  for (int k = 0; k < KU; k++) {
+    accU[k] = 0.0;
+    const int u = lane + 32 * k;
+    mu[k] = (u < dU) ? mU[u] : 0.0;
+  }
+#pragma unroll
+  for (int j = 0; j < KD; j++) {
+    accD[j] = 0.0;
+    const int d = warp + nw * j;
+    md[j] = (d < dD) ? mD[d] : 0.0;
+  }
+  for (int lr = lr0; lr < lr1; lr++) {
+    const int l = lr % dL, r = lr / dL;
+    const double w = S.in[2][l] * S.in[3][r];
+    const double* T = S.T + (long long)lr * dU * dD;
+    double ps[KU], wmu[KU];
+#pragma unroll
+    for (int k = 0; k < KU; k++) { ps[k] = 0.0; wmu[k] = w * mu[k]; }
+    // all loads of the slice first (columns past dD are clamped to a valid one: their md is 0 and
+    // their accD is never stored), then the arithmetic: KU*KD independent loads in flight per lane
+    constexpr int JB = (KD * KU <= 16) ? KD : (16 / KU);     // columns per load batch (16 loads per lane)
+#pragma unroll
+    for (int j0 = 0; j0 < KD; j0 += JB) {
+      double tv[JB][KU];
+#pragma unroll
+      for (int j = 0; j < JB; j++) {
+        const int d = min(warp + nw * (j0 + j), dD - 1);
+        const double* col = T + (long long)d * dU;
+#pragma unroll
+        for (int k = 0; k < KU; k++) {
+          const int u = lane + 32 * k;
+          tv[j][k] = (u < dU) ? __ldg(col + u) : 0.0;
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < JB; j++) {
+#pragma unroll
+        for (int k = 0; k < KU; k++) {
+          ps[k] = fma(tv[j][k], md[j0 + j], ps[k]);
+          accD[j0 + j] = fma(tv[j][k], wmu[k], accD[j0 + j]);
+        }
+      }
+    }
+    double sp = 0.0;
+#pragma unroll
+    for (int k = 0; k < KU; k++) { accU[k] = fma(w, ps[k], accU[k]); sp = fma(mu[k], ps[k], sp); }
+    sp = warp_sum(sp);
+    if (lane == 0) sS[lr - lr0][warp] = sp;
+  }
+#pragma unroll
+  for (int k = 0; k < KU; k++) sU[warp][lane + 32 * k] = accU[k];
+#pragma unroll
+  for (int j = 0; j < KD; j++) {
+    const int d = warp + nw * j;
+    const double v = warp_sum(accD[j]);
+    if (lane == 0 && d < dD) S.partD[(long long)blk * dD + d] = v;
+  }
+  __syncthreads();
+  for (int u = threadIdx.x; u < dU; u += BP_THREADS) {
+    double p = 0.0;
+#pragma unroll
+    for (int w2 = 0; w2 < nw; w2++) p += sU[w2][u];
+    S.partU[(long long)blk * dU + u] = p;
+  }
   for (int i = threadIdx.x; i < lr1 - lr0; i += BP_THREADS) {
     double sv = 0.0;
 #pragma unroll
@@ -274,13 +372,21 @@ int launch_bp_partial(cudaStream_t st, const BpBatch& b) {
   dim3 grid(maxlr, b.count);
   int dumax = 1;
   for (int t = 0; t < b.count; t++) dumax = std::max(dumax, b.s[t].d[0]);
-  if (dumax <= 64) bp_partial_kernel<2><<<grid, BP_THREADS, 0, st>>>(b);
-  else if (dumax <= 128) bp_partial_kernel<4><<<grid, BP_THREADS, 0, st>>>(b);
+  int ddmax = 1;
+  for (int t = 0; t < b.count; t++) ddmax = std::max(ddmax, b.s[t].d[1]);
+  if (g_bp_form == 1) {
+    if (dumax <= 64) bp_partial_kernel<2><<<grid, BP_THREADS, 0, st>>>(b);
+    else if (dumax <= 128) bp_partial_kernel<4><<<grid, BP_THREADS, 0, st>>>(b);
+    else bp_partial_kernel<8><<<grid, BP_THREADS, 0, st>>>(b);
+  } else if (dumax <= 64 && ddmax <= 64) bp_partial2_kernel<2, 8><<<grid, BP_THREADS, 0, st>>>(b);
+  else if (dumax <= 128 && ddmax <= 128) bp_partial2_kernel<4, 16><<<grid, BP_THREADS, 0, st>>>(b);
   else bp_partial_kernel<8><<<grid, BP_THREADS, 0, st>>>(b);
   PEPO_COUNT_LAUNCH();
   PEPO_CUDA_OK(cudaGetLastError());
   return 0;
 }
+
+void set_bp_form(int f) { g_bp_form = (f == 1) ? 1 : 2; }
 
 int launch_bp_finalize(cudaStream_t st, const BpBatch& b, double damping, int update,
                        unsigned long long* delta_bits, int* flag) {

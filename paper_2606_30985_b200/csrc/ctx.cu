@@ -655,6 +655,7 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "svd_block") set_svd_block((int)v);
   else if (k == "svd_c16") set_svd_c16((int)v);
   else if (k == "jacobi_early") set_svd_early(v);
+  else if (k == "bp_form") set_bp_form((int)v);
   else if (k == "pipeline") c->pipeline = (int)v;
   else if (k == "trace") c->prof.trace = (int)v;
   else if (k == "piece_stride") c->piece_stride = (int)v;
