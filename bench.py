@@ -195,11 +195,27 @@ def run_ours(args):
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     ms = e0.elapsed_time(e1)
-    prof = sim.profile()
+    prof_overlapped = sim.profile()
     sim.set_option("profile", 0)
     launches = sim.stats()["kernel_launches"] - launches0
     ms = R.max_over_ranks(ms, dev)
     stats = sim.stats()
+    # per-kernel durations with the GPU to itself: PROF_STEPS more steps on the serial schedule
+    # (pipeline = 0) right after the timed region.  In the timed region the default schedule runs
+    # the pieces of a colour class on several streams, so a kernel's event-to-event time there
+    # includes the SMs it shared with concurrent kernels (reported as kernels_overlapped).
+    pipe = 4
+    for kv in args.opt:
+        if kv.startswith("pipeline="):
+            pipe = int(float(kv.split("=")[1]))
+    PROF_STEPS = 2
+    sim.set_option("pipeline", 0)
+    sim.set_option("profile", 2)
+    for _ in range(PROF_STEPS):
+        one_step(sim)
+    prof = sim.profile()
+    sim.set_option("profile", 0)
+    sim.set_option("pipeline", pipe)
 
     # ---- end-to-end: host buffers in, host scalar out, copies inside the timed region ----------
     e2e = None
@@ -240,16 +256,22 @@ def run_ours(args):
     # dominant kernel class by accumulated device time
     dom = max(prof, key=lambda k: prof[k]["ms"])
     fp64_peak = peaks["bf16_tflops_sustained"] * FP64_NOMINAL_RATIO
-    per = {}
-    for k, v in prof.items():
-        if v["count"] == 0:
-            continue
-        per[k] = {"ms_per_step": v["ms"] / args.steps, "share": v["ms"] / max(ms, 1e-9),
-                  "launch_groups_per_step": v["count"] / args.steps}
-        if v["flops"] > 0 and v["ms"] > 0:
-            per[k]["tflops"] = v["flops"] / v["ms"] * 1e-9
-        if v["bytes"] > 0 and v["ms"] > 0:
-            per[k]["gbs"] = v["bytes"] / v["ms"] * 1e-6
+    def per_kernel(pr, nsteps):
+        out = {}
+        tot = sum(v["ms"] for v in pr.values())
+        for k, v in pr.items():
+            if v["count"] == 0:
+                continue
+            out[k] = {"ms_per_step": v["ms"] / nsteps, "share": v["ms"] / max(tot, 1e-9),
+                      "launch_groups_per_step": v["count"] / nsteps}
+            if v["flops"] > 0 and v["ms"] > 0:
+                out[k]["tflops"] = v["flops"] / v["ms"] * 1e-9
+            if v["bytes"] > 0 and v["ms"] > 0:
+                out[k]["gbs"] = v["bytes"] / v["ms"] * 1e-6
+        return out
+
+    per = per_kernel(prof, PROF_STEPS)
+    per_overlapped = per_kernel(prof_overlapped, args.steps)
     alu_peak = 148 * 64 * 2 * 1.965e9 * 1e-12     # fp64 DFMA: 148 SMs x 64 FMA/clk x 2 x 1.965 GHz
 
     def roof_of(k):
@@ -291,13 +313,19 @@ def run_ours(args):
                                "all bonds saturated; step = trotter_step + bp_converge(tol %g, damping %g) + correlation"
                                % (L, L, args.cx, args.cy, chi, args.bp_tol, args.bp_damping),
                    "state": info["prep"], "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "l2": "working set per step (%.1f GB of site tensors) exceeds the 126 MB L2" % (stats["arena_high_water"] / 1e9)},
+                   "l2": "working set per step (%.1f GB of site tensors) exceeds the 126 MB L2" % (stats["arena_high_water"] / 1e9),
+                   "schedule": "pipeline=%d piece streams in the timed region (0 = serial)" % pipe,
+                   "rooflines": "per-kernel durations (kernels, roofline, rooflines) from %d extra steps on the serial "
+                                "schedule right after the timed region, CUDA events on the launching stream; "
+                                "kernels_overlapped = the same event pairs inside the timed region, where kernels of "
+                                "different streams share the SMs" % PROF_STEPS},
         "trotter_only_steps_per_s": world * args.steps / (t_trot * 1e-3),
         "trotter_ms_per_step": t_trot / args.steps,
         "bp_sweeps_per_step": sweeps_tot / args.steps, "jacobi_sweeps_per_step": jac / args.steps,
         "last_C": c_last, "gate_err_last_step": stats["gate_err"],
         "qr": {"cholesky": stats["n_cholesky"], "householder": stats["n_householder"], "chol_rejected": stats["n_chol_failed"]},
         "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "rooflines": rooflines, "kernels": per,
+        "kernels_overlapped": per_overlapped,
         "arena": {"high_water_bytes": stats["arena_high_water"], "model_bytes": stats["arena_model_bytes"],
                   "inflight_gates": stats["max_inflight_gates"]},
         "e2e": e2e,

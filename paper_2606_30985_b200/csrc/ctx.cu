@@ -224,7 +224,8 @@ struct pepo_ctx {
   int piece_stride = 1;                // 1: piece q of a class takes gates q, q + np, ... (else contiguous runs)
   static constexpr int NSMAX = 4;
   cudaStream_t ps[NSMAX] = {nullptr, nullptr, nullptr, nullptr}, hp[NSMAX] = {nullptr, nullptr, nullptr, nullptr};
-  cudaEvent_t pev[4 * NSMAX + 1] = {nullptr};
+  cudaEvent_t pev[5 * NSMAX + 1] = {nullptr};
+  int svd_gate = 0;                    // 1: heavy kernels queued after a Jacobi launch wait until its blocks have begun
   std::vector<cudaEvent_t> done_ev;    // completion events of the pieces of a pipelined step
   int n_sites, n_bonds, n_hb;
   std::vector<SiteInfo> sites;
@@ -595,7 +596,7 @@ extern "C" int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, doub
       ok = cudaStreamCreateWithPriority(&c->ps[i], cudaStreamNonBlocking, pr) == cudaSuccess &&
            cudaStreamCreateWithPriority(&c->hp[i], cudaStreamNonBlocking, hi) == cudaSuccess;
     }
-    for (int i = 0; i < 4 * pepo_ctx::NSMAX + 1 && ok; i++) ok = cudaEventCreateWithFlags(&c->pev[i], cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; i < 5 * pepo_ctx::NSMAX + 1 && ok; i++) ok = cudaEventCreateWithFlags(&c->pev[i], cudaEventDisableTiming) == cudaSuccess;
     if (!ok) { set_error("init: stream / event creation failed"); delete c; return -3; }
   }
   c->cur_st = c->st;
@@ -631,7 +632,7 @@ extern "C" int pepo_destroy(pepo_ctx* c) {
     if (c->ps[i]) { cudaStreamSynchronize(c->ps[i]); cudaStreamDestroy(c->ps[i]); }
     if (c->hp[i]) { cudaStreamSynchronize(c->hp[i]); cudaStreamDestroy(c->hp[i]); }
   }
-  for (int i = 0; i < 4 * pepo_ctx::NSMAX + 1; i++) if (c->pev[i]) cudaEventDestroy(c->pev[i]);
+  for (int i = 0; i < 5 * pepo_ctx::NSMAX + 1; i++) if (c->pev[i]) cudaEventDestroy(c->pev[i]);
   for (auto e : c->done_ev) cudaEventDestroy(e);
   cudaFreeHost(c->h_ints); cudaFreeHost(c->h_dbls); cudaFreeHost(c->h_chi_msg);
   cudaFreeHost(c->h_scal); cudaFreeHost(c->h_delta); cudaFreeHost(c->h_bpints);
@@ -656,6 +657,7 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "svd_c16") set_svd_c16((int)v);
   else if (k == "jacobi_early") set_svd_early(v);
   else if (k == "bp_form") set_bp_form((int)v);
+  else if (k == "svd_gate") c->svd_gate = (int)v;
   else if (k == "pipeline") c->pipeline = (int)v;
   else if (k == "trace") c->prof.trace = (int)v;
   else if (k == "piece_stride") c->piece_stride = (int)v;
@@ -798,6 +800,7 @@ struct BatchState {        // one batch of gates moving through the three phases
   cudaStream_t st = nullptr;       // stream of this batch
   cudaStream_t hp = nullptr;       // high-priority stream for the Jacobi kernel (nullptr: st)
   cudaEvent_t ev[2] = {nullptr, nullptr};
+  cudaEvent_t started = nullptr;   // if set: fires when the blocks of this batch's Jacobi kernel have begun
   bool piped = false;              // another batch is in flight: keep the profiling events until the class ends
   bool have_chol = false;
   SvdFinishBatch fb;
@@ -1018,7 +1021,10 @@ int batch_p2(pepo_ctx* c, BatchState& S) {
       c->cur_st = ss;
       {
         ProfScope ps(c, PC_SVD, 0, 0);
-        rc = launch_svd_jacobi(ss, sb, c->jacobi_tol, c->jacobi_max_sweeps, false, c->svd_precond_min); if (rc) return rc;
+        set_svd_started_event(S.started);
+        rc = launch_svd_jacobi(ss, sb, c->jacobi_tol, c->jacobi_max_sweeps, false, c->svd_precond_min);
+        set_svd_started_event(nullptr);
+        if (rc) return rc;
       }
       c->cur_st = st;
       if (S.hp) {
@@ -1251,6 +1257,7 @@ int run_step_piped(pepo_ctx* c) {
     pc.S.hp = c->hp[s];
     pc.S.ev[0] = c->pev[3 * s]; pc.S.ev[1] = c->pev[3 * s + 1];
     pc.S.piped = true;
+    pc.S.started = c->svd_gate ? c->pev[4 * pepo_ctx::NSMAX + 1 + s] : nullptr;
   }
   // the piece streams start after everything already queued on the caller's stream (the field gate)
   cudaEvent_t fork = c->pev[3 * pepo_ctx::NSMAX];
@@ -1289,6 +1296,10 @@ int run_step_piped(pepo_ctx* c) {
         if (u.phase == 1) {
           rc = batch_p2(c, u.S);
           if (!rc) { PEPO_CUDA_OK(cudaEventRecord(rb, u.S.st)); }
+          // the Jacobi kernel needs whole SMs: heavy kernels the other streams queue from now on
+          // wait until its blocks are resident (launch-completion event)
+          if (!rc && u.S.started)
+            for (int s2 = 0; s2 < NS; s2++) if (s2 != s) PEPO_CUDA_OK(cudaStreamWaitEvent(c->ps[s2], u.S.started, 0));
           u.phase = 2;
         } else {
           rc = batch_p3(c, u.S);

@@ -65,6 +65,7 @@ void set_svd_min_cluster(int cs);
 void set_svd_block(int on);
 void set_svd_c16(int on);
 void set_svd_early(double cosine);
+void set_svd_started_event(cudaEvent_t e);   // launch-completion event of the next hot-path SVD launch (nullptr: none)
 
 struct SvdFinishBatch {
   int count;

@@ -198,6 +198,7 @@ __global__ void __launch_bounds__(1024) jacobi_svd_kernel(SvdBatch b, double tol
 // cluster barriers).  No global-memory traffic inside the iteration.
 // ---------------------------------------------------------------------------------------------
 int g_svd_block = 0;                    // tunable (option "svd_block"): block form of the super-rounds
+cudaEvent_t g_svd_started = nullptr;    // if set: recorded when all blocks of the next hot-path launch have begun
 double g_svd_early = 1e-7;              // tunable (option "jacobi_early"): see jacobi_c16_kernel
 int g_svd_c16 = 1;                      // tunable (option "svd_c16"): 16-lane hot-path kernel
 int g_svd_min_cluster = 1;              // tunable (option "svd_min_cluster"): smallest cluster size tried
@@ -1238,6 +1239,7 @@ __global__ void set_identity_kernel(double* Q, long long m, int k) {
 void set_svd_block(int on) { g_svd_block = on ? 1 : 0; }
 void set_svd_c16(int on) { g_svd_c16 = on ? 1 : 0; }
 void set_svd_early(double c) { g_svd_early = c < 0.0 ? 0.0 : c; }
+void set_svd_started_event(cudaEvent_t e) { g_svd_started = e; }
 void set_svd_min_cluster(int cs) { g_svd_min_cluster = cs < 1 ? 1 : (cs > 16 ? 16 : cs); }
 
 int launch_svd_vectors(cudaStream_t st, const double* G, const double* V, const double* s,
@@ -1320,10 +1322,16 @@ static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int 
       cfg.blockDim = dim3(J16_THREADS);
       cfg.dynamicSmemBytes = smem;
       cfg.stream = st;
-      cudaLaunchAttribute at[1];
+      cudaLaunchAttribute at[2];
       at[0].id = cudaLaunchAttributeClusterDimension;
       at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
       cfg.attrs = at; cfg.numAttrs = 1;
+      if (g_svd_started) {
+        at[1].id = cudaLaunchAttributeLaunchCompletionEvent;
+        at[1].val.launchCompletionEvent.event = g_svd_started;
+        at[1].val.launchCompletionEvent.flags = 0;
+        cfg.numAttrs = 2;
+      }
       static bool attr_done = false;
       if (!attr_done) {
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
