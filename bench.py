@@ -28,6 +28,11 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 J, H, DT = 1.0, 0.9, 0.05
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the class's main kernel on the 4x4 chi=60
+# saturated state, from the `ncu --set full` captures summarised in profiles/r1c_ncu_top_kernels.md and
+# profiles/r1_ncu_top_kernels.md (bytes; None = not captured).  Launch shapes: svd = 8 cores of 240^2 in one
+# launch; apply_gemm = 216000 x 240 x 240; permute = one 4 x 60^4 interior tensor; bp = partial sweep over all 16 sites.
+NCU_TRAFFIC_4x4_CHI60 = {"svd": 3.75e6, "apply_gemm": 790.3e6, "permute": 784.1e6, "bp": 433.8e6, "gram": None}
 FP64_NOMINAL_RATIO = 45.0 / 2250.0     # B200 fp64 tensor / bf16 tensor, blackwell guide table
 
 
@@ -301,6 +306,9 @@ def run_ours(args):
         return None
 
     rooflines = {k: r for k in prof for r in [roof_of(k)] if r is not None}
+    if (L, chi) == (4, 60):
+        for k, r in rooflines.items():
+            r["traffic"] = NCU_TRAFFIC_4x4_CHI60.get(k)
     roof = rooflines.get(dom) or {"kernel": dom, "bound": "alu", "achieved": None, "peak": alu_peak,
                                   "unit": "TFLOP/s", "frac": None, "traffic": None,
                                   "peak_source": "latency-bound small dense kernel"}
