@@ -61,6 +61,7 @@ int launch_dgemm_batched(cudaStream_t st, int transA, int transB, const GemmProb
 int launch_gram_reduce(cudaStream_t st, const double* part, int ksplit, int n, double* C,
                        long long ldc);
 void gram_plan(long long m, int n, int* ksplit, int* kchunk);
+void set_gram_waves(int waves);   // only lowering it after pepo_init is safe (the partial buffers are sized at init)
 
 // ---- permutation -------------------------------------------------------------------------
 // dst[sum_j o_j * dst_stride[j]] = src[sum_d i_d * src_stride[d]] * prod_d scale_d(i_d),

@@ -223,7 +223,7 @@ struct pepo_ctx {
   int pipeline = 4;
   int piece_stride = 1;                // 1: piece q of a class takes gates q, q + np, ... (else contiguous runs)
   static constexpr int NSMAX = 4;
-  cudaStream_t ps[NSMAX] = {nullptr, nullptr, nullptr, nullptr}, hp[NSMAX] = {nullptr, nullptr, nullptr, nullptr};
+  cudaStream_t ps[NSMAX] = {nullptr}, hp[NSMAX] = {nullptr};
   cudaEvent_t pev[5 * NSMAX + 1] = {nullptr};
   int svd_gate = 0;                    // 1: heavy kernels queued after a Jacobi launch wait until its blocks have begun
   std::vector<cudaEvent_t> done_ev;    // completion events of the pieces of a pipelined step
@@ -658,6 +658,7 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "jacobi_early") set_svd_early(v);
   else if (k == "bp_form") set_bp_form((int)v);
   else if (k == "svd_gate") c->svd_gate = (int)v;
+  else if (k == "gram_waves") set_gram_waves(std::min((int)v, 2));
   else if (k == "pipeline") c->pipeline = (int)v;
   else if (k == "trace") c->prof.trace = (int)v;
   else if (k == "piece_stride") c->piece_stride = (int)v;
@@ -1264,7 +1265,7 @@ int run_step_piped(pepo_ctx* c) {
   PEPO_CUDA_OK(cudaEventRecord(fork, c->st));
   for (int s = 0; s < NS; s++) PEPO_CUDA_OK(cudaStreamWaitEvent(c->ps[s], fork, 0));
   std::vector<char> mark(c->n_sites, 0);
-  size_t pos[pepo_ctx::NSMAX] = {0, 0, 0, 0};
+  size_t pos[pepo_ctx::NSMAX] = {0};
   int rc = 0, left = np;
   while (!rc && left > 0) {
     bool progressed = false;

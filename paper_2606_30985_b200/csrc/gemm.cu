@@ -268,15 +268,24 @@ int launch_dgemm_batched(cudaStream_t st, int transA, int transB, const GemmProb
   return launch_trans<64, 64, 32, 32, 4>(st, transA, transB, dummy, probs_dev, batch, max_M, max_N, 1, 0, nullptr, false);
 }
 
+int g_gram_waves = 2;              // tunable (option "gram_waves"): waves of resident CTAs of the 80x80 Gram kernel
+void set_gram_waves(int w) { g_gram_waves = std::min(std::max(w, 1), 4); }
+
 void gram_plan(long long m, int n, int* ksplit, int* kchunk) {
   // upper-triangle tiles at the tile size launch_dgemm will pick (the choice between the 128 and
   // 64 tiles depends on ksplit itself: plan with the 128 tile first, as before)
   int bt = 128, target = 148 * 2, cap = 128;
-  if (n % 80 == 0) { bt = 80; target = 148 * 4; cap = 100; }     // 128-thread CTAs, 4 resident per SM
+  bool whole_waves = false;
+  if (n % 80 == 0) {
+    // 80x80 tile kernel: 197 registers x 128 threads -> 2 resident CTAs per SM = 296 slots.  The
+    // working CTAs (upper tiles x splits) must fill a whole number of waves: 99 splits x 6 tiles =
+    // 594 CTAs ran as two waves plus a third one of 2 CTAs (ncu: 558 us against 2/3 of that).
+    bt = 80; target = 148 * 2 * g_gram_waves; cap = 100 * g_gram_waves; whole_waves = true;
+  }
   else if (n <= 64) bt = 64;
   const int tn = (n + bt - 1) / bt;
   const int upper = tn * (tn + 1) / 2;
-  int ks = (target + upper - 1) / upper;
+  int ks = whole_waves ? std::max(1, target / upper) : (target + upper - 1) / upper;
   long long maxsplit = (m + 255) / 256;             // at least 256 rows per split
   if (ks > maxsplit) ks = (int)maxsplit;
   if (ks > cap) ks = cap;
