@@ -255,7 +255,7 @@ class PEPOState:
     """
 
     def __init__(self, Lx, Ly, cx, cy, J, h, dt, chi_max, eps_cut=1e-11,
-                 bond_pauli="Z", field_pauli="X", obs_pauli="Z"):
+                 bond_pauli="Z", field_pauli="X", obs_pauli="Z", order=1):
         self.lat = Lattice(Lx, Ly)
         if not (0 <= cx < Lx and 0 <= cy < Ly):
             raise ValueError("centre outside grid")
@@ -268,6 +268,12 @@ class PEPOState:
         # R2/R15: U = exp(-iH dt) = exp(+i dt (J sum PP + h sum F)) for H = -J sum PP - h sum F
         self.G1 = ptm_one_site(self.h * self.dt, field_pauli)
         self.G2 = ptm_two_site(self.J * self.dt, bond_pauli)
+        # order 2 = the symmetric step of PAPER eq. (6): half field gate,
+        # all bond gates, half field gate.  order 1 (R2, BASELINE) leaves everything above as it was.
+        if order not in (1, 2):
+            raise ValueError("order must be 1 or 2")
+        self.order = int(order)
+        self.G1_half = ptm_one_site(0.5 * self.h * self.dt, field_pauli)
         self.psi = []
         for v in range(self.lat.n_sites):
             t = np.zeros([1] * len(self.lat.legs(v)) + [4])
@@ -290,10 +296,12 @@ class PEPOState:
         self.psi[v] = np.asarray(flat, dtype=np.float64).reshape(self.psi[v].shape, order="F").copy()
 
     # -- a1: field gate ----------------------------------------------------------------
-    def apply_field_gate(self):
-        """a1 (R2): psi_v[...,p'] = sum_p G1[p',p] psi_v[...,p], all sites."""
+    def apply_field_gate(self, half=False):
+        """a1 (R2): psi_v[...,p'] = sum_p G1[p',p] psi_v[...,p], all sites
+        (half = True: the half-angle gate of the symmetric step, eq. (6))."""
+        G = self.G1_half if half else self.G1
         for v in range(self.lat.n_sites):
-            self.psi[v] = np.tensordot(self.psi[v], self.G1, axes=([-1], [1]))
+            self.psi[v] = np.tensordot(self.psi[v], G, axes=([-1], [1]))
 
     # -- a2..a13: Algorithm 1 ------------------------------------------------------------
     def _cv_matrix(self, v, d_cut):
@@ -387,6 +395,14 @@ class PEPOState:
         """One first-order step (R2): a1 on all sites, then colours 0..3 (R3), each bond in
         the class order.  PAPER Fig. 1 L310-L342."""
         self.gate_err = 0.0
+        if self.order == 2:
+            # eq. (6): R(h dt/2) on all sites, the bond sweep, R(h dt/2) on all sites
+            self.apply_field_gate(half=True)
+            for cls in self.lat.colour_classes():
+                for e in cls:
+                    self.apply_bond_gate(e)
+            self.apply_field_gate(half=True)
+            return
         self.apply_field_gate()
         for cls in self.lat.colour_classes():
             for e in cls:
