@@ -84,7 +84,13 @@ int pepo_destroy(pepo_ctx* ctx);
 /* Options (key, value): "eps_cut" (1e-11, eq. (11)), "bp_max_sweeps" (100, L256),
  * "bp_max_sweeps_damped" (1000, R7), "chol_min_ratio" (Cholesky when m >= ratio*n, 4, R9),
  * "chol_tau" (diag-ratio rejection threshold 1e-7, R9), "force_householder" (0/1),
- * "jacobi_tol" (1e-15), "jacobi_max_sweeps" (60).  -1 on unknown key. */
+ * "jacobi_tol" (1e-15), "jacobi_max_sweeps" (60), "jacobi_early" (cosine below which a sweep
+ * counts as the last one, 1e-7; 0 = always run the confirming sweep),
+ * "trotter_order" (1 = first-order step, R2; 2 = symmetric step of eq. (6)),
+ * "pipeline" (number of piece streams of a Trotter step, 4; 0 = serial schedule; the results do
+ * not depend on it), and kernel-selection tunables used by the benchmarks ("svd_c16",
+ * "svd_min_cluster", "svd_precond_min", "svd_block", "bp_form", "piece_stride", "gram_waves",
+ * "svd_gate", "profile", "trace").  -1 on unknown key. */
 int pepo_set_option(pepo_ctx* ctx, const char* key, double value);
 
 /* One full first-order Trotter step (Fig. 1; R2, R3): field gate on all
@@ -93,7 +99,7 @@ int pepo_set_option(pepo_ctx* ctx, const char* key, double value);
  * truncation (a9), bridge + reconstruction (a10), inverse permute + deabsorb + write-back
  * (a11-a13).  Asynchronous work on the context stream with one host read of the new bond
  * dimensions per batch of gates. */
-int pepo_trotter_step(pepo_ctx* ctx);
+int pepo_trotter_step(pepo_ctx* ctx);   /* "trotter_order" 2: half field gate, bond sweep, half field gate */
 /* The two halves, for gate-replay tests. */
 int pepo_apply_field(pepo_ctx* ctx);
 int pepo_apply_bond(pepo_ctx* ctx, int bond);

@@ -245,8 +245,10 @@ struct pepo_ctx {
   std::vector<double*> partU, partD, partS;
   double *dG1, *dGamma[2], *dAhat[2], *dSigma;
   int NA;
-  double G1[16];
+  double G1[16], G1h[16];              // field PTM at h dt and at h dt / 2 (symmetric step, eq. (6))
   int f_row_mask, f_col_mask;
+  int trotter_order = 1;               // option "trotter_order": 1 = R2 (BASELINE), 2 = symmetric step of eq. (6)
+  double h_dt = 0.0; int field_pauli_id = 1;
   std::vector<LaneWs> lanes;
   int* lane_ints; double* lane_dbls;      // device readback blocks (B*4 ints, B*2 doubles)
   // pinned host
@@ -525,6 +527,7 @@ extern "C" int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, doub
   c->chi.assign(c->n_bonds, 1);
   // gate tables: field PTM, bond PTM and its operator-Schmidt decomposition
   ptm_one_site(h * dt, field_pauli, c->G1);
+  ptm_one_site(0.5 * h * dt, field_pauli, c->G1h);     // same sparsity pattern as G1
   c->f_row_mask = 0; c->f_col_mask = 0;
   for (int q = 0; q < 4; q++) {
     bool ident = true;
@@ -659,6 +662,10 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "bp_form") set_bp_form((int)v);
   else if (k == "svd_gate") c->svd_gate = (int)v;
   else if (k == "gram_waves") set_gram_waves(std::min((int)v, 2));
+  else if (k == "trotter_order") {
+    if ((int)v != 1 && (int)v != 2) { set_error("set_option: trotter_order must be 1 or 2"); return -1; }
+    c->trotter_order = (int)v;
+  }
   else if (k == "pipeline") c->pipeline = (int)v;
   else if (k == "trace") c->prof.trace = (int)v;
   else if (k == "piece_stride") c->piece_stride = (int)v;
@@ -759,8 +766,15 @@ extern "C" int pepo_get_stats(pepo_ctx* c, pepo_stats* s) {
 // ============================================================================================
 // Trotter step
 // ============================================================================================
+namespace {
+int apply_field_impl(pepo_ctx* c, bool half);
+}
 extern "C" int pepo_apply_field(pepo_ctx* c) {
   if (!c) { set_error("apply_field: NULL"); return -1; }
+  return apply_field_impl(c, false);
+}
+namespace {
+int apply_field_impl(pepo_ctx* c, bool half) {
   if (c->f_row_mask == 0) return 0;
   for (int v0 = 0; v0 < c->n_sites; v0 += PEPO_BP_MAXS) {
     FieldBatch fb;
@@ -769,7 +783,7 @@ extern "C" int pepo_apply_field(pepo_ctx* c) {
       fb.psi[i] = c->sites[v0 + i].psi;
       fb.slab[i] = (long long)(site_live_size(c, v0 + i) / 4);
     }
-    memcpy(fb.G, c->G1, sizeof(fb.G));
+    memcpy(fb.G, half ? c->G1h : c->G1, sizeof(fb.G));
     fb.row_mask = c->f_row_mask; fb.col_mask = c->f_col_mask;
     double fbytes = 0; for (int i = 0; i < fb.count; i++) fbytes += 8.0 * fb.slab[i] * 2 * __builtin_popcount(fb.row_mask);
     ProfScope ps(c, PC_FIELD, 0, fbytes);
@@ -779,6 +793,7 @@ extern "C" int pepo_apply_field(pepo_ctx* c) {
   c->msgs_valid = false;
   return 0;
 }
+}  // namespace
 
 namespace {
 
@@ -1337,17 +1352,24 @@ extern "C" int pepo_apply_bond(pepo_ctx* c, int bond) {
 extern "C" int pepo_trotter_step(pepo_ctx* c) {
   if (!c) { set_error("trotter_step: NULL"); return -1; }
   c->stats.gate_err = 0.0; c->stats.min_cut_gap = 1.0; c->stats.jacobi_sweeps = 0;
-  int rc = pepo_apply_field(c);
+  // order 1 (R2): field gate, bond sweep.  order 2 (PAPER eq. (6)):
+  // half field gate, bond sweep, half field gate.
+  const bool sym = c->trotter_order == 2;
+  int rc = apply_field_impl(c, sym);
   if (rc) return rc;
-  if (c->pipeline >= 2 && c->B >= 2) return run_step_piped(c);
-  for (auto& cls : c->classes) {
-    for (size_t i0 = 0; i0 < cls.size(); i0 += c->B) {
-      std::vector<int> g(cls.begin() + i0, cls.begin() + std::min(cls.size(), i0 + (size_t)c->B));
-      rc = run_batch(c, g);
-      if (rc) return rc;
+  if (c->pipeline >= 2 && c->B >= 2) rc = run_step_piped(c);
+  else {
+    for (auto& cls : c->classes) {
+      for (size_t i0 = 0; i0 < cls.size() && !rc; i0 += c->B) {
+        std::vector<int> g(cls.begin() + i0, cls.begin() + std::min(cls.size(), i0 + (size_t)c->B));
+        rc = run_batch(c, g);
+      }
+      if (rc) break;
     }
   }
-  return 0;
+  if (rc) return rc;
+  if (sym) rc = apply_field_impl(c, true);
+  return rc;
 }
 
 // ============================================================================================

@@ -190,3 +190,32 @@ def test_pipelined_schedule_is_bit_identical_to_serial(gpu):
         assert res[0][0] == r[0]
         assert list(res[0][1]) == list(r[1])
         assert (res[0][2] == r[2]).all() and (res[0][3] == r[3]).all()
+
+
+def test_symmetric_trotter_step_vs_oracle(gpu):
+    """SURVEY NEXT-3, PAPER eq. (6): option trotter_order = 2 (half field gate, bond sweep, half
+    field gate) against the oracle's order = 2 (itself pinned to the dense symmetric splitting in
+    test_oracle_pins.py): untruncated window of 3x3 to 1e-10, truncated 4x4 chi 8 to 1e-6, and the
+    closed form C(n dt) = cos(2 h n dt) at J = 0."""
+    import math
+    torch, B = gpu
+    from oracle import pepo_oracle as po
+    from oracle import dense_check as dc
+    sim, out_g = _run_gpu(B, 3, 3, 1, 1, 8, 10, 1e-10, opts={"trotter_order": 2})
+    st, out_o = po.run_trajectory(3, 3, 1, 1, J, H, DT, 8, 10, 1e-10, order=2)
+    _compare(out_g, out_o, 1e-10, sweeps_slack=1)
+    dense = dc.dense_trotter_correlation(3, 3, 1, 1, J, H, DT, 3, order=2)
+    for t in range(3):                       # chi_max = 8 truncates from step 4 on
+        assert abs(out_g[t]["C"] - dense[t]) < 1e-12
+    sim.close()
+    sim, out_g = _run_gpu(B, 4, 4, 1, 1, 8, 16, 1e-10, damping=0.5, opts={"trotter_order": 2})
+    st, out_o = po.run_trajectory(4, 4, 1, 1, J, H, DT, 8, 16, 1e-10, 0.5, order=2)
+    _compare(out_g, out_o, 1e-6, sweeps_slack=4)
+    sim.close()
+    sim = B.Pepo(3, 3, 1, 1, 0.0, H, DT, 8, 1e-12, 0.0)
+    sim.set_option("trotter_order", 2)
+    for n in range(1, 5):
+        sim.trotter_step()
+        sim.bp_converge()
+        assert abs(sim.correlation() - math.cos(2 * H * n * DT)) < 1e-13
+    sim.close()
