@@ -52,6 +52,8 @@ typedef struct pepo_stats {
   size_t arena_model_bytes; /* closed-form model for the same configuration (eq. (15)-(17) analogue) */
   int max_inflight_gates;   /* gates of one colour class processed concurrently */
   int chi_max_live;         /* largest live bond dimension */
+  int last_bp_trap;         /* trap flag of the diagnostics: the last bp_converge
+                               converged (delta < tol) but needed >= 30 sweeps */
 } pepo_stats;
 
 const char* pepo_last_error(void);
@@ -132,6 +134,11 @@ int pepo_get_site(pepo_ctx* ctx, int x, int y, double* h_dst, size_t n);
 int pepo_set_site(pepo_ctx* ctx, int x, int y, const double* h_src, size_t n);
 int pepo_get_lambda(pepo_ctx* ctx, int bond, double* h_dst, int n);
 int pepo_set_lambda(pepo_ctx* ctx, int bond, const double* h_src, int n);
+/* Diagnostics of PAPER.md Table 1 (L373-L380): bond entanglement entropies
+ * S_e = -sum_k lambda_k^2 log lambda_k^2 over the live Schmidt weights of every bond (lambda is
+ * normalised, eq. (12)), computed on the device.  h_S: host array of n >= n_bonds doubles.
+ * Synchronises the context stream.  -1 on a bad argument. */
+int pepo_bond_entropy(pepo_ctx* ctx, double* h_S, int n);
 /* Device pointer of a packed site tensor (valid until the next gate touching the site). */
 double* pepo_site_ptr(pepo_ctx* ctx, int x, int y);
 

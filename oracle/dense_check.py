@@ -96,3 +96,21 @@ def dense_exact_correlation(Lx, Ly, cx, cy, J, h, t, bond="Z", field="X", obs="Z
     U = _expm_herm(hamiltonian(Lx, Ly, J, h, bond, field), -1j * t)
     O = U.conj().T @ Zc @ U
     return float(np.trace(O @ Zc).real) / 2 ** n
+
+
+def dense_chain_operator_schmidt(n, c, J, h, dt, n_steps, cut, bond="Z", field="X", obs="Z"):
+    """Operator-Schmidt coefficients (normalised to unit 2-norm, descending) of the Trotter-evolved
+    operator O(n_steps) = (U^dag)^n P_c U^n on an open chain of ``n`` sites, across the cut between
+    sites ``cut`` and ``cut + 1``: singular values of O reshaped to (left in x left out) x (right in x
+    right out).  On a tree the simple-update bond weights lambda_e of the untruncated network are
+    exactly these numbers (Vidal gauge), so this pins lambda and the entanglement-entropy diagnostic
+    (PAPER Table 1) to the dense evolution."""
+    U = trotter_unitary(1, n, J, h, dt, bond, field)
+    O = _embed({c: _SIG[obs]}, n)
+    for _ in range(n_steps):
+        O = U.conj().T @ O @ U
+    nl = cut + 1
+    dl, dr = 2 ** nl, 2 ** (n - nl)
+    T = O.reshape(dl, dr, dl, dr).transpose(0, 2, 1, 3).reshape(dl * dl, dr * dr)
+    s = np.linalg.svd(T, compute_uv=False)
+    return s / np.linalg.norm(s)

@@ -408,6 +408,14 @@ class PEPOState:
             for e in cls:
                 self.apply_bond_gate(e)
 
+    # -- diagnostics (Table 1) ---------------------------
+    def bond_entropy(self, e):
+        """S_e = -sum_k lambda_k^2 log lambda_k^2 of the normalised Schmidt weights of bond e
+        (eq. (12): sum_k lambda_k^2 = 1)."""
+        w = self.lam[e] ** 2
+        w = w[w > 0.0]
+        return float(-(w * np.log(w)).sum())
+
     # -- a14: BP on the pinned single-layer network -----------------------------------
     def pinned(self, v):
         """T_v = psi_v[..., p_v], p_c = observable Pauli, else I (step 1)."""

@@ -30,7 +30,7 @@ class PepoStats(C.Structure):
                 ("kernel_launches", C.c_longlong), ("last_bp_sweeps", C.c_int),
                 ("last_bp_status", C.c_int), ("last_bp_delta", C.c_double),
                 ("arena_high_water", C.c_size_t), ("arena_model_bytes", C.c_size_t),
-                ("max_inflight_gates", C.c_int), ("chi_max_live", C.c_int)]
+                ("max_inflight_gates", C.c_int), ("chi_max_live", C.c_int), ("last_bp_trap", C.c_int)]
 
 
 def _load():
@@ -63,6 +63,7 @@ def _load():
         "pepo_get_site": (i, [vp, i, i, vp, sz]),
         "pepo_set_site": (i, [vp, i, i, vp, sz]),
         "pepo_get_lambda": (i, [vp, i, vp, i]),
+        "pepo_bond_entropy": (i, [vp, vp, i]),
         "pepo_set_lambda": (i, [vp, i, vp, i]),
         "pepo_site_ptr": (vp, [vp, i, i]),
         "pepo_permute": (i, [dp, dp, ip, ip, i, vp]),
@@ -205,6 +206,11 @@ class Pepo:
     def set_site(self, x, y, flat):
         flat = np.ascontiguousarray(flat, dtype=np.float64).ravel()
         _check(_lib.pepo_set_site(self._h, x, y, flat.ctypes.data_as(C.c_void_p), flat.size))
+
+    def bond_entropy(self):
+        out = np.empty(self.n_bonds, dtype=np.float64)
+        _check(_lib.pepo_bond_entropy(self._h, out.ctypes.data_as(C.c_void_p), self.n_bonds))
+        return out
 
     def get_lambda(self, bond):
         n = self.bond_dims()[bond]

@@ -401,6 +401,33 @@ int launch_bp_finalize(cudaStream_t st, const BpBatch& b, double damping, int up
   return 0;
 }
 
+// Bond entanglement entropy of the diagnostics table: S_e = -sum_k l_k^2 log l_k^2
+// over the live Schmidt weights of bond e (lambda is normalised, eq. (12)); one warp per bond,
+// fixed-order reduction.  chi_of_msg[2e] = live dimension of bond e.
+__global__ void bond_entropy_kernel(const double* lambda, const int* chi_of_msg, int n_bonds, int chi_max,
+                                    double* out) {
+  const int e = blockIdx.x;
+  if (e >= n_bonds) return;
+  const int chi = chi_of_msg[2 * e];
+  const double* l = lambda + (size_t)e * chi_max;
+  double s = 0.0;
+  for (int k = threadIdx.x; k < chi; k += 32) {
+    const double w = l[k] * l[k];
+    if (w > 0.0) s -= w * log(w);
+  }
+  s = warp_sum(s);
+  if (threadIdx.x == 0) out[e] = s;
+}
+
+int launch_bond_entropy(cudaStream_t st, const double* lambda, const int* chi_of_msg, int n_bonds, int chi_max,
+                        double* out) {
+  if (n_bonds == 0) return 0;
+  bond_entropy_kernel<<<n_bonds, 32, 0, st>>>(lambda, chi_of_msg, n_bonds, chi_max, out);
+  PEPO_COUNT_LAUNCH();
+  PEPO_CUDA_OK(cudaGetLastError());
+  return 0;
+}
+
 int launch_bp_init(cudaStream_t st, double* msgs, const int* chi_of_msg, int n_msgs, int chi_max) {
   if (n_msgs == 0) return 0;
   bp_init_kernel<<<n_msgs, 128, 0, st>>>(msgs, chi_of_msg, n_msgs, chi_max);

@@ -37,5 +37,7 @@ int launch_bp_init(cudaStream_t st, double* msgs, const int* chi_of_msg, int n_m
 int launch_bethe(cudaStream_t st, const double* vs, int n_sites, const double* msgs,
                  const int* chi_of_msg, int n_bonds, int chi_max, double* out_C, int* out_status);
 int launch_field_gate(cudaStream_t st, const FieldBatch& b);
+int launch_bond_entropy(cudaStream_t st, const double* lambda, const int* chi_of_msg, int n_bonds, int chi_max,
+                        double* out);
 
 }  // namespace pepo

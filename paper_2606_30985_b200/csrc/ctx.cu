@@ -1471,6 +1471,7 @@ extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
   }
   c->msgs_valid = true;
   c->stats.last_bp_sweeps = sweeps; c->stats.last_bp_status = status; c->stats.last_bp_delta = delta;
+  c->stats.last_bp_trap = (status == 0 && sweeps >= 30) ? 1 : 0;      // trap flag of PAPER.md L451-L457
   if (h_sweeps) *h_sweeps = sweeps;
   if (h_delta) *h_delta = delta;
   return status;
@@ -1488,6 +1489,21 @@ extern "C" int pepo_correlation(pepo_ctx* c, double* h_C) {
   PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
   *h_C = c->h_scal[0];
   if (c->h_bpints[1] != 0) { set_error("correlation: zero or non-finite Z_e / vs_v"); return -4; }
+  return 0;
+}
+
+// Diagnostics of PAPER.md Table 1 (L373-L380): bond entanglement entropies.
+// Uses the message-partial scratch of the BP sweep (free between sweeps) as the output buffer.
+extern "C" int pepo_bond_entropy(pepo_ctx* c, double* h_S, int n) {
+  if (!c || !h_S || n < c->n_bonds) { set_error("bond_entropy: bad argument (need n >= n_bonds)"); return -1; }
+  if (c->n_bonds == 0) return 0;
+  for (int e = 0; e < c->n_bonds; e++) { c->h_chi_msg[2 * e] = c->chi[e]; c->h_chi_msg[2 * e + 1] = c->chi[e]; }
+  PEPO_CUDA_OK(cudaMemcpyAsync(c->chi_of_msg, c->h_chi_msg, (size_t)2 * c->n_bonds * 4, cudaMemcpyHostToDevice, c->st));
+  double* d_out = c->msgs[c->cur_msg ^ 1];             // spare message buffer: >= n_bonds doubles, rewritten by the next sweep
+  int rc = launch_bond_entropy(c->st, c->lambda, c->chi_of_msg, c->n_bonds, c->chi_max, d_out);
+  if (rc) return rc;
+  PEPO_CUDA_OK(cudaMemcpyAsync(h_S, d_out, (size_t)c->n_bonds * 8, cudaMemcpyDeviceToHost, c->st));
+  PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
   return 0;
 }
 

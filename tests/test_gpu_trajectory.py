@@ -219,3 +219,24 @@ def test_symmetric_trotter_step_vs_oracle(gpu):
         sim.bp_converge()
         assert abs(sim.correlation() - math.cos(2 * H * n * DT)) < 1e-13
     sim.close()
+
+
+def test_diagnostics_bond_entropy_and_trap_flag(gpu):
+    """SURVEY NEXT-2, PAPER Table 1 (L373-L380, L451-L457): pepo_bond_entropy against the oracle's
+    S_e (pinned to the dense operator-Schmidt spectrum in test_oracle_pins.py) along a truncated
+    4x4 run, S = 0 on the product operator, and the trap flag = converged with >= 30 sweeps."""
+    torch, B = gpu
+    from oracle import pepo_oracle as po
+    sim = B.Pepo(4, 4, 1, 1, J, H, DT, 8, 1e-10, 0.5)
+    st = po.PEPOState(4, 4, 1, 1, J, H, DT, 8)
+    assert np.all(sim.bond_entropy() == 0.0)
+    for step in range(12):
+        sim.trotter_step()
+        st.trotter_step()
+        S_g = sim.bond_entropy()
+        S_o = np.array([st.bond_entropy(e) for e in range(st.lat.n_bonds)])
+        assert np.allclose(S_g, S_o, rtol=0, atol=1e-9), (step, np.abs(S_g - S_o).max())
+        status, sweeps, delta = sim.bp_converge()
+        assert sim.stats()["last_bp_trap"] == (1 if (status == 0 and sweeps >= 30) else 0)
+    assert S_g.max() > 0.1
+    sim.close()

@@ -334,3 +334,27 @@ def test_symmetric_step_is_second_order_and_keeps_closed_forms():
         st.trotter_step()
         st.bp_converge(1e-12)
         assert abs(st.correlation() - 1.0) < 1e-13
+
+
+# ---------------------------------------------------------------- diagnostics (Table 1) ----
+def test_bond_weights_and_entropy_equal_dense_operator_schmidt_on_a_chain():
+    """SURVEY NEXT-2 / PAPER Table 1 (L373-L380): S_e = -sum lambda^2 log lambda^2.  On a chain (a
+    tree) the untruncated simple-update weights lambda_e are the operator-Schmidt coefficients of
+    Z_c(t) across the bond, which the dense 2^N evolution gives independently; closed forms:
+    S = 0 for the product operator, S = log chi for a flat spectrum."""
+    n, c, steps = 4, 1, 5
+    st = po.PEPOState(1, n, 0, c, J, H, DT, 64)
+    assert all(st.bond_entropy(e) == 0.0 for e in range(st.lat.n_bonds))
+    for _ in range(steps):
+        st.trotter_step()
+    for cut in range(n - 1):
+        e = st.lat.bond_id(st.lat.site(0, cut), "D")
+        s = dc.dense_chain_operator_schmidt(n, c, J, H, DT, steps, cut)
+        lam = st.lam[e]
+        # weights down to ~1e-10 are kept; those below 1e-8 carry the 1e-11 pruning of eq. (11)
+        assert np.allclose(lam, s[:lam.size], rtol=0, atol=1e-10), (cut, lam, s[:lam.size])
+        assert np.all(s[lam.size:] < 1e-9)
+        w = s[s > 1e-14] ** 2
+        assert abs(st.bond_entropy(e) - float(-(w * np.log(w)).sum())) < 1e-9
+    st.lam[0] = np.full(8, 1 / math.sqrt(8))
+    assert abs(st.bond_entropy(0) - math.log(8)) < 1e-14
