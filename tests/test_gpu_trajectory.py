@@ -240,3 +240,31 @@ def test_diagnostics_bond_entropy_and_trap_flag(gpu):
         assert sim.stats()["last_bp_trap"] == (1 if (status == 0 and sweeps >= 30) else 0)
     assert S_g.max() > 0.1
     sim.close()
+
+
+@pytest.mark.parametrize("shape", [(3, 3, 1, 1), (1, 5, 0, 2), (5, 2, 3, 0), (4, 3, 2, 1), (2, 2, 0, 0)])
+def test_pipelined_schedule_on_irregular_lattices(gpu, shape):
+    """Classes with one gate, empty classes, chains and non-square grids: the multi-stream schedule
+    must give the serial schedule's C(t), bond dimensions and tensors bit for bit, with and without
+    the confirming Jacobi sweep being skipped only at the 1e-12 level (jacobi_early)."""
+    torch, B = gpu
+    Lx, Ly, cx, cy = shape
+    res = {}
+    for name, opts in (("serial", {"pipeline": 0}), ("piped", {"pipeline": 4}), ("piped2", {"pipeline": 2}),
+                       ("noearly", {"pipeline": 4, "jacobi_early": 0.0})):
+        sim = B.Pepo(Lx, Ly, cx, cy, J, H, DT, 6, 1e-10, 0.5)
+        for k, v in opts.items():
+            sim.set_option(k, v)
+        cs = []
+        for _ in range(12):
+            sim.trotter_step()
+            sim.bp_converge()
+            cs.append(sim.correlation())
+        res[name] = (cs, list(sim.bond_dims()), sim.get_site(cx, cy).copy())
+        sim.close()
+    for name in ("piped", "piped2"):
+        assert res[name][0] == res["serial"][0], name
+        assert res[name][1] == res["serial"][1], name
+        assert (res[name][2] == res["serial"][2]).all(), name
+    assert res["noearly"][1] == res["serial"][1]
+    assert max(abs(a - b) for a, b in zip(res["noearly"][0], res["serial"][0])) < 1e-12
