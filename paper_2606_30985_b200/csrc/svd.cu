@@ -730,7 +730,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
 //    the block exchange costs ONE cluster barrier and no extra pass over the columns;
 //  * the cluster-wide "any rotation" flag rides on the last barrier of the sweep.
 // ---------------------------------------------------------------------------------------------
-constexpr int J16_THREADS = 512;
+constexpr int J16_THREADS = 512;       // NREG <= 8 (columns of <= 256 doubles); 256 threads above (255 registers)
 
 __device__ __forceinline__ double half_sum1(double v) {
 #pragma unroll
@@ -748,8 +748,8 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-template <int NREG>
-__global__ void __launch_bounds__(J16_THREADS, 1)
+template <int NREG, int NTHR>
+__global__ void __launch_bounds__(NTHR, 1)
 jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int precond_min, int pw,
                   double early2) {
   constexpr int LEN = 32 * NREG, LEN2 = 16 * NREG;
@@ -773,20 +773,20 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
   double* flags = (double*)(idbuf + ((4 * bs + 3) & ~3));
   double* scal = flags + 16;
   double* vbuf = scal + 4;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = J16_THREADS / 32;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = NTHR / 32;
   int cur = 0;
   double* cols = colbuf;
   int* ids = idbuf;
   // ---- load ---------------------------------------------------------------------------------
   double fro = 0.0;
-  for (int e = tid; e < per; e += J16_THREADS) {
+  for (int e = tid; e < per; e += NTHR) {
     const int k = e % LEN, ci = e / LEN;
     const int j = ((ci / bs) ? 2 * CS - 1 - crank : crank) * bs + (ci % bs);
     double v = 0.0;
     if (j < Nc && k < M) { v = tr ? K[j + (long long)k * ldk] : K[k + (long long)j * ldk]; fro += v * v; }
     cols[e] = v;
   }
-  for (int e = tid; e < 2 * bs; e += J16_THREADS) ids[e] = ((e / bs) ? 2 * CS - 1 - crank : crank) * bs + (e % bs);
+  for (int e = tid; e < 2 * bs; e += NTHR) ids[e] = ((e / bs) ? 2 * CS - 1 - crank : crank) * bs + (e % bs);
   __shared__ double s_red[32];
   __shared__ int s_flag;                  // a pair with cos^2 > early2 was rotated in this sweep
   fro = warp_sum1(fro);
@@ -850,7 +850,7 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
           for (int c = 0; c < CS; c++) {
             if (c == crank) continue;
             double* rv = cluster.map_shared_rank(vbuf, c);
-            for (int e = tid; e < tot; e += J16_THREADS) rv[e] = vbuf[e];
+            for (int e = tid; e < tot; e += NTHR) rv[e] = vbuf[e];
           }
         }
         cluster.sync();
@@ -943,13 +943,14 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
       __syncthreads();
     }
     // squared norms of the resident columns, fresh once per sweep
-    if (hw < 2 * bs) {
-      const double2* c2 = reinterpret_cast<const double2*>(cols + (size_t)hw * LEN);
+    for (int c0 = 0; c0 < 2 * bs; c0 += 2 * nw) {          // 2 bs is even: whole warps stay together
+      const int cc = c0 + hw;
+      const double2* c2 = reinterpret_cast<const double2*>(cols + (size_t)min(cc, 2 * bs - 1) * LEN);
       double a0 = 0.0, a1 = 0.0;
 #pragma unroll
       for (int u = 0; u < NREG; u++) { const double2 x = c2[l16 + 16 * u]; a0 = fma(x.x, x.x, a0); a1 = fma(x.y, x.y, a1); }
       a0 = half_sum1(a0 + a1);
-      if (l16 == 0) nrm[hw] = a0;
+      if (l16 == 0 && cc < 2 * bs) nrm[cc] = a0;
     }
     __syncthreads();
     // super-rounds
@@ -1075,7 +1076,7 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
   __threadfence();
   cluster.sync();
   if (crank == 0) {
-    for (int j = tid; j < Nc; j += J16_THREADS) {
+    for (int j = tid; j < Nc; j += NTHR) {
       const double sj = svu[j];
       int rank = 0;
       for (int l = 0; l < Nc; l++) {
@@ -1309,17 +1310,26 @@ static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int 
     const int bs = (ncmax + 2 * CS - 1) / (2 * CS);
     int mmax = 2;
     for (int t = 0; t < b.count; t++) mmax = std::max(mmax, std::max(b.r1[t], b.r2[t]));
-    const int nreg = (mmax + 31) / 32 <= 2 ? 2 : (mmax + 31) / 32 <= 4 ? 4 : (mmax + 31) / 32 <= 6 ? 6 : 8;
-    if (CS <= 16 && bs <= 16 && mmax <= 256) {
+    int nreg = (mmax + 31) / 32 <= 2 ? 2 : (mmax + 31) / 32 <= 4 ? 4 : (mmax + 31) / 32 <= 6 ? 6 : 8;
+    int CSx = CS, bsx = bs, nthr = J16_THREADS;
+    if (mmax > 256 && mmax <= 416) {
+      // chi in 65..104: cluster of 16 (non-portable size), <= 13 pairs per CTA, columns of <= 416
+      // doubles in registers of a 256-thread CTA; the two column buffers fill shared memory
+      CSx = 16; bsx = (ncmax + 31) / 32; nthr = 256;
+      nreg = (mmax + 31) / 32 <= 10 ? 10 : 13;
+    }
+    if (CSx <= 16 && bsx <= 16 && mmax <= 416 && (mmax <= 256 || bsx <= 13)) {
+      const int CS = CSx, bs = bsx;
       const int LENc = 32 * nreg;
+      const size_t cap = (nthr == 256) ? (size_t)225 * 1024 : JC_SMEM_CAP;
       const size_t base = ((size_t)4 * bs * LENc + 4 * bs) * 8 + (size_t)((4 * bs + 3) & ~3) * 4 + (16 + 4) * 8;
       const size_t vs8 = (size_t)(((mmax + 1) & ~1) + 2) * 8;
       int pw = 1;
-      if (precond_min > 0) pw = (int)std::max<size_t>(1, std::min<size_t>((size_t)bs, (JC_SMEM_CAP - base) / vs8));
+      if (precond_min > 0 && cap > base + vs8) pw = (int)std::max<size_t>(1, std::min<size_t>((size_t)bs, (cap - base) / vs8));
       const size_t smem = base + (size_t)pw * vs8;
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3((unsigned)(b.count * CS));
-      cfg.blockDim = dim3(J16_THREADS);
+      cfg.blockDim = dim3(nthr);
       cfg.dynamicSmemBytes = smem;
       cfg.stream = st;
       cudaLaunchAttribute at[2];
@@ -1334,22 +1344,29 @@ static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int 
       }
       static bool attr_done = false;
       if (!attr_done) {
-        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
-        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
-        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
-        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
-        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<2>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<4>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<6>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<8>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        const int mx = 226 * 1024;                 // 227 KB per CTA less the static shared memory
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<2, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<4, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<6, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<8, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<10, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<13, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<2, 512>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<4, 512>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<6, 512>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<8, 512>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<10, 256>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<13, 256>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         attr_done = true;
       }
       const double early2 = g_svd_early * g_svd_early;
       cudaError_t e;
-      if (nreg == 2) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<2>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
-      else if (nreg == 4) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<4>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
-      else if (nreg == 6) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<6>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
-      else e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<8>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
+      if (nreg == 2) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<2, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
+      else if (nreg == 4) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<4, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
+      else if (nreg == 6) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<6, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
+      else if (nreg == 8) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<8, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
+      else if (nreg == 10) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<10, 256>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
+      else e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<13, 256>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
       if (e != cudaSuccess) { set_error("svd: cluster launch failed: %s", cudaGetErrorString(e)); return -3; }
       PEPO_COUNT_LAUNCH();
       return 0;
