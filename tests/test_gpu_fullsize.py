@@ -175,3 +175,38 @@ def test_config2_saturated_properties(gpu):
     assert 0.0 <= s["gate_err"] < 1e-3
     assert s["arena_high_water"] <= s["arena_model_bytes"] * 1.02 + 65536
     sim.close()
+
+
+@pytest.mark.parametrize("chi", [72, 100])
+def test_gate_replay_large_core_3x3(gpu, chi):
+    """Cores above 256 (chi 65..104) take the cluster-of-16 form of the Jacobi kernel:
+    one Algorithm-1 gate on a corner-edge bond of the 3x3 chi = 72 / 100 synthetic state (core
+    288^2 / 400^2) against the oracle on the same seeded inputs: lambda, and the gated two-site tensor
+    on sampled entries (gauge-invariant, R17)."""
+    torch, B = gpu
+    from paper_2606_30985_b200 import inputs
+    L = 3
+    bond = inputs.bond_id(L, L, 0, 0, "R")
+    sim = B.Pepo(L, L, 1, 1, J, H, DT, chi, 1e-10, 0.5)
+    _load_synthetic(sim, L, chi)
+    st = _oracle_state(L, chi)
+    sim.apply_bond(bond)
+    st.apply_bond_gate(bond)
+    assert sim.bond_dims()[bond] == st.lam[bond].size == chi
+    assert np.allclose(sim.get_lambda(bond), st.lam[bond], rtol=1e-9, atol=1e-13)
+    v1, d1, v2, d2 = st.lat.bond_sites(bond)
+    legs1, legs2 = st.lat.legs(v1), st.lat.legs(v2)
+    g1 = sim.get_site(v1 % L, v1 // L).reshape(st.psi[v1].shape, order="F")
+    g2 = sim.get_site(v2 % L, v2 // L).reshape(st.psi[v2].shape, order="F")
+    ax1, ax2 = legs1.index(d1), legs2.index(d2)
+    rng = np.random.default_rng(11)
+    ns = 4000
+    sh1 = [s for a, s in enumerate(g1.shape) if a != ax1]
+    sh2 = [s for a, s in enumerate(g2.shape) if a != ax2]
+    idx1 = np.stack([rng.integers(0, s, ns) for s in sh1], axis=1)
+    idx2 = np.stack([rng.integers(0, s, ns) for s in sh2], axis=1)
+    th_g = _two_site_samples(g1, ax1, g2, ax2, idx1, idx2)
+    th_o = _two_site_samples(st.psi[v1], ax1, st.psi[v2], ax2, idx1, idx2)
+    scale = np.linalg.norm(th_o) / np.sqrt(ns)
+    assert np.max(np.abs(th_g - th_o)) <= 1e-9 * scale, np.max(np.abs(th_g - th_o)) / scale
+    sim.close()
