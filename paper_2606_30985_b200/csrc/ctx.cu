@@ -248,7 +248,6 @@ struct pepo_ctx {
   double G1[16], G1h[16];              // field PTM at h dt and at h dt / 2 (symmetric step, eq. (6))
   int f_row_mask, f_col_mask;
   int trotter_order = 1;               // option "trotter_order": 1 = R2 (BASELINE), 2 = symmetric step of eq. (6)
-  double h_dt = 0.0; int field_pauli_id = 1;
   std::vector<LaneWs> lanes;
   int* lane_ints; double* lane_dbls;      // device readback blocks (B*4 ints, B*2 doubles)
   // pinned host
