@@ -91,7 +91,7 @@ int pepo_destroy(pepo_ctx* ctx);
  * "trotter_order" (1 = first-order step, R2; 2 = symmetric step of eq. (6)),
  * "pipeline" (number of piece streams of a Trotter step, 4; 0 = serial schedule; the results do
  * not depend on it), and kernel-selection tunables used by the benchmarks ("svd_c16",
- * "svd_min_cluster", "svd_precond_min", "svd_block", "bp_form", "piece_stride", "gram_waves",
+ * "svd_min_cluster", "svd_precond_min", "svd_block", "bp_form", "bp_group", "piece_stride", "gram_waves",
  * "svd_gate", "profile", "trace").  -1 on unknown key. */
 int pepo_set_option(pepo_ctx* ctx, const char* key, double value);
 

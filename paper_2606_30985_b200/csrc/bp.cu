@@ -29,6 +29,7 @@ constexpr int BP_MAXK = 8;     // dU <= 256 (kernel instantiated for 32*KU >= dU
 
 template <int KU>
 __global__ void __launch_bounds__(BP_THREADS) bp_partial_kernel(BpBatch b) {
+  if (b.skip_if && __longlong_as_double((long long)*b.skip_if) < b.skip_tol) return;
   constexpr int nw = BP_THREADS / 32;
   __shared__ double sU[nw][32 * KU];
   __shared__ double sS[PEPO_BP_MAXCHUNK][nw];
@@ -122,6 +123,7 @@ __global__ void __launch_bounds__(BP_THREADS) bp_partial_kernel(BpBatch b) {
 // flight per lane.  Sums are in a fixed order: deterministic.
 template <int KU, int KD>
 __global__ void __launch_bounds__(BP_THREADS) bp_partial2_kernel(BpBatch b) {
+  if (b.skip_if && __longlong_as_double((long long)*b.skip_if) < b.skip_tol) return;
   constexpr int nw = BP_THREADS / 32;
   __shared__ double sU[nw][32 * KU];
   __shared__ double sS[PEPO_BP_MAXCHUNK][nw];
@@ -213,6 +215,7 @@ __global__ void __launch_bounds__(BP_THREADS) bp_partial2_kernel(BpBatch b) {
 __global__ void __launch_bounds__(256) bp_finalize_kernel(BpBatch b, double damping, int update,
                                                           unsigned long long* delta_bits,
                                                           int* flag) {
+  if (b.skip_if && __longlong_as_double((long long)*b.skip_if) < b.skip_tol) return;
   __shared__ double sred[8];
   __shared__ double s_bcast[2];
   const int t = blockIdx.y;

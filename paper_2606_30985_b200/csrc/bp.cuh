@@ -19,7 +19,15 @@ struct BpSite {
   int chunk, nchunks;         // (l,r) slices per CTA of bp_partial_kernel, CTAs for this site
   double* vs;                 // site scalar of eq. (7)
 };
-struct BpBatch { int count; BpSite s[PEPO_BP_MAXS]; };
+struct BpBatch {
+  int count; BpSite s[PEPO_BP_MAXS];
+  // grouped sweeps: if skip_if != nullptr and the delta stored there (bit pattern of a non-negative
+  // double, written by the previous sweep of the group) is below skip_tol, the kernels of this sweep
+  // return at once: the previous sweep had converged (eq. (14)); a skipped sweep leaves its own
+  // delta slot at 0, so every later sweep of the group is skipped too
+  const unsigned long long* skip_if = nullptr;
+  double skip_tol = 0.0;
+};
 
 struct FieldBatch {
   int count;

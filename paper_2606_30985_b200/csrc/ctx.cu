@@ -206,6 +206,8 @@ struct Prof {
 
 using namespace pepo;
 
+constexpr int BP_GROUP = 8;            // delta slots (sweeps per read-back, upper bound)
+
 struct pepo_ctx {
   int Lx, Ly, cx, cy, center;
   double J, h, dt, bp_tol, bp_damping;
@@ -225,6 +227,7 @@ struct pepo_ctx {
   static constexpr int NSMAX = 4;
   cudaStream_t ps[NSMAX] = {nullptr}, hp[NSMAX] = {nullptr};
   cudaEvent_t pev[5 * NSMAX + 1] = {nullptr};
+  int bp_group = 8;                    // option "bp_group": BP sweeps enqueued per delta read-back (1..BP_GROUP)
   int svd_gate = 0;                    // 1: heavy kernels queued after a Jacobi launch wait until its blocks have begun
   std::vector<cudaEvent_t> done_ev;    // completion events of the pieces of a pipelined step
   int n_sites, n_bonds, n_hb;
@@ -371,7 +374,7 @@ int layout(pepo_ctx* c) {
   c->ones = (double*)A.take(8);
   c->vs = (double*)A.take(c->n_sites * 8);
   c->bp_scalars = (double*)A.take(16);
-  c->delta_bits = (unsigned long long*)A.take(8);
+  c->delta_bits = (unsigned long long*)A.take(8 * BP_GROUP);
   c->bp_ints = (int*)A.take(16);
   c->partU.assign(c->n_sites, nullptr); c->partD.assign(c->n_sites, nullptr); c->partS.assign(c->n_sites, nullptr);
   for (int v = 0; v < c->n_sites; v++) {
@@ -582,7 +585,7 @@ extern "C" int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, doub
       cudaMallocHost((void**)&c->h_dbls, (size_t)c->B * 2 * 8 + 16) != cudaSuccess ||
       cudaMallocHost((void**)&c->h_chi_msg, (size_t)2 * c->n_bonds * 4 + 16) != cudaSuccess ||
       cudaMallocHost((void**)&c->h_scal, 64) != cudaSuccess ||
-      cudaMallocHost((void**)&c->h_delta, 16) != cudaSuccess ||
+      cudaMallocHost((void**)&c->h_delta, 8 * BP_GROUP + 16) != cudaSuccess ||
       cudaMallocHost((void**)&c->h_bpints, 16) != cudaSuccess) {
     set_error("init: cudaMallocHost failed"); delete c; return -3;
   }
@@ -660,6 +663,7 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "jacobi_early") set_svd_early(v);
   else if (k == "bp_form") set_bp_form((int)v);
   else if (k == "svd_gate") c->svd_gate = (int)v;
+  else if (k == "bp_group") c->bp_group = (int)v;
   else if (k == "gram_waves") set_gram_waves(std::min((int)v, 2));
   else if (k == "trotter_order") {
     if ((int)v != 1 && (int)v != 2) { set_error("set_option: trotter_order must be 1 or 2"); return -1; }
@@ -1409,11 +1413,15 @@ void fill_bp_site(pepo_ctx* c, int v, int cur, BpSite& S) {
   S.vs = c->vs + v;
 }
 
-int bp_sweep(pepo_ctx* c, double damping, int update) {
+// one sweep from message set `cur`; delta goes to slot `slot` of delta_bits; if prev_slot >= 0 the
+// sweep is skipped on the device when the delta in that slot is already below the tolerance
+int bp_sweep(pepo_ctx* c, double damping, int update, int cur = -1, int slot = 0, int prev_slot = -1) {
+  if (cur < 0) cur = c->cur_msg;
   for (int v0 = 0; v0 < c->n_sites; v0 += PEPO_BP_MAXS) {
     BpBatch bb;
     bb.count = std::min(PEPO_BP_MAXS, c->n_sites - v0);
-    for (int i = 0; i < bb.count; i++) fill_bp_site(c, v0 + i, c->cur_msg, bb.s[i]);
+    if (prev_slot >= 0) { bb.skip_if = c->delta_bits + prev_slot; bb.skip_tol = c->bp_tol; }
+    for (int i = 0; i < bb.count; i++) fill_bp_site(c, v0 + i, cur, bb.s[i]);
     double bbytes = 0; for (int i = 0; i < bb.count; i++) bbytes += 8.0 * bb.s[i].d[0] * bb.s[i].d[1] * bb.s[i].d[2] * bb.s[i].d[3];
     // chunking: ~8 CTAs per SM over the batch, each CTA a contiguous run of (l,r) slices
     const double per_cta = std::max(bbytes / (148.0 * 8.0), 32768.0);
@@ -1427,7 +1435,7 @@ int bp_sweep(pepo_ctx* c, double damping, int update) {
     }
     ProfScope ps(c, PC_BP, 0, bbytes);
     int rc = launch_bp_partial(c->st, bb); if (rc) return rc;
-    rc = launch_bp_finalize(c->st, bb, damping, update, c->delta_bits, c->bp_ints); if (rc) return rc;
+    rc = launch_bp_finalize(c->st, bb, damping, update, c->delta_bits + slot, c->bp_ints); if (rc) return rc;
   }
   return 0;
 }
@@ -1455,17 +1463,29 @@ extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
     const int budget = phase == 0 ? c->bp_max_sweeps : c->bp_max_sweeps_damped;
     if (phase == 1 && !(c->bp_damping > 0.0)) break;
     int rc = bp_init_messages(c); if (rc) return rc;
-    for (int it = 0; it < budget; it++) {
-      PEPO_CUDA_OK(cudaMemsetAsync(c->delta_bits, 0, 8, c->st));
-      rc = bp_sweep(c, damping, 1); if (rc) return rc;
-      PEPO_CUDA_OK(cudaMemcpyAsync(c->h_delta, c->delta_bits, 8, cudaMemcpyDeviceToHost, c->st));
+    // sweeps go out in groups of up to BP_GROUP with one read-back of their deltas per group (one
+    // host round trip instead of BP_GROUP); inside a group the stop test of eq. (14) is taken on the
+    // device: the kernels of a sweep return at once when the previous sweep's delta is below tol
+    for (int it = 0; it < budget && status;) {
+      const int ngr = std::min(c->bp_group < 1 ? 1 : std::min(c->bp_group, BP_GROUP), budget - it);
+      PEPO_CUDA_OK(cudaMemsetAsync(c->delta_bits, 0, 8 * ngr, c->st));
+      for (int g = 0; g < ngr; g++) {
+        rc = bp_sweep(c, damping, 1, c->cur_msg ^ (g & 1), g, g - 1); if (rc) return rc;
+      }
+      PEPO_CUDA_OK(cudaMemcpyAsync(c->h_delta, c->delta_bits, 8 * ngr, cudaMemcpyDeviceToHost, c->st));
       PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
       prof_flush(c);
-      c->cur_msg ^= 1;
-      sweeps++;
-      memcpy(&delta, c->h_delta, 8);
-      if (c->n_bonds == 0) delta = 0.0;
-      if (delta < c->bp_tol) { status = 0; break; }
+      int done = ngr;                                   // sweeps of the group that actually ran
+      for (int g = 0; g < ngr; g++) {
+        double dg;
+        memcpy(&dg, c->h_delta + g, 8);
+        if (c->n_bonds == 0) dg = 0.0;
+        delta = dg;
+        if (dg < c->bp_tol) { status = 0; done = g + 1; break; }
+      }
+      if (done & 1) c->cur_msg ^= 1;
+      sweeps += done;
+      it += done;
     }
   }
   c->msgs_valid = true;
