@@ -908,13 +908,24 @@ int batch_p1(pepo_ctx* c, BatchState& S) {
       int p = pb.count++;
       pb.A[p] = W.Rx; pb.ld[p] = t.N; pb.m[p] = t.N; pb.n[p] = t.N; infos[p] = W.info;
     }
+    // the latency-bound small kernels of the gate's critical chain (dressing, POTRF here; the whole
+    // of p2; bridges and W in p3) go to the piece's high-priority stream, so that their few CTAs do
+    // not queue behind the GEMM / permutation CTAs of the other pieces (seen: POTRF 1.05 ms instead
+    // of 0.42, core GEMM 0.4 instead of 0.1)
+    cudaStream_t sh = S.hp ? S.hp : st;
+    if (sh != st) {
+      PEPO_CUDA_OK(cudaEventRecord(S.ev[0], st));
+      PEPO_CUDA_OK(cudaStreamWaitEvent(sh, S.ev[0], 0));
+      c->cur_st = sh;
+    }
     if (db.count) {
       int rc;
-      { ProfScope ps(c, PC_DRESS, 0, 0); rc = launch_dress_gram(st, db, gt); if (rc) return rc; }
-      { ProfScope ps(c, PC_CHOL, 0, 0); rc = launch_potrf(st, pb, infos, c->chol_tau); if (rc) return rc; }
-      PEPO_CUDA_OK(cudaMemcpyAsync(c->h_ints + 4 * S.lane0, c->lane_ints + 4 * S.lane0, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
+      { ProfScope ps(c, PC_DRESS, 0, 0); rc = launch_dress_gram(sh, db, gt); if (rc) return rc; }
+      { ProfScope ps(c, PC_CHOL, 0, 0); rc = launch_potrf(sh, pb, infos, c->chol_tau); if (rc) return rc; }
+      PEPO_CUDA_OK(cudaMemcpyAsync(c->h_ints + 4 * S.lane0, c->lane_ints + 4 * S.lane0, (size_t)ng * 16, cudaMemcpyDeviceToHost, sh));
       S.have_chol = true;
     }
+    c->cur_st = st;
   }
   return 0;
 }
@@ -922,7 +933,7 @@ int batch_p1(pepo_ctx* c, BatchState& S) {
 // phase 2: Cholesky flags (host), Householder fallback, core, SVD, truncation (ends with the chi_new read-back)
 int batch_p2(pepo_ctx* c, BatchState& S) {
   const int ng = S.ng;
-  cudaStream_t st = S.st;
+  cudaStream_t st = S.hp ? S.hp : S.st;     // p2 is all small kernels + the Jacobi kernel: high-priority stream
   std::vector<TaskGeo>& T = S.T;
   const std::vector<int>& gate_bonds = S.gate_bonds;
   const int NA = c->NA;
@@ -1031,24 +1042,12 @@ int batch_p2(pepo_ctx* c, BatchState& S) {
     {
       // the Jacobi kernel needs whole SMs (a cluster per core): on the pipelined schedule it goes to
       // a high-priority stream so that it is placed ahead of the other half-batch's GEMM CTAs
-      cudaStream_t ss = st;
-      if (S.hp) {
-        PEPO_CUDA_OK(cudaEventRecord(S.ev[0], st));
-        PEPO_CUDA_OK(cudaStreamWaitEvent(S.hp, S.ev[0], 0));
-        ss = S.hp;
-      }
-      c->cur_st = ss;
       {
         ProfScope ps(c, PC_SVD, 0, 0);
         set_svd_started_event(S.started);
-        rc = launch_svd_jacobi(ss, sb, c->jacobi_tol, c->jacobi_max_sweeps, false, c->svd_precond_min);
+        rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps, false, c->svd_precond_min);
         set_svd_started_event(nullptr);
         if (rc) return rc;
-      }
-      c->cur_st = st;
-      if (S.hp) {
-        PEPO_CUDA_OK(cudaEventRecord(S.ev[1], S.hp));
-        PEPO_CUDA_OK(cudaStreamWaitEvent(st, S.ev[1], 0));
       }
       ProfScope ps(c, PC_SVD, 0, 0);
       rc = launch_svd_truncate(st, fb, c->chi_max, c->eps_cut); if (rc) return rc;
@@ -1063,6 +1062,7 @@ int batch_p2(pepo_ctx* c, BatchState& S) {
 int batch_p3(pepo_ctx* c, BatchState& S) {
   const int ng = S.ng;
   cudaStream_t st = S.st;
+  cudaStream_t sh = S.hp ? S.hp : st;       // small kernels of the chain (see batch_p1)
   std::vector<TaskGeo>& T = S.T;
   const std::vector<int>& gate_bonds = S.gate_bonds;
   const int NA = c->NA;
@@ -1070,12 +1070,12 @@ int batch_p3(pepo_ctx* c, BatchState& S) {
   gt.Gamma[0] = c->dGamma[0]; gt.Gamma[1] = c->dGamma[1];
   gt.Ahat[0] = c->dAhat[0]; gt.Ahat[1] = c->dAhat[1];
   gt.sigma = c->dSigma;
-  c->cur_st = st;
+  c->cur_st = sh;
   (void)gate_bonds; (void)gt; (void)NA;
   {
     SvdFinishBatch& fb = S.fb;
     int rc = 0;
-    PEPO_CUDA_OK(cudaStreamSynchronize(st));
+    PEPO_CUDA_OK(cudaStreamSynchronize(sh));
     if (!S.piped) prof_flush(c);
     int chi_cap = 1;
     for (int g = 0; g < ng; g++) {
@@ -1103,7 +1103,7 @@ int batch_p3(pepo_ctx* c, BatchState& S) {
       c->stats.gate_err += c->h_dbls[2 * (S.lane0 + g)];
       c->stats.min_cut_gap = std::min(c->stats.min_cut_gap, c->h_dbls[2 * (S.lane0 + g) + 1]);
     }
-    rc = launch_svd_bridge(st, fb, chi_cap); if (rc) return rc;
+    rc = launch_svd_bridge(sh, fb, chi_cap); if (rc) return rc;
   }
   // ---- E: bridge + reconstruction ------------------------------------------------------------------
   {
@@ -1126,7 +1126,7 @@ int batch_p3(pepo_ctx* c, BatchState& S) {
         gp.A = W.Rxinv; gp.lda = t.N; gp.B = UV; gp.ldb = t.r; gp.C = W.T; gp.ldc = t.N;
         gp.M = t.N; gp.N = t.chi_new; gp.K = t.N;
         { ProfScope ps(c, PC_SMALL_GEMM, 2.0 * t.N * t.N * t.chi_new, 0);
-          rc = launch_dgemm(st, 0, 0, gp, 1, 0, nullptr, false); if (rc) return rc; }
+          rc = launch_dgemm(sh, 0, 0, gp, 1, 0, nullptr, false); if (rc) return rc; }
         int q = bw.count++;
         bw.in[q] = W.T; bw.out[q] = W.W; bw.chi[q] = t.chi_c; bw.k[q] = t.chi_new; bw.site[q] = t.site_idx;
         bw.ld_in[q] = t.N; bw.ld_out[q] = t.n; cn_w[q] = L.ints;
@@ -1152,7 +1152,14 @@ int batch_p3(pepo_ctx* c, BatchState& S) {
       }
     }
     if (bw.count) {
-      { ProfScope ps(c, PC_DRESS, 0, 0); rc = launch_build_W(st, bw, gt, cn_w); if (rc) return rc; }
+      { ProfScope ps(c, PC_DRESS, 0, 0); rc = launch_build_W(sh, bw, gt, cn_w); if (rc) return rc; }
+    }
+    if (sh != st) {                                       // join: the heavy kernels run on the piece stream
+      PEPO_CUDA_OK(cudaEventRecord(S.ev[1], sh));
+      PEPO_CUDA_OK(cudaStreamWaitEvent(st, S.ev[1], 0));
+    }
+    c->cur_st = st;
+    if (bw.count) {
       for (auto& t : T) {
         if (!t.chol) continue;
         SiteWs& W = c->lanes[t.lane].s[t.slot];
@@ -1309,12 +1316,12 @@ int run_step_piped(pepo_ctx* c) {
         if (!ready) continue;
         for (int d : deps) PEPO_CUDA_OK(cudaStreamWaitEvent(u.S.st, c->done_ev[d], 0));
         rc = batch_p1(c, u.S);
-        if (!rc) { PEPO_CUDA_OK(cudaEventRecord(rb, u.S.st)); }
+        if (!rc) { PEPO_CUDA_OK(cudaEventRecord(rb, u.S.hp ? u.S.hp : u.S.st)); }
         u.phase = 1; progressed = true;
       } else if (cudaEventQuery(rb) == cudaSuccess) {
         if (u.phase == 1) {
           rc = batch_p2(c, u.S);
-          if (!rc) { PEPO_CUDA_OK(cudaEventRecord(rb, u.S.st)); }
+          if (!rc) { PEPO_CUDA_OK(cudaEventRecord(rb, u.S.hp ? u.S.hp : u.S.st)); }
           // the Jacobi kernel needs whole SMs: heavy kernels the other streams queue from now on
           // wait until its blocks are resident (launch-completion event)
           if (!rc && u.S.started)
