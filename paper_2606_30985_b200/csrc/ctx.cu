@@ -1093,6 +1093,7 @@ int batch_p3(pepo_ctx* c, BatchState& S) {
       T[2 * g].chi_new = T[2 * g + 1].chi_new = cn;
       chi_cap = std::max(chi_cap, cn);
       c->stats.jacobi_sweeps += c->h_ints[4 * (S.lane0 + g) + 1];
+      if (c->prof.trace) fprintf(stderr, "SWEEPS bond %d core %dx%d sweeps %d\n", gate_bonds[g], T[2 * g].r, T[2 * g + 1].r, c->h_ints[4 * (S.lane0 + g) + 1]);
       if (c->prof.on) {
         // algorithmic flops of the one-sided Jacobi iteration: per sweep Nc(Nc-1)/2 pairs, each
         // 3 inner products (6 L flop) + one plane rotation of two L-vectors (6 L flop)
@@ -1252,10 +1253,24 @@ int run_step_piped(pepo_ctx* c) {
     int np = (n + hb - 1) / hb;
     np = ((np + NS - 1) / NS) * NS;              // a multiple of the stream count: stream q % NS keeps its part of the grid
     np = std::min(np, n);
+    // piece_stride = 2: gates ordered by the size of their site tensors, pieces = contiguous runs of
+    // that order (pieces of like gates: a slow light gate never holds up a heavy one in its launch)
+    std::vector<int> ord(cls.begin(), cls.end());
+    if (c->piece_stride == 2) {
+      auto weight = [&](int e) {
+        double w = 0;
+        for (int v : {c->bonds[e].v1, c->bonds[e].v2}) w += (double)site_live_size(c, v);
+        return w;
+      };
+      std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) { return weight(a) > weight(b); });
+    }
     for (int q = 0; q < np; q++) {
       Piece pc;
       pc.stream = q % NS;
-      if (c->piece_stride) {
+      if (c->piece_stride == 2) {
+        const int a = (int)((long long)n * q / np), b = (int)((long long)n * (q + 1) / np);
+        pc.S.gate_bonds.assign(ord.begin() + a, ord.begin() + b);
+      } else if (c->piece_stride) {
         for (int g = q; g < n; g += np) pc.S.gate_bonds.push_back(cls[g]);
       } else {
         const int a = (int)((long long)n * q / np), b = (int)((long long)n * (q + 1) / np);
