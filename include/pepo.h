@@ -132,6 +132,16 @@ int pepo_set_bond_dims(pepo_ctx* ctx, const int* h_chi /* n_bonds */);
 size_t pepo_site_size(pepo_ctx* ctx, int x, int y);              /* elements at live dims */
 int pepo_get_site(pepo_ctx* ctx, int x, int y, double* h_dst, size_t n);
 int pepo_set_site(pepo_ctx* ctx, int x, int y, const double* h_src, size_t n);
+/* Asynchronous pepo_set_site: the host-to-device copy is queued on an internal copy stream and
+ * the call returns at once.  h_src (pinned memory, else the copy is staged synchronously by the
+ * driver) must stay valid and unchanged until pepo_trotter_step or a call returning a host value
+ * (bp_converge, correlation, getters) has returned.  The next pepo_trotter_step starts on the
+ * sites that have arrived while the others are still in flight: the field gate (a1) and the
+ * first bond gate of a site wait for that site's copy only.  Same errors as pepo_set_site. */
+int pepo_set_site_async(pepo_ctx* ctx, int x, int y, const double* h_src, size_t n);
+/* Order (site index = y * Lx + x, n >= Lx * Ly ints) in which the next pepo_trotter_step first
+ * touches the sites; uploading in this order lets the step start earliest.  -1 on a bad argument. */
+int pepo_site_order(pepo_ctx* ctx, int* h_order, int n);
 int pepo_get_lambda(pepo_ctx* ctx, int bond, double* h_dst, int n);
 int pepo_set_lambda(pepo_ctx* ctx, int bond, const double* h_src, int n);
 /* Diagnostics of PAPER.md Table 1 (L373-L380): bond entanglement entropies

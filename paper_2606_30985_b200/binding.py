@@ -62,6 +62,8 @@ def _load():
         "pepo_site_size": (sz, [vp, i, i]),
         "pepo_get_site": (i, [vp, i, i, vp, sz]),
         "pepo_set_site": (i, [vp, i, i, vp, sz]),
+        "pepo_set_site_async": (i, [vp, i, i, vp, sz]),
+        "pepo_site_order": (i, [vp, vp, i]),
         "pepo_get_lambda": (i, [vp, i, vp, i]),
         "pepo_bond_entropy": (i, [vp, vp, i]),
         "pepo_set_lambda": (i, [vp, i, vp, i]),
@@ -206,6 +208,20 @@ class Pepo:
     def set_site(self, x, y, flat):
         flat = np.ascontiguousarray(flat, dtype=np.float64).ravel()
         _check(_lib.pepo_set_site(self._h, x, y, flat.ctypes.data_as(C.c_void_p), flat.size))
+
+    def set_site_async(self, x, y, flat):
+        """flat: contiguous float64 array (pinned for a truly asynchronous copy) that the caller
+        keeps alive and unchanged until trotter_step / bp_converge / correlation has returned."""
+        if flat.dtype != np.float64 or not flat.flags["C_CONTIGUOUS"]:
+            raise ValueError("set_site_async needs a contiguous float64 array")
+        _check(_lib.pepo_set_site_async(self._h, x, y, flat.ctypes.data_as(C.c_void_p), flat.size))
+
+    def site_order(self):
+        """(x, y) of the sites in the order the next trotter_step first touches them."""
+        n = self.Lx * self.Ly
+        out = np.empty(n, dtype=np.int32)
+        _check(_lib.pepo_site_order(self._h, out.ctypes.data_as(C.c_void_p), n))
+        return [(int(v) % self.Lx, int(v) // self.Lx) for v in out]
 
     def bond_entropy(self):
         out = np.empty(self.n_bonds, dtype=np.float64)

@@ -250,6 +250,15 @@ struct pepo_ctx {
   int NA;
   double G1[16], G1h[16];              // field PTM at h dt and at h dt / 2 (symmetric step, eq. (6))
   int f_row_mask, f_col_mask;
+  // asynchronous site uploads (pepo_set_site_async): copies on copy_st, one event per site; the
+  // first kernels that touch a site wait for its event (field gate of the piece that owns it)
+  cudaStream_t copy_st = nullptr;
+  cudaEvent_t copy_ev = nullptr;
+  bool lazy_field = false, lazy_half = false;   // this step applies the field gate piece by piece
+  std::vector<cudaEvent_t> site_ev;
+  std::vector<char> site_pending, field_todo;
+  bool copy_forked = false;            // copy_st already ordered after the compute queued so far
+  int n_pending = 0;
   int trotter_order = 1;               // option "trotter_order": 1 = R2 (BASELINE), 2 = symmetric step of eq. (6)
   std::vector<LaneWs> lanes;
   int* lane_ints; double* lane_dbls;      // device readback blocks (B*4 ints, B*2 doubles)
@@ -303,6 +312,10 @@ struct ProfScope {
   }
 };
 }  // namespace
+
+namespace {
+int wait_pending_uploads(pepo_ctx* c, cudaStream_t st);
+}
 
 namespace {
 
@@ -604,6 +617,15 @@ extern "C" int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, doub
     for (int i = 0; i < 5 * pepo_ctx::NSMAX + 1 && ok; i++) ok = cudaEventCreateWithFlags(&c->pev[i], cudaEventDisableTiming) == cudaSuccess;
     if (!ok) { set_error("init: stream / event creation failed"); delete c; return -3; }
   }
+  {
+    bool ok = cudaStreamCreateWithFlags(&c->copy_st, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaEventCreateWithFlags(&c->copy_ev, cudaEventDisableTiming) == cudaSuccess;
+    c->site_ev.assign(c->n_sites, nullptr);
+    for (int v = 0; v < c->n_sites && ok; v++) ok = cudaEventCreateWithFlags(&c->site_ev[v], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) { set_error("init: stream / event creation failed"); delete c; return -3; }
+    c->site_pending.assign(c->n_sites, 0);
+    c->field_todo.assign(c->n_sites, 0);
+  }
   c->cur_st = c->st;
   int rc = 0;
   double one = 1.0;
@@ -639,6 +661,9 @@ extern "C" int pepo_destroy(pepo_ctx* c) {
   }
   for (int i = 0; i < 5 * pepo_ctx::NSMAX + 1; i++) if (c->pev[i]) cudaEventDestroy(c->pev[i]);
   for (auto e : c->done_ev) cudaEventDestroy(e);
+  if (c->copy_st) { cudaStreamSynchronize(c->copy_st); cudaStreamDestroy(c->copy_st); }
+  for (auto e : c->site_ev) if (e) cudaEventDestroy(e);
+  if (c->copy_ev) cudaEventDestroy(c->copy_ev);
   cudaFreeHost(c->h_ints); cudaFreeHost(c->h_dbls); cudaFreeHost(c->h_chi_msg);
   cudaFreeHost(c->h_scal); cudaFreeHost(c->h_delta); cudaFreeHost(c->h_bpints);
   delete c;
@@ -705,6 +730,7 @@ extern "C" int pepo_get_bond_dims(pepo_ctx* c, int* h_chi) {
 }
 extern "C" int pepo_set_bond_dims(pepo_ctx* c, const int* h_chi) {
   if (!c || !h_chi) { set_error("set_bond_dims: NULL"); return -1; }
+  { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
   for (int e = 0; e < c->n_bonds; e++)
     if (h_chi[e] < 1 || h_chi[e] > c->chi_max) { set_error("set_bond_dims: chi[%d]=%d out of range", e, h_chi[e]); return -1; }
   for (int e = 0; e < c->n_bonds; e++) c->chi[e] = h_chi[e];
@@ -721,14 +747,53 @@ extern "C" double* pepo_site_ptr(pepo_ctx* c, int x, int y) {
 }
 extern "C" int pepo_get_site(pepo_ctx* c, int x, int y, double* h_dst, size_t n) {
   if (!c || !h_dst || x < 0 || x >= c->Lx || y < 0 || y >= c->Ly) { set_error("get_site: bad argument"); return -1; }
+  { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
   int v = y * c->Lx + x;
   if (n != site_live_size(c, v)) { set_error("get_site: size %zu != live size %zu", n, site_live_size(c, v)); return -1; }
   PEPO_CUDA_OK(cudaMemcpyAsync(h_dst, c->sites[v].psi, n * 8, cudaMemcpyDeviceToHost, c->st));
   PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
   return 0;
 }
+namespace {
+// every pending asynchronous site upload becomes visible to `st` (and stops being pending)
+int wait_pending_uploads(pepo_ctx* c, cudaStream_t st) {
+  if (c->n_pending == 0) { c->copy_forked = false; return 0; }
+  for (int v = 0; v < c->n_sites; v++) {
+    if (!c->site_pending[v]) continue;
+    PEPO_CUDA_OK(cudaStreamWaitEvent(st, c->site_ev[v], 0));
+    c->site_pending[v] = 0;
+  }
+  c->n_pending = 0;
+  c->copy_forked = false;
+  return 0;
+}
+}  // namespace
+
+// Asynchronous pepo_set_site: the copy is queued on an internal copy stream and the call returns;
+// h_src (pinned memory for a truly asynchronous copy) must stay valid and unchanged until the next
+// call that returns a host value (bp_converge, correlation, getters) or pepo_trotter_step has
+// returned.  The next pepo_trotter_step starts on the sites already uploaded while the others are
+// still in flight (the field gate and the first bond gate of a site wait for that site only).
+extern "C" int pepo_set_site_async(pepo_ctx* c, int x, int y, const double* h_src, size_t n) {
+  if (!c || !h_src || x < 0 || x >= c->Lx || y < 0 || y >= c->Ly) { set_error("set_site_async: bad argument"); return -1; }
+  const int v = y * c->Lx + x;
+  if (n != site_live_size(c, v)) { set_error("set_site_async: size %zu != live size %zu", n, site_live_size(c, v)); return -1; }
+  if (!c->copy_forked) {
+    // the slot may still be read by kernels queued on the context stream (BP of the previous step)
+    PEPO_CUDA_OK(cudaEventRecord(c->copy_ev, c->st));
+    PEPO_CUDA_OK(cudaStreamWaitEvent(c->copy_st, c->copy_ev, 0));
+    c->copy_forked = true;
+  }
+  PEPO_CUDA_OK(cudaMemcpyAsync(c->sites[v].psi, h_src, n * 8, cudaMemcpyHostToDevice, c->copy_st));
+  PEPO_CUDA_OK(cudaEventRecord(c->site_ev[v], c->copy_st));
+  if (!c->site_pending[v]) { c->site_pending[v] = 1; c->n_pending++; }
+  c->msgs_valid = false;
+  return 0;
+}
+
 extern "C" int pepo_set_site(pepo_ctx* c, int x, int y, const double* h_src, size_t n) {
   if (!c || !h_src || x < 0 || x >= c->Lx || y < 0 || y >= c->Ly) { set_error("set_site: bad argument"); return -1; }
+  { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
   int v = y * c->Lx + x;
   if (n != site_live_size(c, v)) { set_error("set_site: size %zu != live size %zu", n, site_live_size(c, v)); return -1; }
   c->msgs_valid = false;
@@ -778,6 +843,7 @@ extern "C" int pepo_apply_field(pepo_ctx* c) {
 }
 namespace {
 int apply_field_impl(pepo_ctx* c, bool half) {
+  { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
   if (c->f_row_mask == 0) return 0;
   for (int v0 = 0; v0 < c->n_sites; v0 += PEPO_BP_MAXS) {
     FieldBatch fb;
@@ -1243,6 +1309,42 @@ struct Piece {
   std::vector<int> sites;
 };
 
+// field gate (a1) of the sites of `sites` that have not had it in this step, on `st`, each after its
+// own pending upload
+int lazy_field_gate(pepo_ctx* c, const std::vector<int>& sites, cudaStream_t st) {
+  FieldBatch fb; fb.count = 0;
+  double fbytes = 0;
+  for (int v : sites) {
+    if (!c->field_todo[v]) continue;
+    c->field_todo[v] = 0;
+    if (c->site_pending[v]) {
+      PEPO_CUDA_OK(cudaStreamWaitEvent(st, c->site_ev[v], 0));
+      c->site_pending[v] = 0; c->n_pending--;
+    }
+    if (c->f_row_mask == 0) continue;
+    fb.psi[fb.count] = c->sites[v].psi;
+    fb.slab[fb.count] = (long long)(site_live_size(c, v) / 4);
+    fbytes += 8.0 * fb.slab[fb.count] * 2 * __builtin_popcount(c->f_row_mask);
+    if (++fb.count == PEPO_BP_MAXS) {
+      memcpy(fb.G, c->lazy_half ? c->G1h : c->G1, sizeof(fb.G));
+      fb.row_mask = c->f_row_mask; fb.col_mask = c->f_col_mask;
+      int rc = launch_field_gate(st, fb); if (rc) return rc;
+      fb.count = 0;
+    }
+  }
+  if (fb.count) {
+    memcpy(fb.G, c->lazy_half ? c->G1h : c->G1, sizeof(fb.G));
+    fb.row_mask = c->f_row_mask; fb.col_mask = c->f_col_mask;
+    cudaStream_t keep = c->cur_st; c->cur_st = st;
+    ProfScope ps(c, PC_FIELD, 0, fbytes);
+    int rc = launch_field_gate(st, fb);
+    c->cur_st = keep;
+    if (rc) return rc;
+  }
+  if (c->n_pending == 0) c->copy_forked = false;
+  return 0;
+}
+
 int run_step_piped(pepo_ctx* c) {
   const int NS = std::min(std::min(c->pipeline, pepo_ctx::NSMAX), c->B);
   const int hb = c->B / NS;                      // lanes per stream
@@ -1330,6 +1432,7 @@ int run_step_piped(pepo_ctx* c) {
         for (int v : u.sites) mark[v] = 0;
         if (!ready) continue;
         for (int d : deps) PEPO_CUDA_OK(cudaStreamWaitEvent(u.S.st, c->done_ev[d], 0));
+        if (c->lazy_field) { rc = lazy_field_gate(c, u.sites, u.S.st); if (rc) break; }
         rc = batch_p1(c, u.S);
         if (!rc) { PEPO_CUDA_OK(cudaEventRecord(rb, u.S.hp ? u.S.hp : u.S.st)); }
         u.phase = 1; progressed = true;
@@ -1352,6 +1455,13 @@ int run_step_piped(pepo_ctx* c) {
     }
     if (!progressed) std::this_thread::yield();
   }
+  if (c->lazy_field && !rc) {                 // sites no gate touched (none on connected grids)
+    std::vector<int> all(c->n_sites);
+    for (int v = 0; v < c->n_sites; v++) all[v] = v;
+    // ordered after the piece streams by the join below: do it on the first piece stream
+    rc = lazy_field_gate(c, all, c->ps[0]);
+    c->lazy_field = false;
+  }
   // join: the caller's stream continues after all piece streams
   for (int s = 0; s < NS; s++) {
     cudaEventRecord(c->pev[3 * pepo_ctx::NSMAX + 1 + s], c->ps[s]);
@@ -1368,8 +1478,34 @@ int run_step_piped(pepo_ctx* c) {
 
 }  // namespace
 
+// Order in which a Trotter step first touches the sites (piece by piece of the pipelined schedule,
+// class by class): uploading the site tensors in this order (pepo_set_site_async) lets the step
+// start earliest.  h_order: n_sites ints (site index = y * Lx + x).
+extern "C" int pepo_site_order(pepo_ctx* c, int* h_order, int n) {
+  if (!c || !h_order || n < c->n_sites) { set_error("site_order: bad argument"); return -1; }
+  std::vector<char> seen(c->n_sites, 0);
+  int k = 0;
+  const int NS = std::max(1, std::min(std::min(c->pipeline, pepo_ctx::NSMAX), c->B));
+  const int hb = std::max(1, c->B / NS);
+  for (auto& cls : c->classes) {
+    const int nc = (int)cls.size();
+    if (nc == 0) continue;
+    int np = (nc + hb - 1) / hb;
+    np = ((np + NS - 1) / NS) * NS;
+    np = std::min(np, nc);
+    for (int q = 0; q < np; q++)
+      for (int g = (c->piece_stride == 1 ? q : (int)((long long)nc * q / np));
+           g < (c->piece_stride == 1 ? nc : (int)((long long)nc * (q + 1) / np)); g += (c->piece_stride == 1 ? np : 1))
+        for (int v : {c->bonds[cls[g]].v1, c->bonds[cls[g]].v2})
+          if (!seen[v]) { seen[v] = 1; h_order[k++] = v; }
+  }
+  for (int v = 0; v < c->n_sites; v++) if (!seen[v]) h_order[k++] = v;
+  return 0;
+}
+
 extern "C" int pepo_apply_bond(pepo_ctx* c, int bond) {
   if (!c || bond < 0 || bond >= c->n_bonds) { set_error("apply_bond: bad bond"); return -1; }
+  { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
   std::vector<int> g(1, bond);
   return run_batch(c, g);
 }
@@ -1380,9 +1516,15 @@ extern "C" int pepo_trotter_step(pepo_ctx* c) {
   // order 1 (R2): field gate, bond sweep.  order 2 (PAPER eq. (6)):
   // half field gate, bond sweep, half field gate.
   const bool sym = c->trotter_order == 2;
-  int rc = apply_field_impl(c, sym);
+  const bool piped = c->pipeline >= 2 && c->B >= 2;
+  int rc = 0;
+  // asynchronous uploads in flight: the field gate is applied piece by piece, each piece waiting
+  // only for its own sites, so the step starts while the rest of the state is still arriving
+  c->lazy_field = piped && c->n_pending > 0;
+  if (c->lazy_field) { c->lazy_half = sym; std::fill(c->field_todo.begin(), c->field_todo.end(), 1); }
+  else rc = apply_field_impl(c, sym);
   if (rc) return rc;
-  if (c->pipeline >= 2 && c->B >= 2) rc = run_step_piped(c);
+  if (piped) rc = run_step_piped(c);
   else {
     for (auto& cls : c->classes) {
       for (size_t i0 = 0; i0 < cls.size() && !rc; i0 += c->B) {
@@ -1477,6 +1619,7 @@ int bp_init_messages(pepo_ctx* c) {
 
 extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
   if (!c) { set_error("bp_converge: NULL"); return -1; }
+  { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
   int sweeps = 0;
   double delta = INFINITY;
   int status = 1;
@@ -1520,6 +1663,7 @@ extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
 
 extern "C" int pepo_correlation(pepo_ctx* c, double* h_C) {
   if (!c || !h_C) { set_error("correlation: NULL"); return -1; }
+  { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
   if (!c->msgs_valid) { set_error("correlation: no converged messages (call pepo_bp_converge after the last state change)"); return -1; }
   int rc = bp_sweep(c, 0.0, 0); if (rc) return rc;
   rc = launch_bethe(c->st, c->vs, c->n_sites, c->msgs[c->cur_msg], c->chi_of_msg, c->n_bonds, c->chi_max,

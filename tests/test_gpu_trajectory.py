@@ -268,3 +268,44 @@ def test_pipelined_schedule_on_irregular_lattices(gpu, shape):
         assert (res[name][2] == res["serial"][2]).all(), name
     assert res["noearly"][1] == res["serial"][1]
     assert max(abs(a - b) for a, b in zip(res["noearly"][0], res["serial"][0])) < 1e-12
+
+
+def test_async_site_upload_equals_synchronous(gpu):
+    """pepo_set_site_async + the piece-by-piece field gate (the step starts on the sites that have
+    arrived) must give bit for bit what pepo_set_site gives, on both schedules and both Trotter
+    orders; pepo_site_order lists every site once."""
+    torch, B = gpu
+    L, chi = 4, 12
+    sim = B.Pepo(L, L, 1, 1, J, H, DT, chi, 1e-10, 0.5)
+    while min(sim.bond_dims()) < chi:
+        sim.trotter_step()
+    order = sim.site_order()
+    assert sorted(order) == sorted((x, y) for y in range(L) for x in range(L))
+    host = {}
+    for (x, y) in order:
+        a = sim.get_site(x, y)
+        p = torch.empty(a.size, dtype=torch.float64).pin_memory()
+        p.numpy()[:] = a
+        host[(x, y)] = p
+    lam = [sim.get_lambda(e) for e in range(sim.n_bonds)]
+    chis = sim.bond_dims()
+
+    def step(use_async):
+        sim.set_bond_dims(chis)
+        for e, l in enumerate(lam):
+            sim.set_lambda(e, l)
+        for (x, y) in order:
+            (sim.set_site_async if use_async else sim.set_site)(x, y, host[(x, y)].numpy())
+        sim.trotter_step()
+        sim.bp_converge()
+        return sim.correlation(), sim.get_site(1, 1).copy(), sim.get_site(3, 0).copy(), list(sim.bond_dims())
+
+    for opts in ({"pipeline": 4, "trotter_order": 1}, {"pipeline": 4, "trotter_order": 2},
+                 {"pipeline": 0, "trotter_order": 1}):
+        for k, v in opts.items():
+            sim.set_option(k, v)
+        a, b, c2 = step(False), step(True), step(True)
+        for r in (b, c2):
+            assert a[0] == r[0] and a[3] == r[3], opts
+            assert (a[1] == r[1]).all() and (a[2] == r[2]).all(), opts
+    sim.close()
