@@ -22,6 +22,7 @@
 #include "dense.cuh"
 
 #include <algorithm>
+#include <chrono>
 #include <cmath>
 #include <complex>
 #include <cstdarg>
@@ -1409,6 +1410,7 @@ int run_step_piped(pepo_ctx* c) {
   std::vector<char> mark(c->n_sites, 0);
   size_t pos[pepo_ctx::NSMAX] = {0};
   int rc = 0, left = np;
+  double t_enq = 0.0; const auto t_all0 = std::chrono::steady_clock::now();
   while (!rc && left > 0) {
     bool progressed = false;
     for (int s = 0; s < NS && !rc; s++) {
@@ -1432,11 +1434,14 @@ int run_step_piped(pepo_ctx* c) {
         for (int v : u.sites) mark[v] = 0;
         if (!ready) continue;
         for (int d : deps) PEPO_CUDA_OK(cudaStreamWaitEvent(u.S.st, c->done_ev[d], 0));
+        const auto tq0 = std::chrono::steady_clock::now();
         if (c->lazy_field) { rc = lazy_field_gate(c, u.sites, u.S.st); if (rc) break; }
         rc = batch_p1(c, u.S);
+        t_enq += std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - tq0).count();
         if (!rc) { PEPO_CUDA_OK(cudaEventRecord(rb, u.S.hp ? u.S.hp : u.S.st)); }
         u.phase = 1; progressed = true;
       } else if (cudaEventQuery(rb) == cudaSuccess) {
+        const auto tq0 = std::chrono::steady_clock::now();
         if (u.phase == 1) {
           rc = batch_p2(c, u.S);
           if (!rc) { PEPO_CUDA_OK(cudaEventRecord(rb, u.S.hp ? u.S.hp : u.S.st)); }
@@ -1450,6 +1455,7 @@ int run_step_piped(pepo_ctx* c) {
           if (!rc) { PEPO_CUDA_OK(cudaEventRecord(c->done_ev[i], u.S.st)); }
           u.phase = 3; pos[s]++; left--;
         }
+        t_enq += std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - tq0).count();
         progressed = true;
       }
     }
@@ -1462,6 +1468,9 @@ int run_step_piped(pepo_ctx* c) {
     rc = lazy_field_gate(c, all, c->ps[0]);
     c->lazy_field = false;
   }
+  if (c->prof.trace)
+    fprintf(stderr, "HOST step %.3f ms, of which enqueueing phases %.3f ms\n",
+            std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_all0).count(), t_enq);
   // join: the caller's stream continues after all piece streams
   for (int s = 0; s < NS; s++) {
     cudaEventRecord(c->pev[3 * pepo_ctx::NSMAX + 1 + s], c->ps[s]);
