@@ -54,6 +54,9 @@ typedef struct pepo_stats {
   int chi_max_live;         /* largest live bond dimension */
   int last_bp_trap;         /* trap flag of the diagnostics: the last bp_converge
                                converged (delta < tol) but needed >= 30 sweeps */
+  int last_bp_flags;        /* bit 0: some message update of the last bp_converge had zero norm and kept its
+                               old value (R7); bit 1: some update had a non-finite norm (bp_converge then
+                               returns -4) */
 } pepo_stats;
 
 const char* pepo_last_error(void);
@@ -109,7 +112,9 @@ int pepo_apply_bond(pepo_ctx* ctx, int bond);
 /* BP on the pinned single-layer network (eq. (13),(14),(19) PAPER.md:L243-L256, L444-L449; R6,
  * R7): Jacobi-schedule sweeps from the deterministic init until delta < tol or the budget
  * is spent; undamped phase first, damped restart if configured.  Writes the total sweep
- * count and the last delta.  Returns 0 converged, 1 budget exhausted. */
+ * count and the last delta.  Returns 0 converged, 1 budget exhausted (messages still usable),
+ * -4 if a message update produced a non-finite norm.  A zero-norm update keeps the old message
+ * and sets bit 0 of pepo_stats.last_bp_flags (R7). */
 int pepo_bp_converge(pepo_ctx* ctx, int* h_sweeps, double* h_delta);
 /* Bethe evaluation (eq. (7)-(9) PAPER.md:L112-L128) from the current messages, log-space with
  * sign tracking.  -4 if some Z_e is 0 (R14). */
@@ -143,6 +148,10 @@ int pepo_set_site_async(pepo_ctx* ctx, int x, int y, const double* h_src, size_t
  * touches the sites; uploading in this order lets the step start earliest.  -1 on a bad argument. */
 int pepo_site_order(pepo_ctx* ctx, int* h_order, int n);
 int pepo_get_lambda(pepo_ctx* ctx, int bond, double* h_dst, int n);
+/* Current BP message over `bond` (eq. (13)): from_v1 != 0 gives the message
+ * sent by the bond's smaller-coordinate site v1 to v2, else v2 -> v1; n = live dimension of the
+ * bond.  Valid after pepo_bp_converge (else -1).  For parity tests against the oracle. */
+int pepo_get_message(pepo_ctx* ctx, int bond, int from_v1, double* h_dst, int n);
 int pepo_set_lambda(pepo_ctx* ctx, int bond, const double* h_src, int n);
 /* Diagnostics of PAPER.md Table 1 (L373-L380): bond entanglement entropies
  * S_e = -sum_k lambda_k^2 log lambda_k^2 over the live Schmidt weights of every bond (lambda is

@@ -30,7 +30,8 @@ class PepoStats(C.Structure):
                 ("kernel_launches", C.c_longlong), ("last_bp_sweeps", C.c_int),
                 ("last_bp_status", C.c_int), ("last_bp_delta", C.c_double),
                 ("arena_high_water", C.c_size_t), ("arena_model_bytes", C.c_size_t),
-                ("max_inflight_gates", C.c_int), ("chi_max_live", C.c_int), ("last_bp_trap", C.c_int)]
+                ("max_inflight_gates", C.c_int), ("chi_max_live", C.c_int), ("last_bp_trap", C.c_int),
+                ("last_bp_flags", C.c_int)]
 
 
 def _load():
@@ -66,6 +67,7 @@ def _load():
         "pepo_site_order": (i, [vp, vp, i]),
         "pepo_get_lambda": (i, [vp, i, vp, i]),
         "pepo_bond_entropy": (i, [vp, vp, i]),
+        "pepo_get_message": (i, [vp, i, i, vp, i]),
         "pepo_set_lambda": (i, [vp, i, vp, i]),
         "pepo_site_ptr": (vp, [vp, i, i]),
         "pepo_permute": (i, [dp, dp, ip, ip, i, vp]),
@@ -232,6 +234,12 @@ class Pepo:
         n = self.bond_dims()[bond]
         out = np.empty(n, dtype=np.float64)
         _check(_lib.pepo_get_lambda(self._h, bond, out.ctypes.data_as(C.c_void_p), n))
+        return out
+
+    def get_message(self, bond, from_v1=True):
+        n = self.bond_dims()[bond]
+        out = np.empty(n, dtype=np.float64)
+        _check(_lib.pepo_get_message(self._h, bond, 1 if from_v1 else 0, out.ctypes.data_as(C.c_void_p), n))
         return out
 
     def set_lambda(self, bond, lam):

@@ -276,8 +276,14 @@ __global__ void __launch_bounds__(256) bp_finalize_kernel(BpBatch b, double damp
   const double nrm = sqrt(red[0]);
   double* outn = S.out_new[slot];
   if (!(nrm > 0.0) || !isfinite(nrm)) {
+    // R7: a zero-norm update keeps the old message and is flagged (bit 0); a non-finite norm (bit 1)
+    // also poisons delta with +inf so that the sweep can never count as converged
     for (int i = threadIdx.x; i < dl; i += blockDim.x) outn[i] = old[i];
-    if (threadIdx.x == 0) atomicOr(flag, 1);
+    if (threadIdx.x == 0) {
+      const bool bad = !isfinite(nrm);
+      atomicOr(flag, bad ? 2 : 1);
+      if (bad) atomicMax(delta_bits, 0x7ff0000000000000ull);
+    }
     return;
   }
   const double sgn = (red[1] < 0.0) ? -1.0 : 1.0;
@@ -287,11 +293,13 @@ __global__ void __launch_bounds__(256) bp_finalize_kernel(BpBatch b, double damp
     double o = old[i];
     double mn = damping * o + (1.0 - damping) * mh;
     outn[i] = mn;
-    dmax = fmax(dmax, fabs(mn - o));
+    const double ch = fabs(mn - o);
+    dmax = (ch == ch) ? fmax(dmax, ch) : INFINITY;        // fmax would drop a NaN change
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) dmax = fmax(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
   if (lane == 0) atomicMax(delta_bits, (unsigned long long)__double_as_longlong(dmax));
+  (void)0;
   (void)s_bcast;
 }
 

@@ -1632,6 +1632,7 @@ extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
   int sweeps = 0;
   double delta = INFINITY;
   int status = 1;
+  int flags = 0;                 // bit 0: a message with zero norm kept its old value (R7); bit 1: non-finite norm
   for (int phase = 0; phase < 2 && status; phase++) {
     const double damping = phase == 0 ? 0.0 : c->bp_damping;
     const int budget = phase == 0 ? c->bp_max_sweeps : c->bp_max_sweeps_damped;
@@ -1647,8 +1648,10 @@ extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
         rc = bp_sweep(c, damping, 1, c->cur_msg ^ (g & 1), g, g - 1); if (rc) return rc;
       }
       PEPO_CUDA_OK(cudaMemcpyAsync(c->h_delta, c->delta_bits, 8 * ngr, cudaMemcpyDeviceToHost, c->st));
+      PEPO_CUDA_OK(cudaMemcpyAsync(c->h_bpints, c->bp_ints, 8, cudaMemcpyDeviceToHost, c->st));
       PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
       prof_flush(c);
+      flags |= c->h_bpints[0];
       int done = ngr;                                   // sweeps of the group that actually ran
       for (int g = 0; g < ngr; g++) {
         double dg;
@@ -1665,8 +1668,10 @@ extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
   c->msgs_valid = true;
   c->stats.last_bp_sweeps = sweeps; c->stats.last_bp_status = status; c->stats.last_bp_delta = delta;
   c->stats.last_bp_trap = (status == 0 && sweeps >= 30) ? 1 : 0;      // trap flag of PAPER.md L451-L457
+  c->stats.last_bp_flags = flags;
   if (h_sweeps) *h_sweeps = sweeps;
   if (h_delta) *h_delta = delta;
+  if (flags & 2) { set_error("bp_converge: a message update had a non-finite norm (NaN / Inf in the site tensors or messages)"); return -4; }
   return status;
 }
 
@@ -1683,6 +1688,16 @@ extern "C" int pepo_correlation(pepo_ctx* c, double* h_C) {
   PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
   *h_C = c->h_scal[0];
   if (c->h_bpints[1] != 0) { set_error("correlation: zero or non-finite Z_e / vs_v"); return -4; }
+  return 0;
+}
+
+// Current BP message over `bond` (from_v1 != 0: v1 -> v2, else v2 -> v1), for parity tests.
+extern "C" int pepo_get_message(pepo_ctx* c, int bond, int from_v1, double* h_dst, int n) {
+  if (!c || !h_dst || bond < 0 || bond >= c->n_bonds || n != c->chi[bond]) { set_error("get_message: bad argument"); return -1; }
+  if (!c->msgs_valid) { set_error("get_message: no messages (call pepo_bp_converge after the last state change)"); return -1; }
+  const size_t idx = (size_t)(2 * bond + (from_v1 ? 0 : 1));
+  PEPO_CUDA_OK(cudaMemcpyAsync(h_dst, c->msgs[c->cur_msg] + idx * c->chi_max, (size_t)n * 8, cudaMemcpyDeviceToHost, c->st));
+  PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
   return 0;
 }
 

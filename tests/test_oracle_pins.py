@@ -358,3 +358,152 @@ def test_bond_weights_and_entropy_equal_dense_operator_schmidt_on_a_chain():
         assert abs(st.bond_entropy(e) - float(-(w * np.log(w)).sum())) < 1e-9
     st.lam[0] = np.full(8, 1 / math.sqrt(8))
     assert abs(st.bond_entropy(0) - math.log(8)) < 1e-14
+
+
+# ---------------------------------------------------------------- damped BP (eq. (19), R7) ---
+def _state_4x4_chi8(steps):
+    st = po.PEPOState(4, 4, 1, 1, J, H, DT, 8)
+    for _ in range(steps):
+        st.trotter_step()
+    return st
+
+
+def test_damped_sweep_is_eq19_without_renormalisation():
+    """eq. (19) PAPER L444-L449 with d = 1 - alpha (R7): one damped sweep from the init m0 = 1/sqrt(chi)
+    equals d*m0 + (1-d)*mhat, where mhat is what ONE UNDAMPED sweep from the same init gives (normalised,
+    sign-aligned); no renormalisation afterwards.  d = 0.3 tells d from 1-d; the norm of the result is
+    d^2 + (1-d)^2 + 2d(1-d)<m0,mhat> < 1 whenever mhat != m0."""
+    st = _state_4x4_chi8(12)
+    d = 0.3
+    st.bp_converge(1e-30, 0.0, max_sweeps=1)
+    mhat = {k: v.copy() for k, v in st.msgs.items()}
+    status, sweeps, _ = st.bp_converge(1e-30, d, max_sweeps=0, max_sweeps_damped=1)
+    assert (status, sweeps) == (1, 1)
+    some_shorter = False
+    for k, m1 in st.msgs.items():
+        chi = m1.size
+        m0 = np.full(chi, 1.0 / math.sqrt(chi))
+        assert abs(np.linalg.norm(mhat[k]) - 1.0) < 1e-14 and float(mhat[k] @ m0) >= 0.0
+        assert np.allclose(m1, d * m0 + (1 - d) * mhat[k], rtol=0, atol=1e-15)
+        some_shorter |= np.linalg.norm(m1) < 1.0 - 1e-6
+    assert some_shorter
+
+
+@pytest.mark.parametrize("grid,steps", [((3, 3, 1, 1), 8), ((4, 4, 1, 1), 30)])
+def test_damped_restart_lands_on_the_undamped_fixed_point(grid, steps):
+    """phase 2 (restart from the init with damping) converges to the same fixed
+    point as the undamped iteration, so the Bethe value agrees to rounding; forced here by a phase-1
+    budget of one sweep."""
+    st = po.PEPOState(*grid, J, H, DT, 8)
+    for _ in range(steps):
+        st.trotter_step()
+    s0, n0, _ = st.bp_converge(1e-13, 0.0)
+    c0 = st.correlation()
+    m0 = {k: v.copy() for k, v in st.msgs.items()}
+    s1, n1, d1 = st.bp_converge(1e-13, 0.5, max_sweeps=1)
+    c1 = st.correlation()
+    assert s0 == 0 and s1 == 0 and d1 < 1e-13
+    assert n1 > n0 + 1                       # 1 undamped sweep + a slower damped run
+    assert abs(c1 - c0) <= 1e-14 * max(1.0, abs(c0)) + 1e-15
+    for k in m0:
+        # same ray and the same norm 1 (the fixed point of the un-renormalised damped iteration); the
+        # overall sign of a message is a free choice of the iteration history (C does not depend on it)
+        a, b = st.msgs[k], m0[k]
+        assert min(np.abs(a - b).max(), np.abs(a + b).max()) < 1e-10
+
+
+def test_damped_contraction_rate_obeys_eq19():
+    """Linearised eq. (19): the damped iteration matrix is d*I + (1-d)*Jac, so with rho the late-time
+    undamped ratio delta_{k+1}/delta_k the damped ratio lies in [d - (1-d) rho, d + (1-d) rho].  With
+    d = 0.75 and rho <= 0.4 that is [0.65, 0.85]; swapping d and 1-d would give <= 0.55."""
+    st = _state_4x4_chi8(30)
+    rates = {}
+    for d in (0.0, 0.75):
+        msgs, dl = st._init_messages(), []
+        for _ in range(400):
+            msgs, de, _ = st._bp_sweep(msgs, d)
+            dl.append(de)
+            if de < 1e-12:
+                break
+        r = [dl[i + 1] / dl[i] for i in range(len(dl) - 1)]
+        rates[d] = r[-8:]
+    rho = max(rates[0.0])
+    assert rho < 0.4
+    for r in rates[0.75]:
+        assert 0.75 - 0.25 * rho - 0.01 <= r <= 0.75 + 0.25 * rho + 0.01, (r, rho)
+
+
+def test_exhausted_budget_and_restart_from_the_init():
+    """when both budgets are spent bp_converge returns status 1 with the sweep count
+    = both budgets and delta >= tol; the messages stay usable (finite C).  The damped phase restarts
+    from the init (L456 'retry'): its result does not depend on how long phase 1 ran."""
+    st = _state_4x4_chi8(40)
+    s, n, de = st.bp_converge(1e-10, 0.5, max_sweeps=3, max_sweeps_damped=4)
+    assert (s, n) == (1, 7) and de >= 1e-10
+    ma = {k: v.copy() for k, v in st.msgs.items()}
+    ca = st.correlation()
+    assert math.isfinite(ca)
+    s, n, de2 = st.bp_converge(1e-10, 0.5, max_sweeps=6, max_sweeps_damped=4)
+    assert (s, n) == (1, 10) and de2 == de
+    for k in ma:
+        assert np.array_equal(ma[k], st.msgs[k])
+    # no damping configured: only phase 1 runs
+    s, n, _ = st.bp_converge(1e-10, 0.0, max_sweeps=3, max_sweeps_damped=4)
+    assert (s, n) == (1, 3)
+    # golden trajectory (tests/golden/oracle_4x4_chi8.txt): step 49 needs the damped restart, 100 + 60 sweeps
+    for _ in range(9):
+        st.trotter_step()
+    s, n, _ = st.bp_converge(1e-10, 0.5)
+    assert s == 0 and n > 100
+
+
+def test_lambda_is_normalised_over_the_kept_values_when_truncating():
+    """eq. (11)-(12), R8, on a gate that DOES truncate: chi_new = chi_max and lambda = s[:chi]/||s[:chi]||
+    with s the singular values of the gated, environment-weighted two-site tensor (computed here from
+    the contracted tensor, not from the QR cores); gate_err = discarded weight."""
+    st = po.PEPOState(2, 3, 0, 1, J, H, DT, 3)
+    for _ in range(4):
+        st.trotter_step()
+    st.apply_field_gate()
+    lat = st.lat
+    e = lat.bond_id(lat.site(0, 1), "R")
+    v1, d1, v2, d2 = lat.bond_sites(e)
+    a, b = st.psi[v1].copy(), st.psi[v2].copy()
+    w = lambda v: (np.sqrt(st.lam[lat.bond_id(v, "U")])[:, None] * np.sqrt(st.lam[lat.bond_id(v, "D")])[None, :])
+    theta = np.einsum("udcp,efcq->udpefq", a * w(v1)[:, :, None, None], b * w(v2)[:, :, None, None])
+    theta = np.einsum("xypq,udpefq->udxefy", st.G2.reshape(4, 4, 4, 4), theta)
+    s = np.linalg.svd(theta.reshape(theta.shape[0] * theta.shape[1] * 4, -1), compute_uv=False)
+    assert np.count_nonzero(s >= 1e-11 * s[0]) > 3          # the gate really truncates
+    st.gate_err = 0.0
+    st.apply_bond_gate(e)
+    assert st.lam[e].size == 3
+    assert np.allclose(st.lam[e], s[:3] / np.linalg.norm(s[:3]), rtol=0, atol=1e-13)
+    assert abs(np.sum(st.lam[e] ** 2) - 1) < 1e-14
+    assert abs(st.gate_err - np.sum(s[3:] ** 2) / np.sum(s ** 2)) < 1e-13
+
+
+# ---------------------------------------------------------------- the paper's own convention ---
+@pytest.mark.parametrize("case", [(2, 2, 0, 0), (2, 3, 0, 1), (1, 4, 0, 1)])
+def test_paper_convention_xx_plus_z_equals_dense(case):
+    """PAPER eq. (1): H = -J sum XX - h sum Z with J = h = -1, dt = 0.1,
+    observable Z_c.  The Paulis are parameters of the oracle; untruncated, it must equal the dense
+    Trotterised evolution of that model (first order, field then bonds, R2)."""
+    Lx, Ly, cx, cy = case
+    Jp, hp, dtp = -1.0, -1.0, 0.1
+    dense = dc.dense_trotter_correlation(Lx, Ly, cx, cy, Jp, hp, dtp, 6, bond="X", field="Z", obs="Z")
+    # eps_cut 1e-14: the 1e-11 pruning of eq. (11) itself drifts the network off the dense value by
+    # ~1e-10 after a few steps (SURVEY P2)
+    st = po.PEPOState(Lx, Ly, cx, cy, Jp, hp, dtp, 256, eps_cut=1e-14, bond_pauli="X", field_pauli="Z",
+                      obs_pauli="Z")
+    for t in range(6):
+        st.trotter_step()
+        # the tensor update is exact while untruncated: brute-force contraction of the pinned network
+        # (1e-12 while no Schmidt weight is near the pruning threshold; the 1/sqrt(lambda) of the
+        # de-absorb amplifies rounding once the 2x2 / 2x3 operator space saturates)
+        assert abs(st.exact_contraction() - dense[t]) < (1e-12 if t < 4 else 1e-10), (t, st.exact_contraction(), dense[t])
+        st.bp_converge(1e-13)
+        # BP + Bethe: exact on the chain (tree), approximate on loops (P4; dt = 0.1 doubles the angle)
+        assert abs(st.correlation() - dense[t]) < (1e-12 if Lx == 1 else (2e-9 if t < 4 else 1e-6))
+    # Z_c commutes with the field, not with the bonds: C(dt) = cos(2 J dt)^deg(c) != the ZZ+X value cos(2 h dt)
+    deg = len(st.lat.legs(st.center))
+    assert abs(dense[0] - math.cos(2 * Jp * dtp) ** deg) < 1e-14
