@@ -93,9 +93,10 @@ int pepo_destroy(pepo_ctx* ctx);
  * counts as the last one, 1e-7; 0 = always run the confirming sweep),
  * "trotter_order" (1 = first-order step, R2; 2 = symmetric step of eq. (6)),
  * "pipeline" (number of piece streams of a Trotter step, 4; 0 = serial schedule; the results do
- * not depend on it), and kernel-selection tunables used by the benchmarks ("svd_c16",
- * "svd_min_cluster", "svd_precond_min", "svd_block", "bp_form", "bp_group", "piece_stride", "gram_waves",
- * "svd_gate", "profile", "trace").  -1 on unknown key. */
+ * not depend on it), "bp_tol", "bp_damping", "bp_group" (BP sweeps enqueued per delta read-back,
+ * 1..8; results do not depend on it), "svd_precond_min" (QR-precondition cores of at least this
+ * order, 32; 0 = never), "profile", "trace".  Options belong to the context: two contexts in one
+ * process do not share any setting.  -1 on unknown key. */
 int pepo_set_option(pepo_ctx* ctx, const char* key, double value);
 
 /* One full first-order Trotter step (Fig. 1; R2, R3): field gate on all

@@ -152,7 +152,7 @@ extern "C" int pepo_svd_jacobi(const double* d_A, int m, int n, int lda, double*
   SvdBatch sb; sb.count = 1;
   sb.K[0] = d_A; sb.ldk[0] = lda; sb.r1[0] = m; sb.r2[0] = n; sb.G[0] = G; sb.V[0] = V; sb.sv[0] = d_s;
   sb.order[0] = order; sb.sweeps[0] = d_sweeps ? d_sweeps : ints + 1;
-  int rc = launch_svd_jacobi(st, sb, 1e-15, 60, true, 0); if (rc) return rc;
+  int rc = launch_svd_jacobi(st, sb, 1e-15, 60, true, 0, 0.0); if (rc) return rc;
   return launch_svd_vectors(st, G, V, d_s, order, m, n, d_U, d_V);
 }
 

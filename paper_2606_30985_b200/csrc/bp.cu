@@ -23,7 +23,6 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 constexpr int BP_THREADS = 256;
-int g_bp_form = 2;             // tunable (option "bp_form"): 1 = per-column reductions, 2 = per-chunk reductions
 constexpr int BP_MAXK = 8;     // dU <= 256 (kernel instantiated for 32*KU >= dU, KU in {2,4,8}: fewer
                                // registers -> more resident CTAs -> more bytes in flight)
 
@@ -385,19 +384,13 @@ int launch_bp_partial(cudaStream_t st, const BpBatch& b) {
   for (int t = 0; t < b.count; t++) dumax = std::max(dumax, b.s[t].d[0]);
   int ddmax = 1;
   for (int t = 0; t < b.count; t++) ddmax = std::max(ddmax, b.s[t].d[1]);
-  if (g_bp_form == 1) {
-    if (dumax <= 64) bp_partial_kernel<2><<<grid, BP_THREADS, 0, st>>>(b);
-    else if (dumax <= 128) bp_partial_kernel<4><<<grid, BP_THREADS, 0, st>>>(b);
-    else bp_partial_kernel<8><<<grid, BP_THREADS, 0, st>>>(b);
-  } else if (dumax <= 64 && ddmax <= 64) bp_partial2_kernel<2, 8><<<grid, BP_THREADS, 0, st>>>(b);
+  if (dumax <= 64 && ddmax <= 64) bp_partial2_kernel<2, 8><<<grid, BP_THREADS, 0, st>>>(b);
   else if (dumax <= 128 && ddmax <= 128) bp_partial2_kernel<4, 16><<<grid, BP_THREADS, 0, st>>>(b);
   else bp_partial_kernel<8><<<grid, BP_THREADS, 0, st>>>(b);
   PEPO_COUNT_LAUNCH();
   PEPO_CUDA_OK(cudaGetLastError());
   return 0;
 }
-
-void set_bp_form(int f) { g_bp_form = (f == 1) ? 1 : 2; }
 
 int launch_bp_finalize(cudaStream_t st, const BpBatch& b, double damping, int update,
                        unsigned long long* delta_bits, int* flag) {

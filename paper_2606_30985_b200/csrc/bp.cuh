@@ -38,7 +38,6 @@ struct FieldBatch {
 };
 
 int launch_bp_partial(cudaStream_t st, const BpBatch& b);
-void set_bp_form(int form);
 int launch_bp_finalize(cudaStream_t st, const BpBatch& b, double damping, int update,
                        unsigned long long* delta_bits, int* flag);
 int launch_bp_init(cudaStream_t st, double* msgs, const int* chi_of_msg, int n_msgs, int chi_max);

@@ -21,8 +21,22 @@ void set_error(const char* fmt, ...);
     }                                                                               \
   } while (0)
 
-extern long long g_launch_count;   // kernels launched by this library (stats)
-#define PEPO_COUNT_LAUNCH() (++pepo::g_launch_count)
+// Kernel-launch counter of the context the calling thread is working for (every extern "C" entry
+// that takes a pepo_ctx points it at that context's counter; the kernel-level entry points count
+// into a per-thread scratch counter).  No process-global mutable state: two contexts on two host
+// threads do not interfere.
+extern thread_local long long* t_launch_counter;
+#define PEPO_COUNT_LAUNCH() (++*pepo::t_launch_counter)
+
+// One-time per-device setup (cudaFuncSetAttribute): flags[dev] is set on first use on that device.
+#define PEPO_MAX_DEVICES 64
+inline bool first_use_on_device(char* flags) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= PEPO_MAX_DEVICES) return true;
+  if (flags[dev]) return false;
+  flags[dev] = 1;
+  return true;
+}
 
 // ---- fast division by a runtime constant (index arithmetic of the permute kernels) -------
 struct FastDiv {
@@ -61,7 +75,6 @@ int launch_dgemm_batched(cudaStream_t st, int transA, int transB, const GemmProb
 int launch_gram_reduce(cudaStream_t st, const double* part, int ksplit, int n, double* C,
                        long long ldc);
 void gram_plan(long long m, int n, int* ksplit, int* kchunk);
-void set_gram_waves(int waves);   // only lowering it after pepo_init is safe (the partial buffers are sized at init)
 
 // ---- permutation -------------------------------------------------------------------------
 // dst[sum_j o_j * dst_stride[j]] = src[sum_d i_d * src_stride[d]] * prod_d scale_d(i_d),

@@ -34,7 +34,8 @@
 
 namespace pepo {
 
-long long g_launch_count = 0;
+static thread_local long long t_scratch_launches = 0;
+thread_local long long* t_launch_counter = &t_scratch_launches;
 static thread_local char g_err[512] = "";
 void set_error(const char* fmt, ...) {
   va_list ap;
@@ -224,12 +225,11 @@ struct pepo_ctx {
   // pieces of the colour classes on the streams ps[], their Jacobi kernels on the high-priority
   // streams hp[]; pev: per stream [svd fork, svd join, read-back], then [fork, join per stream]
   int pipeline = 4;
-  int piece_stride = 1;                // 1: piece q of a class takes gates q, q + np, ... (else contiguous runs)
   static constexpr int NSMAX = 4;
   cudaStream_t ps[NSMAX] = {nullptr}, hp[NSMAX] = {nullptr};
   cudaEvent_t pev[5 * NSMAX + 1] = {nullptr};
   int bp_group = 8;                    // option "bp_group": BP sweeps enqueued per delta read-back (1..BP_GROUP)
-  int svd_gate = 0;                    // 1: heavy kernels queued after a Jacobi launch wait until its blocks have begun
+  double jacobi_early = 1e-7;          // option "jacobi_early": cosine below which a Jacobi sweep counts as the last one
   std::vector<cudaEvent_t> done_ev;    // completion events of the pieces of a pipelined step
   int n_sites, n_bonds, n_hb;
   std::vector<SiteInfo> sites;
@@ -264,16 +264,24 @@ struct pepo_ctx {
   std::vector<LaneWs> lanes;
   int* lane_ints; double* lane_dbls;      // device readback blocks (B*4 ints, B*2 doubles)
   // pinned host
-  int* h_ints; double* h_dbls; int* h_chi_msg; double* h_scal; unsigned long long* h_delta; int* h_bpints;
+  int* h_ints = nullptr; double* h_dbls = nullptr; int* h_chi_msg = nullptr; double* h_scal = nullptr;
+  unsigned long long* h_delta = nullptr; int* h_bpints = nullptr;
   int cur_msg = 0;
   bool msgs_valid = false;
-  long long launches0 = 0;
+  long long launches = 0;              // kernels launched for this context (PEPO_COUNT_LAUNCH via t_launch_counter)
   pepo_stats stats;
   size_t model_bytes = 0;
   Prof prof;
 };
 
 namespace {
+// Kernel launches made while an API call works for a context are counted into that context.
+struct CtxScope {
+  long long* prev;
+  explicit CtxScope(pepo_ctx* c) : prev(pepo::t_launch_counter) { pepo::t_launch_counter = &c->launches; }
+  ~CtxScope() { pepo::t_launch_counter = prev; }
+};
+
 void prof_flush(pepo_ctx* c) {        // call only after a stream synchronize
   Prof& P = c->prof;
   for (size_t i = 0; i < P.used; i++) {
@@ -527,7 +535,11 @@ extern "C" int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, doub
                             int bond_pauli, int field_pauli, int obs_pauli) {
   if (!out) { set_error("init: out is NULL"); return -1; }
   *out = nullptr;
-  if (Lx < 1 || Ly < 1 || cx < 0 || cx >= Lx || cy < 0 || cy >= Ly || chi_max < 1 || chi_max > 256 ||
+  if (chi_max > 256) {
+    set_error("init: chi_max %d > 256 is not supported (the BP kernels hold a message in 256 lanes x 8 registers)", chi_max);
+    return -1;
+  }
+  if (Lx < 1 || Ly < 1 || cx < 0 || cx >= Lx || cy < 0 || cy >= Ly || chi_max < 1 ||
       !(dt > 0.0) || bond_pauli < 1 || bond_pauli > 3 || field_pauli < 1 || field_pauli > 3 ||
       obs_pauli < 1 || obs_pauli > 3 || bp_damping < 0.0 || bp_damping >= 1.0 || !d_arena) {
     set_error("init: bad argument (grid %dx%d centre (%d,%d) chi_max %d dt %g)", Lx, Ly, cx, cy, chi_max, dt);
@@ -601,7 +613,7 @@ extern "C" int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, doub
       cudaMallocHost((void**)&c->h_scal, 64) != cudaSuccess ||
       cudaMallocHost((void**)&c->h_delta, 8 * BP_GROUP + 16) != cudaSuccess ||
       cudaMallocHost((void**)&c->h_bpints, 16) != cudaSuccess) {
-    set_error("init: cudaMallocHost failed"); delete c; return -3;
+    set_error("init: cudaMallocHost failed"); pepo_destroy(c); return -3;
   }
   {
     int lo = 0, hi = 0;
@@ -616,14 +628,14 @@ extern "C" int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, doub
            cudaStreamCreateWithPriority(&c->hp[i], cudaStreamNonBlocking, hi) == cudaSuccess;
     }
     for (int i = 0; i < 5 * pepo_ctx::NSMAX + 1 && ok; i++) ok = cudaEventCreateWithFlags(&c->pev[i], cudaEventDisableTiming) == cudaSuccess;
-    if (!ok) { set_error("init: stream / event creation failed"); delete c; return -3; }
+    if (!ok) { set_error("init: stream / event creation failed"); pepo_destroy(c); return -3; }
   }
   {
     bool ok = cudaStreamCreateWithFlags(&c->copy_st, cudaStreamNonBlocking) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->copy_ev, cudaEventDisableTiming) == cudaSuccess;
     c->site_ev.assign(c->n_sites, nullptr);
     for (int v = 0; v < c->n_sites && ok; v++) ok = cudaEventCreateWithFlags(&c->site_ev[v], cudaEventDisableTiming) == cudaSuccess;
-    if (!ok) { set_error("init: stream / event creation failed"); delete c; return -3; }
+    if (!ok) { set_error("init: stream / event creation failed"); pepo_destroy(c); return -3; }
     c->site_pending.assign(c->n_sites, 0);
     c->field_todo.assign(c->n_sites, 0);
   }
@@ -638,10 +650,10 @@ extern "C" int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, doub
   }
   rc |= upload(c, c->dSigma, sig.data(), 32);
   if (!rc) rc = reset_state(c);
-  if (rc) { delete c; return -3; }
+  if (rc) { pepo_destroy(c); return -3; }
   memset(&c->stats, 0, sizeof(c->stats));
   c->stats.min_cut_gap = 1.0;
-  c->launches0 = g_launch_count;
+  c->launches = 0;
   *out = c;
   return 0;
 }
@@ -656,6 +668,7 @@ extern "C" int pepo_init(pepo_ctx** out, int Lx, int Ly, int cx, int cy, double 
 extern "C" int pepo_destroy(pepo_ctx* c) {
   if (!c) return 0;
   cudaStreamSynchronize(c->st);
+  for (auto& e : c->prof.ev) if (e) cudaEventDestroy(e);
   for (int i = 0; i < pepo_ctx::NSMAX; i++) {
     if (c->ps[i]) { cudaStreamSynchronize(c->ps[i]); cudaStreamDestroy(c->ps[i]); }
     if (c->hp[i]) { cudaStreamSynchronize(c->hp[i]); cudaStreamDestroy(c->hp[i]); }
@@ -682,22 +695,15 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "force_householder") c->force_hh = (int)v;
   else if (k == "jacobi_tol") c->jacobi_tol = v;
   else if (k == "jacobi_max_sweeps") c->jacobi_max_sweeps = (int)v;
-  else if (k == "svd_min_cluster") set_svd_min_cluster((int)v);
   else if (k == "svd_precond_min") c->svd_precond_min = (int)v;
-  else if (k == "svd_block") set_svd_block((int)v);
-  else if (k == "svd_c16") set_svd_c16((int)v);
-  else if (k == "jacobi_early") set_svd_early(v);
-  else if (k == "bp_form") set_bp_form((int)v);
-  else if (k == "svd_gate") c->svd_gate = (int)v;
+  else if (k == "jacobi_early") c->jacobi_early = v < 0.0 ? 0.0 : v;
   else if (k == "bp_group") c->bp_group = (int)v;
-  else if (k == "gram_waves") set_gram_waves(std::min((int)v, 2));
   else if (k == "trotter_order") {
     if ((int)v != 1 && (int)v != 2) { set_error("set_option: trotter_order must be 1 or 2"); return -1; }
     c->trotter_order = (int)v;
   }
   else if (k == "pipeline") c->pipeline = (int)v;
   else if (k == "trace") c->prof.trace = (int)v;
-  else if (k == "piece_stride") c->piece_stride = (int)v;
   else if (k == "profile") {
     Prof& P = c->prof;
     if (v != 0.0 && P.ev.empty()) {
@@ -821,7 +827,7 @@ extern "C" int pepo_set_lambda(pepo_ctx* c, int bond, const double* h_src, int n
 
 extern "C" int pepo_get_stats(pepo_ctx* c, pepo_stats* s) {
   if (!c || !s) { set_error("get_stats: NULL"); return -1; }
-  c->stats.kernel_launches = g_launch_count - c->launches0;
+  c->stats.kernel_launches = c->launches;
   c->stats.arena_high_water = c->arena.top;
   c->stats.arena_model_bytes = c->model_bytes;
   c->stats.max_inflight_gates = c->B;
@@ -840,6 +846,7 @@ int apply_field_impl(pepo_ctx* c, bool half);
 }
 extern "C" int pepo_apply_field(pepo_ctx* c) {
   if (!c) { set_error("apply_field: NULL"); return -1; }
+  CtxScope scope(c);
   return apply_field_impl(c, false);
 }
 namespace {
@@ -886,7 +893,6 @@ struct BatchState {        // one batch of gates moving through the three phases
   cudaStream_t st = nullptr;       // stream of this batch
   cudaStream_t hp = nullptr;       // high-priority stream for the Jacobi kernel (nullptr: st)
   cudaEvent_t ev[2] = {nullptr, nullptr};
-  cudaEvent_t started = nullptr;   // if set: fires when the blocks of this batch's Jacobi kernel have begun
   bool piped = false;              // another batch is in flight: keep the profiling events until the class ends
   bool have_chol = false;
   SvdFinishBatch fb;
@@ -1111,9 +1117,7 @@ int batch_p2(pepo_ctx* c, BatchState& S) {
       // a high-priority stream so that it is placed ahead of the other half-batch's GEMM CTAs
       {
         ProfScope ps(c, PC_SVD, 0, 0);
-        set_svd_started_event(S.started);
-        rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps, false, c->svd_precond_min);
-        set_svd_started_event(nullptr);
+        rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps, false, c->svd_precond_min, c->jacobi_early);
         if (rc) return rc;
       }
       ProfScope ps(c, PC_SVD, 0, 0);
@@ -1346,7 +1350,7 @@ int lazy_field_gate(pepo_ctx* c, const std::vector<int>& sites, cudaStream_t st)
   return 0;
 }
 
-int run_step_piped(pepo_ctx* c) {
+int run_step_piped_impl(pepo_ctx* c) {
   const int NS = std::min(std::min(c->pipeline, pepo_ctx::NSMAX), c->B);
   const int hb = c->B / NS;                      // lanes per stream
   std::vector<Piece> P;
@@ -1356,29 +1360,11 @@ int run_step_piped(pepo_ctx* c) {
     int np = (n + hb - 1) / hb;
     np = ((np + NS - 1) / NS) * NS;              // a multiple of the stream count: stream q % NS keeps its part of the grid
     np = std::min(np, n);
-    // piece_stride = 2: gates ordered by the size of their site tensors, pieces = contiguous runs of
-    // that order (pieces of like gates: a slow light gate never holds up a heavy one in its launch)
-    std::vector<int> ord(cls.begin(), cls.end());
-    if (c->piece_stride == 2) {
-      auto weight = [&](int e) {
-        double w = 0;
-        for (int v : {c->bonds[e].v1, c->bonds[e].v2}) w += (double)site_live_size(c, v);
-        return w;
-      };
-      std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) { return weight(a) > weight(b); });
-    }
+    // piece q of a class takes gates q, q + np, ...: each piece holds a similar mix of interior / edge gates
     for (int q = 0; q < np; q++) {
       Piece pc;
       pc.stream = q % NS;
-      if (c->piece_stride == 2) {
-        const int a = (int)((long long)n * q / np), b = (int)((long long)n * (q + 1) / np);
-        pc.S.gate_bonds.assign(ord.begin() + a, ord.begin() + b);
-      } else if (c->piece_stride) {
-        for (int g = q; g < n; g += np) pc.S.gate_bonds.push_back(cls[g]);
-      } else {
-        const int a = (int)((long long)n * q / np), b = (int)((long long)n * (q + 1) / np);
-        pc.S.gate_bonds.assign(cls.begin() + a, cls.begin() + b);
-      }
+      for (int g = q; g < n; g += np) pc.S.gate_bonds.push_back(cls[g]);
       if (pc.S.gate_bonds.empty()) continue;
       pc.S.ng = (int)pc.S.gate_bonds.size();
       for (int e : pc.S.gate_bonds) { pc.sites.push_back(c->bonds[e].v1); pc.sites.push_back(c->bonds[e].v2); }
@@ -1401,7 +1387,6 @@ int run_step_piped(pepo_ctx* c) {
     pc.S.hp = c->hp[s];
     pc.S.ev[0] = c->pev[3 * s]; pc.S.ev[1] = c->pev[3 * s + 1];
     pc.S.piped = true;
-    pc.S.started = c->svd_gate ? c->pev[4 * pepo_ctx::NSMAX + 1 + s] : nullptr;
   }
   // the piece streams start after everything already queued on the caller's stream (the field gate)
   cudaEvent_t fork = c->pev[3 * pepo_ctx::NSMAX];
@@ -1445,10 +1430,6 @@ int run_step_piped(pepo_ctx* c) {
         if (u.phase == 1) {
           rc = batch_p2(c, u.S);
           if (!rc) { PEPO_CUDA_OK(cudaEventRecord(rb, u.S.hp ? u.S.hp : u.S.st)); }
-          // the Jacobi kernel needs whole SMs: heavy kernels the other streams queue from now on
-          // wait until its blocks are resident (launch-completion event)
-          if (!rc && u.S.started)
-            for (int s2 = 0; s2 < NS; s2++) if (s2 != s) PEPO_CUDA_OK(cudaStreamWaitEvent(c->ps[s2], u.S.started, 0));
           u.phase = 2;
         } else {
           rc = batch_p3(c, u.S);
@@ -1485,6 +1466,23 @@ int run_step_piped(pepo_ctx* c) {
   return rc;
 }
 
+// Every exit of the pipelined step - also an error return from the middle of the state machine -
+// leaves the piece streams joined and idle and the lazy field-gate state cleared.
+int run_step_piped(pepo_ctx* c) {
+  const int rc = run_step_piped_impl(c);
+  if (rc) {
+    cudaStreamSynchronize(c->st);
+    for (int s = 0; s < pepo_ctx::NSMAX; s++) { if (c->ps[s]) cudaStreamSynchronize(c->ps[s]); if (c->hp[s]) cudaStreamSynchronize(c->hp[s]); }
+    if (c->copy_st) cudaStreamSynchronize(c->copy_st);
+    c->lazy_field = false;
+    std::fill(c->site_pending.begin(), c->site_pending.end(), 0);
+    c->n_pending = 0; c->copy_forked = false;
+    c->cur_st = c->st;
+    c->prof.used = 0;
+  }
+  return rc;
+}
+
 }  // namespace
 
 // Order in which a Trotter step first touches the sites (piece by piece of the pipelined schedule,
@@ -1503,8 +1501,7 @@ extern "C" int pepo_site_order(pepo_ctx* c, int* h_order, int n) {
     np = ((np + NS - 1) / NS) * NS;
     np = std::min(np, nc);
     for (int q = 0; q < np; q++)
-      for (int g = (c->piece_stride == 1 ? q : (int)((long long)nc * q / np));
-           g < (c->piece_stride == 1 ? nc : (int)((long long)nc * (q + 1) / np)); g += (c->piece_stride == 1 ? np : 1))
+      for (int g = q; g < nc; g += np)
         for (int v : {c->bonds[cls[g]].v1, c->bonds[cls[g]].v2})
           if (!seen[v]) { seen[v] = 1; h_order[k++] = v; }
   }
@@ -1514,6 +1511,7 @@ extern "C" int pepo_site_order(pepo_ctx* c, int* h_order, int n) {
 
 extern "C" int pepo_apply_bond(pepo_ctx* c, int bond) {
   if (!c || bond < 0 || bond >= c->n_bonds) { set_error("apply_bond: bad bond"); return -1; }
+  CtxScope scope(c);
   { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
   std::vector<int> g(1, bond);
   return run_batch(c, g);
@@ -1521,6 +1519,7 @@ extern "C" int pepo_apply_bond(pepo_ctx* c, int bond) {
 
 extern "C" int pepo_trotter_step(pepo_ctx* c) {
   if (!c) { set_error("trotter_step: NULL"); return -1; }
+  CtxScope scope(c);
   c->stats.gate_err = 0.0; c->stats.min_cut_gap = 1.0; c->stats.jacobi_sweeps = 0;
   // order 1 (R2): field gate, bond sweep.  order 2 (PAPER eq. (6)):
   // half field gate, bond sweep, half field gate.
@@ -1628,12 +1627,13 @@ int bp_init_messages(pepo_ctx* c) {
 
 extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
   if (!c) { set_error("bp_converge: NULL"); return -1; }
+  CtxScope scope(c);
   { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
   int sweeps = 0;
   double delta = INFINITY;
   int status = 1;
   int flags = 0;                 // bit 0: a message with zero norm kept its old value (R7); bit 1: non-finite norm
-  for (int phase = 0; phase < 2 && status; phase++) {
+  for (int phase = 0; phase < 2 && status && !(flags & 2); phase++) {
     const double damping = phase == 0 ? 0.0 : c->bp_damping;
     const int budget = phase == 0 ? c->bp_max_sweeps : c->bp_max_sweeps_damped;
     if (phase == 1 && !(c->bp_damping > 0.0)) break;
@@ -1652,6 +1652,7 @@ extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
       PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
       prof_flush(c);
       flags |= c->h_bpints[0];
+      if (flags & 2) break;                               // non-finite norm: no point in spending the budget
       int done = ngr;                                   // sweeps of the group that actually ran
       for (int g = 0; g < ngr; g++) {
         double dg;
@@ -1677,6 +1678,7 @@ extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
 
 extern "C" int pepo_correlation(pepo_ctx* c, double* h_C) {
   if (!c || !h_C) { set_error("correlation: NULL"); return -1; }
+  CtxScope scope(c);
   { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
   if (!c->msgs_valid) { set_error("correlation: no converged messages (call pepo_bp_converge after the last state change)"); return -1; }
   int rc = bp_sweep(c, 0.0, 0); if (rc) return rc;
@@ -1705,6 +1707,7 @@ extern "C" int pepo_get_message(pepo_ctx* c, int bond, int from_v1, double* h_ds
 // Uses the message-partial scratch of the BP sweep (free between sweeps) as the output buffer.
 extern "C" int pepo_bond_entropy(pepo_ctx* c, double* h_S, int n) {
   if (!c || !h_S || n < c->n_bonds) { set_error("bond_entropy: bad argument (need n >= n_bonds)"); return -1; }
+  CtxScope scope(c);
   if (c->n_bonds == 0) return 0;
   for (int e = 0; e < c->n_bonds; e++) { c->h_chi_msg[2 * e] = c->chi[e]; c->h_chi_msg[2 * e + 1] = c->chi[e]; }
   PEPO_CUDA_OK(cudaMemcpyAsync(c->chi_of_msg, c->h_chi_msg, (size_t)2 * c->n_bonds * 4, cudaMemcpyHostToDevice, c->st));

@@ -522,11 +522,11 @@ int launch_potrf(cudaStream_t st, const MatBatch& b, int* const* info, double ta
   int nmax = 0;
   for (int t = 0; t < b.count; t++) { ip.p[t] = info[t]; nmax = std::max(nmax, b.n[t]); }
   size_t smem = (size_t)(PB * (PB + 1) + (PB + 1) * std::max(nmax, 1)) * sizeof(double);
-  static size_t attr = 0;
-  if (smem > attr) {
-    PEPO_CUDA_OK(cudaFuncSetAttribute(potrf_upper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(smem, (size_t)48 * 1024)));
-    attr = std::max(smem, (size_t)48 * 1024);
-  }
+  // largest shared-memory size the kernel may ask for (chi_max <= 256: n <= 1024), set once per device
+  static char attr[PEPO_MAX_DEVICES] = {0};
+  if (first_use_on_device(attr))
+    PEPO_CUDA_OK(cudaFuncSetAttribute(potrf_upper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+  if (smem > (size_t)200 * 1024) { set_error("potrf: matrix of order %d too large", nmax); return -1; }
   potrf_upper_kernel<<<b.count, 512, smem, st>>>(b, ip, tau);
   PEPO_COUNT_LAUNCH();
   PEPO_CUDA_OK(cudaGetLastError());
@@ -550,11 +550,10 @@ int launch_trtri(cudaStream_t st, const MatBatch& R, const MatBatch& Rinv) {
   for (int t = 0; t < R.count; t++) nmax = std::max(nmax, R.n[t]);
   int nblk = (nmax + PB - 1) / PB;
   size_t smem = ((size_t)(nblk + 1) * PB * PB + PB * (PB + 1)) * sizeof(double);
-  static size_t attr = 0;
-  if (smem > attr) {
-    PEPO_CUDA_OK(cudaFuncSetAttribute(trtri_upper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(smem, (size_t)48 * 1024)));
-    attr = std::max(smem, (size_t)48 * 1024);
-  }
+  static char attr[PEPO_MAX_DEVICES] = {0};
+  if (first_use_on_device(attr))
+    PEPO_CUDA_OK(cudaFuncSetAttribute(trtri_upper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+  if (smem > (size_t)200 * 1024) { set_error("trtri: matrix of order %d too large", nmax); return -1; }
   dim3 grid(nblk, R.count);
   trtri_upper_kernel<<<grid, 256, smem, st>>>(R, Rinv);
   PEPO_COUNT_LAUNCH();

@@ -59,13 +59,10 @@ struct SvdBatch {
 // with_v = false: V is not accumulated (launch_svd_bridge then derives it from K, SvdFinishBatch::K)
 // precond_min > 0 (only with_v = false): problems with min(r1,r2) >= precond_min are QR-preconditioned
 // (the Jacobi iteration runs on R^T); launch_svd_bridge must get the same value.
+// early: cosine below which a sweep counts as the last one (jacobi_c16_kernel; 0 = always run the
+// confirming sweep)
 int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
-                      int precond_min);
-void set_svd_min_cluster(int cs);
-void set_svd_block(int on);
-void set_svd_c16(int on);
-void set_svd_early(double cosine);
-void set_svd_started_event(cudaEvent_t e);   // launch-completion event of the next hot-path SVD launch (nullptr: none)
+                      int precond_min, double early);
 
 struct SvdFinishBatch {
   int count;

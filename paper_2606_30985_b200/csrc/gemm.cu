@@ -202,11 +202,9 @@ int launch_cfg(cudaStream_t st, const GemmProb& p, const GemmProb* probs, int gz
   constexpr int NT = (BM / WM) * (BN / WN) * 32;
   size_t smem = (size_t)STAGES * (BM + BN) * BK * sizeof(double);
   auto kern = dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static char attr_set[PEPO_MAX_DEVICES] = {0};
+  if (first_use_on_device(attr_set))
     PEPO_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_set = true;
-  }
   long long tiles = ((maxM + BM - 1) / BM) * ((maxN + BN - 1) / BN);
   if (tiles <= 0 || gz <= 0) return 0;
   dim3 grid((unsigned)tiles, 1, (unsigned)gz);
@@ -268,8 +266,7 @@ int launch_dgemm_batched(cudaStream_t st, int transA, int transB, const GemmProb
   return launch_trans<64, 64, 32, 32, 4>(st, transA, transB, dummy, probs_dev, batch, max_M, max_N, 1, 0, nullptr, false);
 }
 
-int g_gram_waves = 2;              // tunable (option "gram_waves"): waves of resident CTAs of the 80x80 Gram kernel
-void set_gram_waves(int w) { g_gram_waves = std::min(std::max(w, 1), 4); }
+constexpr int GRAM_WAVES = 2;      // waves of resident CTAs of the 80x80 Gram kernel (1 and 2 measured equal, 3+ slower)
 
 void gram_plan(long long m, int n, int* ksplit, int* kchunk) {
   // upper-triangle tiles at the tile size launch_dgemm will pick (the choice between the 128 and
@@ -280,7 +277,7 @@ void gram_plan(long long m, int n, int* ksplit, int* kchunk) {
     // 80x80 tile kernel: 197 registers x 128 threads -> 2 resident CTAs per SM = 296 slots.  The
     // working CTAs (upper tiles x splits) must fill a whole number of waves: 99 splits x 6 tiles =
     // 594 CTAs ran as two waves plus a third one of 2 CTAs (ncu: 558 us against 2/3 of that).
-    bt = 80; target = 148 * 2 * g_gram_waves; cap = 100 * g_gram_waves; whole_waves = true;
+    bt = 80; target = 148 * 2 * GRAM_WAVES; cap = 100 * GRAM_WAVES; whole_waves = true;
   }
   else if (n <= 64) bt = 64;
   const int tn = (n + bt - 1) / bt;

@@ -197,11 +197,6 @@ __global__ void __launch_bounds__(1024) jacobi_svd_kernel(SvdBatch b, double tol
 // the round-robin circle through distributed shared memory (staged in registers between two
 // cluster barriers).  No global-memory traffic inside the iteration.
 // ---------------------------------------------------------------------------------------------
-int g_svd_block = 0;                    // tunable (option "svd_block"): block form of the super-rounds
-cudaEvent_t g_svd_started = nullptr;    // if set: recorded when all blocks of the next hot-path launch have begun
-double g_svd_early = 1e-7;              // tunable (option "jacobi_early"): see jacobi_c16_kernel
-int g_svd_c16 = 1;                      // tunable (option "svd_c16"): 16-lane hot-path kernel
-int g_svd_min_cluster = 1;              // tunable (option "svd_min_cluster"): smallest cluster size tried
 constexpr int JC_THREADS = 1024;
 constexpr int JC_STAGE = 26;            // doubles staged per thread during a block exchange
 constexpr size_t JC_SMEM_CAP = 200 * 1024;
@@ -235,141 +230,10 @@ __device__ __forceinline__ bool rotate_pair(double* cp, double* cq, int MP2, int
   return true;
 }
 
-// ---------------------------------------------------------------------------------------------
-// Block form of one super-round (top block x bottom block, bs rounds of bs disjoint pairs).
-// The pair rotations of a round need only the Gram matrix of the 2 bs resident columns, so:
-//   A. W = X^T X from the columns (fresh inner products, once per super-round);
-//   B. the bs rounds run on W alone (two-sided update of a 2bs x 2bs matrix) and accumulate the
-//      rotations into J (orthogonal by construction: a product of plane rotations);
-//   C. X <- X J, one pass over the columns (ALU-bound, 2 LEN (2bs)^2 flop).
-// Same pairs, same order, same angle formula as the column-wise rounds; the latency-bound part
-// (reductions + the scalar rotation arithmetic of every pair) now touches 2bs-vectors instead of
-// LEN-vectors.  The "any rotation" flag is taken from the fresh W (step A), i.e. from inner
-// products of the actual columns, as in the column-wise form.
-// Shared: Wm, Jm: n2 x PW (PW even >= n2), rc/rs: bs doubles each.  LEN/2 odd: conflict-free.
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void rot_params(double al, double be, double ga, double tol2, double noise2,
-                                           double& cs, double& sn) {
-  cs = 1.0; sn = 0.0;
-  if (al < noise2 || be < noise2 || !(al > 0.0) || !(be > 0.0)) return;
-  if (ga * ga <= tol2 * al * be) return;
-  jacobi_cs(al, be, ga, cs, sn);
-}
-
-__device__ bool block_superround(double* top, int bs, int LEN, int MP2, double tol2, double noise2,
-                                 double* Wm, double* Jm, double* rc, double* rs, int PW) {
-  const int tid = threadIdx.x, lane = tid & 31;
-  const int n2 = 2 * bs, LEN2 = LEN >> 1;
-  const double2* X2 = reinterpret_cast<const double2*>(top);      // column c at X2 + c*LEN2
-  // ---- A: Gram (upper triangle, two threads per entry) ---------------------------------------
-  const int npair = n2 * (n2 + 1) / 2;
-  bool rot = false;
-  for (int e0 = 0; e0 < npair; e0 += JC_THREADS / 2) {
-    const int e = e0 + (tid >> 1);
-    double v = 0.0;
-    int i = 0, j = 0;
-    if (e < npair) {
-      // e -> (i <= j): row-major enumeration of the upper triangle
-      int rem = e;
-      i = 0;
-      int rowlen = n2;
-      while (rem >= rowlen) { rem -= rowlen; rowlen--; i++; }
-      j = i + rem;
-      const double2* xi = X2 + (size_t)i * LEN2;
-      const double2* xj = X2 + (size_t)j * LEN2;
-      for (int k = (tid & 1); k < MP2; k += 2) {
-        const double2 a = xi[k], b = xj[k];
-        v += a.x * b.x;
-        v += a.y * b.y;
-      }
-    }
-    v += __shfl_xor_sync(0xffffffffu, v, 1);
-    if (e < npair && (tid & 1) == 0) { Wm[i * PW + j] = v; Wm[j * PW + i] = v; }
-  }
-  for (int e = tid; e < n2 * PW; e += JC_THREADS) Jm[e] = ((e / PW) == (e % PW)) ? 1.0 : 0.0;
-  __syncthreads();
-  // ---- B: bs rounds on W, rotations accumulated in J -----------------------------------------
-  for (int r = 0; r < bs; r++) {
-    if (tid < bs) {
-      const int pp = tid;
-      int q = tid + r; if (q >= bs) q -= bs;
-      q += bs;
-      double cs, sn;
-      rot_params(Wm[pp * PW + pp], Wm[q * PW + q], Wm[pp * PW + q], tol2, noise2, cs, sn);
-      rc[tid] = cs; rs[tid] = sn;
-      rot |= (sn != 0.0);
-    }
-    __syncthreads();
-    // column phase: W[:,p], W[:,q] and J[:,p], J[:,q]
-    {
-      const int half = JC_THREADS / 2;
-      double* Mx = (tid < half) ? Wm : Jm;
-      for (int e = (tid < half ? tid : tid - half); e < n2 * bs; e += half) {
-        const int t = e % bs, i = e / bs;
-        int q = t + r; if (q >= bs) q -= bs;
-        q += bs;
-        const double cs = rc[t], sn = rs[t];
-        if (sn != 0.0) {
-          const double x = Mx[i * PW + t], y = Mx[i * PW + q];
-          Mx[i * PW + t] = cs * x - sn * y;
-          Mx[i * PW + q] = sn * x + cs * y;
-        }
-      }
-    }
-    __syncthreads();
-    // row phase: W[p,:], W[q,:]
-    for (int e = tid; e < n2 * bs; e += JC_THREADS) {
-      const int j = e % n2, t = e / n2;
-      int q = t + r; if (q >= bs) q -= bs;
-      q += bs;
-      const double cs = rc[t], sn = rs[t];
-      if (sn != 0.0) {
-        const double x = Wm[t * PW + j], y = Wm[q * PW + j];
-        Wm[t * PW + j] = cs * x - sn * y;
-        Wm[q * PW + j] = sn * x + cs * y;
-      }
-    }
-    __syncthreads();
-  }
-  // ---- C: X <- X J (rows independent: in place after a barrier per pass) ----------------------
-  {
-    double2* Xw = reinterpret_cast<double2*>(top);
-    const int ng = (n2 + 3) / 4;                       // groups of 4 output columns
-    const int rpp = JC_THREADS / ng;                   // row pairs per pass (all groups of a row in one pass)
-    for (int k0 = 0; k0 < LEN2; k0 += rpp) {
-      const int k2 = k0 + tid % rpp, jg = tid / rpp;
-      const bool act = (jg < ng) && (k2 < LEN2);
-      const int j0 = jg * 4;
-      double2 acc0 = make_double2(0.0, 0.0), acc1 = acc0, acc2 = acc0, acc3 = acc0;
-      if (act) {
-        for (int i = 0; i < n2; i++) {
-          const double2 x = Xw[(size_t)i * LEN2 + k2];
-          const double2 ja = *reinterpret_cast<const double2*>(Jm + i * PW + j0);
-          const double2 jb = *reinterpret_cast<const double2*>(Jm + i * PW + j0 + 2);
-          acc0.x += x.x * ja.x; acc0.y += x.y * ja.x;
-          acc1.x += x.x * ja.y; acc1.y += x.y * ja.y;
-          acc2.x += x.x * jb.x; acc2.y += x.y * jb.x;
-          acc3.x += x.x * jb.y; acc3.y += x.y * jb.y;
-        }
-      }
-      __syncthreads();
-      if (act) {
-        Xw[(size_t)j0 * LEN2 + k2] = acc0;
-        if (j0 + 1 < n2) Xw[(size_t)(j0 + 1) * LEN2 + k2] = acc1;
-        if (j0 + 2 < n2) Xw[(size_t)(j0 + 2) * LEN2 + k2] = acc2;
-        if (j0 + 3 < n2) Xw[(size_t)(j0 + 3) * LEN2 + k2] = acc3;
-      }
-      __syncthreads();
-    }
-  }
-  (void)lane;
-  return rot;
-}
-
 template <int STAGE, int NREG>
 __global__ void __launch_bounds__(JC_THREADS, 1)
 jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int with_v, int LEN,
-                      int precond_min, int pw, int use_block) {
+                      int precond_min, int pw) {
   extern __shared__ __align__(16) double jsm[];
   cg::cluster_group cluster = cg::this_cluster();
   const int crank = (int)cluster.block_rank();
@@ -552,9 +416,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
     __syncthreads();
     // super-rounds
     for (int sr = 0; sr < 2 * CS - 1; sr++) {
-      if (use_block) {
-        rot |= block_superround(top, bs, LEN, MP2, tol2, noise2, Wm, Jm, rc, rs, PW);
-      } else if (NREG > 0) {
+      if (NREG > 0) {
         // The pair rotations are shared-memory-bandwidth and latency bound.  Warp i keeps top column
         // i in registers for the bs rounds of the super-round, so only the bottom column of each pair
         // moves through shared memory; the squared norms of the columns are carried along (al in a
@@ -1237,11 +1099,6 @@ __global__ void set_identity_kernel(double* Q, long long m, int k) {
 
 }  // namespace
 
-void set_svd_block(int on) { g_svd_block = on ? 1 : 0; }
-void set_svd_c16(int on) { g_svd_c16 = on ? 1 : 0; }
-void set_svd_early(double c) { g_svd_early = c < 0.0 ? 0.0 : c; }
-void set_svd_started_event(cudaEvent_t e) { g_svd_started = e; }
-void set_svd_min_cluster(int cs) { g_svd_min_cluster = cs < 1 ? 1 : (cs > 16 ? 16 : cs); }
 
 int launch_svd_vectors(cudaStream_t st, const double* G, const double* V, const double* s,
                        const int* order, int m, int n, double* U, double* Vout) {
@@ -1263,14 +1120,14 @@ int launch_set_identity(cudaStream_t st, double* Q, long long m, int k) {
 }
 
 static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
-                            int precond_min);
+                            int precond_min, double early);
 
 // The launch configuration (cluster size, columns per CTA, register tile) fixes the order of the
 // pair rotations, i.e. the rounding of the result.  It is therefore chosen per problem SIZE, never
 // from the composition of the batch: problems of equal (min, max) dimension share a launch, and a
 // gate gives bit-identical results whichever other gates run beside it (serial or pipelined class).
 int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
-                      int precond_min) {
+                      int precond_min, double early) {
   if (b.count == 0) return 0;
   bool done[PEPO_MAXT] = {false};
   for (int t0 = 0; t0 < b.count; t0++) {
@@ -1284,14 +1141,14 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
       g.G[q] = b.G[t]; g.V[q] = b.V[t]; g.sv[q] = b.sv[t]; g.order[q] = b.order[t]; g.sweeps[q] = b.sweeps[t];
       done[t] = true;
     }
-    int rc = launch_svd_group(st, g, tol, max_sweeps, with_v, precond_min);
+    int rc = launch_svd_group(st, g, tol, max_sweeps, with_v, precond_min, early);
     if (rc) return rc;
   }
   return 0;
 }
 
 static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
-                            int precond_min) {
+                            int precond_min, double early) {
   if (b.count == 0) return 0;
   int ncmax = 1, lenmax = 2;
   for (int t = 0; t < b.count; t++) {
@@ -1305,8 +1162,8 @@ static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int 
   int cs0 = 1;
   while (cs0 < 8 && (ncmax + 2 * cs0 - 1) / (2 * cs0) > 16) cs0 *= 2;
   // hot path: 16-lane kernel (no V, cluster >= 2, columns of <= 256 doubles, <= 16 pairs per CTA)
-  if (!with_v && g_svd_c16) {
-    const int CS = std::max(std::max(cs0, g_svd_min_cluster), 2);
+  if (!with_v) {
+    const int CS = std::max(cs0, 2);
     const int bs = (ncmax + 2 * CS - 1) / (2 * CS);
     int mmax = 2;
     for (int t = 0; t < b.count; t++) mmax = std::max(mmax, std::max(b.r1[t], b.r2[t]));
@@ -1332,18 +1189,12 @@ static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int 
       cfg.blockDim = dim3(nthr);
       cfg.dynamicSmemBytes = smem;
       cfg.stream = st;
-      cudaLaunchAttribute at[2];
+      cudaLaunchAttribute at[1];
       at[0].id = cudaLaunchAttributeClusterDimension;
       at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
       cfg.attrs = at; cfg.numAttrs = 1;
-      if (g_svd_started) {
-        at[1].id = cudaLaunchAttributeLaunchCompletionEvent;
-        at[1].val.launchCompletionEvent.event = g_svd_started;
-        at[1].val.launchCompletionEvent.flags = 0;
-        cfg.numAttrs = 2;
-      }
-      static bool attr_done = false;
-      if (!attr_done) {
+      static char attr_done[PEPO_MAX_DEVICES] = {0};
+      if (first_use_on_device(attr_done)) {
         const int mx = 226 * 1024;                 // 227 KB per CTA less the static shared memory
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<2, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<4, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
@@ -1357,9 +1208,8 @@ static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int 
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<8, 512>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<10, 256>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<13, 256>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        attr_done = true;
       }
-      const double early2 = g_svd_early * g_svd_early;
+      const double early2 = early * early;
       cudaError_t e;
       if (nreg == 2) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<2, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
       else if (nreg == 4) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<4, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
@@ -1372,7 +1222,7 @@ static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int 
       return 0;
     }
   }
-  for (int CS = std::max(cs0, g_svd_min_cluster); CS <= 16; CS *= 2) {
+  for (int CS = cs0; CS <= 16; CS *= 2) {
     int bs = (ncmax + 2 * CS - 1) / (2 * CS);
     const int PW = (2 * bs + 3) & ~3;
     size_t smem0 = ((size_t)2 * bs * lenmax) * 8 + (size_t)(2 * bs + 4) * 4 + 64 +
@@ -1398,37 +1248,33 @@ static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int 
     const int pwk = std::max(pw, 1), wv = with_v ? 1 : 0;
     cudaError_t e;
     if (need <= 8 && lenmax / 2 <= 128 && bs <= JC_THREADS / 32) {
-      static bool done84 = false;
-      if (!done84) {
+      static char done84[PEPO_MAX_DEVICES] = {0};
+      if (first_use_on_device(done84)) {
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<8, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<8, 4>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        done84 = true;
       }
-      e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel<8, 4>, b, tol, max_sweeps, bs, CS, wv, lenmax, pmin, pwk, g_svd_block);
+      e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel<8, 4>, b, tol, max_sweeps, bs, CS, wv, lenmax, pmin, pwk);
     } else if (need <= 8) {
-      static bool done8 = false;
-      if (!done8) {
+      static char done8[PEPO_MAX_DEVICES] = {0};
+      if (first_use_on_device(done8)) {
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<8, 0>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        done8 = true;
       }
-      e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel<8, 0>, b, tol, max_sweeps, bs, CS, wv, lenmax, pmin, pwk, g_svd_block);
+      e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel<8, 0>, b, tol, max_sweeps, bs, CS, wv, lenmax, pmin, pwk);
     } else if (need <= 16) {
-      static bool done16 = false;
-      if (!done16) {
+      static char done16[PEPO_MAX_DEVICES] = {0};
+      if (first_use_on_device(done16)) {
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<16, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<16, 0>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        done16 = true;
       }
-      e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel<16, 0>, b, tol, max_sweeps, bs, CS, wv, lenmax, pmin, pwk, g_svd_block);
+      e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel<16, 0>, b, tol, max_sweeps, bs, CS, wv, lenmax, pmin, pwk);
     } else {
-      static bool done26 = false;
-      if (!done26) {
+      static char done26[PEPO_MAX_DEVICES] = {0};
+      if (first_use_on_device(done26)) {
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<JC_STAGE, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)JC_SMEM_CAP + 1024));
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_cluster_kernel<JC_STAGE, 0>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        done26 = true;
       }
-      e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel<JC_STAGE, 0>, b, tol, max_sweeps, bs, CS, wv, lenmax, pmin, pwk, g_svd_block);
+      e = cudaLaunchKernelEx(&cfg, jacobi_cluster_kernel<JC_STAGE, 0>, b, tol, max_sweeps, bs, CS, wv, lenmax, pmin, pwk);
     }
     if (e == cudaSuccess) { PEPO_COUNT_LAUNCH(); return 0; }
     (void)cudaGetLastError();                      // e.g. cluster of 16 not schedulable: try the fallback

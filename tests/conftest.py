@@ -29,3 +29,18 @@ def golden_dense():
             key, vals = line.split("|")
             out[tuple(int(t) for t in key.split())] = [float(t) for t in vals.split()]
     return out
+
+
+def read_oracle_trajectory(name):
+    """Rows of a stored oracle trajectory written by tests/golden/make_oracle_twin.py:
+    dicts with step, C, sweeps, status, delta, chi_max_live, gate_err, chi_sum."""
+    path = os.path.join(ROOT, "tests", "golden", name)
+    rows = []
+    with open(path) as f:
+        for line in f:
+            if line.startswith("#"):
+                continue
+            t = line.split()
+            rows.append(dict(step=int(t[0]), C=float(t[1]), sweeps=int(t[2]), status=int(t[3]), delta=float(t[4]),
+                             chi_max_live=int(t[5]), gate_err=float(t[6]), chi_sum=int(t[7])))
+    return rows
