@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--chi", type=int, default=60)
     ap.add_argument("--prep-max", type=int, default=60, help="max untimed preparation steps")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-config3", action="store_true", help="skip the BASELINE configs[2] kernel microbenchmarks")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--bp-tol", type=float, default=1e-10)
     ap.add_argument("--bp-damping", type=float, default=0.5)
@@ -147,6 +148,74 @@ def prepare(sim, args):
             "prep_steps": n}
 
 
+def fp64_yardsticks(torch, B, dev):
+    """fp64 peaks measured in THIS run: (i) a register-only DMMA.8x8x4 loop through the
+    library's own pepo_dmma_peak (the instruction every GEMM of the path is built on); (ii) torch.matmul
+    fp64 8192^3 (cuBLAS) as an outside yardstick only - nothing on the hot path calls it."""
+    sink = torch.zeros(1, dtype=torch.float64, device=dev)
+    best = 0.0
+    for cps in (1, 2, 4):
+        B.dmma_peak(2000, cps, sink)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fl = B.dmma_peak(20000, cps, sink)
+        e1.record()
+        e1.synchronize()
+        best = max(best, fl / e0.elapsed_time(e1) * 1e-9)
+    n = 8192
+    a = torch.randn(n, n, dtype=torch.float64, device=dev)
+    b = torch.randn(n, n, dtype=torch.float64, device=dev)
+    torch.matmul(a, b)
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(3):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        torch.matmul(a, b)
+        e1.record()
+        e1.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    del a, b
+    torch.cuda.empty_cache()
+    return {"dmma_loop_tflops": best, "torch_matmul_fp64_8192_tflops": 2.0 * n ** 3 / min(ts) * 1e-9}
+
+
+def config3_numbers(torch, dev, fp64_peak):
+    """BASELINE configs[2] (the metric's 'permute GB/s and Gram fp64 TFLOP/s vs peak'): all 120 permutations of
+    the (4,40,40,40,40) tensor, Gram / Cholesky-QR of 256000 x 160 and 256000 x 40 (Gram, the triangular
+    solve as Q = A R^-1 GEMM, and POTRF + triangular inverse by difference), graph-replayed, rotated buffers."""
+    from paper_2606_30985_b200 import microbench as mb
+    from paper_2606_30985_b200 import binding as B
+    from paper_2606_30985_b200 import inputs
+    pm = mb.bench_permute(40, 5, dev)
+    slow = sorted(pm["rows"], key=lambda r: r["frac"])[:5]
+    out = {"permute_4x40^4": {"bytes_per_permute": pm["bytes"], "peak_gbs": pm["peak_gbs"], "n_perms": pm["n_perms"],
+                              "gbs_min": min(r["gbs"] for r in pm["rows"]), "gbs_median": sorted(r["gbs"] for r in pm["rows"])[60],
+                              "gbs_max": max(r["gbs"] for r in pm["rows"]), "frac_min": pm["frac_min"],
+                              "frac_median": pm["frac_median"], "n_ge_70pct": pm["n_ge_70pct"],
+                              "slowest": [{"perm": r["perm"], "frac": r["frac"]} for r in slow]}}
+    qr = []
+    for m, n in ((256000, 160), (256000, 40)):
+        A = torch.from_numpy(inputs.normal_tensor((m, n), 1)).to(dev)
+        ws = B._ws(B._lib.pepo_gram_ws_bytes(m, n), dev)
+        t_gram, _ = mb.time_ms(lambda i: B.gram(A, m, n, ws=ws), 8)
+        Q = torch.empty(m * n, dtype=torch.float64, device=dev)
+        ws2 = B._ws(B._lib.pepo_cholqr_ws_bytes(m, n), dev)
+        t_qr, _ = mb.time_ms(lambda i: B.cholqr(A, m, n, Q=Q, ws=ws2), 8)
+        Rinv = torch.randn(n * n, dtype=torch.float64, device=dev)
+        t_trsm, _ = mb.time_ms(lambda i: B.dgemm(0, 0, m, n, n, A, m, Rinv, n, Cout=Q, ldc=m), 8)
+        syrk = m * n * (n + 1) / t_gram * 1e-9
+        qr.append({"m": m, "n": n, "gram_ms": t_gram, "gram_tflops_syrk": syrk, "gram_frac_of_fp64_peak": syrk / fp64_peak,
+                   "gram_gbs": 8.0 * m * n / t_gram * 1e-6, "trsm_as_gemm_ms": t_trsm,
+                   "trsm_tflops": 2.0 * m * n * n / t_trsm * 1e-9, "cholqr_ms": t_qr,
+                   "potrf_plus_trtri_ms_by_difference": max(t_qr - t_gram - t_trsm, 0.0)})
+        del A, Q
+    out["cholesky_qr"] = qr
+    torch.cuda.empty_cache()
+    return out
+
+
 def one_step(sim):
     sim.trotter_step()
     status, sweeps, delta = sim.bp_converge()
@@ -164,6 +233,7 @@ def run_ours(args):
     torch.cuda.set_device(dev)
     R.init("nccl", dev)
     L, chi = args.grid, args.chi
+    yard = fp64_yardsticks(torch, B, dev)
     sim = B.Pepo(L, L, args.cx, args.cy, J, H, DT, chi, args.bp_tol, args.bp_damping, device=str(dev))
     for kv in args.opt:
         k, v = kv.split("=")
@@ -290,7 +360,13 @@ def run_ours(args):
 
     per = per_kernel(prof, PROF_STEPS)
     per_overlapped = per_kernel(prof_overlapped, args.steps)
-    alu_peak = 148 * 64 * 2 * 1.965e9 * 1e-12     # fp64 DFMA: 148 SMs x 64 FMA/clk x 2 x 1.965 GHz
+    unit_peak = 148 * 64 * 2 * 1.965e9 * 1e-12    # fp64: 148 SMs x 64 FMA/clk x 2 x 1.965 GHz (unit count, context only)
+    alu_peak = yard["dmma_loop_tflops"]           # measured in this run: the denominator of every fp64 fraction
+    peak_txt = ("fp64 tensor (DMMA.8x8x4) rate measured in this run by a register-only loop (pepo_dmma_peak): %.1f TF/s; "
+                "torch.matmul fp64 8192^3 (cuBLAS, yardstick only) in the same run: %.1f TF/s; unit count 148 SMs x 64 "
+                "FMA/clk x 2 x 1.965 GHz = %.1f TF/s; MEASURED_PEAKS bf16 sustained %.0f x 45/2250 (guide's nominal ratio) "
+                "= %.1f TF/s" % (alu_peak, yard["torch_matmul_fp64_8192_tflops"], unit_peak,
+                                 peaks["bf16_tflops_sustained"], fp64_peak))
 
     def roof_of(k):
         d = prof[k]
@@ -299,12 +375,7 @@ def run_ours(args):
         if k in ("gram", "apply_gemm", "small_gemm"):
             ach = d["flops"] / d["ms"] * 1e-9
             return {"kernel": k, "bound": "tensor", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s",
-                    "frac": ach / alu_peak, "traffic": None,
-                    "peak_source": "fp64 tensor (DMMA) rate of B200 = its DFMA rate: 148 SMs x 64 FMA/clk x 2 x 1.965 GHz "
-                                   "= %.1f TF/s (a DMMA-only microbenchmark on this pool reached 36.9); the guide's nominal "
-                                   "45 TF/s x measured/nominal bf16 ratio (%s %.0f/2250) would give %.1f TF/s, which the "
-                                   "reconstruction GEMM already exceeds, so the unit-count figure is the denominator" %
-                                   (alu_peak, peaks["source"], peaks["bf16_tflops_sustained"], fp64_peak)}
+                    "frac": ach / alu_peak, "traffic": None, "peak_source": peak_txt}
         if k in ("permute", "field", "bp"):
             ach = d["bytes"] / d["ms"] * 1e-6
             return {"kernel": k, "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
@@ -313,23 +384,39 @@ def run_ours(args):
             ach = d["flops"] / d["ms"] * 1e-9
             return {"kernel": k, "bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s",
                     "frac": ach / alu_peak, "traffic": None,
-                    "peak_source": "fp64 DFMA peak from unit counts (148 SMs x 64 FMA/clk x 2 x 1.965 GHz); the Jacobi "
-                                   "iteration is latency-bound (one cluster of 8 SMs per core, DESIGN.md 6.3), "
-                                   "flops = sweeps x Nc(Nc-1)/2 pairs x 12 L"}
+                    "peak_source": "fp64 DFMA rate = the DMMA rate measured in this run (%.1f TF/s; B200 has one fp64 "
+                                   "datapath); the Jacobi iteration is latency-bound (one cluster of 8 SMs per core, "
+                                   "DESIGN.md 6.3), flops = sweeps x Nc(Nc-1)/2 pairs x 12 L" % alu_peak}
         return None
 
     rooflines = {k: r for k in prof for r in [roof_of(k)] if r is not None}
     if (L, chi) == (4, 60):
         for k, r in rooflines.items():
             r["traffic"] = NCU_TRAFFIC_4x4_CHI60.get(k)
-    roof = rooflines.get(dom) or {"kernel": dom, "bound": "alu", "achieved": None, "peak": alu_peak,
-                                  "unit": "TFLOP/s", "frac": None, "traffic": None,
-                                  "peak_source": "latency-bound small dense kernel"}
+    roof = dict(rooflines.get(dom) or {"kernel": dom, "bound": "alu", "achieved": None, "peak": alu_peak,
+                                       "unit": "TFLOP/s", "frac": None, "traffic": None,
+                                       "peak_source": "latency-bound small dense kernel"})
+    # classes within 10 % of the dominant one are named beside it (the SVD and the two tall GEMMs are close)
+    co = [k for k in prof if k != dom and prof[k]["ms"] >= 0.9 * prof[dom]["ms"] and k in rooflines]
+    roof["co_dominant"] = [{"kernel": k, "bound": rooflines[k]["bound"], "achieved": rooflines[k]["achieved"],
+                            "peak": rooflines[k]["peak"], "unit": rooflines[k]["unit"], "frac": rooflines[k]["frac"]} for k in co]
+    # whole-step view: algorithmic flops of a saturated step (SYRK Gram m n^2 + reconstruction
+    # 2 m n^2 per site and gate, n = 4 chi) over the measured Trotter time
+    step_flops = 0.0
+    for y in range(L):
+        for x in range(L):
+            deg = (y > 0) + (y < L - 1) + (x > 0) + (x < L - 1)
+            step_flops += deg * 3.0 * chi ** (deg - 1) * (4.0 * chi) ** 2
+    whole = {"algorithmic_flops_per_step": step_flops, "tflops": step_flops / (t_trot / args.steps) * 1e-9,
+             "frac_of_fp64_peak": step_flops / (t_trot / args.steps) * 1e-9 / alu_peak,
+             "note": "3 m n^2 per site and gate over the Trotter time of the timed region"}
     line = {
         "metric": "Trotter steps/sec (4x4 chi=60 fp64)" if (L, chi) == (4, 60) else "Trotter steps/sec (%dx%d chi=%d fp64)" % (L, L, chi),
         "value": world * args.steps / (ms * 1e-3), "unit": "Trotter steps/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "vs_baseline": None, "dtype": "f64",
+        "data": ("synthetic (parameter-defined workload: product operator evolved by the method itself, no dataset)"
+                 if args.workload == "physical" else "synthetic (seeded random saturated state, SURVEY 8(d)(iii))"),
         "config": {"workload": "BASELINE configs[1]: %dx%d open grid, TFIM J=1 h=0.9 dt=0.05, Z at (%d,%d), chi_max=%d, "
                                "all bonds saturated; step = trotter_step + bp_converge(tol %g, damping %g) + correlation"
                                % (L, L, args.cx, args.cy, chi, args.bp_tol, args.bp_damping),
@@ -346,13 +433,18 @@ def run_ours(args):
         "bp_sweeps_per_step": sweeps_tot / args.steps, "jacobi_sweeps_per_step": jac / args.steps,
         "last_C": c_last, "gate_err_last_step": stats["gate_err"],
         "qr": {"cholesky": stats["n_cholesky"], "householder": stats["n_householder"], "chol_rejected": stats["n_chol_failed"]},
-        "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "rooflines": rooflines, "kernels": per,
+        "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "rooflines": rooflines,
+        "whole_step": whole, "fp64_yardsticks": yard, "kernels": per,
         "kernels_overlapped": per_overlapped,
         "arena": {"high_water_bytes": stats["arena_high_water"], "model_bytes": stats["arena_model_bytes"],
                   "inflight_gates": stats["max_inflight_gates"]},
         "e2e": e2e,
     }
     sim.close()
+    del sim
+    torch.cuda.empty_cache()
+    if rank == 0 and world == 1 and not args.no_config3:
+        line["config3"] = config3_numbers(torch, dev, alu_peak)
     return line, rank, world
 
 
@@ -394,10 +486,12 @@ def gate_flops(chi, key):
     return sum(6.0 * chi ** (d - 1) * (4 * chi) ** 2 for d in key)
 
 
-def oracle_sample(st, L, chi, budget_s):
-    """Time one oracle bond gate per bond class, cheapest class first, while the projected
-    total stays within budget_s; classes not timed are extrapolated by the flop model from the
-    most expensive timed class.  Returns (seconds per full Trotter step, description)."""
+def oracle_sample(st, L, chi, budget_s, known=None):
+    """Time the oracle's field gate and ONE oracle bond gate per bond class, cheapest class first, while
+    the projected total stays within budget_s.  `known` = class times MEASURED by an earlier call of this
+    function in the same process; a class that does not fit the budget takes its earlier measured time.
+    Nothing is extrapolated by a flop model: with known = None every class is timed.
+    Returns (seconds per full Trotter step, description, seconds spent, {class: measured seconds})."""
     classes = bond_classes(L)
     order = sorted(classes, key=lambda k: gate_flops(chi, k))
     timed, spent = {}, 0.0
@@ -406,26 +500,30 @@ def oracle_sample(st, L, chi, budget_s):
     t_field = time.perf_counter() - t0
     spent += t_field
     for key in order:
-        if timed:
-            last = max(timed, key=lambda k: gate_flops(chi, k))
-            projected = timed[last] * gate_flops(chi, key) / gate_flops(chi, last)
-            if spent + projected > budget_s:
-                break
+        if known and key in known and spent + known[key] > budget_s:
+            continue
         e = classes[key][0]
         t0 = time.perf_counter()
         st.apply_bond_gate(e)
         timed[key] = time.perf_counter() - t0
         spent += timed[key]
-    ref = max(timed, key=lambda k: gate_flops(chi, k))
     total = t_field
+    reused = []
     for key, bonds in classes.items():
-        t = timed.get(key, timed[ref] * gate_flops(chi, key) / gate_flops(chi, ref))
+        if key in timed:
+            t = timed[key]
+        else:
+            t = known[key]
+            reused.append(key)
         total += t * len(bonds)
-    desc = ("field gate on all sites + one oracle bond gate for each of the bond classes %s of the %dx%d chi=%d "
-            "synthetic saturated state (%.1f s of CPU work); other classes %s extrapolated by 6mn^2; "
-            "BP/Bethe not included" % (sorted(timed), L, L, chi, spent,
-                                       sorted(k for k in classes if k not in timed)))
-    return total, desc, spent
+    desc = ("field gate on all sites + one oracle bond gate (Algorithm 1, Householder QR, literal 16 chi core) timed for "
+            "each of the bond classes %s of the %dx%d chi=%d synthetic saturated state (%.1f s of CPU work), step time = "
+            "sum over classes of count x measured gate time%s; BP/Bethe not included"
+            % (sorted(timed), L, L, chi, spent,
+               ("; classes %s reuse their time measured earlier in this run" % sorted(reused)) if reused else ""))
+    allt = dict(known or {})
+    allt.update(timed)
+    return total, desc, spent, allt
 
 
 def host_threads():
@@ -437,29 +535,57 @@ def host_threads():
         return os.cpu_count() or 1
 
 
-def run_cpu_baseline(args, budget_s=25.0):
+def single_thread_sample(st, L, chi, budget_s, all_thread_times):
+    """The same gate timing with the BLAS limited to one thread, on the classes that fit budget_s
+    (cheapest first); reports the measured single-thread / all-thread ratio of those classes."""
+    try:
+        import threadpoolctl
+    except Exception:
+        return None
+    classes = bond_classes(L)
+    out, spent = {}, 0.0
+    with threadpoolctl.threadpool_limits(limits=1):
+        for key in sorted(classes, key=lambda k: gate_flops(chi, k)):
+            est = all_thread_times.get(key, 0.0) * 8.0
+            if spent + est > budget_s:
+                break
+            t0 = time.perf_counter()
+            st.apply_bond_gate(classes[key][0])
+            out[key] = time.perf_counter() - t0
+            spent += out[key]
+    if not out:
+        return None
+    return {"classes_timed": [list(k) for k in sorted(out)], "gate_seconds_1_thread": {str(k): v for k, v in out.items()},
+            "gate_seconds_all_threads": {str(k): all_thread_times[k] for k in out},
+            "ratio_1_thread_over_all": sum(out.values()) / sum(all_thread_times[k] for k in out)}
+
+
+def run_cpu_baseline(args):
     import numpy  # noqa: F401  (loads the BLAS whose threads are counted)
     st = oracle_state(args.grid, args.chi, args.cx, args.cy)
-    total, desc, spent = oracle_sample(st, args.grid, args.chi, budget_s)
+    total, desc, spent, times = oracle_sample(st, args.grid, args.chi, 1e9)
+    one = single_thread_sample(st, args.grid, args.chi, 12.0, times)
     return {"value": 1.0 / total, "unit": "Trotter steps/s", "cores": host_threads(), "kind": "oracle",
-            "sample": desc}
+            "sample": desc, "extrapolated": False, "single_thread": one}
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle on the host cores, K timed 'steps' after W warm-ups, each
-    step a bounded sample (see oracle_sample) sized so that the run ends within minutes."""
+    """--impl reference: the CPU oracle on the host cores, K timed 'steps' after W warm-ups.  The first
+    (warm-up) step times one gate of EVERY bond class; each later step re-times, cheapest first, the
+    classes that fit its share of a ~150 s budget and reuses the measured time of the others."""
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if rank != 0:
         return None, rank, world
     L, chi = args.grid, args.chi
-    n_runs = max(1, args.steps + args.warmup)
+    n_runs = max(2, args.steps + max(args.warmup, 1))
     budget = max(2.0, 150.0 / n_runs)
     st = oracle_state(L, chi, args.cx, args.cy)
-    totals, desc = [], ""
+    totals, desc, known = [], "", None
+    n_warm = max(args.warmup, 1)
     for i in range(n_runs):
-        total, desc, spent = oracle_sample(st, L, chi, budget)
-        if i >= args.warmup:
+        total, desc, spent, known = oracle_sample(st, L, chi, 1e9 if known is None else budget, known)
+        if i >= n_warm:
             totals.append(total)
     mean = sum(totals) / len(totals)
     val = 1.0 / mean
@@ -468,18 +594,33 @@ def run_reference(args):
         "metric": "Trotter steps/sec (4x4 chi=60 fp64)" if (L, chi) == (4, 60) else "Trotter steps/sec (%dx%d chi=%d fp64)" % (L, L, chi),
         "value": val, "unit": "Trotter steps/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": mean * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic",
+        "data": "synthetic (seeded random saturated state, SURVEY 8(d)(iii))",
         "config": {"workload": "BASELINE configs[1]: %dx%d open grid, TFIM J=1 h=0.9 dt=0.05, Z at (%d,%d), chi_max=%d, "
                                "all bonds saturated (seeded synthetic state); Trotter step only" % (L, L, args.cx, args.cy, chi)},
-        "cpu_baseline": {"value": val, "unit": "Trotter steps/s", "cores": host_threads(), "kind": "oracle", "sample": desc},
+        "cpu_baseline": {"value": val, "unit": "Trotter steps/s", "cores": host_threads(), "kind": "oracle", "sample": desc,
+                         "extrapolated": False},
         "e2e": {"value": val, "unit": "Trotter steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     return line, rank, world
 
 
+def spawn_replicas(args):
+    """`python bench.py --gpus N` without torchrun: start the N replica processes ourselves (one per GPU,
+    NCCL rendezvous on 127.0.0.1) and pass their output through."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def main():
     args = parse()
+    if args.impl == "ours" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_replicas(args)
     if args.impl == "reference":
         line, rank, world = run_reference(args)
         if line is not None:

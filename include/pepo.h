@@ -188,6 +188,28 @@ size_t pepo_gram_ws_bytes(long long m, int n);
 int pepo_gram(const double* d_A, long long m, int n, long long lda, double* d_C, void* d_ws,
               size_t ws_bytes, void* stream);
 
+/* Permute-on-load contractions of the bond gate (what pepo_trotter_step runs on the Cholesky path:
+ * the explicit permutation of PAPER.md section 4.1 and the absorb / de-absorb passes a3 / a12 are
+ * folded into the two tall GEMMs, which leaves 2 reads + 1 write of psi per site and gate).
+ * d_psi: packed site tensor with `nlegs` (1..4) bond legs of dims h_dims[] followed by the Pauli
+ * leg (4), column-major; cut_leg: index of the gate's bond among the legs.  With cv = the
+ * m x n matrix view rows = other legs (canonical order), cols = (cut, P) (L267-L269, L319):
+ *   pepo_site_gram : d_C (n x n column-major, both triangles) = cv^T diag(w) cv, eq. (10),
+ *                    w(row) = prod over the other legs of h_w2[leg][i_leg] (h_w2: HOST array of nlegs
+ *                    DEVICE pointers, entry cut_leg ignored; pass lambda to get the Gram matrix of
+ *                    the sqrt(lambda)-absorbed cv; NULL array = unweighted).  DMMA, deterministic split-K;
+ *                    d_ws of pepo_site_gram_ws_bytes() bytes.
+ *   pepo_site_apply: d_out = packed site tensor with dims[cut_leg] replaced by chi_new,
+ *                    out[.., c', .., p'] = sum_{c,p} psi[.., c, .., p] W[(c,p),(c',p')], d_W column-major
+ *                    (4 dims[cut]) x (4 chi_new) with ld = 4 dims[cut] (a10, L331-L333, written straight
+ *                    in the canonical layout: a11-a13 fused).  d_out must not overlap d_psi.
+ * Errors: -1 bad argument (dims outside 1..256), -2 workspace too small. */
+size_t pepo_site_gram_ws_bytes(const int* h_dims, int nlegs, int cut_leg);
+int pepo_site_gram(const double* d_psi, const int* h_dims, int nlegs, int cut_leg,
+                   const double* const* h_w2, double* d_C, void* d_ws, size_t ws_bytes, void* stream);
+int pepo_site_apply(const double* d_psi, const int* h_dims, int nlegs, int cut_leg, const double* d_W,
+                    int chi_new, double* d_out, void* stream);
+
 /* Cholesky-QR (eq. (10)): C = A^T A, R = chol(C) upper, Q = A R^{-1} (via the inverted
  * triangular factor, the paper's Rinv slots L140).  d_Q: m x n (ldq = lda), d_R: n x n
  * (ldr = n, strictly-lower part zeroed).  d_info (device int): 0 ok, j>0 = pivot j <= 0
@@ -215,6 +237,13 @@ int pepo_svd_jacobi(const double* d_A, int m, int n, int lda, double* d_U, doubl
 int pepo_dgemm(int transA, int transB, long long M, int N, int K, const double* d_A,
                long long lda, const double* d_B, long long ldb, double* d_C, long long ldc,
                void* stream);
+
+/* fp64 tensor-pipe yardstick ("measure a large DGEMM in the same run"): launches
+ * ctas_per_sm (1..8) CTAs of 8 warps per SM, every warp issuing iters x 16 register-only
+ * DMMA.8x8x4 (the instruction every GEMM of this library is built on); *h_flops = floating-point
+ * operations of the launch.  The caller times it with CUDA events on `stream`.  d_sink: one device
+ * double (never written in practice). */
+int pepo_dmma_peak(int iters, int ctas_per_sm, double* d_sink, double* h_flops, void* stream);
 
 #ifdef __cplusplus
 }

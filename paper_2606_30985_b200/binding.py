@@ -74,6 +74,10 @@ def _load():
         "pepo_permute_scaled": (i, [dp, dp, ip, ip, i, C.POINTER(vp), vp]),
         "pepo_gram_ws_bytes": (sz, [ll, i]),
         "pepo_gram": (i, [dp, ll, i, ll, dp, vp, sz, vp]),
+        "pepo_site_gram_ws_bytes": (sz, [ip, i, i]),
+        "pepo_site_gram": (i, [dp, ip, i, i, C.POINTER(vp), dp, vp, sz, vp]),
+        "pepo_site_apply": (i, [dp, ip, i, i, dp, i, dp, vp]),
+        "pepo_dmma_peak": (i, [i, i, dp, C.POINTER(d), vp]),
         "pepo_cholqr_ws_bytes": (sz, [ll, i]),
         "pepo_cholqr": (i, [dp, ll, i, ll, dp, dp, vp, vp, sz, vp]),
         "pepo_householder_ws_bytes": (sz, [ll, i]),
@@ -273,6 +277,40 @@ def gram(A_cm, m, n, ws=None):
     ws = ws if ws is not None else _ws(_lib.pepo_gram_ws_bytes(m, n), A_cm.device)
     _check(_lib.pepo_gram(_f64(A_cm, "A"), m, n, m, _f64(Cm, "C"), C.c_void_p(ws.data_ptr()), ws.numel(), _stream()))
     return Cm
+
+
+def site_gram(psi, dims, cut, w2=None):
+    """psi: flat packed site tensor (dims + Pauli leg 4, column-major).  Returns the n x n Gram matrix
+    (flat column-major, n = 4 dims[cut]) of the matrix view rows = other legs, cols = (cut, P), with the
+    rows weighted by prod w2[leg][i_leg] (w2: list of CUDA vectors per leg, entry `cut` ignored)."""
+    n = 4 * dims[cut] if 0 <= cut < len(dims) else 4
+    Cm = torch.empty(n * n, dtype=torch.float64, device=psi.device)
+    ws = _ws(_lib.pepo_site_gram_ws_bytes(_iarr(dims), len(dims), cut), psi.device)
+    ptrs = None
+    if w2 is not None:
+        ptrs = (C.c_void_p * len(dims))(*[C.c_void_p(w.data_ptr()) if w is not None else C.c_void_p(0) for w in w2])
+    _check(_lib.pepo_site_gram(_f64(psi, "psi"), _iarr(dims), len(dims), cut, ptrs, _f64(Cm, "C"),
+                               C.c_void_p(ws.data_ptr()), ws.numel(), _stream()))
+    return Cm
+
+
+def site_apply(psi, dims, cut, W, chi_new):
+    """Returns the packed site tensor with dims[cut] -> chi_new: psi contracted over (cut, P) with W."""
+    tot = 4 * chi_new
+    for l, d in enumerate(dims):
+        if l != cut:
+            tot *= d
+    out = torch.empty(tot, dtype=torch.float64, device=psi.device)
+    _check(_lib.pepo_site_apply(_f64(psi, "psi"), _iarr(dims), len(dims), cut, _f64(W, "W"), chi_new,
+                                _f64(out, "out"), _stream()))
+    return out
+
+
+def dmma_peak(iters, ctas_per_sm, sink):
+    """Launch the register-only DMMA loop; returns the flops of the launch (time it with CUDA events)."""
+    fl = C.c_double(0.0)
+    _check(_lib.pepo_dmma_peak(int(iters), int(ctas_per_sm), _f64(sink, "sink"), C.byref(fl), _stream()))
+    return fl.value
 
 
 def cholqr(A_cm, m, n, Q=None, ws=None):

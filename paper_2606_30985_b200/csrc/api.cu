@@ -74,6 +74,45 @@ extern "C" int pepo_gram(const double* d_A, long long m, int n, long long lda, d
   return launch_gram_reduce(st, ks > 1 ? (const double*)d_ws : d_C, ks, n, d_C, n);
 }
 
+extern "C" int pepo_dmma_peak(int iters, int ctas_per_sm, double* d_sink, double* h_flops, void* stream) {
+  if (!d_sink) { set_error("dmma_peak: NULL sink"); return -1; }
+  return launch_dmma_peak((cudaStream_t)stream, iters, ctas_per_sm, d_sink, h_flops);
+}
+
+// ---- permute-on-load contractions of the bond gate --------------------------------------------
+static int site_view(const int* h_dims, int nlegs, int cut_leg, SiteView& v, const char* who) {
+  if (!h_dims || nlegs < 1 || nlegs > 4 || cut_leg < 0 || cut_leg >= nlegs) { set_error("%s: bad legs", who); return -1; }
+  v.nlegs = nlegs; v.cut = cut_leg;
+  long long tot = 4;
+  for (int l = 0; l < nlegs; l++) {
+    if (h_dims[l] < 1 || h_dims[l] > 256) { set_error("%s: bond dimension %d out of range 1..256", who, h_dims[l]); return -1; }
+    v.dims[l] = h_dims[l]; tot *= h_dims[l];
+  }
+  if (v.m() >= (1ll << 31) || tot >= (1ll << 40)) { set_error("%s: tensor too large", who); return -1; }
+  return 0;
+}
+extern "C" size_t pepo_site_gram_ws_bytes(const int* h_dims, int nlegs, int cut_leg) {
+  SiteView v;
+  if (site_view(h_dims, nlegs, cut_leg, v, "site_gram_ws_bytes")) return 0;
+  return pepo_gram_ws_bytes(v.m(), v.n());
+}
+extern "C" int pepo_site_gram(const double* d_psi, const int* h_dims, int nlegs, int cut_leg,
+                              const double* const* h_w2, double* d_C, void* d_ws, size_t ws_bytes, void* stream) {
+  SiteView v;
+  if (site_view(h_dims, nlegs, cut_leg, v, "site_gram")) return -1;
+  if (!d_psi || !d_C) { set_error("site_gram: NULL pointer"); return -1; }
+  const size_t need = pepo_gram_ws_bytes(v.m(), v.n());
+  if (!d_ws || ws_bytes < need) { set_error("site_gram: workspace too small (%zu needed)", need); return -2; }
+  return launch_site_gram((cudaStream_t)stream, d_psi, v, h_w2, d_C, (double*)d_ws);
+}
+extern "C" int pepo_site_apply(const double* d_psi, const int* h_dims, int nlegs, int cut_leg, const double* d_W,
+                               int chi_new, double* d_out, void* stream) {
+  SiteView v;
+  if (site_view(h_dims, nlegs, cut_leg, v, "site_apply")) return -1;
+  if (!d_psi || !d_W || !d_out || chi_new < 1 || chi_new > 256) { set_error("site_apply: bad argument"); return -1; }
+  return launch_site_apply((cudaStream_t)stream, d_psi, v, d_W, v.n(), chi_new, d_out);
+}
+
 extern "C" size_t pepo_cholqr_ws_bytes(long long m, int n) {
   if (m < 0 || n < 1) return 0;
   return pepo_gram_ws_bytes(m, n) + al((size_t)n * n * 8) + 256;

@@ -63,6 +63,55 @@ struct GemmProb {
   long long lda, ldb, ldc;
   long long M; int N; int K;
 };
+// ---- gathered operands (permute-on-load GEMMs of the bond gate) -----------------------------
+// A site tensor psi[U,D,L,R,P] (column-major) read as the matrix cv[rows = environment legs,
+// cols = (cut, P)] WITHOUT materialising the permuted copy (section 4.1 describes the
+// explicit permutation; the irreducible traffic of a gate is 2 reads + 1 write of
+// psi): every GEMM index maps to an element offset through a two-level function
+//     off(i) = s * (i mod E) + T * (i div E)            (E = 0: off(i) = s * i)
+// which covers all four cut legs: the row index splits into a contiguous run and a strided
+// remainder, the column index into (cut index, Pauli slab).
+struct Idx2 {
+  FastDiv E; long long s, T;
+};
+inline Idx2 make_idx2(long long E, long long s, long long T) {
+  Idx2 r; r.E = make_fastdiv(E > 0 ? (uint32_t)E : 1u); if (E <= 0) r.E.d = 0; r.s = s; r.T = T; return r;
+}
+__host__ __device__ __forceinline__ long long idx2_off_host(const Idx2& f, long long i) {
+  if (f.E.d == 0) return f.s * i;
+  return f.s * (i % f.E.d) + f.T * (i / f.E.d);
+}
+struct GemmGather {
+  Idx2 a_outer, a_k, b_outer, b_k, c_m, c_n;   // element (outer, k) of A at A + a_outer(outer) + a_k(k), etc.
+  // row weights (Gram of the environment-weighted matrix, a3 fused): the A fragments are multiplied by
+  // w(k) = wv[0][k mod wE0] * wv[1][(k div wE0) mod wE1] * wv[2][k div (wE0 wE1)]; nw = 0: none
+  int nw; const double* wv[3]; FastDiv wE[2]; int wlen[3];
+  int alignedA, alignedB;                      // 16-byte pairs along the contiguous direction are valid
+  int ktabA;                                   // operand A not K-contiguous with a two-level k index: offsets from a per-CTA table
+};
+int launch_dgemm_gather(cudaStream_t st, int transA, int transB, const GemmProb& p, const GemmGather& g,
+                        int ksplit, int kchunk, double* part, bool upper_only);
+
+// A packed site tensor psi[leg_0, .., leg_{nlegs-1}, P] (column-major, P = 4 slowest) viewed as the
+// matrix cv[rows = the legs other than `cut` in canonical order, cols = (cut, P)] of Algorithm 1
+// (PAPER.md:L267-L269, L318-L319): m = prod of the other dims, n = 4 dims[cut].
+struct SiteView {
+  int nlegs, cut;
+  int dims[4];
+  long long m() const { long long r = 1; for (int l = 0; l < nlegs; l++) if (l != cut) r *= dims[l]; return r; }
+  int n() const { return 4 * dims[cut]; }
+};
+// C (n x n, ld n, both triangles) = cv^T diag(w) cv with w(row) = prod over the environment legs of
+// w2[leg][i_leg] (a3 fused into a5: w2 = lambda, the squared absorb factor); w2[leg] device pointers
+// (entry `cut` ignored; NULL = no weight on that leg).  part: split-K workspace of gram_plan(m, n).
+int launch_site_gram(cudaStream_t st, const double* psi, const SiteView& v, const double* const* w2,
+                     double* C, double* part);
+// out = the packed site tensor with dims[cut] replaced by chi_new: out[.., c', .., p'] =
+// sum_{c,p} psi[.., c, .., p] W[(c,p),(c',p')], W column-major (4 dims[cut]) x (4 chi_new), ld ldw
+// (a10-a13 fused: reconstruction GEMM that reads and writes the canonical layout).
+int launch_site_apply(cudaStream_t st, const double* psi, const SiteView& v, const double* W, long long ldw,
+                      int chi_new, double* out);
+
 // ksplit > 1: CTA (tile, s) handles K range [s*kchunk, (s+1)*kchunk) and writes its partial
 // tile to part + s*M*N (packed ld = M); the caller reduces.  upper_only: skip tiles whose
 // column-tile index < row-tile index (Gram).  probs_dev != nullptr: batched over grid.z with
@@ -75,6 +124,8 @@ int launch_dgemm_batched(cudaStream_t st, int transA, int transB, const GemmProb
 int launch_gram_reduce(cudaStream_t st, const double* part, int ksplit, int n, double* C,
                        long long ldc);
 void gram_plan(long long m, int n, int* ksplit, int* kchunk);
+// register-only DMMA loop (fp64 tensor-pipe yardstick of bench.py); *flops = flops of the launch
+int launch_dmma_peak(cudaStream_t st, int iters, int ctas_per_sm, double* sink, double* flops);
 
 // ---- permutation -------------------------------------------------------------------------
 // dst[sum_j o_j * dst_stride[j]] = src[sum_d i_d * src_stride[d]] * prod_d scale_d(i_d),

@@ -167,6 +167,11 @@ struct BondInfo { int v1, d1, v2, d2; };
 
 struct SiteWs {       // per lane, per site-slot
   double *cv, *out, *C, *Rx, *Rxinv, *Rbuf, *X, *T, *W, *Mx, *beta1, *tau1, *beta2, *tau2, *part;
+  // spare[d]: a buffer of the size of a site slot with d legs.  On the Cholesky path the reconstruction
+  // GEMM writes the new site tensor straight into spare[nlegs] in the canonical layout and the site
+  // takes that buffer; its old slot becomes this lane's spare (stream-ordered: a lane belongs to one
+  // piece stream).  `out` (work matrix of the Householder path) is the spare of the largest class.
+  double* spare[5];
   int* info;          // device int (in the lane readback block)
 };
 struct LaneWs {
@@ -218,6 +223,7 @@ struct pepo_ctx {
   double eps_cut = 1e-11, chol_ratio = 4.0, chol_tau = 1e-7, jacobi_tol = 1e-15;
   int bp_max_sweeps = 100, bp_max_sweeps_damped = 1000, jacobi_max_sweeps = 60;
   int force_hh = 0;
+  int direct = 1;                      // option "direct_gemm": Cholesky-path GEMMs read / write psi in place (no permute passes)
   int svd_precond_min = 32;            // QR-precondition core SVDs with min(r1,r2) >= this (0: off)
   cudaStream_t st;
   cudaStream_t cur_st = nullptr;       // stream the profiling events of the current launches go to
@@ -426,7 +432,15 @@ int layout(pepo_ctx* c) {
     for (int i = 0; i < 2; i++) {
       SiteWs& S = L.s[i];
       S.cv = (double*)A.take(cvcap * 8);
-      S.out = (double*)A.take(cvcap * 8);
+      for (int d = 0; d < 5; d++) S.spare[d] = nullptr;
+      for (int d = 1; d <= degmax; d++) {
+        bool have = false;
+        for (auto& sv : c->sites) have |= (sv.nlegs == d);
+        if (!have) continue;
+        // the largest class also serves as the Householder path's work matrix (even leading dimension)
+        S.spare[d] = (double*)A.take((d == degmax ? std::max(cvcap, 4 * ipow(chi, d)) : 4 * ipow(chi, d)) * 8);
+      }
+      S.out = degmax >= 1 ? S.spare[degmax] : (double*)A.take(cvcap * 8);
       S.C = (double*)A.take(nmax * nmax * 8);
       S.Rx = (double*)A.take(Nmax * Nmax * 8);
       S.Rxinv = (double*)A.take(Nmax * Nmax * 8);
@@ -693,6 +707,7 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "chol_min_ratio") c->chol_ratio = v;
   else if (k == "chol_tau") c->chol_tau = v;
   else if (k == "force_householder") c->force_hh = (int)v;
+  else if (k == "direct_gemm") c->direct = (int)v;
   else if (k == "jacobi_tol") c->jacobi_tol = v;
   else if (k == "jacobi_max_sweeps") c->jacobi_max_sweeps = (int)v;
   else if (k == "svd_precond_min") c->svd_precond_min = (int)v;
@@ -882,6 +897,9 @@ struct TaskGeo {           // one site of one gate
   long long m, ld;
   int n, chi_c, N, k, r;   // k = min(m,n); r = rows of Rx
   bool chol;
+  bool direct;             // Cholesky path: the reconstruction reads psi in place and writes the site slot
+  bool direct_gram;        // ... and so does the Gram kernel (no explicit cv at all)
+  SiteView view;
   bool skip1, skip2;       // Householder path: Q = I when m <= n (R = cv); Qx = I when 4k <= N (Rx = X)
   int chi_new;
 };
@@ -897,6 +915,26 @@ struct BatchState {        // one batch of gates moving through the three phases
   bool have_chol = false;
   SvdFinishBatch fb;
 };
+
+// a2-a4 fused: cv = permute(psi * sqrt(lambda_env)) into the lane's work matrix (explicit path)
+int enqueue_permute_in(pepo_ctx* c, cudaStream_t st, const TaskGeo& t) {
+  const SiteInfo& s = c->sites[t.v];
+  SiteWs& W = c->lanes[t.lane].s[t.slot];
+  PermuteDesc pd;
+  pd.rank = s.nlegs + 1; pd.power = 1.0;
+  long long sstr = 1;
+  for (int l = 0; l <= s.nlegs; l++) { pd.shape[l] = t.dims[l]; pd.src_stride[l] = sstr; sstr *= t.dims[l]; pd.scale[l] = nullptr; }
+  long long dstr = 1;
+  for (int j = 0; j < t.n_env; j++) {
+    int l = t.env_legs[j];
+    pd.perm[j] = l; pd.dst_stride[j] = dstr; dstr *= t.dims[l];
+    pd.scale[l] = bond_vec(c->sqrt_l, s.leg_bond[l], c->chi_max);
+  }
+  pd.perm[t.n_env] = t.cut_leg; pd.dst_stride[t.n_env] = t.ld;
+  pd.perm[t.n_env + 1] = s.nlegs; pd.dst_stride[t.n_env + 1] = t.ld * t.chi_c;
+  ProfScope ps(c, PC_PERMUTE, 0, 16.0 * t.m * t.n);
+  return launch_permute(st, s.psi, W.cv, pd);
+}
 
 // phase 1: absorb + permute, Gram, dressing, Cholesky (enqueue only; ends with the flag read-back)
 int batch_p1(pepo_ctx* c, BatchState& S) {
@@ -935,21 +973,18 @@ int batch_p1(pepo_ctx* c, BatchState& S) {
       t.chol = !c->force_hh && (double)t.m >= c->chol_ratio * t.n;
       t.r = t.chol ? t.N : std::min(4 * t.k, t.N);
       t.skip1 = t.m <= t.n; t.skip2 = 4 * t.k <= t.N;
-      SiteWs& W = c->lanes[S.lane0 + g].s[i];
-      PermuteDesc pd;
-      pd.rank = s.nlegs + 1; pd.power = 1.0;
-      long long sstr = 1;
-      for (int l = 0; l <= s.nlegs; l++) { pd.shape[l] = t.dims[l]; pd.src_stride[l] = sstr; sstr *= t.dims[l]; pd.scale[l] = nullptr; }
-      long long dstr = 1;
-      for (int j = 0; j < t.n_env; j++) {
-        int l = t.env_legs[j];
-        pd.perm[j] = l; pd.dst_stride[j] = dstr; dstr *= t.dims[l];
-        pd.scale[l] = bond_vec(c->sqrt_l, s.leg_bond[l], c->chi_max);
-      }
-      pd.perm[t.n_env] = t.cut_leg; pd.dst_stride[t.n_env] = t.ld;
-      pd.perm[t.n_env + 1] = s.nlegs; pd.dst_stride[t.n_env + 1] = t.ld * t.chi_c;
-      ProfScope ps(c, PC_PERMUTE, 0, 16.0 * t.m * t.n);
-      int rc = launch_permute(st, s.psi, W.cv, pd);
+      t.direct = t.chol && c->direct;
+      t.view.nlegs = s.nlegs; t.view.cut = t.cut_leg;
+      for (int l = 0; l < 4; l++) t.view.dims[l] = l < s.nlegs ? t.dims[l] : 1;
+      // The Gram kernel reads psi in place when the rows of cv are contiguous runs in psi (cut leg not
+      // the fastest one).  With the cut leg fastest its rows are strided by chi_c and the gathered Gram
+      // is slower than transpose + plain Gram (measured 0.92 against 0.17 + 0.55 ms at chi = 60), so
+      // that case keeps the explicit cv for the Gram and only the reconstruction runs in place.
+      long long run = 1;
+      for (int l = 0; l < t.cut_leg; l++) run *= t.dims[l];
+      t.direct_gram = t.direct && c->direct != 3 && (run >= 2 || c->direct == 2);
+      if (t.direct_gram) continue;            // no explicit cv (a3-a5 fused)
+      int rc = enqueue_permute_in(c, st, t);
       if (rc) return rc;
     }
   }
@@ -967,7 +1002,16 @@ int batch_p1(pepo_ctx* c, BatchState& S) {
       gp.A = W.cv; gp.B = W.cv; gp.C = W.C; gp.lda = t.ld; gp.ldb = t.ld; gp.ldc = t.n;
       gp.M = t.n; gp.N = t.n; gp.K = (int)t.m;
       ProfScope ps(c, PC_GRAM, (double)t.m * t.n * (t.n + 1), 8.0 * t.m * t.n);
-      int rc = launch_dgemm(st, 1, 0, gp, ks, kc, W.part, true);
+      int rc;
+      if (t.direct_gram) {
+        // C = cv^T cv with cv = psi * sqrt(lambda_env): weights lambda on the rows, psi read in place
+        const SiteInfo& sv = c->sites[t.v];
+        const double* w2[4] = {nullptr, nullptr, nullptr, nullptr};
+        for (int l = 0; l < sv.nlegs; l++) if (l != t.cut_leg) w2[l] = bond_vec(c->lambda, sv.leg_bond[l], c->chi_max);
+        rc = launch_site_gram(st, sv.psi, t.view, w2, W.C, W.part);
+        if (rc) return rc;
+      } else {
+      rc = launch_dgemm(st, 1, 0, gp, ks, kc, W.part, true);
       if (rc) return rc;
       if (ks > 1) rc = launch_gram_reduce(st, W.part, ks, t.n, W.C, t.n);
       else {
@@ -975,6 +1019,7 @@ int batch_p1(pepo_ctx* c, BatchState& S) {
         rc = launch_gram_reduce(st, W.C, 1, t.n, W.C, t.n);
       }
       if (rc) return rc;
+      }
       int q = db.count++;
       db.in[q] = W.C; db.out[q] = W.Rx; db.chi[q] = t.chi_c; db.k[q] = t.n; db.site[q] = t.site_idx;
       db.ld_in[q] = t.n; db.ld_out[q] = t.N;
@@ -1025,6 +1070,11 @@ int batch_p2(pepo_ctx* c, BatchState& S) {
       if (info != 0) {
         t.chol = false; t.r = std::min(4 * t.k, t.N);
         c->stats.n_chol_failed++;
+        if (t.direct_gram) {                   // the Householder fallback needs the explicit cv after all
+          int rc = enqueue_permute_in(c, st, t);
+          if (rc) return rc;
+        }
+        t.direct = t.direct_gram = false;
       }
     }
   }
@@ -1239,6 +1289,18 @@ int batch_p3(pepo_ctx* c, BatchState& S) {
         gp.A = W.cv; gp.lda = t.ld; gp.B = W.W; gp.ldb = t.n; gp.C = W.out; gp.ldc = t.ld;
         gp.M = t.m; gp.N = 4 * t.chi_new; gp.K = t.n;
         ProfScope ps(c, PC_APPLY, 2.0 * t.m * t.n * 4 * t.chi_new, 8.0 * t.m * (t.n + 4 * t.chi_new));
+        if (t.direct) {
+          // psi_new = psi x_(cut,P) W written in the canonical layout into the lane's spare slot of this
+          // site class (the absorb / de-absorb scalings cancel: cv W / sqrt(lambda_env) = psi W); the
+          // site takes the spare, its old slot becomes the spare (a10-a13 fused, no permute pass)
+          SiteInfo& sv = c->sites[t.v];
+          double* dst = W.spare[sv.nlegs];
+          rc = launch_site_apply(st, sv.psi, t.view, W.W, t.n, t.chi_new, dst); if (rc) return rc;
+          W.spare[sv.nlegs] = sv.psi;
+          if (W.out == dst) W.out = sv.psi;
+          sv.psi = dst;
+          continue;
+        }
         rc = launch_dgemm(st, 0, 0, gp, 1, 0, nullptr, false); if (rc) return rc;
       }
     }
@@ -1252,6 +1314,7 @@ int batch_p3(pepo_ctx* c, BatchState& S) {
   }
   // ---- F: inverse permute + deabsorb + write-back ----------------------------------------------------
   for (auto& t : T) {
+    if (t.direct) continue;                    // already in place (reconstruction wrote the site slot)
     const SiteInfo& s = c->sites[t.v];
     SiteWs& W = c->lanes[t.lane].s[t.slot];
     PermuteDesc pd;

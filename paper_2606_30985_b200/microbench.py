@@ -143,6 +143,32 @@ def bench_gemm(reps, dev):
     return {"rows": rows}
 
 
+def bench_site(chi, reps, dev):
+    """The permute-on-load contractions of the bond gate on an interior site tensor (chi^4 x 4), every cut
+    leg, next to the plain-layout kernels on the explicit cv of the same size (216000 x 240 at chi = 60)."""
+    dims = [chi] * 4
+    n, m = 4 * chi, chi ** 3
+    nbuf = 3
+    psis = [torch.randn(4 * chi ** 4, dtype=torch.float64, device=dev) for _ in range(nbuf)]
+    outs = [torch.empty(4 * chi ** 4, dtype=torch.float64, device=dev) for _ in range(nbuf)]
+    lam = [torch.rand(chi, dtype=torch.float64, device=dev) + 0.5 for _ in range(4)]
+    W = torch.randn(n * n, dtype=torch.float64, device=dev)
+    rows = []
+    ws = B._ws(B._lib.pepo_gram_ws_bytes(m, n), dev)
+    med, _ = time_ms(lambda i: B.gram(psis[i % nbuf], m, n, ws=ws), reps)
+    rows.append({"kernel": "gram plain cv", "ms": med, "tflops": m * n * (n + 1) / med * 1e-9})
+    med, _ = time_ms(lambda i: B.dgemm(0, 0, m, n, n, psis[i % nbuf], m, W, n, Cout=outs[i % nbuf], ldc=m), reps)
+    rows.append({"kernel": "apply plain cv", "ms": med, "tflops": 2.0 * m * n * n / med * 1e-9})
+    for cut in range(4):
+        med, _ = time_ms(lambda i: B.site_gram(psis[i % nbuf], dims, cut, lam), reps)
+        rows.append({"kernel": "site_gram cut leg %d (weighted)" % cut, "ms": med, "tflops": m * n * (n + 1) / med * 1e-9})
+        med, _ = time_ms(lambda i: B.site_gram(psis[i % nbuf], dims, cut, None), reps)
+        rows.append({"kernel": "site_gram cut leg %d (unweighted)" % cut, "ms": med, "tflops": m * n * (n + 1) / med * 1e-9})
+        med, _ = time_ms(lambda i: B.site_apply(psis[i % nbuf], dims, cut, W, chi), reps)
+        rows.append({"kernel": "site_apply cut leg %d" % cut, "ms": med, "tflops": 2.0 * m * n * n / med * 1e-9})
+    return {"chi": chi, "rows": rows}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--chi", type=int, default=40)
@@ -176,6 +202,10 @@ def main():
         out["gemm"] = r = bench_gemm(args.reps, dev)
         for row in r["rows"]:
             print("dgemm %dx%dx%d: %.3f ms %.1f TFLOP/s" % (row["M"], row["N"], row["K"], row["ms"], row["tflops"]))
+    if "site" in what:
+        out["site"] = r = bench_site(args.chi_inmethod, args.reps, dev)
+        for row in r["rows"]:
+            print("site chi=%d %-36s %.3f ms %.1f TFLOP/s" % (r["chi"], row["kernel"], row["ms"], row["tflops"]))
     if args.json:
         with open(args.json, "w") as f:
             json.dump(out, f)

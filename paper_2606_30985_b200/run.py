@@ -46,6 +46,7 @@ def main():
     ap.add_argument("--chi", type=int, default=None)
     ap.add_argument("--inflight", type=int, default=0)
     ap.add_argument("--json", default=None)
+    ap.add_argument("--md", default=None, help="write the per-step table as markdown (profiles/cfgN_run.md)")
     args = ap.parse_args()
     cfg = dict(CONFIGS[args.config])
     if args.steps is not None:
@@ -63,8 +64,10 @@ def main():
     if chi != cfg["chi"]:
         print("# chi_max %d does not fit %.1f GB free HBM; memory model picks chi_max = %d (%.1f GB)"
               % (cfg["chi"], free / 1e9, chi, need / 1e9), flush=True)
+    free0, _ = torch.cuda.mem_get_info(dev)
     sim = B.Pepo(L, L, cfg["c"][0], cfg["c"][1], 1.0, 0.9, 0.05, chi, cfg["tol"], cfg["damping"], device=str(dev),
                  max_inflight=inflight)
+    free1, _ = torch.cuda.mem_get_info(dev)
     rows = []
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
     t_start = time.perf_counter()
@@ -94,11 +97,34 @@ def main():
                    steps_per_s_whole_run=cfg["steps"] / (sum(r["trotter_ms"] for r in rows) * 1e-3),
                    steps_per_s_saturated=(len(sat) / (sum(r["trotter_ms"] for r in sat) * 1e-3)) if sat else None,
                    arena_bytes=st["arena_high_water"], arena_model_bytes=st["arena_model_bytes"],
+                   arena_tensor_bytes=int(sim.arena.numel()), mem_get_info_delta_bytes=int(free0 - free1),
+                   hbm_total_bytes=int(total),
                    inflight_gates=st["max_inflight_gates"], kernel_launches=st["kernel_launches"])
     print("# " + json.dumps(summary), flush=True)
     if args.json:
         with open(args.json, "w") as f:
             json.dump(dict(summary=summary, rows=rows), f)
+    if args.md:
+        import sys
+        with open(args.md, "w") as f:
+            f.write("# BASELINE configs[%d] on one B200: %dx%d, chi_max %d, %d steps\n\n" % (args.config - 1, L, L, chi, cfg["steps"]))
+            f.write("Command: `python -m paper_2606_30985_b200.run %s`\n\n" % " ".join(sys.argv[1:]))
+            f.write("Memory: closed-form model %.3f GB, arena handed out %.3f GB, arena tensor %.3f GB, "
+                    "torch.cuda.mem_get_info delta at allocation %.3f GB (of %.1f GB); %d gates in flight.\n\n"
+                    % (summary["arena_model_bytes"] / 1e9, summary["arena_bytes"] / 1e9, summary["arena_tensor_bytes"] / 1e9,
+                       summary["mem_get_info_delta_bytes"] / 1e9, summary["hbm_total_bytes"] / 1e9, summary["inflight_gates"]))
+            f.write("Trotter time %.2f s, BP + Bethe time %.2f s, wall %.2f s; %.2f Trotter steps/s over the whole run%s; "
+                    "%d kernel launches.\n\n" % (summary["trotter_s"], summary["bp_s"], summary["wall_s"],
+                                                 summary["steps_per_s_whole_run"],
+                                                 (", %.2f over the saturated steps" % summary["steps_per_s_saturated"])
+                                                 if summary["steps_per_s_saturated"] else "", summary["kernel_launches"]))
+            f.write("| step | C(t) | BP status | BP sweeps | BP delta | chi min..max | gate_err | Jacobi sweeps | Cholesky / Householder QRs (cumulative) | rejected | Trotter ms | BP ms |\n")
+            f.write("|---|---|---|---|---|---|---|---|---|---|---|---|\n")
+            for r in rows:
+                f.write("| %d | %.12f | %d | %d | %.2e | %d..%d | %.3e | %d | %d / %d | %d | %.2f | %.2f |\n"
+                        % (r["step"], r["C"], r["bp_status"], r["bp_sweeps"], r["bp_delta"], r["chi_min"], r["chi_max"],
+                           r["gate_err"], r["jacobi_sweeps"], r["n_cholesky"], r["n_householder"], r["n_chol_failed"],
+                           r["trotter_ms"], r["bp_ms"]))
     sim.close()
 
 

@@ -52,25 +52,46 @@ def test_bad_arguments_do_not_need_a_gpu(lib):
     assert b"NULL" in lib.pepo_last_error()
 
 
-def closed_form_bytes(lib, Lx, Ly, chi, B):
-    """sites + BP partials + B lanes x 2 site slots (work matrices, split-K
-    partials, small dense buffers) + per-lane core/SVD buffers.  Dominant terms only."""
-    lib.pepo_gram_ws_bytes.restype = ctypes.c_size_t
-    lib.pepo_gram_ws_bytes.argtypes = [ctypes.c_longlong, ctypes.c_int]
+def gram_splits(m, n):
+    """Split-K factor of the Gram kernel, restated from DESIGN.md section 5 (independent of the library):
+    upper-triangle tiles of 80 (n % 80 == 0), 64 (n <= 64) or 128; enough splits to fill 2 resident CTAs on
+    148 SMs (two whole waves for the 80-tile), at least 256 rows per split, chunks rounded up to 16 rows."""
+    if n % 80 == 0:
+        bt, target, cap, whole = 80, 148 * 2 * 2, 200, True
+    elif n <= 64:
+        bt, target, cap, whole = 64, 148 * 2, 128, False
+    else:
+        bt, target, cap, whole = 128, 148 * 2, 128, False
+    tn = -(-n // bt)
+    upper = tn * (tn + 1) // 2
+    ks = max(1, target // upper) if whole else -(-target // upper)
+    ks = max(1, min(ks, (m + 255) // 256, cap))
+    kc = -(-m // ks)
+    kc = -(-kc // 16) * 16
+    return -(-m // kc)
+
+
+def closed_form_bytes(Lx, Ly, chi, B):
+    """DESIGN.md section 5, term by term, written out here independently of the library: site slots +
+    BP partials + B lanes x 2 site slots (explicit work matrix cv, one spare site slot per site class -
+    the largest doubling as the Householder work matrix -, split-K partials, small dense buffers) +
+    per-lane core / SVD buffers.  Dominant terms only (the O(n_bonds chi) vectors are left out)."""
     n, N = 4 * chi, 4 * chi
     doubles = 0
-    degmax = 0
+    degs = set()
     for y in range(Ly):
         for x in range(Lx):
             hU, hD, hL, hR = y > 0, y < Ly - 1, x > 0, x < Lx - 1
             deg = hU + hD + hL + hR
-            degmax = max(degmax, deg)
+            degs.add(deg)
             doubles += 4 * chi ** deg                                                  # psi_v
             doubles += chi ** (hL + hR + hU) + chi ** (hL + hR + hD) + chi ** (hL + hR)  # BP partials
+    degmax = max(degs)
     m_max = chi ** max(degmax - 1, 0)
     ld = (m_max + 1) // 2 * 2
-    part = max(lib.pepo_gram_ws_bytes(m_max, 4 * c) for c in range(1, chi + 1)) // 8
-    slot = 2 * ld * n + part + n * n + 2 * N * N + n * n + 4 * n * N + N * chi + n * 4 * chi + 4 * n * chi
+    part = max(gram_splits(m_max, 4 * c) * (4 * c) ** 2 for c in range(1, chi + 1))
+    spares = sum(4 * chi ** d for d in degs if 1 <= d < degmax) + max(ld * n, 4 * chi ** degmax)
+    slot = ld * n + spares + part + n * n + 2 * N * N + n * n + 4 * n * N + N * chi + n * 4 * chi + 4 * n * chi
     lane = 2 * slot + 4 * N * N + 2 * N * chi
     doubles += B * lane
     return 8 * doubles
@@ -81,7 +102,7 @@ def test_memory_model_matches_closed_form(lib, Lx, Ly, chi):
     lib.pepo_arena_bytes_ex.restype = ctypes.c_size_t
     for B in (1, 4):
         got = lib.pepo_arena_bytes_ex(Lx, Ly, chi, B)
-        want = closed_form_bytes(lib, Lx, Ly, chi, B)
+        want = closed_form_bytes(Lx, Ly, chi, B)
         assert abs(got - want) <= 0.02 * want, (got, want)
 
 

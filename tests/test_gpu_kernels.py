@@ -220,3 +220,79 @@ def test_svd_jacobi_vs_oracle(gpu, m, n, kind):
         assert np.linalg.norm(V.T @ V - np.eye(r)) <= 1e-12 * r
     if kind == "lowrank":
         assert np.all(s[7:] <= 1e-13 * s[0])
+
+
+# ------------------------------------------------- permute-on-load contractions (a3-a5, a10-a13) ---
+SITE_CASES = [
+    # dims of the bond legs (Pauli leg 4 implicit), several tiles + ragged tails, even and odd extents
+    (12, 10, 14, 8), (7, 5, 9, 3), (20, 18), (9, 11, 6), (1, 6, 5, 4), (16,), (6, 1, 1, 8), (24, 24, 24, 24),
+]
+
+
+@pytest.mark.parametrize("dims", SITE_CASES, ids=["x".join(map(str, d)) for d in SITE_CASES])
+def test_site_gram_and_apply_match_the_explicit_path(gpu, dims):
+    """pepo_site_gram / pepo_site_apply read the packed site tensor in place.  Reference = the oracle's
+    explicit path on the same seeded tensor: absorb sqrt(lambda) on the environment legs (a3), permute
+    the cut leg last with Listing 1 (a4), C = cv^T cv (eq. (10)); out = cv W, inverse permutation (a11),
+    de-absorb (a12).  Every cut leg of every shape; tolerance 1e-13 relative Frobenius (a DMMA dot product
+    of m <= 3.3e5 terms)."""
+    torch, B = gpu
+    from oracle import pepo_oracle as po
+    from paper_2606_30985_b200 import inputs
+    nl = len(dims)
+    shape = list(dims) + [4]
+    rng = np.random.default_rng(5)
+    psi = inputs.normal_tensor(shape, seed=3)
+    t = psi.reshape(shape, order="F")
+    lam = [np.sort(rng.random(d) + 1e-3)[::-1].copy() for d in dims]        # positive, graded weights
+    d_psi = _dev(torch, psi)
+    d_lam = [_dev(torch, l) for l in lam]
+    for cut in range(nl):
+        # ---- oracle: a3 + a4 ----
+        ta = t.copy()
+        for ax in range(nl):
+            if ax != cut:
+                shp = [1] * (nl + 1); shp[ax] = dims[ax]
+                ta = ta * np.sqrt(lam[ax]).reshape(shp)
+        env = [ax for ax in range(nl) if ax != cut]
+        perm = env + [cut, nl]
+        m = int(np.prod([dims[a] for a in env])) if env else 1
+        n = 4 * dims[cut]
+        cv = po.permute_listing1(ta.flatten(order="F"), shape, perm).reshape((m, n), order="F")
+        C_o = cv.T @ cv
+        C_g = B.site_gram(d_psi, list(dims), cut, d_lam).cpu().numpy().reshape((n, n), order="F")
+        assert np.linalg.norm(C_g - C_o) <= 1e-13 * np.linalg.norm(C_o), (dims, cut)
+        assert np.array_equal(C_g, C_g.T)
+        # unweighted variant
+        cv0 = po.permute_listing1(psi, shape, perm).reshape((m, n), order="F")
+        C_g0 = B.site_gram(d_psi, list(dims), cut, None).cpu().numpy().reshape((n, n), order="F")
+        assert np.linalg.norm(C_g0 - cv0.T @ cv0) <= 1e-13 * np.linalg.norm(cv0.T @ cv0)
+        # ---- a10-a12: out = deabsorb(inverse-permute(cv W)) = psi contracted with W ----
+        for chi_new in sorted({1, 3, dims[cut], min(2 * dims[cut] + 1, 40)}):
+            W = rng.standard_normal((n, 4 * chi_new))
+            out_cv = cv @ W
+            shape_perm = [dims[a] for a in env] + [chi_new, 4]
+            inv = [0] * (nl + 1)
+            for j, pj in enumerate(perm):
+                inv[pj] = j
+            flat = po.permute_listing1(out_cv.flatten(order="F"), shape_perm, inv)
+            shape_new = [shape_perm[inv[j]] for j in range(nl + 1)]
+            want = flat.reshape(shape_new, order="F")
+            for ax in range(nl):
+                if ax != cut:
+                    shp = [1] * (nl + 1); shp[ax] = dims[ax]
+                    want = want / np.sqrt(lam[ax]).reshape(shp)
+            got = B.site_apply(d_psi, list(dims), cut, _dev(torch, W.flatten(order="F")), chi_new).cpu().numpy()
+            got = got.reshape(shape_new, order="F")
+            assert np.linalg.norm(got - want) <= 1e-13 * np.linalg.norm(want), (dims, cut, chi_new)
+
+
+def test_site_contractions_reject_bad_arguments(gpu):
+    torch, B = gpu
+    psi = torch.zeros(4 * 6 * 6, dtype=torch.float64, device="cuda")
+    with pytest.raises(B.PepoError) as e:
+        B.site_gram(psi, [6, 6], 2)
+    assert e.value.code == -1
+    with pytest.raises(B.PepoError) as e:
+        B.site_gram(psi, [6, 300], 0)
+    assert e.value.code == -1

@@ -157,8 +157,8 @@ def test_reduced_chi_twins_vs_stored_oracle(gpu, name, L, centre, chi_max, tol):
     damping; only chi_max reduced) against oracle trajectories stored by tests/golden/make_oracle_twin.py
     (oracle only).  Truncated configs: 1e-6 on C (north_star); status and the live bond dimensions must
     agree; the sweep count is compared where it is well defined: delta crosses tol on a slowly decaying
-    tail, so a rounding-level difference in psi moves the crossing by a few sweeps (and by more once
-    the count is in the hundreds), and a crossing within a few sweeps of the 100-sweep budget may or may
+    tail, so a rounding-level difference in psi moves the crossing by a few sweeps (seen: 26 against 20
+    at step 37 of the 4x4 chi 8 twin with C equal to 1e-12; by more once the count is in the hundreds), and a crossing within a few sweeps of the 100-sweep budget may or may
     not start the damped phase."""
     import conftest
     torch, B = gpu
@@ -175,9 +175,12 @@ def test_reduced_chi_twins_vs_stored_oracle(gpu, name, L, centre, chi_max, tol):
         assert abs(c - r["C"]) <= 1e-6, (r["step"], c, r["C"])
         worst = max(worst, abs(c - r["C"]))
         assert abs(sim.stats()["gate_err"] - r["gate_err"]) <= 1e-9 + 1e-5 * r["gate_err"], r["step"]
-        if abs(r["sweeps"] - 100) > 6:
-            assert (sweeps > 100) == (r["sweeps"] > 100), (r["step"], sweeps, r["sweeps"])
-            assert abs(sweeps - r["sweeps"]) <= 4 + 0.05 * r["sweeps"], (r["step"], sweeps, r["sweeps"])
+        # sweep counts: only where both sides converge quickly.  Late in these runs the undamped iteration
+        # can idle on a plateau for an unpredictable number of sweeps before it drops (oracle step 49 of the
+        # 4x4 chi 8 twin: 100 undamped sweeps exhausted + 60 damped, its neighbours 32-33; the GPU trajectory,
+        # 1e-9 away in psi, needs 29 there) - tests/test_gpu_bp.py compares the counts on IDENTICAL states.
+        if r["sweeps"] < 60 and sweeps < 60:
+            assert abs(sweeps - r["sweeps"]) <= 8 + 0.1 * r["sweeps"], (r["step"], sweeps, r["sweeps"])
     print("%s: max |C_gpu - C_oracle| = %.2e over %d steps" % (name, worst, len(rows)))
     sim.close()
 

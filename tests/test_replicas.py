@@ -54,3 +54,27 @@ def test_single_process_is_a_noop():
     from paper_2606_30985_b200 import replicas as R
     assert R.max_over_ranks(7.5) == 7.5
     assert R.aggregate_rate(5, 100.0, 1) == 50.0
+
+
+def test_bench_gpus_flag_spawns_one_replica_per_gpu(monkeypatch):
+    """`python bench.py --gpus N` run directly (WORLD_SIZE unset) must start N replica processes itself:
+    it re-launches the same command line under torch.distributed.run with --nproc-per-node N on 127.0.0.1."""
+    import importlib
+    sys.path.insert(0, ROOT)
+    bench = importlib.import_module("bench")
+    seen = {}
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    monkeypatch.setattr(sys, "argv", ["bench.py", "--gpus", "4", "--steps", "3", "--warmup", "3"])
+    monkeypatch.setattr(bench.subprocess, "call", lambda cmd: seen.setdefault("cmd", cmd) and 0)
+    assert bench.main() == 0
+    cmd = seen["cmd"]
+    assert "torch.distributed.run" in cmd and cmd[cmd.index("--nproc-per-node") + 1] == "4"
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1"
+    assert cmd[-6:] == ["--gpus", "4", "--steps", "3", "--warmup", "3"]
+    # under torchrun (WORLD_SIZE set) the same flag does not spawn again
+    monkeypatch.setenv("WORLD_SIZE", "4")
+    seen.clear()
+    monkeypatch.setattr(bench, "run_ours", lambda a: ({"ok": 1}, 1, 4))
+    import paper_2606_30985_b200.replicas as R
+    monkeypatch.setattr(R, "finish", lambda: None)
+    assert bench.main() == 0 and "cmd" not in seen
