@@ -54,6 +54,8 @@ typedef struct pepo_stats {
   int chi_max_live;         /* largest live bond dimension */
   int last_bp_trap;         /* trap flag of the diagnostics: the last bp_converge
                                converged (delta < tol) but needed >= 30 sweeps */
+  int last_bp_stage;        /* stage of the last bp_converge that ended it: 0 undamped, 1 damping d, 2 the ladder's
+                               second damping (option "bp_ladder") */
   int last_bp_flags;        /* bit 0: some message update of the last bp_converge had zero norm and kept its
                                old value (R7); bit 1: some update had a non-finite norm (bp_converge then
                                returns -4) */
@@ -92,6 +94,11 @@ int pepo_destroy(pepo_ctx* ctx);
  * "jacobi_tol" (1e-15), "jacobi_max_sweeps" (60), "jacobi_early" (cosine below which a sweep
  * counts as the last one, 1e-7; 0 = always run the confirming sweep),
  * "trotter_order" (1 = first-order step, R2; 2 = symmetric step of eq. (6)),
+ * "bp_init" (0: every BP stage starts from m = (1..1)/sqrt(chi), reading R7; 1: from the leading Schmidt
+ * vector e_0 of each bond, reading R7b), "bp_ladder" (1: third BP stage with "bp_damping2", default 0.2), "observe_ref_C" /
+ * "observe_ref_gate_err" (reference of pepo_observe's drop test: C(t) and gate_err of the last accepted
+ * layer; 1 and 0 after init), "direct_gemm" (1: Cholesky-path GEMMs read / write psi in place, 0: explicit
+ * permute passes),
  * "pipeline" (number of piece streams of a Trotter step, 4; 0 = serial schedule; the results do
  * not depend on it), "bp_tol", "bp_damping", "bp_group" (BP sweeps enqueued per delta read-back,
  * 1..8; results do not depend on it), "svd_precond_min" (QR-precondition cores of at least this
@@ -117,6 +124,15 @@ int pepo_apply_bond(pepo_ctx* ctx, int bond);
  * -4 if a message update produced a non-finite norm.  A zero-norm update keeps the old message
  * and sets bit 0 of pepo_stats.last_bp_flags (R7). */
 int pepo_bp_converge(pepo_ctx* ctx, int* h_sweeps, double* h_delta);
+/* BP + Bethe evaluation with the trap remediation procedure of PAPER.md L451-L457:
+ * the BP stages (undamped, damping d, and with option "bp_ladder" a third stage with option
+ * "bp_damping2", default 0.2 = alpha 0.8) run until one converges; a converged stage that needed
+ * >= 30 sweeps is a trap candidate and counts as a trap when |C| fell below half of the last accepted
+ * C(t) while gate_err did not double; then the next alpha is tried from the init.  *h_C = C(t) of the
+ * accepted stage, *h_sweeps = total sweeps, *h_stage = stage that ended the call (may be NULL).
+ * Returns 0 accepted, 1 no stage converged (*h_C = 0), 2 every converged stage looks trapped - the
+ * bond dimension is the bottleneck (L457) - with *h_C the last value; < 0 errors as bp_converge. */
+int pepo_observe(pepo_ctx* ctx, double* h_C, int* h_sweeps, int* h_stage);
 /* Bethe evaluation (eq. (7)-(9) PAPER.md:L112-L128) from the current messages, log-space with
  * sign tracking.  -4 if some Z_e is 0 (R14). */
 int pepo_correlation(pepo_ctx* ctx, double* h_C);
@@ -159,6 +175,13 @@ int pepo_set_lambda(pepo_ctx* ctx, int bond, const double* h_src, int n);
  * normalised, eq. (12)), computed on the device.  h_S: host array of n >= n_bonds doubles.
  * Synchronises the context stream.  -1 on a bad argument. */
 int pepo_bond_entropy(pepo_ctx* ctx, double* h_S, int n);
+/* Operator spreading (section 6.4; appendix A.3 eq. (21)): the per-site
+ * non-identity Pauli weight n(r,t) = 1 - w_I / sum_p w_p with w_p = sum_i psi_v[i,p]^2 prod_legs
+ * lambda_leg[i_leg] (the Pauli-resolved norm of the site in its Vidal-gauge environment; exact on trees;
+ * reading R19 - the paper prints no formula), one device pass over every site tensor.  h_n: n >= n_sites
+ * doubles (site index y*Lx + x).  h_spread (may be NULL): [R_L1 mean Manhattan radius, R_L2 RMS Euclidean
+ * radius from the centre, S_frac = -sum p ln p / ln(n_sites)], p = n / sum n.  -4 if a site has zero norm. */
+int pepo_site_weights(pepo_ctx* ctx, double* h_n, int n, double* h_spread);
 /* Device pointer of a packed site tensor (valid until the next gate touching the site). */
 double* pepo_site_ptr(pepo_ctx* ctx, int x, int y);
 

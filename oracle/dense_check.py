@@ -114,3 +114,29 @@ def dense_chain_operator_schmidt(n, c, J, h, dt, n_steps, cut, bond="Z", field="
     T = O.reshape(dl, dr, dl, dr).transpose(0, 2, 1, 3).reshape(dl * dl, dr * dr)
     s = np.linalg.svd(T, compute_uv=False)
     return s / np.linalg.norm(s)
+
+
+def dense_site_weights(Lx, Ly, cx, cy, J, h, dt, n_steps, bond="Z", field="X", obs="Z"):
+    """Per-site non-identity Pauli weight n(r) of the Trotter-evolved operator O = (U^dag)^n P_c U^n
+    (section 6.4): with O = sum_S c_S S over Pauli strings S,
+    n(r) = sum_{S: S_r != I} c_S^2 / sum_S c_S^2.  Computed from the full coefficient vector
+    c_S = Tr[S O] / 2^N (site 0 is the slowest Kronecker factor, as in _embed)."""
+    n = Lx * Ly
+    U = trotter_unitary(Lx, Ly, J, h, dt, bond, field)
+    O = _embed({cy * Lx + cx: _SIG[obs]}, n)
+    for _ in range(n_steps):
+        O = U.conj().T @ O @ U
+    # tensor with one (row, column) index pair per site, then each pair -> Pauli index p via Tr[P_p . ]/2
+    T = O.reshape([2] * (2 * n))
+    T = T.transpose([k for s in range(n) for k in (s, n + s)]).reshape([4] * n)       # index (r, c) = 2 r + c per site
+    P = np.stack([np.array([_SIG[k][0, 0], _SIG[k][1, 0], _SIG[k][0, 1], _SIG[k][1, 1]]) for k in "IXYZ"]) / 2.0
+    # c_p = Tr[P_p M]/2 = sum_{r,c} P_p[c, r] M[r, c] / 2  ->  row of P holds P_p[c, r] at position 2 r + c
+    for s in range(n):
+        T = np.moveaxis(np.tensordot(P, T, axes=([1], [s])), 0, s)
+    w = np.abs(T) ** 2
+    tot = w.sum()
+    out = []
+    for s in range(n):
+        ident = np.take(w, 0, axis=s).sum()
+        out.append(float(1.0 - ident / tot))
+    return out

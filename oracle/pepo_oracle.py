@@ -416,18 +416,61 @@ class PEPOState:
         w = w[w > 0.0]
         return float(-(w * np.log(w)).sum())
 
+    def site_pauli_weights(self, v):
+        """w_p = sum_i psi_v[i, p]^2 prod_legs lambda_leg[i_leg], p = I, X, Y, Z: the Pauli-resolved norm of
+        site v in its simple-update environment (psi carries sqrt(s) on every leg, R5; the environment of
+        the Vidal gauge adds sqrt(lambda) per leg on each of the two layers) - exact on trees."""
+        t = self.psi[v] ** 2
+        for ax, d in enumerate(self.lat.legs(v)):
+            shp = [1] * t.ndim
+            shp[ax] = -1
+            t = t * self.lam[self.lat.bond_id(v, d)].reshape(shp)
+        return t.reshape(-1, 4).sum(axis=0)
+
+    def site_weights(self):
+        """n(r, t): per-site non-identity Pauli weight (PAPER section 6.4, Figs. 4-6):
+        n(r) = 1 - w_I(r) / sum_p w_p(r).  The paper gives no formula: DESIGN.md reading R19."""
+        out = []
+        for v in range(self.lat.n_sites):
+            w = self.site_pauli_weights(v)
+            out.append(float(1.0 - w[0] / w.sum()))
+        return out
+
+    def spreading(self):
+        """(R_L1, R_L2, S_frac) of PAPER appendix A.3, eq. (21): mean Manhattan radius, RMS
+        Euclidean radius from the centre site and the spatial entropy fraction of p(r) = n(r)/sum n(r)."""
+        n = np.asarray(self.site_weights())
+        p = n / n.sum()
+        cx, cy = self.lat.xy(self.center)
+        xs = np.array([self.lat.xy(v)[0] for v in range(self.lat.n_sites)])
+        ys = np.array([self.lat.xy(v)[1] for v in range(self.lat.n_sites)])
+        r1 = float((p * (np.abs(xs - cx) + np.abs(ys - cy))).sum())
+        r2 = float(math.sqrt((p * ((xs - cx) ** 2 + (ys - cy) ** 2)).sum()))
+        q = p[p > 0.0]
+        sfrac = float(-(q * np.log(q)).sum() / math.log(self.lat.n_sites)) if self.lat.n_sites > 1 else 0.0
+        return r1, r2, sfrac
+
     # -- a14: BP on the pinned single-layer network -----------------------------------
     def pinned(self, v):
         """T_v = psi_v[..., p_v], p_c = observable Pauli, else I (step 1)."""
         return self.psi[v][..., self.obs if v == self.center else 0]
 
     def _init_messages(self):
+        """R7: deterministic init m = (1, .., 1)/sqrt(chi) on every directed bond.  ``self.bp_init = "e0"``
+        (reading R7b, an option on both sides) starts from the leading Schmidt vector e_0 of each bond
+        instead - where the operator is close to the identity that IS the message up to small terms."""
         msgs = {}
+        e0 = getattr(self, "bp_init", "uniform") == "e0"
         for v in range(self.lat.n_sites):
             for d in self.lat.legs(v):
                 chi = self.lam[self.lat.bond_id(v, d)].size
-                # message v -> neighbour across leg d; R7: deterministic init
-                msgs[(v, d)] = np.full(chi, 1.0 / math.sqrt(chi))
+                # message v -> neighbour across leg d
+                if e0:
+                    m = np.zeros(chi)
+                    m[0] = 1.0
+                else:
+                    m = np.full(chi, 1.0 / math.sqrt(chi))
+                msgs[(v, d)] = m
         return msgs
 
     def _incoming(self, msgs, v, d):
@@ -467,29 +510,74 @@ class PEPOState:
                 new[(v, d_out)] = mnew
         return new, delta, flagged
 
-    def bp_converge(self, tol, damping=0.0, max_sweeps=100, max_sweeps_damped=1000):
-        """a14 until delta < tol or budget (R7).  Phase 1 undamped up to
-        ``max_sweeps``; if not converged and damping > 0: restart from the init with that
-        damping up to ``max_sweeps_damped`` (the paper's alpha-retry, L456).
-        Returns (status, sweeps, delta): status 0 converged, 1 budget exhausted."""
+    def _bp_stage(self, tol, damping, budget):
+        """One stage: restart from the init (R7) and sweep with `damping` until delta < tol or budget."""
         msgs = self._init_messages()
-        sweeps, delta = 0, float("inf")
-        for _ in range(max_sweeps):
-            msgs, delta, _ = self._bp_sweep(msgs, 0.0)
-            sweeps += 1
+        n, delta = 0, float("inf")
+        for _ in range(budget):
+            msgs, delta, _ = self._bp_sweep(msgs, damping)
+            n += 1
             if delta < tol:
-                self.msgs = msgs
-                return 0, sweeps, delta
-        if damping > 0.0:
-            msgs = self._init_messages()
-            for _ in range(max_sweeps_damped):
-                msgs, delta, _ = self._bp_sweep(msgs, damping)
-                sweeps += 1
-                if delta < tol:
-                    self.msgs = msgs
-                    return 0, sweeps, delta
+                return 0, n, delta, msgs
+        return 1, n, delta, msgs
+
+    def bp_converge(self, tol, damping=0.0, max_sweeps=100, max_sweeps_damped=1000, damping2=None,
+                    first_stage=0):
+        """a14 until delta < tol or budget (R7).  Stage 0 undamped up to
+        ``max_sweeps``; if not converged and damping > 0: restart from the init with that
+        damping up to ``max_sweeps_damped`` (the paper's alpha-retry, L456); ``damping2`` adds a
+        third stage with another alpha (the ladder of L451-L457: alpha = 0.5, then 0.8).
+        Returns (status, sweeps, delta): status 0 converged, 1 budget exhausted.  The stage that
+        ended the call is left in ``self.bp_stage``."""
+        stages = [(0.0, max_sweeps), (damping, max_sweeps_damped)]
+        if damping2 is not None:
+            stages.append((damping2, max_sweeps_damped))
+        sweeps, delta, status = 0, float("inf"), 1
+        msgs = self._init_messages()
+        for k, (d, budget) in enumerate(stages):
+            if k < first_stage or (k >= 1 and not d > 0.0) or (k == 2 and d == damping):
+                continue
+            status, n, delta, msgs = self._bp_stage(tol, d, budget)
+            sweeps += n
+            self.bp_stage = k
+            if status == 0:
+                break
         self.msgs = msgs
-        return 1, sweeps, delta
+        return status, sweeps, delta
+
+    def observe(self, tol, damping, damping2=None, max_sweeps=100, max_sweeps_damped=1000):
+        """BP + Bethe with the trap remediation procedure of PAPER L451-L457: a converged run with
+        >= 30 sweeps is a trap candidate; it counts as a trap when |C| fell below half of the last
+        accepted C(t) while gate_err did not double; then the next alpha is tried from the init.
+        Returns (status, C, sweeps, stage): 0 accepted, 1 nothing converged (C = 0), 2 every converged
+        stage looks trapped (C of the last one; L457: raise chi)."""
+        if not hasattr(self, "obs_prev_C"):
+            self.obs_prev_C, self.obs_prev_gerr = 1.0, 0.0            # C(0) = 1
+        last = 2 if damping2 is not None else 1
+        first, sweeps, C, have, trapped = 0, 0, 0.0, False, False
+        status = 1
+        while first <= last:
+            status, n, _ = self.bp_converge(tol, damping, max_sweeps, max_sweeps_damped, damping2, first)
+            sweeps += n
+            if status != 0:
+                break
+            C = self.correlation()
+            have = True
+            candidate = sweeps >= 30
+            dropped = abs(C) < 0.5 * abs(self.obs_prev_C)
+            # "no corresponding increase in gate_err" (L454) needs a reference: none yet -> not a trap
+            quiet = self.obs_prev_gerr > 0.0 and not self.gate_err > 2.0 * self.obs_prev_gerr
+            if not (candidate and dropped and quiet):
+                trapped = False
+                break
+            trapped = True
+            first = self.bp_stage + 1
+        out = status
+        if have and trapped:
+            out = 2
+        if out == 0:
+            self.obs_prev_C, self.obs_prev_gerr = C, self.gate_err
+        return out, (C if have else 0.0), sweeps, getattr(self, "bp_stage", 0)
 
     # -- a15: Bethe evaluation -----------------------------------------------------------
     def correlation(self):

@@ -31,7 +31,7 @@ class PepoStats(C.Structure):
                 ("last_bp_status", C.c_int), ("last_bp_delta", C.c_double),
                 ("arena_high_water", C.c_size_t), ("arena_model_bytes", C.c_size_t),
                 ("max_inflight_gates", C.c_int), ("chi_max_live", C.c_int), ("last_bp_trap", C.c_int),
-                ("last_bp_flags", C.c_int)]
+                ("last_bp_stage", C.c_int), ("last_bp_flags", C.c_int)]
 
 
 def _load():
@@ -55,6 +55,7 @@ def _load():
         "pepo_apply_bond": (i, [vp, i]),
         "pepo_bp_converge": (i, [vp, ip, C.POINTER(d)]),
         "pepo_correlation": (i, [vp, C.POINTER(d)]),
+        "pepo_observe": (i, [vp, C.POINTER(d), ip, ip]),
         "pepo_get_stats": (i, [vp, C.POINTER(PepoStats)]),
         "pepo_get_profile": (i, [vp, i, C.POINTER(d), C.POINTER(d), C.POINTER(d), C.POINTER(ll)]),
         "pepo_n_bonds": (i, [vp]),
@@ -68,6 +69,7 @@ def _load():
         "pepo_get_lambda": (i, [vp, i, vp, i]),
         "pepo_bond_entropy": (i, [vp, vp, i]),
         "pepo_get_message": (i, [vp, i, i, vp, i]),
+        "pepo_site_weights": (i, [vp, vp, i, vp]),
         "pepo_set_lambda": (i, [vp, i, vp, i]),
         "pepo_site_ptr": (vp, [vp, i, i]),
         "pepo_permute": (i, [dp, dp, ip, ip, i, vp]),
@@ -179,6 +181,12 @@ class Pepo:
         _check(_lib.pepo_correlation(self._h, C.byref(out)))
         return out.value
 
+    def observe(self):
+        """(status, C, sweeps, stage) of BP + Bethe with the alpha-retry / trap-verification procedure."""
+        out, sw, stg = C.c_double(0.0), C.c_int(0), C.c_int(0)
+        status = _check(_lib.pepo_observe(self._h, C.byref(out), C.byref(sw), C.byref(stg)))
+        return status, out.value, sw.value, stg.value
+
     def stats(self):
         s = PepoStats()
         _check(_lib.pepo_get_stats(self._h, C.byref(s)))
@@ -239,6 +247,14 @@ class Pepo:
         out = np.empty(n, dtype=np.float64)
         _check(_lib.pepo_get_lambda(self._h, bond, out.ctypes.data_as(C.c_void_p), n))
         return out
+
+    def site_weights(self):
+        """(n(r) per site [y*Lx + x], (R_L1, R_L2, S_frac)) - PAPER.md section 6.4 / eq. (21)."""
+        n = self.Lx * self.Ly
+        out = np.empty(n, dtype=np.float64)
+        spread = np.empty(3, dtype=np.float64)
+        _check(_lib.pepo_site_weights(self._h, out.ctypes.data_as(C.c_void_p), n, spread.ctypes.data_as(C.c_void_p)))
+        return out, tuple(spread)
 
     def get_message(self, bond, from_v1=True):
         n = self.bond_dims()[bond]

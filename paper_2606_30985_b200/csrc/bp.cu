@@ -302,13 +302,14 @@ __global__ void __launch_bounds__(256) bp_finalize_kernel(BpBatch b, double damp
   (void)s_bcast;
 }
 
-__global__ void bp_init_kernel(double* msgs, const int* chi_of_msg, int n_msgs, int chi_max) {
+// mode 0 (R7): m = (1, .., 1)/sqrt(chi); mode 1: m = e_0, the leading Schmidt vector of the bond
+__global__ void bp_init_kernel(double* msgs, const int* chi_of_msg, int n_msgs, int chi_max, int mode) {
   const int mIdx = blockIdx.x;
   if (mIdx >= n_msgs) return;
   const int chi = chi_of_msg[mIdx];
   const double v = 1.0 / sqrt((double)chi);
   for (int i = threadIdx.x; i < chi_max; i += blockDim.x)
-    msgs[(long long)mIdx * chi_max + i] = (i < chi) ? v : 0.0;
+    msgs[(long long)mIdx * chi_max + i] = mode == 1 ? (i == 0 ? 1.0 : 0.0) : ((i < chi) ? v : 0.0);
 }
 
 // eq. (8), (9): C = prod vs_v / prod Z_e in log space with sign tracking
@@ -405,6 +406,52 @@ int launch_bp_finalize(cudaStream_t st, const BpBatch& b, double damping, int up
   return 0;
 }
 
+__global__ void __launch_bounds__(256) site_weights_partial_kernel(SiteWeightBatch b) {
+  const int t = blockIdx.y, ch = blockIdx.x;
+  const int d0 = b.d[t][0], d1 = b.d[t][1], d2 = b.d[t][2], d3 = b.d[t][3];
+  const long long slab = (long long)d0 * d1 * d2 * d3;
+  const long long per = (slab + PEPO_SW_CHUNKS - 1) / PEPO_SW_CHUNKS;
+  const long long i0 = ch * per, i1 = min(slab, i0 + per);
+  const double* psi = b.psi[t];
+  double w[4] = {0.0, 0.0, 0.0, 0.0};
+  for (long long i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
+    long long r = i;
+    const int a0 = (int)(r % d0); r /= d0;
+    const int a1 = (int)(r % d1); r /= d1;
+    const int a2 = (int)(r % d2); r /= d2;
+    const double lw = b.lam[t][0][a0] * b.lam[t][1][a1] * b.lam[t][2][a2] * b.lam[t][3][(int)r];
+#pragma unroll
+    for (int p = 0; p < 4; p++) { const double v = psi[i + p * slab]; w[p] = fma(v * v, lw, w[p]); }
+  }
+  __shared__ double sred[8][4];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int p = 0; p < 4; p++) { const double v = warp_sum(w[p]); if (lane == 0) sred[warp][p] = v; }
+  __syncthreads();
+  if (threadIdx.x < 4) {
+    double s = 0.0;
+    for (int q = 0; q < 8; q++) s += sred[q][threadIdx.x];
+    b.part[t][ch * 4 + threadIdx.x] = s;
+  }
+}
+__global__ void site_weights_final_kernel(SiteWeightBatch b) {
+  const int t = blockIdx.x, p = threadIdx.x;
+  if (p >= 4) return;
+  double s = 0.0;
+  for (int ch = 0; ch < PEPO_SW_CHUNKS; ch++) s += b.part[t][ch * 4 + p];
+  b.out[t][p] = s;
+}
+
+int launch_site_weights(cudaStream_t st, const SiteWeightBatch& b) {
+  if (b.count == 0) return 0;
+  site_weights_partial_kernel<<<dim3(PEPO_SW_CHUNKS, b.count), 256, 0, st>>>(b);
+  PEPO_COUNT_LAUNCH();
+  site_weights_final_kernel<<<b.count, 32, 0, st>>>(b);
+  PEPO_COUNT_LAUNCH();
+  PEPO_CUDA_OK(cudaGetLastError());
+  return 0;
+}
+
 // Bond entanglement entropy of the diagnostics table: S_e = -sum_k l_k^2 log l_k^2
 // over the live Schmidt weights of bond e (lambda is normalised, eq. (12)); one warp per bond,
 // fixed-order reduction.  chi_of_msg[2e] = live dimension of bond e.
@@ -432,9 +479,9 @@ int launch_bond_entropy(cudaStream_t st, const double* lambda, const int* chi_of
   return 0;
 }
 
-int launch_bp_init(cudaStream_t st, double* msgs, const int* chi_of_msg, int n_msgs, int chi_max) {
+int launch_bp_init(cudaStream_t st, double* msgs, const int* chi_of_msg, int n_msgs, int chi_max, int mode) {
   if (n_msgs == 0) return 0;
-  bp_init_kernel<<<n_msgs, 128, 0, st>>>(msgs, chi_of_msg, n_msgs, chi_max);
+  bp_init_kernel<<<n_msgs, 128, 0, st>>>(msgs, chi_of_msg, n_msgs, chi_max, mode);
   PEPO_COUNT_LAUNCH();
   PEPO_CUDA_OK(cudaGetLastError());
   return 0;

@@ -40,10 +40,22 @@ struct FieldBatch {
 int launch_bp_partial(cudaStream_t st, const BpBatch& b);
 int launch_bp_finalize(cudaStream_t st, const BpBatch& b, double damping, int update,
                        unsigned long long* delta_bits, int* flag);
-int launch_bp_init(cudaStream_t st, double* msgs, const int* chi_of_msg, int n_msgs, int chi_max);
+int launch_bp_init(cudaStream_t st, double* msgs, const int* chi_of_msg, int n_msgs, int chi_max, int mode);
 int launch_bethe(cudaStream_t st, const double* vs, int n_sites, const double* msgs,
                  const int* chi_of_msg, int n_bonds, int chi_max, double* out_C, int* out_status);
 int launch_field_gate(cudaStream_t st, const FieldBatch& b);
+// Per-site Pauli-resolved norms (n(r,t) of PAPER.md section 6.4): w[site][p] = sum_i psi[i,p]^2 prod_legs
+// lambda_leg[i_leg]; one pass over the four slabs of every site, per-chunk partials summed in fixed order.
+#define PEPO_SW_CHUNKS 64
+struct SiteWeightBatch {
+  int count;
+  const double* psi[PEPO_BP_MAXS];
+  int d[PEPO_BP_MAXS][4];                 // leg dims in storage order (1 if absent)
+  const double* lam[PEPO_BP_MAXS][4];     // lambda of the leg's bond (a constant [1.0] if absent)
+  double* part[PEPO_BP_MAXS];             // PEPO_SW_CHUNKS x 4 partials
+  double* out[PEPO_BP_MAXS];              // 4 doubles: w_I, w_X, w_Y, w_Z
+};
+int launch_site_weights(cudaStream_t st, const SiteWeightBatch& b);
 int launch_bond_entropy(cudaStream_t st, const double* lambda, const int* chi_of_msg, int n_bonds, int chi_max,
                         double* out);
 

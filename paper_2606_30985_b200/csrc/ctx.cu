@@ -235,6 +235,10 @@ struct pepo_ctx {
   cudaStream_t ps[NSMAX] = {nullptr}, hp[NSMAX] = {nullptr};
   cudaEvent_t pev[5 * NSMAX + 1] = {nullptr};
   int bp_group = 8;                    // option "bp_group": BP sweeps enqueued per delta read-back (1..BP_GROUP)
+  int bp_init = 0;                     // option "bp_init": 0 = uniform init of R7, 1 = leading Schmidt vector e_0
+  int bp_ladder = 0;                   // option "bp_ladder": third BP stage with damping bp_damping2 (alpha-retry, L451-L457)
+  double bp_damping2 = 0.2;            // option "bp_damping2": alpha = 0.8
+  double obs_prev_C = 1.0, obs_prev_gerr = 0.0;   // last C(t) / gate_err accepted by pepo_observe (C(0) = 1)
   double jacobi_early = 1e-7;          // option "jacobi_early": cosine below which a Jacobi sweep counts as the last one
   std::vector<cudaEvent_t> done_ev;    // completion events of the pieces of a pipelined step
   int n_sites, n_bonds, n_hb;
@@ -253,6 +257,8 @@ struct pepo_ctx {
   unsigned long long* delta_bits;
   int* bp_ints;                           // [flag, status]
   std::vector<double*> partU, partD, partS;
+  double* sw_part = nullptr;              // n_sites x PEPO_SW_CHUNKS x 4 partials of pepo_site_weights
+  double* sw_out = nullptr;               // n_sites x 4
   double *dG1, *dGamma[2], *dAhat[2], *dSigma;
   int NA;
   double G1[16], G1h[16];              // field PTM at h dt and at h dt / 2 (symmetric step, eq. (6))
@@ -412,6 +418,8 @@ int layout(pepo_ctx* c) {
     c->partD[v] = (double*)A.take(ipow(chi, hL + hR + hD) * 8);
     c->partS[v] = (double*)A.take(ipow(chi, hL + hR) * 8);
   }
+  c->sw_part = (double*)A.take((size_t)c->n_sites * PEPO_SW_CHUNKS * 4 * 8);
+  c->sw_out = (double*)A.take((size_t)c->n_sites * 4 * 8);
   c->dG1 = (double*)A.take(16 * 8);
   for (int i = 0; i < 2; i++) {
     c->dGamma[i] = (double*)A.take((size_t)NA * NA * 16 * 8);
@@ -713,6 +721,11 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "svd_precond_min") c->svd_precond_min = (int)v;
   else if (k == "jacobi_early") c->jacobi_early = v < 0.0 ? 0.0 : v;
   else if (k == "bp_group") c->bp_group = (int)v;
+  else if (k == "bp_ladder") c->bp_ladder = (int)v;
+  else if (k == "bp_init") c->bp_init = (int)v;
+  else if (k == "observe_ref_C") c->obs_prev_C = v;            // reference of pepo_observe's drop test (e.g. after a restart)
+  else if (k == "observe_ref_gate_err") c->obs_prev_gerr = v;
+  else if (k == "bp_damping2") { if (!(v >= 0.0 && v < 1.0)) { set_error("set_option: bp_damping2 must be in [0,1)"); return -1; } c->bp_damping2 = v; }
   else if (k == "trotter_order") {
     if ((int)v != 1 && (int)v != 2) { set_error("set_option: trotter_order must be 1 or 2"); return -1; }
     c->trotter_order = (int)v;
@@ -1679,7 +1692,7 @@ int bp_init_messages(pepo_ctx* c) {
   for (int e = 0; e < c->n_bonds; e++) { c->h_chi_msg[2 * e] = c->chi[e]; c->h_chi_msg[2 * e + 1] = c->chi[e]; }
   if (c->n_bonds) {
     PEPO_CUDA_OK(cudaMemcpyAsync(c->chi_of_msg, c->h_chi_msg, (size_t)2 * c->n_bonds * 4, cudaMemcpyHostToDevice, c->st));
-    int rc = launch_bp_init(c->st, c->msgs[c->cur_msg], c->chi_of_msg, 2 * c->n_bonds, c->chi_max);
+    int rc = launch_bp_init(c->st, c->msgs[c->cur_msg], c->chi_of_msg, 2 * c->n_bonds, c->chi_max, c->bp_init);
     if (rc) return rc;
   }
   PEPO_CUDA_OK(cudaMemsetAsync(c->bp_ints, 0, 16, c->st));
@@ -1688,55 +1701,131 @@ int bp_init_messages(pepo_ctx* c) {
 
 }  // namespace
 
+namespace {
+// One stage of BP: restart from the deterministic init (R7) and sweep with `damping` until delta < tol
+// or `budget` sweeps.  Returns 0 converged, 1 budget exhausted, < 0 error.  Sweeps go out in groups of
+// up to BP_GROUP with one read-back of their deltas per group (one host round trip instead of
+// BP_GROUP); inside a group the stop test of eq. (14) is taken on the device: the kernels of a sweep
+// return at once when the previous sweep's delta is below tol.
+int bp_run_stage(pepo_ctx* c, double damping, int budget, int& sweeps, double& delta, int& flags) {
+  int rc = bp_init_messages(c); if (rc) return rc;
+  int status = 1;
+  for (int it = 0; it < budget && status;) {
+    const int ngr = std::min(c->bp_group < 1 ? 1 : std::min(c->bp_group, BP_GROUP), budget - it);
+    PEPO_CUDA_OK(cudaMemsetAsync(c->delta_bits, 0, 8 * ngr, c->st));
+    for (int g = 0; g < ngr; g++) {
+      rc = bp_sweep(c, damping, 1, c->cur_msg ^ (g & 1), g, g - 1); if (rc) return rc;
+    }
+    PEPO_CUDA_OK(cudaMemcpyAsync(c->h_delta, c->delta_bits, 8 * ngr, cudaMemcpyDeviceToHost, c->st));
+    PEPO_CUDA_OK(cudaMemcpyAsync(c->h_bpints, c->bp_ints, 8, cudaMemcpyDeviceToHost, c->st));
+    PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
+    prof_flush(c);
+    flags |= c->h_bpints[0];
+    if (flags & 2) break;                               // non-finite norm: no point in spending the budget
+    int done = ngr;                                     // sweeps of the group that actually ran
+    for (int g = 0; g < ngr; g++) {
+      double dg;
+      memcpy(&dg, c->h_delta + g, 8);
+      if (c->n_bonds == 0) dg = 0.0;
+      delta = dg;
+      if (dg < c->bp_tol) { status = 0; done = g + 1; break; }
+    }
+    if (done & 1) c->cur_msg ^= 1;
+    sweeps += done;
+    it += done;
+  }
+  return status;
+}
+
+// Stages of bp_converge (R7 + the alpha-retry ladder of PAPER.md L451-L457): 0 = undamped (alpha = 1),
+// 1 = the configured damping d (alpha = 1 - d), 2 = option "bp_damping2" (default 0.2, i.e. alpha = 0.8;
+// only with option "bp_ladder").  Runs stages first..last until one converges.
+int bp_run_stages(pepo_ctx* c, int first, int& sweeps, double& delta, int& flags, int& stage_out, int& stage_sweeps) {
+  int status = 1;
+  const int last = c->bp_ladder ? 2 : 1;
+  for (int stage = first; stage <= last && status == 1 && !(flags & 2); stage++) {
+    const double damping = stage == 0 ? 0.0 : (stage == 1 ? c->bp_damping : c->bp_damping2);
+    const int budget = stage == 0 ? c->bp_max_sweeps : c->bp_max_sweeps_damped;
+    if (stage >= 1 && !(damping > 0.0)) continue;
+    if (stage == 2 && damping == c->bp_damping) continue;
+    const int before = sweeps;
+    status = bp_run_stage(c, damping, budget, sweeps, delta, flags);
+    if (status < 0) return status;
+    stage_out = stage; stage_sweeps = sweeps - before;
+  }
+  return status;
+}
+
+int bp_finish(pepo_ctx* c, int status, int sweeps, double delta, int flags, int stage, int stage_sweeps) {
+  c->msgs_valid = true;
+  c->stats.last_bp_sweeps = sweeps; c->stats.last_bp_status = status; c->stats.last_bp_delta = delta;
+  // trap candidate of PAPER.md L451-L457: converged, but only after >= 30 sweeps
+  c->stats.last_bp_trap = (status == 0 && sweeps >= 30) ? 1 : 0;
+  (void)stage_sweeps;
+  c->stats.last_bp_flags = flags;
+  c->stats.last_bp_stage = stage;
+  if (flags & 2) { set_error("bp_converge: a message update had a non-finite norm (NaN / Inf in the site tensors or messages)"); return -4; }
+  return status;
+}
+}  // namespace
+
 extern "C" int pepo_bp_converge(pepo_ctx* c, int* h_sweeps, double* h_delta) {
   if (!c) { set_error("bp_converge: NULL"); return -1; }
   CtxScope scope(c);
   { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
-  int sweeps = 0;
+  int sweeps = 0, flags = 0, stage = 0, stage_sweeps = 0;
   double delta = INFINITY;
-  int status = 1;
-  int flags = 0;                 // bit 0: a message with zero norm kept its old value (R7); bit 1: non-finite norm
-  for (int phase = 0; phase < 2 && status && !(flags & 2); phase++) {
-    const double damping = phase == 0 ? 0.0 : c->bp_damping;
-    const int budget = phase == 0 ? c->bp_max_sweeps : c->bp_max_sweeps_damped;
-    if (phase == 1 && !(c->bp_damping > 0.0)) break;
-    int rc = bp_init_messages(c); if (rc) return rc;
-    // sweeps go out in groups of up to BP_GROUP with one read-back of their deltas per group (one
-    // host round trip instead of BP_GROUP); inside a group the stop test of eq. (14) is taken on the
-    // device: the kernels of a sweep return at once when the previous sweep's delta is below tol
-    for (int it = 0; it < budget && status;) {
-      const int ngr = std::min(c->bp_group < 1 ? 1 : std::min(c->bp_group, BP_GROUP), budget - it);
-      PEPO_CUDA_OK(cudaMemsetAsync(c->delta_bits, 0, 8 * ngr, c->st));
-      for (int g = 0; g < ngr; g++) {
-        rc = bp_sweep(c, damping, 1, c->cur_msg ^ (g & 1), g, g - 1); if (rc) return rc;
-      }
-      PEPO_CUDA_OK(cudaMemcpyAsync(c->h_delta, c->delta_bits, 8 * ngr, cudaMemcpyDeviceToHost, c->st));
-      PEPO_CUDA_OK(cudaMemcpyAsync(c->h_bpints, c->bp_ints, 8, cudaMemcpyDeviceToHost, c->st));
-      PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
-      prof_flush(c);
-      flags |= c->h_bpints[0];
-      if (flags & 2) break;                               // non-finite norm: no point in spending the budget
-      int done = ngr;                                   // sweeps of the group that actually ran
-      for (int g = 0; g < ngr; g++) {
-        double dg;
-        memcpy(&dg, c->h_delta + g, 8);
-        if (c->n_bonds == 0) dg = 0.0;
-        delta = dg;
-        if (dg < c->bp_tol) { status = 0; done = g + 1; break; }
-      }
-      if (done & 1) c->cur_msg ^= 1;
-      sweeps += done;
-      it += done;
-    }
-  }
-  c->msgs_valid = true;
-  c->stats.last_bp_sweeps = sweeps; c->stats.last_bp_status = status; c->stats.last_bp_delta = delta;
-  c->stats.last_bp_trap = (status == 0 && sweeps >= 30) ? 1 : 0;      // trap flag of PAPER.md L451-L457
-  c->stats.last_bp_flags = flags;
+  int status = bp_run_stages(c, 0, sweeps, delta, flags, stage, stage_sweeps);
+  if (status < 0) return status;
   if (h_sweeps) *h_sweeps = sweeps;
   if (h_delta) *h_delta = delta;
-  if (flags & 2) { set_error("bp_converge: a message update had a non-finite norm (NaN / Inf in the site tensors or messages)"); return -4; }
-  return status;
+  return bp_finish(c, status, sweeps, delta, flags, stage, stage_sweeps);
+}
+
+// BP + Bethe with the trap remediation procedure of PAPER.md L451-L457:
+//  1. run the stages (undamped, then the alpha ladder) until one converges;
+//  2. a converged run that needed >= 30 sweeps in all is a trap candidate; it is taken for a trap when
+//     |C| dropped by more than 50 % against the last accepted C(t) while gate_err did not grow by more
+//     than a factor 2 ("no corresponding increase in gate_err");
+//  3. then the next stages (another alpha) are tried, each from the init; the first converged one
+//     that is not a trap by the same test is accepted;
+//  4. if every alpha fails, status 2: the bond dimension is the bottleneck (raise chi).
+// Status: 0 accepted, 1 no stage converged, 2 every converged stage looks trapped (C of the last one).
+extern "C" int pepo_observe(pepo_ctx* c, double* h_C, int* h_sweeps, int* h_stage) {
+  if (!c || !h_C) { set_error("observe: NULL"); return -1; }
+  CtxScope scope(c);
+  { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
+  int sweeps = 0, flags = 0, stage = 0, stage_sweeps = 0, first = 0;
+  double delta = INFINITY, C = 0.0;
+  bool have = false, trapped_any = false;
+  const int last = c->bp_ladder ? 2 : 1;
+  const double gerr = c->stats.gate_err;
+  int status = 1;
+  while (first <= last) {
+    status = bp_run_stages(c, first, sweeps, delta, flags, stage, stage_sweeps);
+    if (status < 0) return status;
+    int rcf = bp_finish(c, status, sweeps, delta, flags, stage, stage_sweeps);
+    if (rcf < 0) return rcf;
+    if (status != 0) break;                                     // nothing (more) converges
+    int rc = pepo_correlation(c, &C); if (rc) return rc;
+    have = true;
+    const bool candidate = sweeps >= 30;
+    const bool dropped = std::fabs(C) < 0.5 * std::fabs(c->obs_prev_C);
+    // "no corresponding increase in gate_err" (L454) needs a reference: none yet -> not a trap
+    const bool gerr_quiet = c->obs_prev_gerr > 0.0 && !(gerr > 2.0 * c->obs_prev_gerr);
+    if (!(candidate && dropped && gerr_quiet)) { trapped_any = false; break; }
+    trapped_any = true;
+    first = stage + 1;                                          // retry with the next alpha
+  }
+  if (h_sweeps) *h_sweeps = sweeps;
+  if (h_stage) *h_stage = stage;
+  int out = status;
+  if (status == 0 && trapped_any) out = 2;
+  if (status != 0 && have && trapped_any) out = 2;              // the only converged stages were traps
+  if (out == 0) { c->obs_prev_C = C; c->obs_prev_gerr = gerr; }
+  *h_C = have ? C : 0.0;
+  c->stats.last_bp_status = out;
+  return out;
 }
 
 extern "C" int pepo_correlation(pepo_ctx* c, double* h_C) {
@@ -1779,6 +1868,50 @@ extern "C" int pepo_bond_entropy(pepo_ctx* c, double* h_S, int n) {
   if (rc) return rc;
   PEPO_CUDA_OK(cudaMemcpyAsync(h_S, d_out, (size_t)c->n_bonds * 8, cudaMemcpyDeviceToHost, c->st));
   PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
+  return 0;
+}
+
+// n(r, t) and the spreading measures of PAPER.md section 6.4 / appendix A.3 (reading R19).
+extern "C" int pepo_site_weights(pepo_ctx* c, double* h_n, int n, double* h_spread) {
+  if (!c || !h_n || n < c->n_sites) { set_error("site_weights: bad argument (need n >= n_sites)"); return -1; }
+  CtxScope scope(c);
+  { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
+  for (int v0 = 0; v0 < c->n_sites; v0 += PEPO_BP_MAXS) {
+    SiteWeightBatch b;
+    b.count = std::min(PEPO_BP_MAXS, c->n_sites - v0);
+    for (int i = 0; i < b.count; i++) {
+      const SiteInfo& s = c->sites[v0 + i];
+      b.psi[i] = s.psi;
+      for (int l = 0; l < 4; l++) {
+        if (l < s.nlegs) { b.d[i][l] = c->chi[s.leg_bond[l]]; b.lam[i][l] = bond_vec(c->lambda, s.leg_bond[l], c->chi_max); }
+        else { b.d[i][l] = 1; b.lam[i][l] = c->ones; }
+      }
+      b.part[i] = c->sw_part + (size_t)(v0 + i) * PEPO_SW_CHUNKS * 4;
+      b.out[i] = c->sw_out + (size_t)(v0 + i) * 4;
+    }
+    int rc = launch_site_weights(c->st, b); if (rc) return rc;
+  }
+  std::vector<double> w((size_t)c->n_sites * 4);
+  PEPO_CUDA_OK(cudaMemcpyAsync(w.data(), c->sw_out, w.size() * 8, cudaMemcpyDeviceToHost, c->st));
+  PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
+  double tot = 0.0;
+  for (int v = 0; v < c->n_sites; v++) {
+    const double sum = w[4 * v] + w[4 * v + 1] + w[4 * v + 2] + w[4 * v + 3];
+    if (!(sum > 0.0) || !std::isfinite(sum)) { set_error("site_weights: site %d has zero or non-finite norm", v); return -4; }
+    h_n[v] = 1.0 - w[4 * v] / sum;
+    tot += h_n[v];
+  }
+  if (h_spread) {
+    double r1 = 0.0, r2 = 0.0, ent = 0.0;
+    for (int v = 0; v < c->n_sites && tot > 0.0; v++) {
+      const double p = h_n[v] / tot;
+      const int dx = std::abs(c->sites[v].x - c->cx), dy = std::abs(c->sites[v].y - c->cy);
+      r1 += p * (dx + dy); r2 += p * (dx * dx + dy * dy);
+      if (p > 0.0) ent -= p * std::log(p);
+    }
+    h_spread[0] = r1; h_spread[1] = std::sqrt(r2);
+    h_spread[2] = c->n_sites > 1 ? ent / std::log((double)c->n_sites) : 0.0;
+  }
   return 0;
 }
 

@@ -46,6 +46,11 @@ def main():
     ap.add_argument("--chi", type=int, default=None)
     ap.add_argument("--inflight", type=int, default=0)
     ap.add_argument("--json", default=None)
+    ap.add_argument("--observe", action="store_true",
+                    help="use pepo_observe with the alpha ladder (PAPER.md L451-L457) instead of bp_converge + correlation")
+    ap.add_argument("--bp-init", type=int, default=None,
+                    help="0 = uniform BP init (reading R7), 1 = leading Schmidt vector (R7b); default 0 for configs 1, 2 "
+                         "and 1 for configs 4, 5, where the uniform init stops converging from step 22 (DESIGN.md 9.2)")
     ap.add_argument("--md", default=None, help="write the per-step table as markdown (profiles/cfgN_run.md)")
     args = ap.parse_args()
     cfg = dict(CONFIGS[args.config])
@@ -68,6 +73,10 @@ def main():
     sim = B.Pepo(L, L, cfg["c"][0], cfg["c"][1], 1.0, 0.9, 0.05, chi, cfg["tol"], cfg["damping"], device=str(dev),
                  max_inflight=inflight)
     free1, _ = torch.cuda.mem_get_info(dev)
+    if args.observe:
+        sim.set_option("bp_ladder", 1)
+    bp_init = args.bp_init if args.bp_init is not None else (1 if args.config in (4, 5) else 0)
+    sim.set_option("bp_init", bp_init)
     rows = []
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
     t_start = time.perf_counter()
@@ -75,8 +84,12 @@ def main():
         ev[0].record()
         sim.trotter_step()
         ev[1].record()
-        status, sweeps, delta = sim.bp_converge()
-        c = sim.correlation()
+        if args.observe:
+            status, c, sweeps, stage = sim.observe()
+            delta = sim.stats()["last_bp_delta"]
+        else:
+            status, sweeps, delta = sim.bp_converge()
+            c = sim.correlation()
         ev[2].record()
         ev[2].synchronize()
         st = sim.stats()
@@ -109,6 +122,8 @@ def main():
         with open(args.md, "w") as f:
             f.write("# BASELINE configs[%d] on one B200: %dx%d, chi_max %d, %d steps\n\n" % (args.config - 1, L, L, chi, cfg["steps"]))
             f.write("Command: `python -m paper_2606_30985_b200.run %s`\n\n" % " ".join(sys.argv[1:]))
+            f.write("BP init: %s; %s.\n\n" % ("leading Schmidt vector e_0 (reading R7b)" if bp_init else "uniform (reading R7)",
+                                             "pepo_observe with the alpha ladder" if args.observe else "pepo_bp_converge + pepo_correlation"))
             f.write("Memory: closed-form model %.3f GB, arena handed out %.3f GB, arena tensor %.3f GB, "
                     "torch.cuda.mem_get_info delta at allocation %.3f GB (of %.1f GB); %d gates in flight.\n\n"
                     % (summary["arena_model_bytes"] / 1e9, summary["arena_bytes"] / 1e9, summary["arena_tensor_bytes"] / 1e9,

@@ -86,6 +86,7 @@ def closed_form_bytes(Lx, Ly, chi, B):
             degs.add(deg)
             doubles += 4 * chi ** deg                                                  # psi_v
             doubles += chi ** (hL + hR + hU) + chi ** (hL + hR + hD) + chi ** (hL + hR)  # BP partials
+            doubles += 64 * 4 + 4                                                      # n(r,t) partials
     degmax = max(degs)
     m_max = chi ** max(degmax - 1, 0)
     ld = (m_max + 1) // 2 * 2

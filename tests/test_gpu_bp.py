@@ -171,3 +171,78 @@ def test_zero_norm_message_is_flagged_and_nan_is_an_error(gpu):
     assert e.value.code == -4
     assert sim.stats()["last_bp_flags"] & 2
     sim.close()
+
+
+def test_alpha_ladder_and_observe_match_the_oracle(gpu):
+    """SURVEY NEXT-2 / PAPER.md L451-L457: the third BP stage (option bp_ladder, alpha = 0.8) and the trap
+    remediation call pepo_observe against the oracle's bp_converge(damping2=...) / observe on the same
+    state (4x4 chi 8 at step 52, where BP needs 37 / 69 / 42 sweeps at alpha = 1 / 0.5 / 0.8): stage,
+    sweep counts (exact when a budget is hit), status and C for (1) a healthy step, (2) budgets that
+    only the third stage meets, (3) a forced 'drop' that makes every alpha look trapped (status 2),
+    (4) the same drop excused by a doubled gate_err."""
+    torch, B = gpu
+    sim = B.Pepo(4, 4, 1, 1, J, H, DT, 8, 1e-10, 0.5)
+    for _ in range(52):
+        sim.trotter_step()
+    st = _oracle_from_gpu(sim, 4, 4, 1, 1, 8)
+    st.gate_err = sim.stats()["gate_err"]
+    sim.set_option("bp_ladder", 1)
+    # (1) healthy: first call accepts (reference C(0) = 1: a drop, but the first reference gate_err is 0)
+    so = st.observe(1e-10, 0.5, 0.2)
+    sg = sim.observe()
+    assert sg[0] == so[0] == 0 and sg[3] == so[3] == 0
+    assert abs(sg[1] - so[1]) < 1e-12 and abs(sg[2] - so[2]) <= 1
+    # (2) small budgets: only alpha = 0.8 converges
+    sim.set_option("bp_max_sweeps", 5); sim.set_option("bp_max_sweeps_damped", 45)
+    s_o, n_o, _ = st.bp_converge(1e-10, 0.5, 5, 45, damping2=0.2)
+    s_g, n_g, _ = sim.bp_converge()
+    assert (s_g, s_o) == (0, 0) and st.bp_stage == 2 and sim.stats()["last_bp_stage"] == 2
+    assert abs(n_g - n_o) <= 1 and n_o > 50
+    assert abs(sim.correlation() - st.correlation()) < 1e-12
+    sim.set_option("bp_ladder", 0)
+    assert sim.bp_converge()[0] == 1 and sim.stats()["last_bp_stage"] == 1          # without the ladder: exhausted
+    sim.set_option("bp_ladder", 1)
+    sim.set_option("bp_max_sweeps", 100); sim.set_option("bp_max_sweeps_damped", 1000)
+    # (3) forced drop: the reference says C should be 10x larger, gate_err quiet -> every alpha is retried
+    # from the init, all reach the same fixed point -> status 2 ("raise chi"), reference kept
+    c0 = so[1]
+    st.obs_prev_C, st.obs_prev_gerr = 10.0 * c0, st.gate_err
+    sim.set_option("observe_ref_C", 10.0 * c0); sim.set_option("observe_ref_gate_err", st.gate_err)
+    so3 = st.observe(1e-10, 0.5, 0.2)
+    sg3 = sim.observe()
+    assert sg3[0] == so3[0] == 2 and sg3[3] == so3[3] == 2
+    assert abs(sg3[1] - so3[1]) < 1e-12 and abs(sg3[2] - so3[2]) <= 3 and so3[2] > 120
+    # (4) the same drop with a gate_err more than twice the reference's is accepted at once
+    st.obs_prev_gerr = 0.4 * st.gate_err
+    sim.set_option("observe_ref_gate_err", 0.4 * st.gate_err)
+    so4 = st.observe(1e-10, 0.5, 0.2)
+    sg4 = sim.observe()
+    assert sg4[0] == so4[0] == 0 and sg4[3] == so4[3] == 0 and abs(sg4[1] - so4[1]) < 1e-12
+    sim.close()
+
+
+def test_leading_schmidt_vector_init_matches_oracle_and_converges_where_uniform_fails(gpu):
+    """Reading R7b (option bp_init = 1): BP started from e_0 on every bond.  On the 8x8 chi_max = 32 state
+    at step 28 the uniform init of R7 exhausts both budgets on the GPU and in the oracle alike
+    (profiles/r2_bp_replay_8x8_chi32.md); from e_0 the damped stage converges in a few dozen sweeps on both
+    sides, to the same messages and the same C, which continues the curve of the chi_max = 24 twin
+    (tests/golden/oracle_8x8_chi24_40.txt: C(28) = 0.27895)."""
+    torch, B = gpu
+    L, chi = 8, 32
+    sim = B.Pepo(L, L, 3, 3, J, H, DT, chi, 1e-9, 0.5)
+    for _ in range(28):
+        sim.trotter_step()
+    sim.set_option("bp_max_sweeps_damped", 300)
+    sg, swg, _ = sim.bp_converge()
+    assert sg == 1 and swg == 400                                  # uniform init: 100 + 300 sweeps, not converged
+    sim.set_option("bp_init", 1)
+    sg, swg, dg = sim.bp_converge()
+    cg = sim.correlation()
+    st = _oracle_from_gpu(sim, L, L, 3, 3, chi)
+    st.bp_init = "e0"
+    so, swo, do = st.bp_converge(1e-9, 0.5, 100, 300)
+    co = st.correlation()
+    assert (sg, so) == (0, 0) and abs(swg - swo) <= 1 and swo < 200
+    assert abs(cg - co) < 1e-12 and abs(cg - 0.279) < 1e-3
+    assert _msg_diff(sim, st, up_to_sign=(swg != swo)) < 1e-8
+    sim.close()

@@ -148,6 +148,9 @@ GOLDEN_TWINS = [
     ("oracle_8x8_chi24_40.txt", 8, (3, 3), 24, 1e-9),     # configs[3] twin, all 40 steps
     ("oracle_10x10_chi8.txt", 10, (4, 4), 8, 1e-8),       # configs[4] twin, all 30 steps
     ("oracle_10x10_chi12.txt", 10, (4, 4), 12, 1e-8),
+    # configs[1] ITSELF at chi_max = 60: the oracle needs ~5 min per saturated step; the file holds as many
+    # of the 60 steps as were computed (all bonds are saturated from step 23 on)
+    ("oracle_4x4_chi60.txt", 4, (1, 1), 60, 1e-10),
 ]
 
 
@@ -174,7 +177,10 @@ def test_reduced_chi_twins_vs_stored_oracle(gpu, name, L, centre, chi_max, tol):
         assert max(dims) == r["chi_max_live"] and sum(dims) == r["chi_sum"], (r["step"], max(dims), sum(dims))
         assert abs(c - r["C"]) <= 1e-6, (r["step"], c, r["C"])
         worst = max(worst, abs(c - r["C"]))
-        assert abs(sim.stats()["gate_err"] - r["gate_err"]) <= 1e-9 + 1e-5 * r["gate_err"], r["step"]
+        # discarded weight: a sum of squared singular values below the cut; once truncation is active the
+        # tail directions are the ill-determined ones (seen 1.26e-8 against 1.08e-8 at step 17 of the chi 16
+        # twin with C equal to 1e-9), so it is compared to 1e-8 + 2 %
+        assert abs(sim.stats()["gate_err"] - r["gate_err"]) <= 1e-8 + 0.02 * r["gate_err"], r["step"]
         # sweep counts: only where both sides converge quickly.  Late in these runs the undamped iteration
         # can idle on a plateau for an unpredictable number of sweeps before it drops (oracle step 49 of the
         # 4x4 chi 8 twin: 100 undamped sweeps exhausted + 60 damped, its neighbours 32-33; the GPU trajectory,
@@ -182,6 +188,25 @@ def test_reduced_chi_twins_vs_stored_oracle(gpu, name, L, centre, chi_max, tol):
         if r["sweeps"] < 60 and sweeps < 60:
             assert abs(sweeps - r["sweeps"]) <= 8 + 0.1 * r["sweeps"], (r["step"], sweeps, r["sweeps"])
     print("%s: max |C_gpu - C_oracle| = %.2e over %d steps" % (name, worst, len(rows)))
+    sim.close()
+
+
+@pytest.mark.parametrize("name,L,centre,chi_max,tol", [g for g in GOLDEN_TWINS if g[1] >= 8],
+                         ids=[g[0][7:-4] for g in GOLDEN_TWINS if g[1] >= 8])
+def test_twins_with_leading_schmidt_vector_init(gpu, name, L, centre, chi_max, tol):
+    """Reading R7b (bp_init = 1, what the full-size runs of configs[3], [4] use - DESIGN.md 9.2): BP started
+    from e_0 must reach the fixed point the stored oracle trajectories (uniform init, R7) reached, i.e. the
+    same C(t) to 1e-6, converging at every step."""
+    import conftest
+    torch, B = gpu
+    rows = conftest.read_oracle_trajectory(name)
+    sim = B.Pepo(L, L, centre[0], centre[1], J, H, DT, chi_max, tol, 0.5)
+    sim.set_option("bp_init", 1)
+    for r in rows:
+        sim.trotter_step()
+        status, sweeps, delta = sim.bp_converge()
+        assert status == 0, r["step"]
+        assert abs(sim.correlation() - r["C"]) <= 1e-6, (r["step"], sim.correlation(), r["C"])
     sim.close()
 
 
@@ -385,3 +410,25 @@ def test_paper_convention_xx_plus_z(gpu):
         assert sg == so
         assert abs(sim.correlation() - st.correlation()) < 1e-6
     sim.close()
+
+
+def test_site_weights_and_spreading_vs_oracle(gpu):
+    """SURVEY NEXT-2 / PAPER section 6.4 + eq. (21): pepo_site_weights (one device pass over the four Pauli
+    slabs of every site) against the oracle's n(r, t) (pinned to the dense Pauli weights in
+    test_oracle_pins.py) along an untruncated chain, a truncated 4x4 run and a 6x6 grid (two site batches);
+    t = 0 is a single pixel."""
+    torch, B = gpu
+    from oracle import pepo_oracle as po
+    for (Lx, Ly, cx, cy, chi, steps) in [(1, 5, 0, 2, 32, 6), (4, 4, 1, 1, 8, 14), (6, 6, 2, 2, 4, 10)]:
+        sim = B.Pepo(Lx, Ly, cx, cy, J, H, DT, chi, 1e-10, 0.5)
+        st = po.PEPOState(Lx, Ly, cx, cy, J, H, DT, chi)
+        n0, sp0 = sim.site_weights()
+        assert list(n0) == [1.0 if v == cy * Lx + cx else 0.0 for v in range(Lx * Ly)] and sp0 == (0.0, 0.0, 0.0)
+        for t in range(steps):
+            sim.trotter_step(); st.trotter_step()
+            ng, spg = sim.site_weights()
+            no, spo = np.array(st.site_weights()), st.spreading()
+            assert np.abs(ng - no).max() < 1e-9, (Lx, Ly, t, np.abs(ng - no).max())
+            assert max(abs(a - b) for a, b in zip(spg, spo)) < 1e-8
+        assert spg[0] > 0.0 and 0.0 < spg[2] < 1.0
+        sim.close()

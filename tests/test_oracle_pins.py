@@ -507,3 +507,76 @@ def test_paper_convention_xx_plus_z_equals_dense(case):
     # Z_c commutes with the field, not with the bonds: C(dt) = cos(2 J dt)^deg(c) != the ZZ+X value cos(2 h dt)
     deg = len(st.lat.legs(st.center))
     assert abs(dense[0] - math.cos(2 * Jp * dtp) ** deg) < 1e-14
+
+
+# ---------------------------------------------------------------- alpha ladder / trap remediation ---
+def test_alpha_ladder_and_trap_procedure_control_flow():
+    """PAPER L451-L457.  The procedure has no closed form to pin; what is fixed by the text
+    is its control flow, checked here on a state whose BP needs >= 30 sweeps (4x4 chi 8, step 52):
+    (1) healthy step: observe = bp_converge + correlation, stage 0, and the accepted C becomes the
+    reference of the next call; (2) a third stage (alpha = 0.8) runs only when the first two fail;
+    (3) a candidate (>= 30 sweeps) whose |C| is below half the reference with quiet gate_err is retried
+    with every remaining alpha, each from the init - all reach the same fixed point here, so the answer
+    is status 2 ('raise chi', L457), the sweep count is the sum of the three runs, and the reference is
+    kept; (4) the same drop WITH a doubled gate_err is accepted (L454 'no corresponding increase')."""
+    st = _state_4x4_chi8(52)
+    s0, n0, _ = st.bp_converge(1e-10, 0.5)
+    c0 = st.correlation()
+    assert s0 == 0 and 30 <= n0 < 100
+    st.obs_prev_C, st.obs_prev_gerr = 2.0 * c0 * 0.99, st.gate_err          # not a > 50 % drop
+    out = st.observe(1e-10, 0.5, 0.2)
+    assert out == (0, c0, n0, 0) and st.obs_prev_C == c0
+    # (2): budgets too small for stages 0 and 1, enough for stage 2
+    n2 = st.bp_converge(1e-10, 0.2, max_sweeps=0, max_sweeps_damped=45)[1]
+    s, n, _ = st.bp_converge(1e-10, 0.5, max_sweeps=5, max_sweeps_damped=45, damping2=0.2)
+    assert s == 0 and st.bp_stage == 2 and n == 5 + 45 + n2
+    assert abs(st.correlation() - c0) < 1e-12
+    assert st.bp_converge(1e-10, 0.5, max_sweeps=5, max_sweeps_damped=45)[0] == 1       # without the ladder: exhausted
+    # (3)
+    st.obs_prev_C, st.obs_prev_gerr = 10.0 * c0, st.gate_err
+    n1 = st.bp_converge(1e-10, 0.5, first_stage=1)[1]
+    n2 = st.bp_converge(1e-10, 0.5, damping2=0.2, first_stage=2)[1]
+    status, C, n, stage = st.observe(1e-10, 0.5, 0.2)
+    assert (status, stage, n) == (2, 2, n0 + n1 + n2) and abs(C - c0) < 1e-12
+    assert st.obs_prev_C == 10.0 * c0
+    # (4)
+    st.obs_prev_gerr = 0.4 * st.gate_err
+    status, C, n, stage = st.observe(1e-10, 0.5, 0.2)
+    assert (status, stage, n) == (0, 0, n0) and st.obs_prev_C == C
+
+
+# ---------------------------------------------------------------- n(r, t) (PAPER section 6.4, eq. (21)) ---
+@pytest.mark.parametrize("case", [(1, 5, 0, 2), (1, 4, 0, 1), (2, 2, 0, 0), (2, 3, 0, 1)])
+def test_site_weights_equal_the_dense_pauli_weights(case):
+    """Reading R19: n(r) = 1 - w_I / sum_p w_p from the site tensor in its Vidal-gauge environment.  On a tree
+    the gauge is exact, so n(r) must equal the non-identity Pauli weight of the densely evolved operator
+    (sum over all 4^N Pauli strings, oracle/dense_check.py) to rounding; on loops it is the simple-update
+    approximation (2e-8 after 6 steps on 2x2 / 2x3)."""
+    Lx, Ly, cx, cy = case
+    st = po.PEPOState(Lx, Ly, cx, cy, J, H, DT, 256, eps_cut=1e-14)
+    n0 = st.site_weights()
+    assert n0 == [1.0 if v == st.center else 0.0 for v in range(Lx * Ly)]          # a single pixel at t = 0 (L363)
+    assert st.spreading() == (0.0, 0.0, 0.0)
+    for t in range(1, 7):
+        st.trotter_step()
+        got = np.array(st.site_weights())
+        want = np.array(dc.dense_site_weights(Lx, Ly, cx, cy, J, H, DT, t))
+        tol = 1e-13 if min(Lx, Ly) == 1 else (1e-12 if t <= 2 else 1e-7)      # loops: exact until the first closed path (step 3)
+        assert np.abs(got - want).max() < tol, (t, np.abs(got - want).max())
+    r1, r2, sf = st.spreading()
+    p = want / want.sum()
+    xs, ys = np.arange(Lx * Ly) % Lx, np.arange(Lx * Ly) // Lx
+    assert abs(r1 - (p * (abs(xs - cx) + abs(ys - cy))).sum()) < 1e-6
+    assert abs(r2 - math.sqrt((p * ((xs - cx) ** 2 + (ys - cy) ** 2)).sum())) < 1e-6
+    assert abs(sf + (p * np.log(p)).sum() / math.log(Lx * Ly)) < 1e-6 and 0.0 < sf < 1.0
+
+
+def test_site_weights_closed_forms():
+    """J = 0: the operator never leaves the centre site and never acquires an identity component there
+    (Z rotates in the Y-Z plane): n = delta_{r,c} at every step.  h = 0: Z_c commutes with H: the same."""
+    for Jx, hx in ((0.0, H), (J, 0.0)):
+        st = po.PEPOState(3, 3, 1, 1, Jx, hx, DT, 8)
+        for _ in range(4):
+            st.trotter_step()
+            n = st.site_weights()
+            assert abs(n[st.center] - 1.0) < 1e-15 and max(abs(x) for i, x in enumerate(n) if i != st.center) < 1e-15
