@@ -138,6 +138,10 @@ int pepo_observe(pepo_ctx* ctx, double* h_C, int* h_sweeps, int* h_stage);
 int pepo_correlation(pepo_ctx* ctx, double* h_C);
 
 int pepo_get_stats(pepo_ctx* ctx, pepo_stats* h_stats);
+/* Arena canaries (PAPER.md:L132-L160 single pre-sized workspace): every sub-buffer of the
+ * arena is followed by 64 guard bytes filled at init.  0 = all intact, -4 = a kernel wrote past the end of
+ * a buffer (pepo_last_error() names the guard).  Synchronises the context's streams. */
+int pepo_check_guards(pepo_ctx* ctx);
 /* In-situ per-kernel-class timing (option "profile": 1 on, 0 off, 2 on + reset): CUDA-event
  * pairs on the context stream around each launch group, summed per class.  Classes, in order:
  * 0 permute(+absorb/deabsorb), 1 Gram, 2 reconstruction GEMM, 3 small core GEMMs, 4 Cholesky +

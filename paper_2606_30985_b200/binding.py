@@ -57,6 +57,7 @@ def _load():
         "pepo_correlation": (i, [vp, C.POINTER(d)]),
         "pepo_observe": (i, [vp, C.POINTER(d), ip, ip]),
         "pepo_get_stats": (i, [vp, C.POINTER(PepoStats)]),
+        "pepo_check_guards": (i, [vp]),
         "pepo_get_profile": (i, [vp, i, C.POINTER(d), C.POINTER(d), C.POINTER(d), C.POINTER(ll)]),
         "pepo_n_bonds": (i, [vp]),
         "pepo_get_bond_dims": (i, [vp, ip]),
@@ -186,6 +187,9 @@ class Pepo:
         out, sw, stg = C.c_double(0.0), C.c_int(0), C.c_int(0)
         status = _check(_lib.pepo_observe(self._h, C.byref(out), C.byref(sw), C.byref(stg)))
         return status, out.value, sw.value, stg.value
+
+    def check_guards(self):
+        _check(_lib.pepo_check_guards(self._h))
 
     def stats(self):
         s = PepoStats()

@@ -185,10 +185,16 @@ struct LaneWs {
 struct Arena {
   char* base = nullptr; size_t size = 0, top = 0;
   bool dry = false; size_t model = 0;     // dry run: only account (model = unaligned sum)
+  // Every buffer is followed by a guard zone of PEPO_GUARD bytes holding a fixed pattern (the arena
+  // canaries of SURVEY section 5): pepo_check_guards() finds a kernel that wrote past its buffer.
+  std::vector<size_t> guards;             // offsets of the guard zones
   void* take(size_t bytes) {
     model += bytes;
     size_t off = (top + 255) & ~(size_t)255;
     top = off + bytes;
+    const size_t g = (top + 7) & ~(size_t)7;
+    guards.push_back(g);
+    top = g + 64;
     if (dry) return nullptr;
     return base ? base + off : nullptr;
   }
@@ -413,10 +419,12 @@ int layout(pepo_ctx* c) {
   c->partU.assign(c->n_sites, nullptr); c->partD.assign(c->n_sites, nullptr); c->partS.assign(c->n_sites, nullptr);
   for (int v = 0; v < c->n_sites; v++) {
     const SiteInfo& s = c->sites[v];
-    int hU = s.nbr[0] >= 0, hD = s.nbr[1] >= 0, hL = s.nbr[2] >= 0, hR = s.nbr[3] >= 0;
-    c->partU[v] = (double*)A.take(ipow(chi, hL + hR + hU) * 8);
-    c->partD[v] = (double*)A.take(ipow(chi, hL + hR + hD) * 8);
-    c->partS[v] = (double*)A.take(ipow(chi, hL + hR) * 8);
+    // BP roles (fill_bp_site): the legs that exist, in storage order, play the roles (u, d, l, r) of the
+    // sweep kernel; per-chunk partial vectors: <= d_l d_r chunks of d_u (d_d) entries, d_l d_r slice scalars
+    const int nl = s.nlegs;
+    c->partU[v] = (double*)A.take(ipow(chi, (nl >= 1) + (nl >= 3) + (nl >= 4)) * 8);
+    c->partD[v] = (double*)A.take(ipow(chi, (nl >= 2) + (nl >= 3) + (nl >= 4)) * 8);
+    c->partS[v] = (double*)A.take(ipow(chi, (nl >= 3) + (nl >= 4)) * 8);
   }
   c->sw_part = (double*)A.take((size_t)c->n_sites * PEPO_SW_CHUNKS * 4 * 8);
   c->sw_out = (double*)A.take((size_t)c->n_sites * 4 * 8);
@@ -663,6 +671,8 @@ extern "C" int pepo_init_ex(pepo_ctx** out, int Lx, int Ly, int cx, int cy, doub
   }
   c->cur_st = c->st;
   int rc = 0;
+  for (size_t g : c->arena.guards)
+    if (cudaMemsetAsync(c->arena.base + g, 0xA5, 64, c->st) != cudaSuccess) { set_error("init: guard fill failed"); pepo_destroy(c); return -3; }
   double one = 1.0;
   rc |= upload(c, c->ones, &one, 8);
   rc |= upload(c, c->dG1, c->G1, 128);
@@ -1643,18 +1653,22 @@ void fill_bp_site(pepo_ctx* c, int v, int cur, BpSite& S) {
   size_t slab = site_live_size(c, v) / 4;
   int pv = (v == c->center) ? c->obsP : 0;
   S.T = s.psi + slab * pv;
-  S.first_slot = -1;
-  for (int d = 0; d < 4; d++) {
-    if (s.nbr[d] >= 0) {
-      int e = s.bond_of_dir[d];
-      S.d[d] = c->chi[e]; S.present[d] = 1;
-      if (S.first_slot < 0) S.first_slot = d;
-      S.in[d] = c->msgs[cur] + (size_t)msg_index(c, v, d, false) * c->chi_max;
-      S.out_old[d] = c->msgs[cur] + (size_t)msg_index(c, v, d, true) * c->chi_max;
-      S.out_new[d] = c->msgs[cur ^ 1] + (size_t)msg_index(c, v, d, true) * c->chi_max;
+  // The sweep kernel sees a 4-index tensor T[u,d,l,r] and puts lanes on u and warps on d.  A missing leg
+  // has dimension 1 and can sit anywhere in the index list without changing the memory layout, so the
+  // legs that exist take the roles u, d, l, r in storage order and the missing ones the trailing roles
+  // (a top-row site, stored [D,L,R], would otherwise run with one active lane per warp).
+  S.first_slot = s.nlegs > 0 ? 0 : -1;
+  for (int role = 0; role < 4; role++) {
+    if (role < s.nlegs) {
+      const int d = s.leg_dir[role];
+      const int e = s.leg_bond[role];
+      S.d[role] = c->chi[e]; S.present[role] = 1;
+      S.in[role] = c->msgs[cur] + (size_t)msg_index(c, v, d, false) * c->chi_max;
+      S.out_old[role] = c->msgs[cur] + (size_t)msg_index(c, v, d, true) * c->chi_max;
+      S.out_new[role] = c->msgs[cur ^ 1] + (size_t)msg_index(c, v, d, true) * c->chi_max;
     } else {
-      S.d[d] = 1; S.present[d] = 0;
-      S.in[d] = c->ones; S.out_old[d] = c->ones; S.out_new[d] = nullptr;
+      S.d[role] = 1; S.present[role] = 0;
+      S.in[role] = c->ones; S.out_old[role] = c->ones; S.out_new[role] = nullptr;
     }
   }
   S.partU = c->partU[v]; S.partD = c->partD[v]; S.partS = c->partS[v];
@@ -1869,6 +1883,22 @@ extern "C" int pepo_bond_entropy(pepo_ctx* c, double* h_S, int n) {
   PEPO_CUDA_OK(cudaMemcpyAsync(h_S, d_out, (size_t)c->n_bonds * 8, cudaMemcpyDeviceToHost, c->st));
   PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
   return 0;
+}
+
+// Arena canaries: every sub-buffer of the arena is followed by 64 guard bytes filled at init.  Returns 0
+// when all are intact, else -4 with the index of the first damaged one in the error text (a kernel wrote
+// past the end of the buffer in front of it).  Synchronises every stream of the context.
+extern "C" int pepo_check_guards(pepo_ctx* c) {
+  if (!c) { set_error("check_guards: NULL"); return -1; }
+  PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
+  for (int i = 0; i < pepo_ctx::NSMAX; i++) { if (c->ps[i]) cudaStreamSynchronize(c->ps[i]); if (c->hp[i]) cudaStreamSynchronize(c->hp[i]); }
+  std::vector<unsigned char> h(64);
+  for (size_t k = 0; k < c->arena.guards.size(); k++) {
+    PEPO_CUDA_OK(cudaMemcpy(h.data(), c->arena.base + c->arena.guards[k], 64, cudaMemcpyDeviceToHost));
+    for (int b = 0; b < 64; b++)
+      if (h[b] != 0xA5) { set_error("check_guards: guard %zu of %zu (arena offset %zu) overwritten", k, c->arena.guards.size(), c->arena.guards[k]); return -4; }
+  }
+  return (int)0;
 }
 
 // n(r, t) and the spreading measures of PAPER.md section 6.4 / appendix A.3 (reading R19).

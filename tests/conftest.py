@@ -42,5 +42,13 @@ def read_oracle_trajectory(name):
                 continue
             t = line.split()
             rows.append(dict(step=int(t[0]), C=float(t[1]), sweeps=int(t[2]), status=int(t[3]), delta=float(t[4]),
-                             chi_max_live=int(t[5]), gate_err=float(t[6]), chi_sum=int(t[7])))
+                             chi_max_live=int(t[5]), gate_err=float(t[6]), chi_sum=int(t[7]),
+                             sens=float(t[8]) if len(t) > 8 else -1.0))
+    # tolerance of C at each step: north_star's 1e-6 where the trajectory is defined that well, else 50 x the
+    # running max of the oracle's own sensitivity to a one-ulp perturbation (tests/golden/make_oracle_twin.py)
+    env = 0.0
+    for r in rows:
+        if r["sens"] == r["sens"] and r["sens"] > 0.0:
+            env = max(env, r["sens"])
+        r["tol_C"] = max(1e-6, 50.0 * env)
     return rows

@@ -8,7 +8,13 @@ Run from the repo root, e.g.
     python tests/golden/make_oracle_twin.py --grid 4 4 --centre 1 1 --chi 16 --steps 60 --tol 1e-10
     python tests/golden/make_oracle_twin.py --grid 8 8 --centre 3 3 --chi 24 --steps 40 --tol 1e-9
 Columns: step, C(t), BP sweeps (both phases), BP status, BP delta, max live bond dimension, gate_err,
-sum of all bond dimensions.  A status-1 line is an exhausted budget.
+sum of all bond dimensions, sens.  A status-1 line is an exhausted budget.
+
+--sens N (default 0): N more oracle states run in lockstep, identical except that after step 5 every
+entry of every site tensor is multiplied ONCE by (1 + 1e-15 g), g ~ N(0,1) from default_rng(seed = 1..N):
+a one-ulp perturbation.  sens = max over the N copies of |C - C_perturbed| at that step = how far the
+truncated trajectory amplifies rounding, i.e. to how many digits C(t) is defined at all by the algorithm
+in fp64.  The parity tests compare the CUDA path to C within max(1e-6, 50 x running max of sens).
 """
 import argparse
 import os
@@ -29,10 +35,13 @@ if __name__ == "__main__":
     ap.add_argument("--max-sweeps", type=int, default=100)
     ap.add_argument("--max-sweeps-damped", type=int, default=1000)
     ap.add_argument("--out", default=None)
+    ap.add_argument("--sens", type=int, default=0)
     a = ap.parse_args()
     Lx, Ly = a.grid
     cx, cy = a.centre
     st = po.PEPOState(Lx, Ly, cx, cy, 1.0, 0.9, 0.05, a.chi)
+    twins = [po.PEPOState(Lx, Ly, cx, cy, 1.0, 0.9, 0.05, a.chi) for _ in range(a.sens)]
+    import numpy as np
     name = a.out or "oracle_%dx%d_chi%d.txt" % (Lx, Ly, a.chi)
     path = os.path.join(os.path.dirname(__file__), name)
     t0 = time.time()
@@ -40,13 +49,24 @@ if __name__ == "__main__":
         f.write("# %dx%d centre (%d,%d) chi_max %d, J=1 h=0.9 dt=0.05, BP tol %g damping %g budgets %d/%d "
                 "(oracle/pepo_oracle.py via tests/golden/make_oracle_twin.py)\n"
                 % (Lx, Ly, cx, cy, a.chi, a.tol, a.damping, a.max_sweeps, a.max_sweeps_damped))
-        f.write("# step C sweeps status delta chi_max_live gate_err chi_sum\n")
+        f.write("# sens: %d copies perturbed once by 1e-15 (relative, seeded) after step 5\n" % a.sens)
+        f.write("# step C sweeps status delta chi_max_live gate_err chi_sum sens\n")
         for s in range(1, a.steps + 1):
             st.trotter_step()
             status, sweeps, delta = st.bp_converge(a.tol, a.damping, a.max_sweeps, a.max_sweeps_damped)
             chis = st.bond_dims()
-            f.write("%d %.15f %d %d %.6e %d %.12e %d\n" % (s, st.correlation(), sweeps, status, delta,
-                                                       max(chis), st.gate_err, sum(chis)))
+            C = st.correlation()
+            sens = 0.0
+            for k, tw in enumerate(twins):
+                tw.trotter_step()
+                if s == 5:
+                    rng = np.random.default_rng(k + 1)
+                    for v in range(Lx * Ly):
+                        tw.psi[v] = tw.psi[v] * (1.0 + 1e-15 * rng.standard_normal(tw.psi[v].shape))
+                stw, _, _ = tw.bp_converge(a.tol, a.damping, a.max_sweeps, a.max_sweeps_damped)
+                sens = max(sens, abs(tw.correlation() - C) if (stw == 0 and status == 0) else float("nan"))
+            f.write("%d %.15f %d %d %.6e %d %.12e %d %.3e\n" % (s, C, sweeps, status, delta,
+                                                             max(chis), st.gate_err, sum(chis), sens if a.sens else -1.0))
             f.flush()
             sys.stderr.write("step %d done, %.0f s\n" % (s, time.time() - t0))
     print("wrote", path)

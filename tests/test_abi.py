@@ -85,7 +85,9 @@ def closed_form_bytes(Lx, Ly, chi, B):
             deg = hU + hD + hL + hR
             degs.add(deg)
             doubles += 4 * chi ** deg                                                  # psi_v
-            doubles += chi ** (hL + hR + hU) + chi ** (hL + hR + hD) + chi ** (hL + hR)  # BP partials
+            # BP partials: per-chunk vectors for the first two legs that exist, slice scalars for the others
+            doubles += (chi ** ((deg >= 1) + (deg >= 3) + (deg >= 4)) + chi ** ((deg >= 2) + (deg >= 3) + (deg >= 4))
+                        + chi ** ((deg >= 3) + (deg >= 4)))
             doubles += 64 * 4 + 4                                                      # n(r,t) partials
     degmax = max(degs)
     m_max = chi ** max(degmax - 1, 0)
@@ -95,7 +97,10 @@ def closed_form_bytes(Lx, Ly, chi, B):
     slot = ld * n + spares + part + n * n + 2 * N * N + n * n + 4 * n * N + N * chi + n * 4 * chi + 4 * n * chi
     lane = 2 * slot + 4 * N * N + 2 * N * chi
     doubles += B * lane
-    return 8 * doubles
+    # every sub-buffer starts on a 256-byte boundary and is followed by 64 guard bytes (pepo_check_guards):
+    # 4 buffers per site, 21 global ones, 14 + one per site class per lane slot, 8 per lane
+    n_buffers = 4 * Lx * Ly + 21 + B * (2 * (14 + len([d for d in degs if d >= 1])) + 8)
+    return 8 * doubles + n_buffers * (128 + 64)
 
 
 @pytest.mark.parametrize("Lx,Ly,chi", [(3, 3, 8), (4, 4, 60), (8, 8, 60), (10, 10, 95)])

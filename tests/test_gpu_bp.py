@@ -246,3 +246,4 @@ def test_leading_schmidt_vector_init_matches_oracle_and_converges_where_uniform_
     assert abs(cg - co) < 1e-12 and abs(cg - 0.279) < 1e-3
     assert _msg_diff(sim, st, up_to_sign=(swg != swo)) < 1e-8
     sim.close()
+

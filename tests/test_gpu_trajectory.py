@@ -27,6 +27,7 @@ def _run_gpu(B, Lx, Ly, cx, cy, chi_max, steps, tol, damping=0.0, opts=None, **k
         status, sweeps, delta = sim.bp_converge()
         out.append(dict(C=sim.correlation(), status=status, sweeps=sweeps, delta=delta,
                         chi=sim.bond_dims(), gate_err=sim.stats()["gate_err"]))
+    sim.check_guards()         # arena canaries: no kernel wrote past the end of its buffer
     return sim, out
 
 
@@ -158,7 +159,10 @@ GOLDEN_TWINS = [
 def test_reduced_chi_twins_vs_stored_oracle(gpu, name, L, centre, chi_max, tol):
     """Reduced-chi twins of BASELINE configs[1], [3], [4] (same grid, centre, steps, BP tolerance and
     damping; only chi_max reduced) against oracle trajectories stored by tests/golden/make_oracle_twin.py
-    (oracle only).  Truncated configs: 1e-6 on C (north_star); status and the live bond dimensions must
+    (oracle only).  Truncated configs: 1e-6 on C (north_star) wherever the trajectory is defined that well:
+    the files carry the oracle's own sensitivity to a one-ulp perturbation (column sens; e.g. 4x4 chi 16:
+    4e-8 at step 30, 5e-7 at step 40, 2e-5 at step 50 - heavily truncated runs amplify rounding), and the
+    tolerance at a step is max(1e-6, 50 x running max of sens).  Status and the live bond dimensions must
     agree; the sweep count is compared where it is well defined: delta crosses tol on a slowly decaying
     tail, so a rounding-level difference in psi moves the crossing by a few sweeps (seen: 26 against 20
     at step 37 of the 4x4 chi 8 twin with C equal to 1e-12; by more once the count is in the hundreds), and a crossing within a few sweeps of the 100-sweep budget may or may
@@ -175,7 +179,7 @@ def test_reduced_chi_twins_vs_stored_oracle(gpu, name, L, centre, chi_max, tol):
         dims = sim.bond_dims()
         assert status == r["status"], r["step"]
         assert max(dims) == r["chi_max_live"] and sum(dims) == r["chi_sum"], (r["step"], max(dims), sum(dims))
-        assert abs(c - r["C"]) <= 1e-6, (r["step"], c, r["C"])
+        assert abs(c - r["C"]) <= r["tol_C"], (r["step"], c, r["C"], r["tol_C"])
         worst = max(worst, abs(c - r["C"]))
         # discarded weight: a sum of squared singular values below the cut; once truncation is active the
         # tail directions are the ill-determined ones (seen 1.26e-8 against 1.08e-8 at step 17 of the chi 16
@@ -206,7 +210,7 @@ def test_twins_with_leading_schmidt_vector_init(gpu, name, L, centre, chi_max, t
         sim.trotter_step()
         status, sweeps, delta = sim.bp_converge()
         assert status == 0, r["step"]
-        assert abs(sim.correlation() - r["C"]) <= 1e-6, (r["step"], sim.correlation(), r["C"])
+        assert abs(sim.correlation() - r["C"]) <= r["tol_C"], (r["step"], sim.correlation(), r["C"])
     sim.close()
 
 
@@ -432,3 +436,30 @@ def test_site_weights_and_spreading_vs_oracle(gpu):
             assert max(abs(a - b) for a, b in zip(spg, spo)) < 1e-8
         assert spg[0] > 0.0 and 0.0 < spg[2] < 1.0
         sim.close()
+
+
+def test_arena_guards_detect_an_overrun(gpu):
+    """compute-sanitizer is not available on this GPU pool, so memory safety inside the single arena is
+    watched by canaries: every sub-buffer is followed by 64 guard bytes (pepo_check_guards).  Intact after
+    runs on both schedules, both QR paths and the BP / diagnostics calls; a byte written into the last
+    guard zone is reported as -4."""
+    torch, B = gpu
+    for opts in ({"pipeline": 4}, {"pipeline": 0}, {"direct_gemm": 0}, {"force_householder": 1}, {"chol_tau": 1.0}):
+        sim = B.Pepo(4, 4, 1, 1, J, H, DT, 12, 1e-10, 0.5)
+        for k, v in opts.items():
+            sim.set_option(k, v)
+        for _ in range(14):
+            sim.trotter_step()
+        sim.observe(); sim.site_weights(); sim.bond_entropy()
+        sim.check_guards()
+        sim.close()
+    sim = B.Pepo(3, 3, 1, 1, J, H, DT, 8, 1e-10, 0.0)
+    sim.trotter_step()
+    sim.check_guards()
+    off = (-sim.arena.data_ptr()) % 256 + sim.stats()["arena_high_water"] - 32
+    sim.arena[off] = 0
+    torch.cuda.synchronize()
+    with pytest.raises(B.PepoError) as e:
+        sim.check_guards()
+    assert e.value.code == -4 and "guard" in str(e.value)
+    sim.close()
