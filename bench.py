@@ -29,10 +29,12 @@ if ROOT not in sys.path:
 
 J, H, DT = 1.0, 0.9, 0.05
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the class's main kernel on the 4x4 chi=60
-# saturated state, from the `ncu --set full` captures summarised in profiles/r1c_ncu_top_kernels.md and
-# profiles/r1_ncu_top_kernels.md (bytes; None = not captured).  Launch shapes: svd = 8 cores of 240^2 in one
-# launch; apply_gemm = 216000 x 240 x 240; permute = one 4 x 60^4 interior tensor; bp = partial sweep over all 16 sites.
-NCU_TRAFFIC_4x4_CHI60 = {"svd": 3.75e6, "apply_gemm": 790.3e6, "permute": 784.1e6, "bp": 433.8e6, "gram": None}
+# saturated state, from the `ncu --set full` captures summarised in profiles/r2_ncu_top_kernels.md (bytes; None =
+# not captured).  Launch shapes: svd = one core of 240^2; apply_gemm = gathered reconstruction of one interior site
+# (216000 x 240 x 240, algorithmic 829.4e6); gram = gathered weighted Gram of one interior site (algorithmic 414.7e6
+# + 17 MB of split-K partials); permute = round 1's capture of one 4 x 60^4 interior tensor; bp = partial sweep
+# over all 16 pinned slabs (algorithmic 428.4e6).
+NCU_TRAFFIC_4x4_CHI60 = {"svd": 0.53e6, "apply_gemm": 792.2e6, "permute": 784.1e6, "bp": 433.7e6, "gram": 434.9e6}
 FP64_NOMINAL_RATIO = 45.0 / 2250.0     # B200 fp64 tensor / bf16 tensor, blackwell guide table
 
 

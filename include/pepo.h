@@ -94,6 +94,8 @@ int pepo_destroy(pepo_ctx* ctx);
  * "jacobi_tol" (1e-15), "jacobi_max_sweeps" (60), "jacobi_early" (cosine below which a sweep
  * counts as the last one, 1e-7; 0 = always run the confirming sweep),
  * "trotter_order" (1 = first-order step, R2; 2 = symmetric step of eq. (6)),
+ * "env" (0: gate environment = diag(sqrt(lambda)), reading R6(i); 1: the matrix messages of
+ * pepo_norm_bp_converge), "psqrt_eps",
  * "bp_init" (0: every BP stage starts from m = (1..1)/sqrt(chi), reading R7; 1: from the leading Schmidt
  * vector e_0 of each bond, reading R7b), "bp_ladder" (1: third BP stage with "bp_damping2", default 0.2), "observe_ref_C" /
  * "observe_ref_gate_err" (reference of pepo_observe's drop test: C(t) and gate_err of the last accepted
@@ -179,6 +181,25 @@ int pepo_set_lambda(pepo_ctx* ctx, int bond, const double* h_src, int n);
  * normalised, eq. (12)), computed on the device.  h_S: host array of n >= n_bonds doubles.
  * Synchronises the context stream.  -1 on a bad argument. */
 int pepo_bond_entropy(pepo_ctx* ctx, double* h_S, int n);
+/* NEXT-1 of SURVEY 8(f): belief propagation on the NORM network <<O|O>> with chi x chi symmetric PSD matrix
+ * messages ("approximate Vidal gauge maintained by BP", L146-L150):
+ *   Mhat_{v->w}[k,k'] = sum_p sum_{i,i'} psi_v[..i..,k,p] psi_v[..i'..,k',p] prod_{u != w} M_{u->v}[i_u,i'_u],
+ * symmetrised, normalised to Frobenius norm 1 (matches sum lambda^2 = 1, eq. (12)), damped as eq. (19),
+ * delta as eq. (14); Jacobi schedule.  pepo_norm_bp_converge sweeps from the CURRENT messages (diag(lambda_e)
+ * in both directions when there are none: after init, set_lambda, set_bond_dims) until delta < tol or
+ * max_sweeps, then refreshes the PSEUDO_SQRT S = V sqrt(w) V^T and its pseudo-inverse of every message
+ * (symmetric Jacobi eigen-decomposition, eigenvalues below option "psqrt_eps" (1e-12) x the largest zeroed,
+ * L315-L317).  Returns 0 converged / 1 budget exhausted / -4 non-finite.  With option "env" = 1 the bond gates
+ * then absorb and de-absorb these matrices by chi x chi GEMMs on every environment leg (L318, L336) instead of
+ * the diagonal sqrt(lambda); a gate resets the two messages of its bond to diag(lambda_new) (a13).  On a tree
+ * the fixed point is diag(lambda) and nothing changes; an untruncated gate is exact for any invertible
+ * environment.  Heavy contractions run on the DMMA GEMM kernels; written for parity at test sizes (chi <= 160).
+ * pepo_bethe_norm: Table 1 (L373-L380, L550), exp(sum_v log f_v - sum_e log Z_e), f_v the full double-layer
+ * site contraction, Z_e = sum_{kk'} M_{a->b}[k,k'] M_{b->a}[k,k'] (1 on a tree).
+ * pepo_get_norm_message: message over `bond` sent by v1 (from_v1 != 0) or v2, chi x chi column-major, n = chi^2. */
+int pepo_norm_bp_converge(pepo_ctx* ctx, double tol, double damping, int max_sweeps, int* h_sweeps, double* h_delta);
+int pepo_bethe_norm(pepo_ctx* ctx, double* h_norm);
+int pepo_get_norm_message(pepo_ctx* ctx, int bond, int from_v1, double* h_dst, int n);
 /* Operator spreading (section 6.4; appendix A.3 eq. (21)): the per-site
  * non-identity Pauli weight n(r,t) = 1 - w_I / sum_p w_p with w_p = sum_i psi_v[i,p]^2 prod_legs
  * lambda_leg[i_leg] (the Pauli-resolved norm of the site in its Vidal-gauge environment; exact on trees;

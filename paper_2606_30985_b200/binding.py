@@ -71,6 +71,9 @@ def _load():
         "pepo_bond_entropy": (i, [vp, vp, i]),
         "pepo_get_message": (i, [vp, i, i, vp, i]),
         "pepo_site_weights": (i, [vp, vp, i, vp]),
+        "pepo_norm_bp_converge": (i, [vp, d, d, i, ip, C.POINTER(d)]),
+        "pepo_bethe_norm": (i, [vp, C.POINTER(d)]),
+        "pepo_get_norm_message": (i, [vp, i, i, vp, i]),
         "pepo_set_lambda": (i, [vp, i, vp, i]),
         "pepo_site_ptr": (vp, [vp, i, i]),
         "pepo_permute": (i, [dp, dp, ip, ip, i, vp]),
@@ -259,6 +262,22 @@ class Pepo:
         spread = np.empty(3, dtype=np.float64)
         _check(_lib.pepo_site_weights(self._h, out.ctypes.data_as(C.c_void_p), n, spread.ctypes.data_as(C.c_void_p)))
         return out, tuple(spread)
+
+    def norm_bp_converge(self, tol, damping=0.0, max_sweeps=100):
+        sw, de = C.c_int(0), C.c_double(0.0)
+        status = _check(_lib.pepo_norm_bp_converge(self._h, float(tol), float(damping), int(max_sweeps), C.byref(sw), C.byref(de)))
+        return status, sw.value, de.value
+
+    def bethe_norm(self):
+        out = C.c_double(0.0)
+        _check(_lib.pepo_bethe_norm(self._h, C.byref(out)))
+        return out.value
+
+    def get_norm_message(self, bond, from_v1=True):
+        chi = self.bond_dims()[bond]
+        out = np.empty(chi * chi, dtype=np.float64)
+        _check(_lib.pepo_get_norm_message(self._h, bond, 1 if from_v1 else 0, out.ctypes.data_as(C.c_void_p), chi * chi))
+        return out.reshape((chi, chi), order="F")
 
     def get_message(self, bond, from_v1=True):
         n = self.bond_dims()[bond]

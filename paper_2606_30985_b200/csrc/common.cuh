@@ -104,8 +104,10 @@ struct SiteView {
 // C (n x n, ld n, both triangles) = cv^T diag(w) cv with w(row) = prod over the environment legs of
 // w2[leg][i_leg] (a3 fused into a5: w2 = lambda, the squared absorb factor); w2[leg] device pointers
 // (entry `cut` ignored; NULL = no weight on that leg).  part: split-K workspace of gram_plan(m, n).
+// psiB != nullptr: the cross Gram cv(psi)^T diag(w) cv(psiB) of two tensors of the same shape (norm-network
+// BP); it must be symmetric by construction, only its upper triangle is computed and mirrored.
 int launch_site_gram(cudaStream_t st, const double* psi, const SiteView& v, const double* const* w2,
-                     double* C, double* part);
+                     double* C, double* part, const double* psiB = nullptr);
 // out = the packed site tensor with dims[cut] replaced by chi_new: out[.., c', .., p'] =
 // sum_{c,p} psi[.., c, .., p] W[(c,p),(c',p')], W column-major (4 dims[cut]) x (4 chi_new), ld ldw
 // (a10-a13 fused: reconstruction GEMM that reads and writes the canonical layout).

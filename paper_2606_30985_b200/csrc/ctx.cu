@@ -20,6 +20,7 @@
 #include "bp.cuh"
 #include "common.cuh"
 #include "dense.cuh"
+#include "normbp.cuh"
 
 #include <algorithm>
 #include <chrono>
@@ -263,6 +264,18 @@ struct pepo_ctx {
   unsigned long long* delta_bits;
   int* bp_ints;                           // [flag, status]
   std::vector<double*> partU, partD, partS;
+  // NEXT-1: norm-network BP with chi x chi matrix messages (option "env" = 1 feeds them to the gates).
+  // Indexed like msgs: 2e = sent by v1 of bond e, 2e + 1 = sent by v2; packed, ld = live chi of the bond.
+  int env_mode = 0;
+  double* nM[2] = {nullptr, nullptr};     // two sets of 2 n_bonds messages (chi_max^2 each)
+  double *nS = nullptr, *nSinv = nullptr; // PSEUDO_SQRT and its pseudo-inverse of the current messages
+  double *nG = nullptr, *nraw = nullptr;  // cross Gram (4 chi)^2; unnormalised message chi^2
+  double *nEg = nullptr, *nEv = nullptr, *nEu = nullptr, *nEw = nullptr, *nEs = nullptr;   // eigen workspace
+  int* nEo = nullptr;                     // order (chi ints) + sweeps
+  double* nscal = nullptr;                // n_sites + n_bonds scalars (f_v, Z_e)
+  int n_cur = 0;
+  bool n_valid = false, n_sqrt_valid = false;
+  double psqrt_eps = 1e-12;               // option "psqrt_eps"
   double* sw_part = nullptr;              // n_sites x PEPO_SW_CHUNKS x 4 partials of pepo_site_weights
   double* sw_out = nullptr;               // n_sites x 4
   double *dG1, *dGamma[2], *dAhat[2], *dSigma;
@@ -425,6 +438,18 @@ int layout(pepo_ctx* c) {
     c->partU[v] = (double*)A.take(ipow(chi, (nl >= 1) + (nl >= 3) + (nl >= 4)) * 8);
     c->partD[v] = (double*)A.take(ipow(chi, (nl >= 2) + (nl >= 3) + (nl >= 4)) * 8);
     c->partS[v] = (double*)A.take(ipow(chi, (nl >= 3) + (nl >= 4)) * 8);
+  }
+  {
+    const size_t x2 = chi * chi;
+    for (int i = 0; i < 2; i++) c->nM[i] = (double*)A.take(2 * nb * x2 * 8 + 8);
+    c->nS = (double*)A.take(2 * nb * x2 * 8 + 8);
+    c->nSinv = (double*)A.take(2 * nb * x2 * 8 + 8);
+    c->nG = (double*)A.take(16 * x2 * 8);
+    c->nraw = (double*)A.take(x2 * 8);
+    c->nEg = (double*)A.take(x2 * 8); c->nEv = (double*)A.take((x2 + chi) * 8);
+    c->nEu = (double*)A.take(x2 * 8); c->nEw = (double*)A.take(x2 * 8); c->nEs = (double*)A.take(chi * 8);
+    c->nEo = (int*)A.take((chi + 4) * 4);
+    c->nscal = (double*)A.take((c->n_sites + nb + 1) * 8);
   }
   c->sw_part = (double*)A.take((size_t)c->n_sites * PEPO_SW_CHUNKS * 4 * 8);
   c->sw_out = (double*)A.take((size_t)c->n_sites * 4 * 8);
@@ -733,6 +758,8 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "bp_group") c->bp_group = (int)v;
   else if (k == "bp_ladder") c->bp_ladder = (int)v;
   else if (k == "bp_init") c->bp_init = (int)v;
+  else if (k == "env") c->env_mode = (int)v ? 1 : 0;
+  else if (k == "psqrt_eps") c->psqrt_eps = v;
   else if (k == "observe_ref_C") c->obs_prev_C = v;            // reference of pepo_observe's drop test (e.g. after a restart)
   else if (k == "observe_ref_gate_err") c->obs_prev_gerr = v;
   else if (k == "bp_damping2") { if (!(v >= 0.0 && v < 1.0)) { set_error("set_option: bp_damping2 must be in [0,1)"); return -1; } c->bp_damping2 = v; }
@@ -779,7 +806,7 @@ extern "C" int pepo_set_bond_dims(pepo_ctx* c, const int* h_chi) {
   for (int e = 0; e < c->n_bonds; e++)
     if (h_chi[e] < 1 || h_chi[e] > c->chi_max) { set_error("set_bond_dims: chi[%d]=%d out of range", e, h_chi[e]); return -1; }
   for (int e = 0; e < c->n_bonds; e++) c->chi[e] = h_chi[e];
-  c->msgs_valid = false;
+  c->msgs_valid = false; c->n_valid = false; c->n_sqrt_valid = false;
   return 0;
 }
 extern "C" size_t pepo_site_size(pepo_ctx* c, int x, int y) {
@@ -857,6 +884,7 @@ extern "C" int pepo_set_lambda(pepo_ctx* c, int bond, const double* h_src, int n
     if (!(h_src[i] > 0.0)) { set_error("set_lambda: non-positive entry"); return -1; }
     sq[i] = std::sqrt(h_src[i]); isq[i] = 1.0 / sq[i];
   }
+  c->n_valid = false; c->n_sqrt_valid = false;
   int rc = upload(c, bond_vec(c->lambda, bond, c->chi_max), h_src, n * 8);
   rc |= upload(c, bond_vec(c->sqrt_l, bond, c->chi_max), sq.data(), n * 8);
   rc |= upload(c, bond_vec(c->isqrt_l, bond, c->chi_max), isq.data(), n * 8);
@@ -939,10 +967,30 @@ struct BatchState {        // one batch of gates moving through the three phases
   SvdFinishBatch fb;
 };
 
-// a2-a4 fused: cv = permute(psi * sqrt(lambda_env)) into the lane's work matrix (explicit path)
+int msg_index(const pepo_ctx* c, int v, int dir, bool outgoing);
+int leg_apply(pepo_ctx* c, cudaStream_t st, const double* src, const int* dims, int nlegs, int leg,
+              const double* Mat, int d_new, double* Wbuf, double* dst);
+inline bool matrix_env(const pepo_ctx* c) { return c->env_mode == 1 && c->n_valid && c->n_sqrt_valid; }
+
+// a2-a4 fused: cv = permute(psi * sqrt(lambda_env)) into the lane's work matrix (explicit path).
+// Matrix environment (NEXT-1, option "env" = 1): the absorb is a chi x chi GEMM per environment leg with
+// the PSEUDO_SQRT of the incoming matrix message, then a plain permutation.
 int enqueue_permute_in(pepo_ctx* c, cudaStream_t st, const TaskGeo& t) {
   const SiteInfo& s = c->sites[t.v];
   SiteWs& W = c->lanes[t.lane].s[t.slot];
+  const double* psrc = s.psi;
+  const bool menv = matrix_env(c);
+  if (menv && t.n_env > 0) {
+    const double* src = s.psi;
+    for (int j = 0; j < t.n_env; j++) {
+      const int l = t.env_legs[j];
+      double* dst = ((t.n_env - 1 - j) % 2 == 0) ? W.out : W.cv;         // the last one lands in W.out
+      const double* Smat = c->nS + (size_t)msg_index(c, t.v, s.leg_dir[l], false) * c->chi_max * c->chi_max;
+      int rc = leg_apply(c, st, src, t.dims, s.nlegs, l, Smat, t.dims[l], W.W, dst); if (rc) return rc;
+      src = dst;
+    }
+    psrc = src;
+  }
   PermuteDesc pd;
   pd.rank = s.nlegs + 1; pd.power = 1.0;
   long long sstr = 1;
@@ -951,12 +999,12 @@ int enqueue_permute_in(pepo_ctx* c, cudaStream_t st, const TaskGeo& t) {
   for (int j = 0; j < t.n_env; j++) {
     int l = t.env_legs[j];
     pd.perm[j] = l; pd.dst_stride[j] = dstr; dstr *= t.dims[l];
-    pd.scale[l] = bond_vec(c->sqrt_l, s.leg_bond[l], c->chi_max);
+    pd.scale[l] = menv ? nullptr : bond_vec(c->sqrt_l, s.leg_bond[l], c->chi_max);
   }
   pd.perm[t.n_env] = t.cut_leg; pd.dst_stride[t.n_env] = t.ld;
   pd.perm[t.n_env + 1] = s.nlegs; pd.dst_stride[t.n_env + 1] = t.ld * t.chi_c;
   ProfScope ps(c, PC_PERMUTE, 0, 16.0 * t.m * t.n);
-  return launch_permute(st, s.psi, W.cv, pd);
+  return launch_permute(st, psrc, W.cv, pd);
 }
 
 // phase 1: absorb + permute, Gram, dressing, Cholesky (enqueue only; ends with the flag read-back)
@@ -996,7 +1044,7 @@ int batch_p1(pepo_ctx* c, BatchState& S) {
       t.chol = !c->force_hh && (double)t.m >= c->chol_ratio * t.n;
       t.r = t.chol ? t.N : std::min(4 * t.k, t.N);
       t.skip1 = t.m <= t.n; t.skip2 = 4 * t.k <= t.N;
-      t.direct = t.chol && c->direct;
+      t.direct = t.chol && c->direct && !matrix_env(c);
       t.view.nlegs = s.nlegs; t.view.cut = t.cut_leg;
       for (int l = 0; l < 4; l++) t.view.dims[l] = l < s.nlegs ? t.dims[l] : 1;
       // The Gram kernel reads psi in place when the rows of cv are contiguous runs in psi (cut leg not
@@ -1354,7 +1402,7 @@ int batch_p3(pepo_ctx* c, BatchState& S) {
     for (int j = 0; j < t.n_env; j++) {
       int l = t.env_legs[j];
       src_leg[j] = l; pd.shape[j] = t.dims[l]; pd.src_stride[j] = sstr; sstr *= t.dims[l];
-      pd.scale[j] = bond_vec(c->isqrt_l, s.leg_bond[l], c->chi_max);
+      pd.scale[j] = matrix_env(c) ? nullptr : bond_vec(c->isqrt_l, s.leg_bond[l], c->chi_max);
     }
     src_leg[t.n_env] = t.cut_leg; pd.shape[t.n_env] = t.chi_new; pd.src_stride[t.n_env] = t.ld; pd.scale[t.n_env] = nullptr;
     src_leg[t.n_env + 1] = s.nlegs; pd.shape[t.n_env + 1] = 4; pd.src_stride[t.n_env + 1] = t.ld * t.chi_new; pd.scale[t.n_env + 1] = nullptr;
@@ -1365,8 +1413,34 @@ int batch_p3(pepo_ctx* c, BatchState& S) {
       pd.perm[j] = sd; pd.dst_stride[j] = dst_stride_of_leg[j];
     }
     ProfScope ps(c, PC_PERMUTE, 0, 16.0 * t.m * 4 * t.chi_new);
+    if (matrix_env(c) && t.n_env > 0) {
+      // de-absorb (a12) by chi x chi GEMMs with the pseudo-inverse square roots
+      int rc = launch_permute(st, W.out, W.cv, pd); if (rc) return rc;
+      const double* src = W.cv;
+      for (int j = 0; j < t.n_env; j++) {
+        const int l = t.env_legs[j];
+        double* dst = (j == t.n_env - 1) ? s.psi : ((j % 2 == 0) ? W.out : W.cv);
+        const double* Si = c->nSinv + (size_t)msg_index(c, t.v, s.leg_dir[l], false) * c->chi_max * c->chi_max;
+        rc = leg_apply(c, st, src, newdims, s.nlegs, l, Si, newdims[l], W.W, dst); if (rc) return rc;
+        src = dst;
+      }
+      continue;
+    }
     int rc = launch_permute(st, W.out, s.psi, pd);
     if (rc) return rc;
+  }
+  if (matrix_env(c)) {
+    // a13: mu <- diag(lambda) on the updated bond, both directions, in the new index basis
+    const size_t x2 = (size_t)c->chi_max * c->chi_max;
+    for (int g = 0; g < ng; g++) {
+      const int e = gate_bonds[g], cn = T[2 * g].chi_new;
+      const double* lam = bond_vec(c->lambda, e, c->chi_max);
+      for (int k = 0; k < 2; k++) {
+        int rc = launch_set_diag(st, lam, cn, 0, c->nM[c->n_cur] + (2 * e + k) * x2); if (rc) return rc;
+        rc = launch_set_diag(st, lam, cn, 1, c->nS + (2 * e + k) * x2); if (rc) return rc;
+        rc = launch_set_diag(st, lam, cn, 2, c->nSinv + (2 * e + k) * x2); if (rc) return rc;
+      }
+    }
   }
   for (int g = 0; g < ng; g++) c->chi[gate_bonds[g]] = T[2 * g].chi_new;
   c->msgs_valid = false;
@@ -1942,6 +2016,157 @@ extern "C" int pepo_site_weights(pepo_ctx* c, double* h_n, int n, double* h_spre
     h_spread[0] = r1; h_spread[1] = std::sqrt(r2);
     h_spread[2] = c->n_sites > 1 ? ent / std::log((double)c->n_sites) : 0.0;
   }
+  return 0;
+}
+
+// ============================================================================================
+// NEXT-1: norm-network BP with chi x chi matrix messages (PAPER.md:L72, L146-L150,
+// L315-L317, L336, Table 1).  Built from the site-level DMMA contractions: "one leg times a matrix" is
+// launch_site_apply with W = I_4 (x) M, the double-layer contraction over all legs but one is the cross
+// Gram of (psi with the incoming messages applied) and psi.  Written for parity at test sizes, not tuned.
+// ============================================================================================
+namespace {
+
+inline double* nmsg(pepo_ctx* c, double* base, int idx) { return base + (size_t)idx * c->chi_max * c->chi_max; }
+
+// dst = src with leg `leg` contracted with Mat (d_leg x d_new, ld d_leg): dims[] = live dims of src
+int leg_apply(pepo_ctx* c, cudaStream_t st, const double* src, const int* dims, int nlegs, int leg,
+              const double* Mat, int d_new, double* Wbuf, double* dst) {
+  int rc = launch_kron_i4(st, Mat, dims[leg], d_new, dims[leg], Wbuf); if (rc) return rc;
+  SiteView v; v.nlegs = nlegs; v.cut = leg;
+  for (int l = 0; l < 4; l++) v.dims[l] = l < nlegs ? dims[l] : 1;
+  return launch_site_apply(st, src, v, Wbuf, 4ll * dims[leg], d_new, dst);
+}
+
+int nbp_init(pepo_ctx* c) {
+  for (int e = 0; e < c->n_bonds; e++)
+    for (int k = 0; k < 2; k++) {
+      int rc = launch_set_diag(c->st, bond_vec(c->lambda, e, c->chi_max), c->chi[e], 0, nmsg(c, c->nM[c->n_cur], 2 * e + k));
+      if (rc) return rc;
+    }
+  c->n_valid = true; c->n_sqrt_valid = false;
+  return 0;
+}
+
+// psi_v with the incoming messages applied on every leg except `skip` (-1: none skipped): result pointer
+// in *out (psi itself when there is nothing to apply); scratch = the explicit-cv buffers of lane 0
+int nbp_dress_site(pepo_ctx* c, int v, int skip, const double** out) {
+  const SiteInfo& s = c->sites[v];
+  int dims[4];
+  for (int l = 0; l < s.nlegs; l++) dims[l] = c->chi[s.leg_bond[l]];
+  double* buf[2] = {c->lanes[0].s[0].cv, c->lanes[0].s[1].cv};
+  const double* src = s.psi;
+  int k = 0;
+  for (int l = 0; l < s.nlegs; l++) {
+    if (l == skip) continue;
+    const double* Min = nmsg(c, c->nM[c->n_cur], msg_index(c, v, s.leg_dir[l], false));
+    int rc = leg_apply(c, c->st, src, dims, s.nlegs, l, Min, dims[l], c->lanes[0].s[0].W, buf[k]); if (rc) return rc;
+    src = buf[k]; k ^= 1;
+  }
+  *out = src;
+  return 0;
+}
+
+// unnormalised, symmetrised message leaving v through its leg lw into c->nraw; with update: also the new
+// damped message into the other set
+int nbp_site_leg(pepo_ctx* c, int v, int lw, double damping, bool update) {
+  const SiteInfo& s = c->sites[v];
+  const double* B = nullptr;
+  int rc = nbp_dress_site(c, v, lw, &B); if (rc) return rc;
+  SiteView sv; sv.nlegs = s.nlegs; sv.cut = lw;
+  for (int l = 0; l < 4; l++) sv.dims[l] = l < s.nlegs ? c->chi[s.leg_bond[l]] : 1;
+  rc = launch_site_gram(c->st, B, sv, nullptr, c->nG, c->lanes[0].s[0].part, s.psi); if (rc) return rc;
+  const int oi = msg_index(c, v, s.leg_dir[lw], true);
+  double* old = nmsg(c, c->nM[c->n_cur], oi);
+  double* out = update ? nmsg(c, c->nM[c->n_cur ^ 1], oi) : c->nEw;      // no update: scratch
+  return launch_norm_msg(c->st, c->nG, sv.dims[lw], old, damping, out, c->nraw, c->delta_bits, c->bp_ints);
+}
+
+int nbp_sqrt_all(pepo_ctx* c) {
+  for (int e = 0; e < c->n_bonds; e++)
+    for (int k = 0; k < 2; k++) {
+      const int chi = c->chi[e], idx = 2 * e + k;
+      SvdBatch sb; sb.count = 1;
+      sb.K[0] = nmsg(c, c->nM[c->n_cur], idx); sb.ldk[0] = chi; sb.r1[0] = chi; sb.r2[0] = chi;
+      sb.G[0] = c->nEg; sb.V[0] = c->nEv; sb.sv[0] = c->nEs; sb.order[0] = c->nEo; sb.sweeps[0] = c->nEo + c->chi_max;
+      int rc = launch_svd_jacobi(c->st, sb, 1e-15, 60, true, 0, 0.0); if (rc) return rc;
+      rc = launch_svd_vectors(c->st, c->nEg, c->nEv, c->nEs, c->nEo, chi, chi, c->nEu, c->nEw); if (rc) return rc;
+      rc = launch_psqrt_build(c->st, c->nEu, c->nEw, c->nEs, chi, c->psqrt_eps, nmsg(c, c->nS, idx), nmsg(c, c->nSinv, idx));
+      if (rc) return rc;
+    }
+  c->n_sqrt_valid = true;
+  return 0;
+}
+
+}  // namespace
+
+// Sweeps of the matrix-message BP from the CURRENT messages (diag(lambda) if there are none) until
+// delta < tol or max_sweeps; afterwards the PSEUDO_SQRTs of all messages are refreshed.
+extern "C" int pepo_norm_bp_converge(pepo_ctx* c, double tol, double damping, int max_sweeps, int* h_sweeps, double* h_delta) {
+  if (!c || !(tol > 0.0) || damping < 0.0 || damping >= 1.0 || max_sweeps < 1) { set_error("norm_bp_converge: bad argument"); return -1; }
+  CtxScope scope(c);
+  { int rcw = wait_pending_uploads(c, c->st); if (rcw) return rcw; }
+  int rc = 0;
+  if (!c->n_valid) { rc = nbp_init(c); if (rc) return rc; }
+  int sweeps = 0, status = 1;
+  double delta = INFINITY;
+  PEPO_CUDA_OK(cudaMemsetAsync(c->bp_ints, 0, 16, c->st));
+  for (int it = 0; it < max_sweeps && status; it++) {
+    PEPO_CUDA_OK(cudaMemsetAsync(c->delta_bits, 0, 8, c->st));
+    for (int v = 0; v < c->n_sites; v++)
+      for (int l = 0; l < c->sites[v].nlegs; l++) { rc = nbp_site_leg(c, v, l, damping, true); if (rc) return rc; }
+    c->n_cur ^= 1;
+    PEPO_CUDA_OK(cudaMemcpyAsync(c->h_delta, c->delta_bits, 8, cudaMemcpyDeviceToHost, c->st));
+    PEPO_CUDA_OK(cudaMemcpyAsync(c->h_bpints, c->bp_ints, 8, cudaMemcpyDeviceToHost, c->st));
+    PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
+    memcpy(&delta, c->h_delta, 8);
+    if (c->n_bonds == 0) delta = 0.0;
+    sweeps++;
+    if (c->h_bpints[0] & 2) { set_error("norm_bp_converge: non-finite message norm"); return -4; }
+    if (delta < tol) status = 0;
+  }
+  c->n_sqrt_valid = false;
+  rc = nbp_sqrt_all(c); if (rc) return rc;
+  if (h_sweeps) *h_sweeps = sweeps;
+  if (h_delta) *h_delta = delta;
+  return status;
+}
+
+// Bethe norm of PAPER.md Table 1 (L373-L380, L550): exp(sum_v log f_v - sum_e log Z_e) of the double-layer
+// network with the current matrix messages (1 on a tree).
+extern "C" int pepo_bethe_norm(pepo_ctx* c, double* h_norm) {
+  if (!c || !h_norm) { set_error("bethe_norm: NULL"); return -1; }
+  CtxScope scope(c);
+  if (!c->n_valid) { int rc = nbp_init(c); if (rc) return rc; }
+  for (int v = 0; v < c->n_sites; v++) {
+    const SiteInfo& s = c->sites[v];
+    if (s.nlegs == 0) { set_error("bethe_norm: single-site lattice"); return -1; }
+    int rc = nbp_site_leg(c, v, 0, 0.0, false); if (rc) return rc;
+    const int chi = c->chi[s.leg_bond[0]];
+    rc = launch_frob_dot(c->st, c->nraw, nmsg(c, c->nM[c->n_cur], msg_index(c, v, s.leg_dir[0], false)), chi * chi, c->nscal + v);
+    if (rc) return rc;
+  }
+  for (int e = 0; e < c->n_bonds; e++) {
+    int rc = launch_frob_dot(c->st, nmsg(c, c->nM[c->n_cur], 2 * e), nmsg(c, c->nM[c->n_cur], 2 * e + 1), c->chi[e] * c->chi[e],
+                             c->nscal + c->n_sites + e);
+    if (rc) return rc;
+  }
+  std::vector<double> h((size_t)c->n_sites + c->n_bonds);
+  PEPO_CUDA_OK(cudaMemcpyAsync(h.data(), c->nscal, h.size() * 8, cudaMemcpyDeviceToHost, c->st));
+  PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
+  double lg = 0.0;
+  for (int v = 0; v < c->n_sites; v++) { if (!(h[v] > 0.0)) { set_error("bethe_norm: f_v <= 0 at site %d", v); return -4; } lg += std::log(h[v]); }
+  for (int e = 0; e < c->n_bonds; e++) { const double z = h[c->n_sites + e]; if (!(z > 0.0)) { set_error("bethe_norm: Z_e <= 0 at bond %d", e); return -4; } lg -= std::log(z); }
+  *h_norm = std::exp(lg);
+  return 0;
+}
+
+// Matrix message over `bond` (from_v1 != 0: sent by v1), chi x chi column-major, n = chi^2.
+extern "C" int pepo_get_norm_message(pepo_ctx* c, int bond, int from_v1, double* h_dst, int n) {
+  if (!c || !h_dst || bond < 0 || bond >= c->n_bonds || n != c->chi[bond] * c->chi[bond]) { set_error("get_norm_message: bad argument"); return -1; }
+  if (!c->n_valid) { set_error("get_norm_message: no matrix messages (call pepo_norm_bp_converge)"); return -1; }
+  PEPO_CUDA_OK(cudaMemcpyAsync(h_dst, nmsg(c, c->nM[c->n_cur], 2 * bond + (from_v1 ? 0 : 1)), (size_t)n * 8, cudaMemcpyDeviceToHost, c->st));
+  PEPO_CUDA_OK(cudaStreamSynchronize(c->st));
   return 0;
 }
 

@@ -466,7 +466,7 @@ static void site_geometry(const SiteView& v, long long& run, long long& slab) {
 }
 
 int launch_site_gram(cudaStream_t st, const double* psi, const SiteView& v, const double* const* w2,
-                     double* C, double* part) {
+                     double* C, double* part, const double* psiB) {
   long long run, slab;
   site_geometry(v, run, slab);
   const long long m = v.m();
@@ -489,10 +489,10 @@ int launch_site_gram(cudaStream_t st, const double* psi, const SiteView& v, cons
   else for (int i = 0; i < g.nw; i++) if (!g.wv[i]) { set_error("site_gram: weights must be given for all environment legs or none"); return -1; }
   g.wE[0] = make_fastdiv((uint32_t)ext[0]); g.wE[1] = make_fastdiv((uint32_t)ext[1]);
   for (int i = 0; i < 3; i++) if (ext[i] > GW_MAXLEN) { set_error("site_gram: bond dimension %d > %d", ext[i], GW_MAXLEN); return -1; }
-  const bool base16 = (((uintptr_t)psi) & 15) == 0;
+  const bool base16 = ((((uintptr_t)psi) & 15) == 0) && (!psiB || (((uintptr_t)psiB) & 15) == 0);
   int ks, kc;
   gram_plan(m, n, &ks, &kc);
-  GemmProb p; p.A = psi; p.B = psi; p.C = C; p.lda = p.ldb = 0; p.ldc = n; p.M = n; p.N = n; p.K = (int)m;
+  GemmProb p; p.A = psi; p.B = psiB ? psiB : psi; p.C = C; p.lda = p.ldb = 0; p.ldc = n; p.M = n; p.N = n; p.K = (int)m;
   int rc;
   if (run >= 2) {
     // rows contiguous in runs: both operands K-contiguous (the layout of the explicit cv)

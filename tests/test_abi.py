@@ -89,6 +89,8 @@ def closed_form_bytes(Lx, Ly, chi, B):
             doubles += (chi ** ((deg >= 1) + (deg >= 3) + (deg >= 4)) + chi ** ((deg >= 2) + (deg >= 3) + (deg >= 4))
                         + chi ** ((deg >= 3) + (deg >= 4)))
             doubles += 64 * 4 + 4                                                      # n(r,t) partials
+    n_bonds = Ly * (Lx - 1) + (Ly - 1) * Lx
+    doubles += 8 * n_bonds * chi * chi + 22 * chi * chi      # matrix messages (2 sets, sqrt, inverse sqrt) + their workspace
     degmax = max(degs)
     m_max = chi ** max(degmax - 1, 0)
     ld = (m_max + 1) // 2 * 2
@@ -99,7 +101,7 @@ def closed_form_bytes(Lx, Ly, chi, B):
     doubles += B * lane
     # every sub-buffer starts on a 256-byte boundary and is followed by 64 guard bytes (pepo_check_guards):
     # 4 buffers per site, 21 global ones, 14 + one per site class per lane slot, 8 per lane
-    n_buffers = 4 * Lx * Ly + 21 + B * (2 * (14 + len([d for d in degs if d >= 1])) + 8)
+    n_buffers = 4 * Lx * Ly + 33 + B * (2 * (14 + len([d for d in degs if d >= 1])) + 8)
     return 8 * doubles + n_buffers * (128 + 64)
 
 
