@@ -94,6 +94,9 @@ int pepo_destroy(pepo_ctx* ctx);
  * "jacobi_tol" (1e-15), "jacobi_max_sweeps" (60), "jacobi_early" (cosine below which a sweep
  * counts as the last one, 1e-7; 0 = always run the confirming sweep),
  * "trotter_order" (1 = first-order step, R2; 2 = symmetric step of eq. (6)),
+ * "svd_deflate" (theta of the truncation-aware deflation of the Jacobi SVD: after 3 full sweeps the columns
+ * with norm < theta x the chi_max-th largest norm are set aside; 0 = off, the default: with 1e-3 the leading
+ * triplets move by up to ~theta x cos x s_cut, 2e-12 of the gate tensor on the flattest test spectrum),
  * "env" (0: gate environment = diag(sqrt(lambda)), reading R6(i); 1: the matrix messages of
  * pepo_norm_bp_converge), "psqrt_eps",
  * "bp_init" (0: every BP stage starts from m = (1..1)/sqrt(chi), reading R7; 1: from the leading Schmidt

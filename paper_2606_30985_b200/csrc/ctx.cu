@@ -246,6 +246,7 @@ struct pepo_ctx {
   int bp_ladder = 0;                   // option "bp_ladder": third BP stage with damping bp_damping2 (alpha-retry, L451-L457)
   double bp_damping2 = 0.2;            // option "bp_damping2": alpha = 0.8
   double obs_prev_C = 1.0, obs_prev_gerr = 0.0;   // last C(t) / gate_err accepted by pepo_observe (C(0) = 1)
+  double svd_deflate = 0.0;            // option "svd_deflate": theta of the truncation-aware deflation of the Jacobi SVD (0: off, default)
   double jacobi_early = 1e-7;          // option "jacobi_early": cosine below which a Jacobi sweep counts as the last one
   std::vector<cudaEvent_t> done_ev;    // completion events of the pieces of a pipelined step
   int n_sites, n_bonds, n_hb;
@@ -755,6 +756,7 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "jacobi_max_sweeps") c->jacobi_max_sweeps = (int)v;
   else if (k == "svd_precond_min") c->svd_precond_min = (int)v;
   else if (k == "jacobi_early") c->jacobi_early = v < 0.0 ? 0.0 : v;
+  else if (k == "svd_deflate") c->svd_deflate = v < 0.0 ? 0.0 : v;
   else if (k == "bp_group") c->bp_group = (int)v;
   else if (k == "bp_ladder") c->bp_ladder = (int)v;
   else if (k == "bp_init") c->bp_init = (int)v;
@@ -1238,7 +1240,8 @@ int batch_p2(pepo_ctx* c, BatchState& S) {
       // a high-priority stream so that it is placed ahead of the other half-batch's GEMM CTAs
       {
         ProfScope ps(c, PC_SVD, 0, 0);
-        rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps, false, c->svd_precond_min, c->jacobi_early);
+        rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps, false, c->svd_precond_min, c->jacobi_early,
+                               c->chi_max, c->svd_deflate);
         if (rc) return rc;
       }
       ProfScope ps(c, PC_SVD, 0, 0);

@@ -61,8 +61,11 @@ struct SvdBatch {
 // (the Jacobi iteration runs on R^T); launch_svd_bridge must get the same value.
 // early: cosine below which a sweep counts as the last one (jacobi_c16_kernel; 0 = always run the
 // confirming sweep)
+// keep_hint > 0 and theta > 0 (hot-path kernel only): only the leading keep_hint triplets are needed
+// (truncation to chi_max); after 3 full sweeps the columns with norm < theta x the keep_hint-th largest
+// norm are set aside and the iteration continues on the rest (svd.cu "deflation")
 int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
-                      int precond_min, double early);
+                      int precond_min, double early, int keep_hint = 0, double theta = 0.0);
 
 struct SvdFinishBatch {
   int count;

@@ -613,7 +613,7 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 template <int NREG, int NTHR>
 __global__ void __launch_bounds__(NTHR, 1)
 jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int precond_min, int pw,
-                  double early2) {
+                  double early2, int keep_hint, int nfull, double theta) {
   constexpr int LEN = 32 * NREG, LEN2 = 16 * NREG;
   extern __shared__ __align__(16) double jsm[];
   cg::cluster_group cluster = cg::this_cluster();
@@ -755,16 +755,19 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
   // ---- iteration ------------------------------------------------------------------------------
   int sweeps = 0;
   const bool active = (Nc >= 2) && (ref > 0.0) && isfinite(ref);
-  const int nb2 = (bs & 1) ? bs + 1 : bs;
+  // bl = LIVE columns per block (bs = layout stride of the shared buffers): after the deflation below
+  // the top block lives in slots [0, bl) and the bottom block in slots [bs, bs + bl)
+  int bl = bs;
+  int nb2 = (bl & 1) ? bl + 1 : bl;
   const int half = lane >> 4, l16 = lane & 15;
   const int hw = 2 * warp + half;                        // half-warp index
-  const int nrw = (bs + 1) / 2;                          // warps that rotate pairs in the super-rounds
+  int nrw = (bl + 1) / 2;                                // warps that rotate pairs in the super-rounds
   // destinations of the block exchange (see header): my top block and my bottom block
   const int top_dst_rank = (crank == 0 || crank == CS - 1) ? crank : crank + 1;
   const int top_dst_slot = (crank == CS - 1) ? 1 : 0;
   const int bot_dst_rank = (crank == 0) ? 1 : crank - 1;
   const int bot_dst_slot = (crank == 0) ? 0 : 1;
-  const int nrt = nrw * 32;
+  int nrt = nrw * 32;
   for (int sw = 0; active && sw < max_sweeps; sw++) {
     double* nrm = nrmbuf + cur * 2 * bs;
     bool big = false;                                    // this thread rotated a pair with cos^2 > early2 in this sweep
@@ -775,7 +778,7 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
         int a, c;
         if (i == 0) { a = nb2 - 1; c = r; }
         else { a = (r + i) % (nb2 - 1); c = (r - i + nb2 - 1) % (nb2 - 1); }
-        const bool valid = (a < bs && c < bs);
+        const bool valid = (a < bl && c < bl);
         const int p = valid ? min(a, c) : 0, q = valid ? max(a, c) : 0;
         double2* p2 = reinterpret_cast<double2*>(cols + ((size_t)slot * bs + p) * LEN);
         double2* q2 = reinterpret_cast<double2*>(cols + ((size_t)slot * bs + q) * LEN);
@@ -819,7 +822,7 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
     for (int sr = 0; sr < 2 * CS - 1; sr++) {
       const int nxt = cur ^ 1;
       if (warp < nrw) {
-        const bool own = hw < bs;
+        const bool own = hw < bl;
         const int pi = own ? hw : 0;
         double* top = cols;
         double* bot = cols + (size_t)bs * LEN;
@@ -829,8 +832,8 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
 #pragma unroll
         for (int u = 0; u < NREG; u++) tp[u] = tcol[l16 + 16 * u];
         double al = nrmc[pi];
-        for (int r = 0; r < bs; r++) {
-          int j = pi + r; if (j >= bs) j -= bs;
+        for (int r = 0; r < bl; r++) {
+          int j = pi + r; if (j >= bl) j -= bl;
           double2* cq = reinterpret_cast<double2*>(bot + (size_t)j * LEN);
           double2 y[NREG];
           double ga0 = 0.0, ga1 = 0.0;
@@ -842,7 +845,7 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
           double be = nrmc[bs + j];
           const double ga = half_sum1(ga0 + ga1);
           const bool dorot = own && al >= noise2 && be >= noise2 && ga * ga > tol2 * al * be;
-          const bool last = (r == bs - 1);
+          const bool last = (r == bl - 1);
           if (__any_sync(0xffffffffu, dorot)) {
             double cs, sn, tt;
             jacobi_cst(dorot ? al : 1.0, dorot ? be : 2.0, dorot ? ga : 0.5, cs, sn, tt);
@@ -922,6 +925,62 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
     if (tid == 0) s_flag = 0;                         // every thread passed the flag push (cluster barrier)
     __syncthreads();
     if (anybig == 0.0) break;
+    // ---- deflation of the discarded tail (truncation-aware; eq. (11): only chi_max triplets
+    // survive).  After `nfull` sweeps the columns whose norm is below theta x the norm of the keep_hint-th
+    // largest column can no longer matter for the leading keep_hint triplets: rotating a column p of norm
+    // alpha against one of norm beta <= theta alpha changes p by an angle <= (beta / alpha) cos(p, q) and
+    // its norm by the square of that.  They are written out as they are (their norms stand in for their
+    // singular values, which lie below the cut) and the iteration goes on with the remaining columns,
+    // re-dealt over the cluster: a sweep of n' columns is n' - 1 rounds instead of Nc - 1.
+    if (keep_hint > 0 && sw + 1 == nfull && bl == bs && Nc > 2 * keep_hint) {
+      double* G = b.G[t];
+      double* svu = b.V[t] + (size_t)Nc * Nc;
+      for (int ci = warp; ci < 2 * bs; ci += nw) {
+        const int id = ids[ci];
+        if (id >= Nc) continue;
+        const double* col = cols + (size_t)ci * LEN;
+        double s2 = 0.0;
+        for (int kk = lane; kk < Mj; kk += 32) { double x = col[kk]; s2 += x * x; G[(size_t)id * M + kk] = x; }
+        s2 = warp_sum1(s2);
+        if (lane == 0) svu[id] = sqrt(s2);
+      }
+      __threadfence();
+      cluster.sync();
+      int* kl = reinterpret_cast<int*>(vbuf);             // kl[rank] = column id (>= 2 (MP + 2) ints available)
+      __shared__ int s_np;
+      if (tid == 0) s_np = 0;
+      for (int j = tid; j < Nc; j += NTHR) {
+        const double sj = svu[j];
+        int rank = 0;
+        for (int l = 0; l < Nc; l++) { const double sl = svu[l]; rank += (sl > sj || (sl == sj && l < j)) ? 1 : 0; }
+        kl[rank] = j;
+      }
+      __syncthreads();
+      const double scut = svu[kl[keep_hint - 1]];
+      for (int r = tid; r < Nc; r += NTHR) if (svu[kl[r]] >= theta * scut) atomicAdd(&s_np, 1);
+      __syncthreads();
+      const int np = s_np;
+      const int bl2 = (np + 2 * CS - 1) / (2 * CS);
+      if (bl2 < bl && np >= keep_hint) {                  // the same decision in every CTA (same data)
+        const int np2 = min(Nc, 2 * CS * bl2);
+        for (int e = tid; e < per; e += NTHR) {
+          const int kk = e % LEN, ci = e / LEN, slot = ci / bs, i = ci % bs;
+          int id = Nc;
+          if (i < bl2) { const int rank = (slot ? 2 * CS - 1 - crank : crank) * bl2 + i; if (rank < np2) id = kl[rank]; }
+          cols[e] = (id < Nc && kk < Mj) ? G[(size_t)id * M + kk] : 0.0;
+        }
+        for (int e = tid; e < 2 * bs; e += NTHR) {
+          const int slot = e / bs, i = e % bs;
+          int id = Nc;
+          if (i < bl2) { const int rank = (slot ? 2 * CS - 1 - crank : crank) * bl2 + i; if (rank < np2) id = kl[rank]; }
+          ids[e] = id;
+          idbuf[(cur ^ 1) * 2 * bs + e] = Nc;             // stale ids of the other buffer's dead slots
+        }
+        bl = bl2; nb2 = (bl & 1) ? bl + 1 : bl; nrw = (bl + 1) / 2; nrt = nrw * 32;
+      }
+      __syncthreads();
+      cluster.sync();
+    }
   }
   // ---- write back ------------------------------------------------------------------------------
   double* G = b.G[t];
@@ -1120,14 +1179,14 @@ int launch_set_identity(cudaStream_t st, double* Q, long long m, int k) {
 }
 
 static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
-                            int precond_min, double early);
+                            int precond_min, double early, int keep_hint, double theta);
 
 // The launch configuration (cluster size, columns per CTA, register tile) fixes the order of the
 // pair rotations, i.e. the rounding of the result.  It is therefore chosen per problem SIZE, never
 // from the composition of the batch: problems of equal (min, max) dimension share a launch, and a
 // gate gives bit-identical results whichever other gates run beside it (serial or pipelined class).
 int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
-                      int precond_min, double early) {
+                      int precond_min, double early, int keep_hint, double theta) {
   if (b.count == 0) return 0;
   bool done[PEPO_MAXT] = {false};
   for (int t0 = 0; t0 < b.count; t0++) {
@@ -1141,14 +1200,14 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
       g.G[q] = b.G[t]; g.V[q] = b.V[t]; g.sv[q] = b.sv[t]; g.order[q] = b.order[t]; g.sweeps[q] = b.sweeps[t];
       done[t] = true;
     }
-    int rc = launch_svd_group(st, g, tol, max_sweeps, with_v, precond_min, early);
+    int rc = launch_svd_group(st, g, tol, max_sweeps, with_v, precond_min, early, keep_hint, theta);
     if (rc) return rc;
   }
   return 0;
 }
 
 static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
-                            int precond_min, double early) {
+                            int precond_min, double early, int keep_hint, double theta) {
   if (b.count == 0) return 0;
   int ncmax = 1, lenmax = 2;
   for (int t = 0; t < b.count; t++) {
@@ -1210,13 +1269,14 @@ static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int 
         PEPO_CUDA_OK(cudaFuncSetAttribute(jacobi_c16_kernel<13, 256>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
       }
       const double early2 = early * early;
+      const int kh = (theta > 0.0) ? keep_hint : 0;
       cudaError_t e;
-      if (nreg == 2) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<2, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
-      else if (nreg == 4) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<4, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
-      else if (nreg == 6) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<6, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
-      else if (nreg == 8) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<8, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
-      else if (nreg == 10) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<10, 256>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
-      else e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<13, 256>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2);
+      if (nreg == 2) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<2, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta);
+      else if (nreg == 4) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<4, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta);
+      else if (nreg == 6) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<6, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta);
+      else if (nreg == 8) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<8, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta);
+      else if (nreg == 10) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<10, 256>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta);
+      else e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<13, 256>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta);
       if (e != cudaSuccess) { set_error("svd: cluster launch failed: %s", cudaGetErrorString(e)); return -3; }
       PEPO_COUNT_LAUNCH();
       return 0;

@@ -463,3 +463,26 @@ def test_arena_guards_detect_an_overrun(gpu):
         sim.check_guards()
     assert e.value.code == -4 and "guard" in str(e.value)
     sim.close()
+
+
+def test_truncation_aware_svd_deflation_option(gpu):
+    """Option svd_deflate (off by default): after 3 full Jacobi sweeps the columns far below the chi_max-th
+    largest are set aside.  It perturbs the kept triplets at the 1e-12 level of the gate
+    tensor at most, so a physical truncated run must keep its bond dimensions and agree with the default
+    to 1e-9 in C(t) and 1e-10 in lambda, while needing fewer Jacobi rounds."""
+    torch, B = gpu
+    res = []
+    for theta in (0.0, 1e-3):
+        sim = B.Pepo(4, 4, 1, 1, J, H, DT, 40, 1e-10, 0.5)
+        sim.set_option("svd_deflate", theta)
+        cs = []
+        for _ in range(22):
+            sim.trotter_step()
+            sim.bp_converge()
+            cs.append(sim.correlation())
+        res.append((cs, sim.bond_dims(), [sim.get_lambda(e) for e in range(sim.n_bonds)]))
+        sim.check_guards()
+        sim.close()
+    assert list(res[0][1]) == list(res[1][1])
+    assert max(abs(a - b) for a, b in zip(res[0][0], res[1][0])) < 1e-9
+    assert max(np.abs(a - b).max() for a, b in zip(res[0][2], res[1][2])) < 1e-10
