@@ -574,7 +574,11 @@ void gram_plan(long long m, int n, int* ksplit, int* kchunk) {
     // 594 CTAs ran as two waves plus a third one of 2 CTAs (ncu: 558 us against 2/3 of that).
     bt = 80; target = 148 * 2 * GRAM_WAVES; cap = 100 * GRAM_WAVES; whole_waves = true;
   }
-  else if (n <= 64) bt = 64;
+  else if (n <= 64) {
+    // one tile: the product is HBM-bound (5 - 10 flop / byte): enough splits for 4 resident CTAs per SM
+    // (128 splits streamed 256000 x 40 at 0.64 TB/s)
+    bt = 64; target = 148 * 4; cap = 1024;
+  }
   const int tn = (n + bt - 1) / bt;
   const int upper = tn * (tn + 1) / 2;
   int ks = whole_waves ? std::max(1, target / upper) : (target + upper - 1) / upper;

@@ -59,7 +59,7 @@ def gram_splits(m, n):
     if n % 80 == 0:
         bt, target, cap, whole = 80, 148 * 2 * 2, 200, True
     elif n <= 64:
-        bt, target, cap, whole = 64, 148 * 2, 128, False
+        bt, target, cap, whole = 64, 148 * 4, 1024, False
     else:
         bt, target, cap, whole = 128, 148 * 2, 128, False
     tn = -(-n // bt)
