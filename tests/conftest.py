@@ -8,6 +8,16 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 
+# The oracle's matrices are small: BLAS threads beyond a few only spin (and on a box that is busy with
+# something else an unlimited pool makes the CPU suite crawl).  Limit the pools for the whole session.
+try:
+    import numpy  # noqa: F401  (loads the BLAS whose pool is limited)
+    import threadpoolctl
+    _BLAS_LIMIT = threadpoolctl.threadpool_limits(limits=min(4, os.cpu_count() or 1))
+except Exception:          # pragma: no cover - threadpoolctl is optional
+    _BLAS_LIMIT = None
+
+
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")
 
