@@ -97,6 +97,8 @@ int pepo_destroy(pepo_ctx* ctx);
  * "svd_deflate" (theta of the truncation-aware deflation of the Jacobi SVD: after 3 full sweeps the columns
  * with norm < theta x the chi_max-th largest norm are set aside; 0 = off, the default: with 1e-3 the leading
  * triplets move by up to ~theta x cos x s_cut, 2e-12 of the gate tensor on the flattest test spectrum),
+ * "svd_orient" (square preconditioned cores: 0 = QR of K, 2 = QR of K^T, 1 = of the one whose column norms
+ * are more graded, the default; the singular triplets are the same to rounding, the Jacobi sweep count is not),
  * "env" (0: gate environment = diag(sqrt(lambda)), reading R6(i); 1: the matrix messages of
  * pepo_norm_bp_converge), "psqrt_eps",
  * "bp_init" (0: every BP stage starts from m = (1..1)/sqrt(chi), reading R7; 1: from the leading Schmidt

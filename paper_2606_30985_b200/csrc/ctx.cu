@@ -180,6 +180,7 @@ struct LaneWs {
   double *K, *Ks, *G, *V, *sv, *Us, *Vs;
   int* order;
   int* ints;          // [chi_new, sweeps, info0, info1]
+  int* orient;        // device int: the Jacobi kernel iterated on K^T (square core, option "svd_orient")
   double* dbls;       // [discarded, gap]
 };
 
@@ -246,6 +247,7 @@ struct pepo_ctx {
   int bp_ladder = 0;                   // option "bp_ladder": third BP stage with damping bp_damping2 (alpha-retry, L451-L457)
   double bp_damping2 = 0.2;            // option "bp_damping2": alpha = 0.8
   double obs_prev_C = 1.0, obs_prev_gerr = 0.0;   // last C(t) / gate_err accepted by pepo_observe (C(0) = 1)
+  int svd_orient = 1;                  // option "svd_orient": 0 QR of K, 1 of the more graded of K / K^T (default), 2 of K^T (square cores)
   double svd_deflate = 0.0;            // option "svd_deflate": theta of the truncation-aware deflation of the Jacobi SVD (0: off, default)
   double jacobi_early = 1e-7;          // option "jacobi_early": cosine below which a Jacobi sweep counts as the last one
   std::vector<cudaEvent_t> done_ev;    // completion events of the pieces of a pipelined step
@@ -294,6 +296,7 @@ struct pepo_ctx {
   int n_pending = 0;
   int trotter_order = 1;               // option "trotter_order": 1 = R2 (BASELINE), 2 = symmetric step of eq. (6)
   std::vector<LaneWs> lanes;
+  int* lane_orient = nullptr;             // B ints (LaneWs::orient)
   int* lane_ints; double* lane_dbls;      // device readback blocks (B*4 ints, B*2 doubles)
   // pinned host
   int* h_ints = nullptr; double* h_dbls = nullptr; int* h_chi_msg = nullptr; double* h_scal = nullptr;
@@ -462,6 +465,7 @@ int layout(pepo_ctx* c) {
   c->dSigma = (double*)A.take(NA * 8);
   c->lane_ints = (int*)A.take((size_t)c->B * 4 * 4);
   c->lane_dbls = (double*)A.take((size_t)c->B * 2 * 8);
+  c->lane_orient = (int*)A.take((size_t)c->B * 4);
   const size_t m_max = ipow(chi, std::max(degmax - 1, 0));
   const size_t ld_max = (m_max + 1) & ~(size_t)1;
   const size_t cvcap = ld_max * nmax;
@@ -471,6 +475,7 @@ int layout(pepo_ctx* c) {
     LaneWs& L = c->lanes[l];
     L.ints = c->lane_ints ? c->lane_ints + 4 * l : nullptr;
     L.dbls = c->lane_dbls ? c->lane_dbls + 2 * l : nullptr;
+    L.orient = c->lane_orient ? c->lane_orient + l : nullptr;
     for (int i = 0; i < 2; i++) {
       SiteWs& S = L.s[i];
       S.cv = (double*)A.take(cvcap * 8);
@@ -757,6 +762,7 @@ extern "C" int pepo_set_option(pepo_ctx* c, const char* key, double v) {
   else if (k == "svd_precond_min") c->svd_precond_min = (int)v;
   else if (k == "jacobi_early") c->jacobi_early = v < 0.0 ? 0.0 : v;
   else if (k == "svd_deflate") c->svd_deflate = v < 0.0 ? 0.0 : v;
+  else if (k == "svd_orient") c->svd_orient = v < 0.5 ? 0 : v < 1.5 ? 1 : 2;
   else if (k == "bp_group") c->bp_group = (int)v;
   else if (k == "bp_ladder") c->bp_ladder = (int)v;
   else if (k == "bp_init") c->bp_init = (int)v;
@@ -1217,6 +1223,7 @@ int batch_p2(pepo_ctx* c, BatchState& S) {
       sc.ld_in[g] = t1.r; sc.ld_out[g] = t1.r;
       sb.K[g] = L.K; sb.ldk[g] = t1.r; sb.r1[g] = t1.r; sb.r2[g] = t2.r;
       sb.G[g] = L.G; sb.V[g] = L.V; sb.sv[g] = L.sv; sb.order[g] = L.order; sb.sweeps[g] = L.ints + 1;
+      sb.orient[g] = L.orient; fb.orient[g] = L.orient;
       fb.K[g] = L.K; fb.ldk[g] = t1.r;
       fb.r1[g] = t1.r; fb.r2[g] = t2.r; fb.G[g] = L.G; fb.V[g] = L.V; fb.sv[g] = L.sv; fb.order[g] = L.order;
       fb.Us[g] = L.Us; fb.ldus[g] = t1.r; fb.Vs[g] = L.Vs; fb.ldvs[g] = t2.r;
@@ -1241,7 +1248,7 @@ int batch_p2(pepo_ctx* c, BatchState& S) {
       {
         ProfScope ps(c, PC_SVD, 0, 0);
         rc = launch_svd_jacobi(st, sb, c->jacobi_tol, c->jacobi_max_sweeps, false, c->svd_precond_min, c->jacobi_early,
-                               c->chi_max, c->svd_deflate);
+                               c->chi_max, c->svd_deflate, c->svd_orient);
         if (rc) return rc;
       }
       ProfScope ps(c, PC_SVD, 0, 0);

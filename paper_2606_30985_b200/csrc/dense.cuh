@@ -55,6 +55,8 @@ struct SvdBatch {
   double* sv[PEPO_MAXT];                            // Nc singular values (sorted, descending)
   int* order[PEPO_MAXT];                            // Nc ints scratch
   int* sweeps[PEPO_MAXT];                           // device int
+  // device int or nullptr, OUT: 1 = a square core (r1 == r2) was iterated as K^T (see `orient` below)
+  int* orient[PEPO_MAXT] = {};
 };
 // with_v = false: V is not accumulated (launch_svd_bridge then derives it from K, SvdFinishBatch::K)
 // precond_min > 0 (only with_v = false): problems with min(r1,r2) >= precond_min are QR-preconditioned
@@ -64,14 +66,20 @@ struct SvdBatch {
 // keep_hint > 0 and theta > 0 (hot-path kernel only): only the leading keep_hint triplets are needed
 // (truncation to chi_max); after 3 full sweeps the columns with norm < theta x the keep_hint-th largest
 // norm are set aside and the iteration continues on the rest (svd.cu "deflation")
+// orient (hot-path kernel, preconditioned SQUARE cores only; needs SvdBatch::orient): which of K, K^T
+// gets the QR preconditioner.  0 = K; 1 = the one whose column norms are more graded (larger variance
+// of ln ||col||^2: an unpivoted QR then leaves an L = R^T that is closer to diagonal, 9 Jacobi sweeps
+// instead of 19-21 on the far-corner cores of the 4x4 chi 60 step); 2 = K^T.  The choice is a function
+// of K alone; launch_svd_bridge reads it back through SvdFinishBatch::orient.
 int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
-                      int precond_min, double early, int keep_hint = 0, double theta = 0.0);
+                      int precond_min, double early, int keep_hint = 0, double theta = 0.0, int orient = 0);
 
 struct SvdFinishBatch {
   int count;
   int r1[PEPO_MAXT]; int r2[PEPO_MAXT];
   const double* G[PEPO_MAXT]; const double* V[PEPO_MAXT]; const double* sv[PEPO_MAXT];
   const int* order[PEPO_MAXT];
+  const int* orient[PEPO_MAXT] = {};                // as written by launch_svd_jacobi (nullptr = 0)
   int with_v;                                       // 1: V accumulated by the Jacobi kernel; 0: derive from K
   int precond_min;                                  // as passed to launch_svd_jacobi (with_v = 0)
   const double* K[PEPO_MAXT]; int ldk[PEPO_MAXT];   // the core (needed when with_v = 0)

@@ -98,6 +98,7 @@ __global__ void __launch_bounds__(1024) jacobi_svd_kernel(SvdBatch b, double tol
   const int ldk = b.ldk[t];
   double* G = b.G[t];
   double* V = b.V[t];
+  if (b.orient[t] != nullptr && threadIdx.x == 0) *b.orient[t] = 0;   // this kernel never flips a square core
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = blockDim.x >> 5;
   // load
   double fro = 0.0;
@@ -241,6 +242,7 @@ jacobi_cluster_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, in
   const int r1 = b.r1[t], r2 = b.r2[t];
   const bool tr = r1 < r2;
   const int M = tr ? r2 : r1, Nc = tr ? r1 : r2;
+  if (b.orient[t] != nullptr && crank == 0 && threadIdx.x == 0) *b.orient[t] = 0;   // never flips a square core
   // column layout: [G part: M, zero-padded to MP (even)] [V part: Nc, zero-padded, only with_v];
   // LEN (even, same for the whole launch) >= MP + (with_v ? Nc : 0)
   const int MP = (M + 1) & ~1;
@@ -613,14 +615,14 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 template <int NREG, int NTHR>
 __global__ void __launch_bounds__(NTHR, 1)
 jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int precond_min, int pw,
-                  double early2, int keep_hint, int nfull, double theta) {
+                  double early2, int keep_hint, int nfull, double theta, int orient_mode) {
   constexpr int LEN = 32 * NREG, LEN2 = 16 * NREG;
   extern __shared__ __align__(16) double jsm[];
   cg::cluster_group cluster = cg::this_cluster();
   const int crank = (int)cluster.block_rank();
   const int t = blockIdx.x / CS;
   const int r1 = b.r1[t], r2 = b.r2[t];
-  const bool tr = r1 < r2;
+  bool tr = r1 < r2;                      // a square core may still be flipped below (orient_mode)
   const int M = tr ? r2 : r1, Nc = tr ? r1 : r2;
   const int MP = (M + 1) & ~1;
   int Mj = M;
@@ -666,6 +668,68 @@ jacobi_c16_kernel(SvdBatch b, double tol, int max_sweeps, int bs, int CS, int pr
   const double noise2 = 1e-30 * ref;
   // ---- QR preconditioning (as in jacobi_cluster_kernel): iterate on L = R^T ------------------
   const bool precond = precond_min > 0 && Nc >= precond_min && ref > 0.0 && isfinite(ref);
+  // ---- which of K, K^T gets the QR (square cores; dense.cuh, launch_svd_jacobi `orient`) -------
+  // An unpivoted QR preconditions well when the COLUMNS it sweeps are strongly graded; which side of a
+  // Schmidt-dressed core is the graded one depends on the bond (measured: 9 sweeps vs 19-21).  The
+  // grading is measured as the variance of ln ||.||^2 over the columns and over the rows; every CTA of
+  // the cluster forms the same sums in the same order, so the decision is uniform and a function of K.
+  int* orient_out = b.orient[t];
+  bool flip = false;
+  if (precond && r1 == r2 && orient_out != nullptr && orient_mode > 0) {
+    flip = orient_mode == 2;
+    if (orient_mode == 1) {
+      for (int k = tid; k < M; k += NTHR) {             // row sums over my columns
+        double a = 0.0;
+        for (int ci = 0; ci < 2 * bs; ci++) { const double x = cols[(size_t)ci * LEN + k]; a = fma(x, x, a); }
+        vbuf[k] = a;
+      }
+      double c1 = 0.0, c2 = 0.0;                        // my columns: sum ln, sum ln^2
+      for (int ci = warp; ci < 2 * bs; ci += nw) {
+        if (ids[ci] >= Nc) continue;
+        double a = 0.0;
+        for (int k = lane; k < M; k += 32) { const double x = cols[(size_t)ci * LEN + k]; a = fma(x, x, a); }
+        a = warp_sum1(a);
+        const double l = log(fmax(a, noise2));
+        c1 += l; c2 += l * l;
+      }
+      __syncthreads();                                  // s_red was read by thread 0 above
+      if (lane == 0) { s_red[warp] = c1; s_red[16 + warp] = c2; }
+      __syncthreads();
+      if (tid == 0) {
+        double a1 = 0.0, a2 = 0.0;
+        for (int w = 0; w < nw; w++) { a1 += s_red[w]; a2 += s_red[16 + w]; }
+        scal[1] = a1; scal[2] = a2;
+      }
+      cluster.sync();
+      double C1 = 0.0, C2 = 0.0;
+      for (int c = 0; c < CS; c++) { const double* sc = cluster.map_shared_rank(scal, c); C1 += sc[1]; C2 += sc[2]; }
+      double q1 = 0.0, q2 = 0.0;                        // rows: full sums through DSMEM
+      for (int k = tid; k < M; k += NTHR) {
+        double a = 0.0;
+        for (int c = 0; c < CS; c++) a += cluster.map_shared_rank(vbuf, c)[k];
+        const double l = log(fmax(a, noise2));
+        q1 += l; q2 += l * l;
+      }
+      q1 = warp_sum1(q1); q2 = warp_sum1(q2);
+      if (lane == 0) { s_red[warp] = q1; s_red[16 + warp] = q2; }
+      __syncthreads();
+      double R1 = 0.0, R2 = 0.0;
+      for (int w = 0; w < nw; w++) { R1 += s_red[w]; R2 += s_red[16 + w]; }
+      const double varC = C2 - C1 * C1 / (double)Nc, varR = R2 - R1 * R1 / (double)M;
+      flip = varR > varC;
+      cluster.sync();                                   // vbuf and scal are free again (panel broadcast below)
+    }
+    if (flip) {
+      tr = true;
+      for (int e = tid; e < per; e += NTHR) {
+        const int k = e % LEN, ci = e / LEN;
+        const int j = ((ci / bs) ? 2 * CS - 1 - crank : crank) * bs + (ci % bs);
+        cols[e] = (j < Nc && k < M) ? K[j + (long long)k * ldk] : 0.0;
+      }
+      __syncthreads();
+    }
+  }
+  if (orient_out != nullptr && crank == 0 && tid == 0) *orient_out = flip ? 1 : 0;
   if (precond) {
     const int VS = MP + 2;
     const int nblk = (Nc + bs - 1) / bs;
@@ -1082,7 +1146,8 @@ __global__ void svd_bridge_kernel(SvdFinishBatch b) {
 __global__ void __launch_bounds__(256) svd_bridge_nov_kernel(SvdFinishBatch b) {
   const int t = blockIdx.y;
   const int r1 = b.r1[t], r2 = b.r2[t];
-  const bool tr = r1 < r2;
+  // a square core may have been iterated as K^T (launch_svd_jacobi `orient`)
+  const bool tr = r1 < r2 || (r1 == r2 && b.orient[t] != nullptr && *b.orient[t] != 0);
   const int M = tr ? r2 : r1, Nc = tr ? r1 : r2;
   const bool precond = b.precond_min > 0 && Nc >= b.precond_min;
   // columns of G (ld M): left vectors of the tall problem A (= K, or K^T if tr) times s; with the
@@ -1179,14 +1244,14 @@ int launch_set_identity(cudaStream_t st, double* Q, long long m, int k) {
 }
 
 static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
-                            int precond_min, double early, int keep_hint, double theta);
+                            int precond_min, double early, int keep_hint, double theta, int orient);
 
 // The launch configuration (cluster size, columns per CTA, register tile) fixes the order of the
 // pair rotations, i.e. the rounding of the result.  It is therefore chosen per problem SIZE, never
 // from the composition of the batch: problems of equal (min, max) dimension share a launch, and a
 // gate gives bit-identical results whichever other gates run beside it (serial or pipelined class).
 int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
-                      int precond_min, double early, int keep_hint, double theta) {
+                      int precond_min, double early, int keep_hint, double theta, int orient) {
   if (b.count == 0) return 0;
   bool done[PEPO_MAXT] = {false};
   for (int t0 = 0; t0 < b.count; t0++) {
@@ -1198,16 +1263,17 @@ int launch_svd_jacobi(cudaStream_t st, const SvdBatch& b, double tol, int max_sw
       const int q = g.count++;
       g.K[q] = b.K[t]; g.ldk[q] = b.ldk[t]; g.r1[q] = b.r1[t]; g.r2[q] = b.r2[t];
       g.G[q] = b.G[t]; g.V[q] = b.V[t]; g.sv[q] = b.sv[t]; g.order[q] = b.order[t]; g.sweeps[q] = b.sweeps[t];
+      g.orient[q] = b.orient[t];
       done[t] = true;
     }
-    int rc = launch_svd_group(st, g, tol, max_sweeps, with_v, precond_min, early, keep_hint, theta);
+    int rc = launch_svd_group(st, g, tol, max_sweeps, with_v, precond_min, early, keep_hint, theta, orient);
     if (rc) return rc;
   }
   return 0;
 }
 
 static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int max_sweeps, bool with_v,
-                            int precond_min, double early, int keep_hint, double theta) {
+                            int precond_min, double early, int keep_hint, double theta, int orient) {
   if (b.count == 0) return 0;
   int ncmax = 1, lenmax = 2;
   for (int t = 0; t < b.count; t++) {
@@ -1271,12 +1337,12 @@ static int launch_svd_group(cudaStream_t st, const SvdBatch& b, double tol, int 
       const double early2 = early * early;
       const int kh = (theta > 0.0) ? keep_hint : 0;
       cudaError_t e;
-      if (nreg == 2) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<2, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta);
-      else if (nreg == 4) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<4, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta);
-      else if (nreg == 6) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<6, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta);
-      else if (nreg == 8) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<8, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta);
-      else if (nreg == 10) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<10, 256>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta);
-      else e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<13, 256>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta);
+      if (nreg == 2) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<2, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta, orient);
+      else if (nreg == 4) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<4, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta, orient);
+      else if (nreg == 6) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<6, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta, orient);
+      else if (nreg == 8) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<8, 512>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta, orient);
+      else if (nreg == 10) e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<10, 256>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta, orient);
+      else e = cudaLaunchKernelEx(&cfg, jacobi_c16_kernel<13, 256>, b, tol, max_sweeps, bs, CS, precond_min, pw, early2, kh, 3, theta, orient);
       if (e != cudaSuccess) { set_error("svd: cluster launch failed: %s", cudaGetErrorString(e)); return -3; }
       PEPO_COUNT_LAUNCH();
       return 0;

@@ -100,8 +100,8 @@ def closed_form_bytes(Lx, Ly, chi, B):
     lane = 2 * slot + 4 * N * N + 2 * N * chi
     doubles += B * lane
     # every sub-buffer starts on a 256-byte boundary and is followed by 64 guard bytes (pepo_check_guards):
-    # 4 buffers per site, 21 global ones, 14 + one per site class per lane slot, 8 per lane
-    n_buffers = 4 * Lx * Ly + 33 + B * (2 * (14 + len([d for d in degs if d >= 1])) + 8)
+    # 4 buffers per site, 34 global ones, 14 + one per site class per lane slot, 8 per lane
+    n_buffers = 4 * Lx * Ly + 34 + B * (2 * (14 + len([d for d in degs if d >= 1])) + 8)
     return 8 * doubles + n_buffers * (128 + 64)
 
 

@@ -201,6 +201,40 @@ def test_config2_first_steps_vs_oracle(gpu):
     sim.close()
 
 
+def test_config2_saturated_whole_step_vs_oracle(gpu):
+    """BASELINE configs[1] at FULL size, one whole Trotter step + BP in the saturated regime (every bond = 60,
+    truncation active: 24 Algorithm-1 gates with 240 x 240 cores, interior m = 216000): the CUDA path's own
+    state after step 30 is loaded into the oracle (tests-only), both sides take step 31 from identical
+    inputs.  Compared: every bond's lambda (gauge invariant), the discarded weight, C(t), BP status.
+    The oracle needs 2-5 min for this step on the box's host cores."""
+    torch, B = gpu
+    from oracle import pepo_oracle as po
+    L, chi = 4, 60
+    sim = B.Pepo(L, L, 1, 1, J, H, DT, chi, 1e-10, 0.5)
+    for _ in range(30):
+        sim.trotter_step()
+    dims = sim.bond_dims()
+    assert min(dims) == chi
+    st = po.PEPOState(L, L, 1, 1, J, H, DT, chi)
+    for e in range(sim.n_bonds):
+        st.lam[e] = sim.get_lambda(e)
+    for v in range(L * L):
+        shape = [dims[st.lat.bond_id(v, d)] for d in st.lat.legs(v)] + [4]
+        st.psi[v] = sim.get_site(v % L, v // L).reshape(shape, order="F").copy()
+    st.trotter_step()
+    so, swo, _ = st.bp_converge(1e-10, 0.5)
+    sim.trotter_step()
+    sg, swg, _ = sim.bp_converge()
+    assert sim.bond_dims() == st.bond_dims()
+    for e in range(sim.n_bonds):
+        assert np.max(np.abs(sim.get_lambda(e) - np.asarray(st.lam[e]))) <= 1e-12, e
+    ge = sim.stats()["gate_err"]
+    assert ge > 1e-8 and abs(ge - st.gate_err) <= 1e-9 * st.gate_err          # truncation is active
+    assert sg == so == 0 and abs(swg - swo) <= 2
+    assert abs(sim.correlation() - st.correlation()) <= 1e-12
+    sim.close()
+
+
 def test_config2_saturated_properties(gpu):
     """On the state bench.py times (every bond = 60 after the physical preparation) no oracle run
     is affordable: check what holds at any size."""
