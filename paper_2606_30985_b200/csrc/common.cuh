@@ -126,6 +126,8 @@ int launch_dgemm_batched(cudaStream_t st, int transA, int transB, const GemmProb
 int launch_gram_reduce(cudaStream_t st, const double* part, int ksplit, int n, double* C,
                        long long ldc);
 void gram_plan(long long m, int n, int* ksplit, int* kchunk);
+// largest split count gram_plan returns for any row count <= m (sizing of a shared split-K workspace)
+int gram_max_splits(long long m, int n);
 // register-only DMMA loop (fp64 tensor-pipe yardstick of bench.py); *flops = flops of the launch
 int launch_dmma_peak(cudaStream_t st, int iters, int ctas_per_sm, double* sink, double* flops);
 

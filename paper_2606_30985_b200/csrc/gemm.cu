@@ -563,6 +563,25 @@ int launch_dgemm_batched(cudaStream_t st, int transA, int transB, const GemmProb
 
 constexpr int GRAM_WAVES = 2;      // waves of resident CTAs of the 80x80 Gram kernel (1 and 2 measured equal, 3+ slower)
 
+// Upper bound of gram_plan's split count over every row count <= m: the count before the chunk is rounded
+// up to 16 rows.  (The rounded count is NOT monotone in m - 62400 rows give 195 splits of 320, 64000 rows
+// 191 of 336 - so a workspace shared by all sites of a run is sized with this bound, not with gram_plan
+// of the largest m.)
+int gram_max_splits(long long m, int n) {
+  int ks, kc;
+  gram_plan(m, n, &ks, &kc);
+  long long best = ks;
+  // ks = ceil(m' / kc) <= the unrounded count, which grows with m' through the 256-rows-per-split rule only
+  int bt = 128, target = 148 * 2, cap = 128; bool whole = false;
+  if (n % 80 == 0) { bt = 80; target = 148 * 2 * GRAM_WAVES; cap = 100 * GRAM_WAVES; whole = true; }
+  else if (n <= 64) { bt = 64; target = 148 * 4; cap = 1024; }
+  const int tn = (n + bt - 1) / bt, upper = tn * (tn + 1) / 2;
+  long long k0 = whole ? std::max(1, target / upper) : (target + upper - 1) / upper;
+  k0 = std::min<long long>(k0, (m + 255) / 256);
+  k0 = std::max<long long>(1, std::min<long long>(k0, cap));
+  return (int)std::max(best, k0);
+}
+
 void gram_plan(long long m, int n, int* ksplit, int* kchunk) {
   // upper-triangle tiles at the tile size launch_dgemm will pick (the choice between the 128 and
   // 64 tiles depends on ksplit itself: plan with the 128 tile first, as before)

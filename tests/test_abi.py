@@ -5,6 +5,7 @@ import ctypes
 import os
 import re
 
+import numpy as np
 import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -52,10 +53,12 @@ def test_bad_arguments_do_not_need_a_gpu(lib):
     assert b"NULL" in lib.pepo_last_error()
 
 
-def gram_splits(m, n):
+def gram_splits(m, n, bound=False):
     """Split-K factor of the Gram kernel, restated from DESIGN.md section 5 (independent of the library):
     upper-triangle tiles of 80 (n % 80 == 0), 64 (n <= 64) or 128; enough splits to fill 2 resident CTAs on
-    148 SMs (two whole waves for the 80-tile), at least 256 rows per split, chunks rounded up to 16 rows."""
+    148 SMs (two whole waves for the 80-tile), at least 256 rows per split, chunks rounded up to 16 rows.
+    bound=True: the count before the chunk rounding = the largest count any m' <= m can get (the rounded
+    count is not monotone in m; the per-lane workspace of a run is sized with the bound)."""
     if n % 80 == 0:
         bt, target, cap, whole = 80, 148 * 2 * 2, 200, True
     elif n <= 64:
@@ -66,6 +69,8 @@ def gram_splits(m, n):
     upper = tn * (tn + 1) // 2
     ks = max(1, target // upper) if whole else -(-target // upper)
     ks = max(1, min(ks, (m + 255) // 256, cap))
+    if bound:
+        return ks
     kc = -(-m // ks)
     kc = -(-kc // 16) * 16
     return -(-m // kc)
@@ -94,7 +99,7 @@ def closed_form_bytes(Lx, Ly, chi, B):
     degmax = max(degs)
     m_max = chi ** max(degmax - 1, 0)
     ld = (m_max + 1) // 2 * 2
-    part = max(gram_splits(m_max, 4 * c) * (4 * c) ** 2 for c in range(1, chi + 1))
+    part = max(gram_splits(m_max, 4 * c, bound=True) * (4 * c) ** 2 for c in range(1, chi + 1))
     spares = sum(4 * chi ** d for d in degs if 1 <= d < degmax) + max(ld * n, 4 * chi ** degmax)
     slot = ld * n + spares + part + n * n + 2 * N * N + n * n + 4 * n * N + N * chi + n * 4 * chi + 4 * n * chi
     lane = 2 * slot + 4 * N * N + 2 * N * chi
@@ -112,6 +117,24 @@ def test_memory_model_matches_closed_form(lib, Lx, Ly, chi):
         got = lib.pepo_arena_bytes_ex(Lx, Ly, chi, B)
         want = closed_form_bytes(Lx, Ly, chi, B)
         assert abs(got - want) <= 0.02 * want, (got, want)
+
+
+def test_split_k_workspace_covers_every_smaller_row_count(lib):
+    """The per-lane split-K workspace is shared by all the sites a lane meets, with every row count m <= m_max
+    (mixed bond dimensions during growth).  pepo_gram_ws_bytes(m, n) is not monotone in m (62400 x 160 needs
+    195 splits, 64000 x 160 only 191: seen as an overwritten arena guard at 4x4 chi 40, step 11), so the
+    layout's bound must cover all of them."""
+    lib.pepo_gram_ws_bytes.restype = ctypes.c_size_t
+    lib.pepo_gram_ws_bytes.argtypes = [ctypes.c_longlong, ctypes.c_int]
+    assert lib.pepo_gram_ws_bytes(62400, 160) > lib.pepo_gram_ws_bytes(64000, 160)
+    rng = np.random.default_rng(3)
+    for chi in (40, 60):
+        m_max = chi ** 3
+        cap = 8 * max(gram_splits(m_max, 4 * c, bound=True) * (4 * c) ** 2 for c in range(1, chi + 1))
+        dims = list(range(max(1, chi - 12), chi + 1))
+        for _ in range(4000):
+            a, b, c3, cc = rng.choice(dims, 4)
+            assert lib.pepo_gram_ws_bytes(int(a * b * c3), int(4 * cc)) <= cap + 256, (a, b, c3, cc)
 
 
 def test_config5_sized_to_fit_180GB(lib):

@@ -199,6 +199,7 @@ def test_reduced_chi_twins_vs_stored_oracle(gpu, name, L, centre, chi_max, tol):
         if r["sweeps"] < 60 and sweeps < 60:
             assert abs(sweeps - r["sweeps"]) <= 8 + 0.1 * r["sweeps"], (r["step"], sweeps, r["sweeps"])
     print("%s: max |C_gpu - C_oracle| = %.2e over %d steps" % (name, worst, len(rows)))
+    sim.check_guards()          # every buffer of the arena kept to its bounds through growth and saturation
     sim.close()
 
 
