@@ -241,6 +241,20 @@ size_t pepo_gram_ws_bytes(long long m, int n);
 int pepo_gram(const double* d_A, long long m, int n, long long lda, double* d_C, void* d_ws,
               size_t ws_bytes, void* stream);
 
+/* The same Gram matrix for callers that may not allocate device memory (CUDA graph capture, serving
+ * loops, harnesses that forbid cudaMalloc): same kernels and split plan as pepo_gram - identical bits -
+ * with the split-K partial sums in a device array built into the library (PEPO_STATIC_SCRATCH_BYTES,
+ * held by every GPU that loads the library until exit) instead of a caller workspace.  Allocates
+ * nothing; looks the array's device address up once per device.  d_A (m x n, lda >= m) and d_C (n x n,
+ * both triangles) are the caller's DEVICE buffers.  Returns -2 with a message naming the needed size
+ * when the plan needs more scratch than the array holds (e.g. 256000 x 40 fits, 256000 x 160 does not).
+ * All calls on a device share the array: calls that overlap on the GPU (different streams, no event
+ * between them) race; the array keeps the last call's contents, none of which a later call reads before
+ * writing it. */
+#define PEPO_STATIC_SCRATCH_BYTES (8u << 20)
+size_t pepo_static_scratch_bytes(void);
+int pepo_gram_static(const double* d_A, long long m, int n, long long lda, double* d_C, void* stream);
+
 /* Permute-on-load contractions of the bond gate (what pepo_trotter_step runs on the Cholesky path:
  * the explicit permutation of PAPER.md section 4.1 and the absorb / de-absorb passes a3 / a12 are
  * folded into the two tall GEMMs, which leaves 2 reads + 1 write of psi per site and gate).

@@ -80,6 +80,8 @@ def _load():
         "pepo_permute_scaled": (i, [dp, dp, ip, ip, i, C.POINTER(vp), vp]),
         "pepo_gram_ws_bytes": (sz, [ll, i]),
         "pepo_gram": (i, [dp, ll, i, ll, dp, vp, sz, vp]),
+        "pepo_static_scratch_bytes": (sz, []),
+        "pepo_gram_static": (i, [dp, ll, i, ll, dp, vp]),
         "pepo_site_gram_ws_bytes": (sz, [ip, i, i]),
         "pepo_site_gram": (i, [dp, ip, i, i, C.POINTER(vp), dp, vp, sz, vp]),
         "pepo_site_apply": (i, [dp, ip, i, i, dp, i, dp, vp]),
@@ -316,6 +318,20 @@ def gram(A_cm, m, n, ws=None):
     ws = ws if ws is not None else _ws(_lib.pepo_gram_ws_bytes(m, n), A_cm.device)
     _check(_lib.pepo_gram(_f64(A_cm, "A"), m, n, m, _f64(Cm, "C"), C.c_void_p(ws.data_ptr()), ws.numel(), _stream()))
     return Cm
+
+
+def static_scratch_bytes():
+    return int(_lib.pepo_static_scratch_bytes())
+
+
+def gram_static(A_cm, m, n, out):
+    """pepo_gram_static: C = A^T A into the caller's `out` (n*n float64 on A's device) with the split-K
+    scratch in the library's built-in device array: no allocation anywhere.  Raises PepoError(-2) when
+    the plan needs more than static_scratch_bytes().  Calls on one device must not overlap on the GPU."""
+    if out.numel() < n * n:
+        raise PepoError(-1, "gram_static: out too small")
+    _check(_lib.pepo_gram_static(_f64(A_cm, "A"), m, n, m, _f64(out, "out"), _stream()))
+    return out
 
 
 def site_gram(psi, dims, cut, w2=None):
