@@ -4,6 +4,8 @@
 //   (a10, L102).  The Jacobi SVD lives in svd.cu.
 #include "dense.cuh"
 #include <algorithm>
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
 
 namespace pepo {
 namespace {
@@ -298,6 +300,68 @@ __device__ void hh_apply_stored(const double* __restrict__ x, double beta, doubl
 }
 
 // single CTA per task: whole factorisation, column per warp
+// hh_reflect<32> for the cluster kernel below: same arithmetic in the same order (bit-identical
+// results), every load through L2 (__ldcg): the column a warp reads may have been written by a
+// warp of another CTA of the cluster one step earlier, and L1 is not coherent between SMs.
+__device__ void hh_reflect_cg(const double* x, double* y, long long len, int lane,
+                              double* beta_out, double* tau_out) {
+  double sxx = 0.0, sxy = 0.0;
+  for (long long i = lane; i < len; i += 32) {
+    double xi = __ldcg(x + i);
+    sxx += xi * xi;
+    if (y) sxy += xi * __ldcg(y + i);
+  }
+  sxx = warp_sum(sxx);
+  if (y) sxy = warp_sum(sxy);
+  const double x0 = __ldcg(x);
+  const double nrm = sqrt(sxx);
+  double beta = (x0 >= 0.0) ? -nrm : nrm;
+  double tau = 0.0;
+  if (sxx > 1e-290) tau = 1.0 / (nrm * (nrm + fabs(x0)));
+  else beta = x0;
+  if (beta_out && lane == 0) { *beta_out = beta; *tau_out = tau; }
+  if (!y || tau == 0.0) return;
+  const double y0 = __ldcg(y);
+  const double w = tau * (sxy - beta * y0);
+  __syncwarp();
+  for (long long i = lane; i < len; i += 32) {
+    double vi = __ldcg(x + i) - (i == 0 ? beta : 0.0);
+    y[i] = __ldcg(y + i) - w * vi;
+  }
+}
+
+// The small factorisation spread over a thread-block cluster: the warps of all CS CTAs take the
+// columns c > j of step j (column per warp, as in the single-CTA kernel), a cluster barrier ends
+// the step.  The matrix stays in global memory (<= 2 MB: L2-resident).  Growth phase of a run:
+// the single-CTA kernel took up to 16 ms for a 1090 x 240 matrix (one SM, 240 dependent steps of
+// 15 column updates per warp).
+__global__ void __launch_bounds__(512) hh_factor_small_cluster_kernel(HHBatch b, int small_limit_log2, int CS) {
+  cg::cluster_group cluster = cg::this_cluster();
+  const int crank = (int)cluster.block_rank();
+  const int t = blockIdx.x / CS;
+  const long long m = b.m[t];
+  const int n = b.n[t];
+  if (m * (long long)n > (1ll << small_limit_log2)) return;      // uniform over the cluster
+  double* A = b.A[t];
+  const long long lda = b.lda[t];
+  const int k = (int)min((long long)n, m);
+  const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+  const int gw = crank * nw + (threadIdx.x >> 5), gnw = CS * nw;
+  for (int j = 0; j < k; j++) {
+    const double* x = A + j + (long long)j * lda;
+    const long long len = m - j;
+    if (j + 1 >= n) {
+      if (gw == 0) hh_reflect_cg(x, nullptr, len, lane, b.beta[t] + j, b.tau[t] + j);
+    } else {
+      for (int c = j + 1 + gw; c < n; c += gnw)
+        hh_reflect_cg(x, A + j + (long long)c * lda, len, lane,
+                      (c == j + 1) ? b.beta[t] + j : nullptr, b.tau[t] + j);
+    }
+    __threadfence();
+    cluster.sync();
+  }
+}
+
 __global__ void __launch_bounds__(512) hh_factor_small_kernel(HHBatch b, int small_limit_log2) {
   const int t = blockIdx.x;
   const long long m = b.m[t];
@@ -368,9 +432,9 @@ __global__ void __launch_bounds__(512) hh_apply_small_kernel(HHApplyBatch b, int
   const int t = blockIdx.x;
   const long long m = b.m[t];
   if (m * (long long)max(b.k[t], b.ncols[t]) > (1ll << small_limit_log2)) return;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  // columns are independent: each warp runs all reflectors over its own columns
-  for (int c = warp; c < b.ncols[t]; c += nw) {
+  const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+  // columns are independent: each warp (of the gridDim.y CTAs of a task) runs all reflectors over its own columns
+  for (int c = blockIdx.y * nw + (threadIdx.x >> 5); c < b.ncols[t]; c += gridDim.y * nw) {
     double* y = b.Y[t] + (long long)c * b.ldy[t];
     for (int j = b.k[t] - 1; j >= 0; j--) {
       hh_apply_stored<32>(b.A[t] + j + (long long)j * b.lda[t], b.beta[t][j], b.tau[t][j], y + j,
@@ -572,7 +636,26 @@ int launch_hh_factor(cudaStream_t st, const HHBatch& b) {
     }
   }
   if (any_small) {
-    hh_factor_small_kernel<<<b.count, 512, 0, st>>>(b, SMALL_LOG2);
+    // matrices of more than a few columns: the cluster form (8 CTAs share the columns of a step)
+    int nsmall = 0; long long wsmall = 0;
+    for (int t = 0; t < b.count; t++)
+      if (b.m[t] * (long long)b.n[t] <= (1ll << SMALL_LOG2)) { nsmall = std::max(nsmall, b.n[t]); wsmall = std::max(wsmall, b.m[t] * (long long)b.n[t]); }
+    bool done = false;
+    if (nsmall > 32 && wsmall > 4096) {
+      const int CS = 8;
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)(b.count * CS));
+      cfg.blockDim = dim3(512);
+      cfg.dynamicSmemBytes = 0;
+      cfg.stream = st;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      cudaError_t e = cudaLaunchKernelEx(&cfg, hh_factor_small_cluster_kernel, b, (int)SMALL_LOG2, CS);
+      if (e == cudaSuccess) done = true; else (void)cudaGetLastError();
+    }
+    if (!done) hh_factor_small_kernel<<<b.count, 512, 0, st>>>(b, SMALL_LOG2);
     PEPO_COUNT_LAUNCH();
   }
   for (int j = 0; j < kbig; j++) {
@@ -607,7 +690,10 @@ int launch_hh_apply_q(cudaStream_t st, const HHApplyBatch& b) {
     else { any_big = true; cbig = std::max(cbig, b.ncols[t]); }
   }
   if (any_small) {
-    hh_apply_small_kernel<<<b.count, 512, 0, st>>>(b, SMALL_LOG2);
+    int csmall = 1;
+    for (int t = 0; t < b.count; t++)
+      if (b.m[t] * (long long)std::max(b.k[t], b.ncols[t]) <= (1ll << SMALL_LOG2)) csmall = std::max(csmall, b.ncols[t]);
+    hh_apply_small_kernel<<<dim3(b.count, std::min((csmall + 15) / 16, 16)), 512, 0, st>>>(b, SMALL_LOG2);
     PEPO_COUNT_LAUNCH();
   }
   if (any_big) {
