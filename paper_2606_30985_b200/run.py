@@ -103,6 +103,7 @@ def main():
               % (step, c, row["trotter_ms"], row["bp_ms"], sweeps, status, row["chi_min"], row["chi_max"], st["gate_err"]),
               flush=True)
     wall = time.perf_counter() - t_start
+    sim.check_guards()          # raises if any kernel wrote past one of the arena's buffers during the run
     st = sim.stats()
     sat = [r for r in rows if r["chi_min"] == chi]
     summary = dict(config=args.config, L=L, chi_max=chi, steps=cfg["steps"], wall_s=wall,
@@ -129,7 +130,7 @@ def main():
                     % (summary["arena_model_bytes"] / 1e9, summary["arena_bytes"] / 1e9, summary["arena_tensor_bytes"] / 1e9,
                        summary["mem_get_info_delta_bytes"] / 1e9, summary["hbm_total_bytes"] / 1e9, summary["inflight_gates"]))
             f.write("Trotter time %.2f s, BP + Bethe time %.2f s, wall %.2f s; %.2f Trotter steps/s over the whole run%s; "
-                    "%d kernel launches.\n\n" % (summary["trotter_s"], summary["bp_s"], summary["wall_s"],
+                    "%d kernel launches; arena guard zones intact after the run (pepo_check_guards).\n\n" % (summary["trotter_s"], summary["bp_s"], summary["wall_s"],
                                                  summary["steps_per_s_whole_run"],
                                                  (", %.2f over the saturated steps" % summary["steps_per_s_saturated"])
                                                  if summary["steps_per_s_saturated"] else "", summary["kernel_launches"]))
