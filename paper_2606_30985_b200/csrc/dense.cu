@@ -21,7 +21,14 @@ constexpr int PB = 32;   // block size
 
 struct InfoPtrs { int* p[PEPO_MAXT]; };
 
-__global__ void __launch_bounds__(512) potrf_upper_kernel(MatBatch b, InfoPtrs info, double tau) {
+// Footprint: 256 threads x 128 registers = half of an SM's register file.  The kernel is latency-bound
+// and was 10 % faster alone with 512 threads, but a CTA that needs the whole register file can only
+// start on an SM that has drained completely, and in a Trotter step the GEMM CTAs of the other pieces
+// keep refilling every SM: measured in the pipelined 4x4 chi = 60 step, POTRF 0.58 ms against 0.40 ms
+// alone, and the step 36.2 ms against 34.6 ms with this footprint (128 threads: 35.4).  Any thread count
+// gives the same bits (every entry is computed by one thread in a fixed order).
+constexpr int POTRF_THREADS = 256;
+__global__ void __launch_bounds__(POTRF_THREADS, 2) potrf_upper_kernel(MatBatch b, InfoPtrs info, double tau) {
   extern __shared__ double sm[];
   const int t = blockIdx.x;
   double* A = b.A[t];
@@ -591,7 +598,7 @@ int launch_potrf(cudaStream_t st, const MatBatch& b, int* const* info, double ta
   if (first_use_on_device(attr))
     PEPO_CUDA_OK(cudaFuncSetAttribute(potrf_upper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   if (smem > (size_t)200 * 1024) { set_error("potrf: matrix of order %d too large", nmax); return -1; }
-  potrf_upper_kernel<<<b.count, 512, smem, st>>>(b, ip, tau);
+  potrf_upper_kernel<<<b.count, POTRF_THREADS, smem, st>>>(b, ip, tau);
   PEPO_COUNT_LAUNCH();
   PEPO_CUDA_OK(cudaGetLastError());
   return 0;
