@@ -1590,6 +1590,19 @@ int run_step_piped_impl(pepo_ctx* c) {
           if (ready) rdy.push_back(g);
         }
         if (rdy.empty()) continue;
+        if (c->lazy_field && c->n_pending > 0) {
+          // asynchronous uploads in flight (pepo_set_site_async): only gates whose two sites have ARRIVED start
+          // now; a piece that mixed an early and a late site would hold its stream until the late one is there
+          std::vector<int> here;
+          for (int g : rdy) {
+            bool ok = true;
+            for (int v : {c->bonds[G[g].bond].v1, c->bonds[G[g].bond].v2})
+              ok &= (!c->site_pending[v] || cudaEventQuery(c->site_ev[v]) == cudaSuccess);
+            if (ok) here.push_back(g);
+          }
+          if (here.empty()) continue;
+          rdy.swap(here);
+        }
         // the heaviest ready gate, then the lightest ones: every piece gets its share of the GEMM-heavy
         // gates (pieces taken in list order put the interior gates of a class on two of the four streams:
         // 38.7 against 36.6 ms per step on 4x4 chi = 60)
