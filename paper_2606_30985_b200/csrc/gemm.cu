@@ -167,8 +167,9 @@ __device__ __forceinline__ void load_tile_gather(double* s, const GatherSlots<RO
 
 constexpr int GW_MAXLEN = 256;      // longest weight vector (chi_max <= 256)
 
+// MINB: resident CTAs per SM the register allocation must allow (3 for the 64 x 80 tile: 170 registers)
 template <int TA, int TB, int BM, int BN, int WM, int WN, int STAGES, bool GATHER>
-__global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32)
+__global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, (BM == 64 && BN == 80) ? 3 : 1)
 dgemm_dmma_kernel(GemmProb p0, const GemmProb* __restrict__ probs, int ksplit, int kchunk,
                   double* __restrict__ part, int upper_only, GemmGather gg) {
   constexpr int NT = (BM / WM) * (BN / WN) * 32;
@@ -241,9 +242,8 @@ dgemm_dmma_kernel(GemmProb p0, const GemmProb* __restrict__ probs, int ksplit, i
     for (int j = 0; j < NI; j++) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
 
   const int nk = (kend - kbeg + BK - 1) / BK;
-  auto issue = [&](int it) {
+  auto issue = [&](int it, int st) {
     if (it < nk) {
-      int st = it % STAGES;
       int k0 = kbeg + it * BK;
       if (GATHER) {
         load_tile_gather<BM, A_KC, NT>(sA + st * BM * BK, gsA, gg.a_k, gg.ktabA ? sK : nullptr, kbeg, k0, kend, alignedA, tid);
@@ -266,15 +266,20 @@ dgemm_dmma_kernel(GemmProb p0, const GemmProb* __restrict__ probs, int ksplit, i
     cp_async_commit();
   };
 #pragma unroll
-  for (int s = 0; s < STAGES - 1; s++) issue(s);
+  for (int s = 0; s < STAGES - 1; s++) issue(s, s);
 
-  for (int it = 0; it < nk; it++) {
+  // the ring position of a stage is a compile-time constant in each of the STAGES unrolled copies of the body
+  for (int it0 = 0; it0 < nk; it0 += STAGES) {
+#pragma unroll
+   for (int sidx = 0; sidx < STAGES; sidx++) {
+    const int it = it0 + sidx;
+    if (it >= nk) break;
     cp_async_wait<STAGES - 2>();
     __syncthreads();
-    issue(it + STAGES - 1);
-    const double* a_s = sA + (it % STAGES) * BM * BK;
-    const double* b_s = sB + (it % STAGES) * BN * BK;
-    const double* w_s = sW + (it % STAGES) * BK;
+    issue(it + STAGES - 1, (sidx + STAGES - 1) % STAGES);
+    const double* a_s = sA + sidx * BM * BK;
+    const double* b_s = sB + sidx * BN * BK;
+    const double* w_s = sW + sidx * BK;
     if (!skip_warp) {
 #pragma unroll
       for (int kk = 0; kk < BK; kk += 4) {
@@ -302,6 +307,7 @@ dgemm_dmma_kernel(GemmProb p0, const GemmProb* __restrict__ probs, int ksplit, i
           for (int j = 0; j < NI; j++) dmma8x8x4(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
       }
     }
+   }
   }
   cp_async_wait<0>();
 
