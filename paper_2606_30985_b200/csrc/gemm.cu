@@ -168,7 +168,10 @@ __device__ __forceinline__ void load_tile_gather(double* s, const GatherSlots<RO
 constexpr int GW_MAXLEN = 256;      // longest weight vector (chi_max <= 256)
 
 // MINB: resident CTAs per SM the register allocation must allow (3 for the 64 x 80 tile: 170 registers)
-template <int TA, int TB, int BM, int BN, int WM, int WN, int STAGES, bool GATHER>
+// AL: the host has checked that both operands take the 16-byte cp.async path in every stage (the
+// 8-byte fallback is then not compiled in: the unrolled main loop is half the size, which matters for
+// the instruction cache of the short-K reconstruction CTAs)
+template <int TA, int TB, int BM, int BN, int WM, int WN, int STAGES, bool GATHER, bool AL>
 __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, (BM == 64 && BN == 80) ? 3 : 1)
 dgemm_dmma_kernel(GemmProb p0, const GemmProb* __restrict__ probs, int ksplit, int kchunk,
                   double* __restrict__ part, int upper_only, GemmGather gg) {
@@ -211,9 +214,9 @@ dgemm_dmma_kernel(GemmProb p0, const GemmProb* __restrict__ probs, int ksplit, i
   const int g = lane >> 2, t = lane & 3;
   const int wm0 = (warp % (BM / WM)) * WM, wn0 = (warp / (BM / WM)) * WN;
 
-  const bool alignedA = GATHER ? (gg.alignedA != 0 && (kbeg & 1) == 0)
+  const bool alignedA = AL ? true : GATHER ? (gg.alignedA != 0 && (kbeg & 1) == 0)
                                : ((((uintptr_t)p.A & 15) == 0) && ((p.lda & 1) == 0) && ((kbeg & 1) == 0));
-  const bool alignedB = GATHER ? (gg.alignedB != 0 && (kbeg & 1) == 0)
+  const bool alignedB = AL ? true : GATHER ? (gg.alignedB != 0 && (kbeg & 1) == 0)
                                : ((((uintptr_t)p.B & 15) == 0) && ((p.ldb & 1) == 0) && ((kbeg & 1) == 0));
   GatherSlots<BM, A_KC, NT> gsA;
   GatherSlots<BN, B_KC, NT> gsB;
@@ -376,12 +379,20 @@ int launch_cfg(cudaStream_t st, const GemmProb& p, const GemmProb* probs, int gz
   // row weights (weighted Gram only): the extra shared memory must not cost a resident CTA elsewhere
   if (GATHER && gg && gg->nw > 0) smem += (size_t)(STAGES * BK + 3 * GW_MAXLEN) * sizeof(double);
   else if (GATHER && gg && gg->ktabA) smem += (size_t)((p.K + 1) & ~1) * sizeof(long long);
-  auto kern = dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER>;
+  // all-aligned flavour: same tests as the kernel's, made here (single problem; every split starts at an even k)
+  bool al = !probs && (ksplit <= 1 || (kchunk & 1) == 0);
+  if (al) {
+    if (GATHER) al = gg && gg->alignedA != 0 && gg->alignedB != 0;
+    else al = (((uintptr_t)p.A & 15) == 0) && ((p.lda & 1) == 0) && (((uintptr_t)p.B & 15) == 0) && ((p.ldb & 1) == 0);
+  }
+  auto kern = al ? dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, true>
+                 : dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, false>;
   static char attr_set[PEPO_MAX_DEVICES] = {0};
   if (first_use_on_device(attr_set)) {
     const size_t smem_max = (size_t)STAGES * (BM + BN) * BK * sizeof(double) +
                             (GATHER ? (size_t)(STAGES * BK + 3 * GW_MAXLEN) * sizeof(double) : 0);
-    PEPO_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
+    PEPO_CUDA_OK(cudaFuncSetAttribute(dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
+    PEPO_CUDA_OK(cudaFuncSetAttribute(dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
   }
   long long tiles = ((maxM + BM - 1) / BM) * ((maxN + BN - 1) / BN);
   if (tiles <= 0 || gz <= 0) return 0;
