@@ -171,7 +171,9 @@ constexpr int GW_MAXLEN = 256;      // longest weight vector (chi_max <= 256)
 // AL: the host has checked that both operands take the 16-byte cp.async path in every stage (the
 // 8-byte fallback is then not compiled in: the unrolled main loop is half the size, which matters for
 // the instruction cache of the short-K reconstruction CTAs)
-template <int TA, int TB, int BM, int BN, int WM, int WN, int STAGES, bool GATHER, bool AL>
+// WGT: row weights on the k index (the weighted Gram); a run-time test of it in the main loop is
+// if-converted into a multiply by 1.0 that every kernel would execute
+template <int TA, int TB, int BM, int BN, int WM, int WN, int STAGES, bool GATHER, bool AL, bool WGT>
 __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, (BM == 64 && BN == 80) ? 3 : 1)
 dgemm_dmma_kernel(GemmProb p0, const GemmProb* __restrict__ probs, int ksplit, int kchunk,
                   double* __restrict__ part, int upper_only, GemmGather gg) {
@@ -220,7 +222,7 @@ dgemm_dmma_kernel(GemmProb p0, const GemmProb* __restrict__ probs, int ksplit, i
                                : ((((uintptr_t)p.B & 15) == 0) && ((p.ldb & 1) == 0) && ((kbeg & 1) == 0));
   GatherSlots<BM, A_KC, NT> gsA;
   GatherSlots<BN, B_KC, NT> gsB;
-  const bool weighted = GATHER && gg.nw > 0;
+  constexpr bool weighted = GATHER && WGT;
   if (GATHER) {
     gather_init<BM, A_KC, NT>(gsA, p.A, gg.a_outer, m0, M, tid);
     gather_init<BN, B_KC, NT>(gsB, p.B, gg.b_outer, n0, N, tid);
@@ -385,14 +387,19 @@ int launch_cfg(cudaStream_t st, const GemmProb& p, const GemmProb* probs, int gz
     if (GATHER) al = gg && gg->alignedA != 0 && gg->alignedB != 0;
     else al = (((uintptr_t)p.A & 15) == 0) && ((p.lda & 1) == 0) && (((uintptr_t)p.B & 15) == 0) && ((p.ldb & 1) == 0);
   }
-  auto kern = al ? dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, true>
-                 : dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, false>;
+  const bool wg = GATHER && gg && gg->nw > 0;
+  auto kern = dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, false, false>;
+  if (GATHER && wg) kern = al ? dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, true, GATHER>
+                              : dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, false, GATHER>;
+  else if (al) kern = dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, true, false>;
   static char attr_set[PEPO_MAX_DEVICES] = {0};
   if (first_use_on_device(attr_set)) {
     const size_t smem_max = (size_t)STAGES * (BM + BN) * BK * sizeof(double) +
                             (GATHER ? (size_t)(STAGES * BK + 3 * GW_MAXLEN) * sizeof(double) : 0);
-    PEPO_CUDA_OK(cudaFuncSetAttribute(dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
-    PEPO_CUDA_OK(cudaFuncSetAttribute(dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
+    PEPO_CUDA_OK(cudaFuncSetAttribute(dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
+    PEPO_CUDA_OK(cudaFuncSetAttribute(dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
+    PEPO_CUDA_OK(cudaFuncSetAttribute(dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, true, GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
+    PEPO_CUDA_OK(cudaFuncSetAttribute(dgemm_dmma_kernel<TA, TB, BM, BN, WM, WN, STAGES, GATHER, false, GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
   }
   long long tiles = ((maxM + BM - 1) / BM) * ((maxN + BN - 1) / BN);
   if (tiles <= 0 || gz <= 0) return 0;
