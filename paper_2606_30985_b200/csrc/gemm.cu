@@ -117,7 +117,10 @@ __device__ __forceinline__ void gather_init(GatherSlots<ROWS, KCONTIG, NT>& G, c
     }
   }
 }
-template <int ROWS, bool KCONTIG, int NT>
+// KTAB (non-K-contiguous operand only): the k offsets come from the per-CTA table, with no run-time choice
+// between table / plain stride / two-level arithmetic inside the chunk loop (that choice compiled to three
+// divergence-guarded branches per 16-byte chunk: ~45 instructions, against ~12 for the look-up)
+template <int ROWS, bool KCONTIG, int NT, bool KTAB = false>
 __device__ __forceinline__ void load_tile_gather(double* s, const GatherSlots<ROWS, KCONTIG, NT>& G,
                                                  const Idx2& fk, const long long* __restrict__ ktab, int kbeg,
                                                  int k0, int kend, bool aligned, int tid) {
@@ -153,7 +156,8 @@ __device__ __forceinline__ void load_tile_gather(double* s, const GatherSlots<RO
       const int nvalid = (gk < kend) ? G.nb[i] : 0;
       double* dst = s + k * ROWS + (rr ^ (4 * (k & 3)));
       long long okk = 0;
-      if (nvalid) okk = (fk.E.d == 0) ? fk.s * (long long)gk : (ktab ? ktab[gk - kbeg] : idx2_off(fk, (uint32_t)gk));
+      if (KTAB) okk = ktab[nvalid ? gk - kbeg : 0];
+      else if (nvalid) okk = (fk.E.d == 0) ? fk.s * (long long)gk : (ktab ? ktab[gk - kbeg] : idx2_off(fk, (uint32_t)gk));
       const double* src = G.p0[i] + okk;
       if (aligned) {
         cp_async16(dst, src, nvalid * 8);
@@ -251,7 +255,8 @@ dgemm_dmma_kernel(GemmProb p0, const GemmProb* __restrict__ probs, int ksplit, i
     if (it < nk) {
       int k0 = kbeg + it * BK;
       if (GATHER) {
-        load_tile_gather<BM, A_KC, NT>(sA + st * BM * BK, gsA, gg.a_k, gg.ktabA ? sK : nullptr, kbeg, k0, kend, alignedA, tid);
+        if (!A_KC && gg.ktabA) load_tile_gather<BM, A_KC, NT, true>(sA + st * BM * BK, gsA, gg.a_k, sK, kbeg, k0, kend, alignedA, tid);
+        else load_tile_gather<BM, A_KC, NT>(sA + st * BM * BK, gsA, gg.a_k, nullptr, kbeg, k0, kend, alignedA, tid);
         load_tile_gather<BN, B_KC, NT>(sB + st * BN * BK, gsB, gg.b_k, nullptr, kbeg, k0, kend, alignedB, tid);
         if (weighted && tid < BK) {
           const int k = k0 + tid;
