@@ -99,7 +99,7 @@ def _two_site_samples(t1, ax1, t2, ax2, idx1, idx2):
     return np.einsum("sc,sc->s", a[tuple(idx1.T)], b[tuple(idx2.T)])
 
 
-def _gate_replay(B, Lx, Ly, chi, bond, seed, ns=6000, max_inflight=0):
+def _gate_replay(B, Lx, Ly, chi, bond, seed, ns=6000, max_inflight=0, opts=None):
     """One Algorithm-1 gate on the seeded synthetic state, GPU vs oracle, through
     gauge-invariant quantities (R17): chi_new, lambda, and the gated two-site tensor Theta = psi1 . psi2
     on sampled entries in the ENVIRONMENT-WEIGHTED norm - the norm the simple update optimises and the
@@ -109,6 +109,8 @@ def _gate_replay(B, Lx, Ly, chi, bond, seed, ns=6000, max_inflight=0):
     Tolerance: 1e-12 relative (north_star: QR/SVD reconstructions within 1e-12 relative Frobenius)."""
     from paper_2606_30985_b200 import inputs
     sim = B.Pepo(Lx, Ly, 1, 1, J, H, DT, chi, 1e-10, 0.5, max_inflight=max_inflight)
+    for k, v in (opts or {}).items():
+        sim.set_option(k, v)
     _load_synthetic(sim, Lx, Ly, chi)
     nh = Ly * (Lx - 1)
     if bond < nh:
@@ -167,6 +169,27 @@ def test_gate_replay_4x4_chi60(gpu, which):
             "interior-interior": inputs.bond_id(L, L, 1, 1, "R")}[which]
     rel, _ = _gate_replay(B, L, L, chi, bond, seed=7)
     assert rel <= 1e-12, rel
+
+
+@pytest.mark.parametrize("orient", [0, 1, 2])
+def test_gate_replay_svd_orientation(gpu, orient):
+    """Option svd_orient: the QR preconditioner of the Jacobi SVD on K (0), on K^T (2) or on whichever is
+    more graded (1, default).  Every choice must give the oracle's gate to 1e-12 - orient 2
+    forces the transposed iteration and the transposed bridges on a square 240 x 240 core - and the adaptive
+    choice may not need more sweeps than the better of the two fixed ones (plus one)."""
+    torch, B = gpu
+    from paper_2606_30985_b200 import inputs
+    L, chi = 4, 60
+    bond = inputs.bond_id(L, L, 1, 1, "R")
+    rel, s = _gate_replay(B, L, L, chi, bond, seed=7, opts={"svd_orient": orient})
+    assert rel <= 1e-12, rel
+    test_gate_replay_svd_orientation.sweeps[orient] = s["jacobi_sweeps"]
+    if len(test_gate_replay_svd_orientation.sweeps) == 3:
+        sw = test_gate_replay_svd_orientation.sweeps
+        assert sw[1] <= min(sw[0], sw[2]) + 1, sw
+
+
+test_gate_replay_svd_orientation.sweeps = {}
 
 
 def test_gate_replay_config5_interior_shape(gpu):
